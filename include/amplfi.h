@@ -1,0 +1,142 @@
+/*
+ * amplfi.h -- C ABI of libamplfi: the GPU data-generation hot path of AMPLFI
+ * (arXiv 2407.19048, section 3 "Simulations on Accelerated Hardware").
+ *
+ * Every step of the path runs in hand-written CUDA kernels for sm_100a (B200).  There is no
+ * CPU fallback: without a CUDA device every compute call returns AMPLFI_ERR_CUDA.
+ *
+ * Conventions ("Boundary"):
+ *  - Every pointer argument below is a DEVICE pointer unless its comment says HOST.
+ *  - All buffers are owned by the caller, row-major, contiguous.  Complex numbers are interleaved
+ *    (re, im) float pairs.  The library allocates device memory only in amplfi_plan_create (tables,
+ *    Welch partial sums, per-sample coefficient workspace) and frees it in amplfi_plan_destroy.
+ *  - Calls enqueue work on the caller's stream (`stream` is a cudaStream_t passed as void*, NULL = the
+ *    legacy default stream) and return without synchronising.  A plan must not be used from two
+ *    streams at once (its workspace is shared).
+ *  - Return value: AMPLFI_OK or a negative AMPLFI_ERR_*; amplfi_last_error() gives a thread-local
+ *    message.  No exceptions, no aborts, nothing printed.
+ *  - Units: masses in solar masses, distance in Mpc, times in seconds, angles in radians.
+ *    Strain buffers (noise, bg, strip) are fp32 in natural strain units (~1e-21).  Frequency-domain
+ *    waveform buffers (hp, hc, h_det) are fp32 in strain/Hz.  Power spectra do not fit fp32's range
+ *    (S ~ 1e-47 strain^2/Hz): every `psd` buffer holds  S(f) * 2^140  (amplfi_psd_scale()).
+ *    Whitened output is dimensionless (unit variance per kept frequency bin).
+ *  - Frequency grid of a plan: f_k = k * fs / n, k = 0 .. K-1, K = n/2 + 1.
+ *  - Fourier convention: forward X[k] = sum_n x[n] exp(-2 pi i k n / N); a signal
+ *    h(f) = A exp(-i Psi), Psi containing +2 pi f t_c, merges at time t_c inside the segment.
+ */
+#ifndef AMPLFI_H
+#define AMPLFI_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define AMPLFI_OK                    0
+#define AMPLFI_ERR_INVALID_ARG      (-1)  /* null pointer, batch/n_det <= 0, f_lo >= f_hi, f_hi > fs/2, bad ids */
+#define AMPLFI_ERR_UNSUPPORTED_SIZE (-2)  /* n or nperseg not a power of two in [2^10, 2^16]; nperseg > n_bg */
+#define AMPLFI_ERR_CUDA             (-3)  /* CUDA runtime/launch error (message in amplfi_last_error) */
+#define AMPLFI_ERR_ALIGNMENT        (-4)  /* a buffer is not aligned as documented */
+
+#define AMPLFI_TAYLORF2    0   /* 3.5PN non-spinning inspiral to f_ISCO (ref. [33]) */
+#define AMPLFI_IMRPHENOMD  1   /* the paper's approximant (ref. [32]), aligned spins */
+
+#define AMPLFI_H1 0
+#define AMPLFI_L1 1
+#define AMPLFI_V1 2
+
+#define AMPLFI_N_PARAMS 11
+/* params row (fp64): 0 mchirp  1 q = m2/m1 in (0,1]  2 chi1  3 chi2  4 dist_mpc  5 theta_jn  6 phi_c
+ *                    7 t_c (seconds from the start of the segment)  8 ra  9 dec  10 psi
+ * = Theta of PAPER.md:151 eq. (4) plus the aligned spins and the arrival time
+ * (PAPER.md:93, :117).  A row with q outside (0,1], |chi| >= 1, dist <= 0, mchirp <= 0 or a
+ * non-finite entry does not fail the call: that sample's waveform is identically zero and
+ * flags[b] = 1 where a flags buffer is given. */
+
+typedef struct amplfi_plan amplfi_plan;   /* opaque */
+
+/* Thread-local description of the last error returned on this thread ("" if none). HOST string. */
+const char* amplfi_last_error(void);
+
+/* 2^140, the factor every psd buffer is multiplied by. */
+double amplfi_psd_scale(void);
+
+/* Library build tag, e.g. "amplfi-b200 sm_100a". HOST string. */
+const char* amplfi_version(void);
+
+/* Copy of the IMRPhenomD fit table the kernels use: 19 rows x 11 doubles, row order
+ * rho1 rho2 rho3 v2 gamma1 gamma2 gamma3 sigma1..4 beta1..3 alpha1..5.  `out` is a HOST buffer of
+ * 209 doubles.  (Used by the tests to check the library's copy against the oracle's.) */
+int amplfi_phenomd_table(double* out);
+
+/* Create a plan for segments of n samples at fs Hz seen by n_det detectors.
+ *   n        power of two, 2^10 .. 2^16 (4 s at 2048 Hz = 8192)
+ *   det_ids  HOST array [n_det] of AMPLFI_H1/L1/V1 ("Hanford and Livingston"), n_det 1..3
+ *   max_batch  largest batch later passed to the per-batch calls (sizes the coefficient workspace
+ *              and, for the fused call, the [max_batch, K] complex h0 workspace)
+ *   nperseg  Welch segment length, power of two 2^10 .. 2^16 with nperseg <= n, or 0 if
+ *            amplfi_psd_welch will not be called
+ * Allocates device tables on the current CUDA device.  *out receives the plan. */
+int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_batch, int nperseg,
+                       amplfi_plan** out);
+void amplfi_plan_destroy(amplfi_plan* plan);
+
+/* a-1 Waveform (section 3.1; "generate the IMRPhenomD waveforms directly on
+ * the GPU").  For each sample b and bin k:
+ *     h+ = (1 + cos^2 theta_jn)/2 * h0,   hx = -i cos(theta_jn) * h0,
+ *     h0(f_k) = A(f_k) exp(-i Psi(f_k)) for f_lo <= f_k <= f_top(b), zero elsewhere (bin 0 and the
+ *     Nyquist bin are always zero);  f_top = min(f_ISCO, f_hi) for TaylorF2, min(0.2/M, f_hi) for
+ *     IMRPhenomD.  Phase is accumulated in fp64, amplitude in fp32.
+ *   params [batch, 11] fp64;  hp, hc [batch, K, 2] fp32;  flags [batch] int32 or NULL. */
+int amplfi_waveform_fd(const amplfi_plan* plan, int approximant, int batch, const double* params,
+                       double f_lo, double f_hi, float* hp, float* hc, int* flags, void* stream);
+
+/* a-2, a-3 Projection ("antenna response ... on-the-fly on the GPU"):
+ *     h_d(f_k) = (F+_d h+ + Fx_d hx) exp(-2 pi i f_k dt_d),
+ * F+, Fx the antenna patterns of detector d for (ra, dec, psi) at Greenwich sidereal angle gmst and
+ * dt_d the arrival-time offset of detector d relative to the geocentre (computed in fp64).
+ *   hp, hc [batch, K, 2];  h_det [batch, n_det, K, 2] fp32;
+ *   resp NULL or [batch, n_det, 3] fp64 receiving (F+, Fx, dt).
+ * hp/hc/h_det may be NULL if only resp is wanted (then resp must not be NULL). */
+int amplfi_project(const amplfi_plan* plan, int batch, const double* params, double gmst,
+                   const float* hp, const float* hc, float* h_det, double* resp, void* stream);
+
+/* a-4 Welch PSD ("power spectra estimation"; "The power spectra is fit to
+ * this background chunk"): per detector, segments of nperseg samples stepping by nperseg - noverlap
+ * (full segments only), optional mean removal, periodic Hann window, |FFT|^2, mean over segments,
+ * one-sided density.
+ *   bg [n_det, n_bg] fp32 strain, row stride n_bg;  noverlap in [0, nperseg);  detrend 0 none / 1 constant;
+ *   average must be 0 (mean);  psd [n_det, nperseg/2+1] fp32 receives S * 2^140.
+ * Deterministic (fixed summation order). */
+int amplfi_psd_welch(const amplfi_plan* plan, const float* bg, long n_bg, int noverlap, int detrend,
+                     int average, float* psd, void* stream);
+
+/* a-5 .. a-9 Gather + inject + whiten ("N small background chunks ... are lazily loaded";
+ * PAPER.md:105 "We then inject the signals into the background chunks ... We whiten the batch using the
+ * estimated power spectra"):
+ *     out[b,d,:] = irfft( ( rfft(x[b,d,:]) + fs * h_d[b,:] ) * w_d ),
+ *     w_d[k] = sqrt(2 / (fs * S_d(f_k))) for f_lo <= f_k <= f_hi, 0 elsewhere.
+ *   noise    offsets == NULL: dense [batch, n_det, n] fp32.
+ *            offsets != NULL: strip [n_det, strip_len] fp32 and x[b,d,:] = strip[d, offsets[b,d] : +n];
+ *            offsets [batch, n_det] int64, each in [0, strip_len - n] (checked on the device: an
+ *            out-of-range offset yields an all-NaN row, never an out-of-bounds read).
+ *   h_det    [batch, n_det, K, 2] fp32 to inject a caller-supplied projected waveform, or NULL.
+ *   params   used when h_det == NULL: [batch, 11] fp64 -> the waveform is generated, projected and
+ *            injected inside the call (fused path; `approximant`, `gmst` as above; the waveform band is
+ *            the same [f_lo, f_hi]).  h_det == NULL and params == NULL: whiten only.
+ *   psd      [n_det, n_psd] fp32, S * 2^140; n_psd == K, or n_psd == (n/r)/2+1 for an integer r >= 1, in
+ *            which case S is linearly interpolated in frequency onto the segment grid.
+ *   out      [batch, n_det, n] fp32.
+ * batch <= the plan's max_batch.  n = 2^16 needs a 2-CTA thread-block cluster per segment. */
+int amplfi_inject_whiten(const amplfi_plan* plan, int batch, const float* noise, const long* offsets,
+                         long strip_len, const float* h_det, int approximant, const double* params,
+                         double gmst, const float* psd, int n_psd, double f_lo, double f_hi,
+                         float* out, void* stream);
+
+/* Number of kernel launches the library has enqueued since it was loaded (all plans, all threads).
+ * bench.py reports the difference across its timed region as "gpu_launches". */
+long amplfi_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AMPLFI_H */

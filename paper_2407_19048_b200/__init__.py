@@ -1,0 +1,196 @@
+"""Thin Python binding of libamplfi (include/amplfi.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of ``libamplfi.so``; torch is used for device
+memory and streams.  There is no CPU fallback: if the shared library is missing, importing this
+package raises, and every compute call needs CUDA tensors.
+
+The functions keep the C names: ``amplfi_waveform_fd``, ``amplfi_project``, ``amplfi_psd_welch``,
+``amplfi_inject_whiten`` (PAPER.md:101-105 for the steps they implement).
+"""
+import ctypes
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libamplfi.so")
+
+OK, ERR_INVALID_ARG, ERR_UNSUPPORTED_SIZE, ERR_CUDA, ERR_ALIGNMENT = 0, -1, -2, -3, -4
+TAYLORF2, IMRPHENOMD = 0, 1
+H1, L1, V1 = 0, 1, 2
+N_PARAMS = 11
+
+EXPORTS = ("amplfi_last_error", "amplfi_psd_scale", "amplfi_version", "amplfi_phenomd_table",
+           "amplfi_plan_create", "amplfi_plan_destroy", "amplfi_waveform_fd", "amplfi_project",
+           "amplfi_psd_welch", "amplfi_inject_whiten", "amplfi_launch_count")
+
+
+class AmplfiError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("libamplfi error %d: %s" % (code, msg))
+        self.code = code
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError("libamplfi.so not found at %s: build it with `python -m paper_2407_19048_b200.build` "
+                          "(there is no CPU fallback)" % LIB_PATH)
+    lib = ctypes.CDLL(LIB_PATH)
+    c = ctypes
+    vp, dbl, i32, i64 = c.c_void_p, c.c_double, c.c_int, c.c_long
+    lib.amplfi_last_error.restype = c.c_char_p
+    lib.amplfi_last_error.argtypes = []
+    lib.amplfi_psd_scale.restype = dbl
+    lib.amplfi_psd_scale.argtypes = []
+    lib.amplfi_version.restype = c.c_char_p
+    lib.amplfi_version.argtypes = []
+    lib.amplfi_launch_count.restype = i64
+    lib.amplfi_launch_count.argtypes = []
+    lib.amplfi_phenomd_table.restype = i32
+    lib.amplfi_phenomd_table.argtypes = [vp]
+    lib.amplfi_plan_create.restype = i32
+    lib.amplfi_plan_create.argtypes = [i32, dbl, i32, c.POINTER(i32), i32, i32, c.POINTER(vp)]
+    lib.amplfi_plan_destroy.restype = None
+    lib.amplfi_plan_destroy.argtypes = [vp]
+    lib.amplfi_waveform_fd.restype = i32
+    lib.amplfi_waveform_fd.argtypes = [vp, i32, i32, vp, dbl, dbl, vp, vp, vp, vp]
+    lib.amplfi_project.restype = i32
+    lib.amplfi_project.argtypes = [vp, i32, vp, dbl, vp, vp, vp, vp, vp]
+    lib.amplfi_psd_welch.restype = i32
+    lib.amplfi_psd_welch.argtypes = [vp, vp, i64, i32, i32, i32, vp, vp]
+    lib.amplfi_inject_whiten.restype = i32
+    lib.amplfi_inject_whiten.argtypes = [vp, i32, vp, vp, i64, vp, i32, vp, dbl, vp, i32, dbl, dbl, vp, vp]
+    return lib
+
+
+_lib = _load()
+
+
+def _check(rc):
+    if rc != OK:
+        raise AmplfiError(rc, _lib.amplfi_last_error().decode())
+
+
+def _ptr(t, dtype=None, name="tensor"):
+    if t is None:
+        return None
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError("%s must be a CUDA tensor (no CPU fallback)" % name)
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError("%s must have dtype %s, got %s" % (name, dtype, t.dtype))
+    if not t.is_contiguous():
+        raise ValueError("%s must be contiguous" % name)
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _stream(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
+
+
+def last_error():
+    return _lib.amplfi_last_error().decode()
+
+
+def psd_scale():
+    return _lib.amplfi_psd_scale()
+
+
+def version():
+    return _lib.amplfi_version().decode()
+
+
+def launch_count():
+    return int(_lib.amplfi_launch_count())
+
+
+def phenomd_table():
+    buf = (ctypes.c_double * 209)()
+    _check(_lib.amplfi_phenomd_table(ctypes.cast(buf, ctypes.c_void_p)))
+    return [list(buf[r * 11:(r + 1) * 11]) for r in range(19)]
+
+
+class Plan:
+    """amplfi_plan_create / amplfi_plan_destroy."""
+
+    def __init__(self, n, fs, det_ids, max_batch, nperseg=0):
+        det_ids = [int(d) for d in det_ids]
+        arr = (ctypes.c_int * max(len(det_ids), 1))(*det_ids)
+        handle = ctypes.c_void_p()
+        _check(_lib.amplfi_plan_create(int(n), float(fs), len(det_ids), arr, int(max_batch), int(nperseg),
+                                       ctypes.byref(handle)))
+        self._h = handle
+        self.n, self.fs, self.det_ids, self.max_batch, self.nperseg = int(n), float(fs), det_ids, int(max_batch), int(nperseg)
+        self.n_det = len(det_ids)
+        self.n_bins = self.n // 2 + 1
+
+    def close(self):
+        if getattr(self, "_h", None):
+            _lib.amplfi_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def amplfi_waveform_fd(plan, approximant, params, f_lo, f_hi, hp=None, hc=None, flags=None, stream=None):
+    """params [B, 11] fp64 cuda -> (hp, hc) [B, K, 2] fp32, flags [B] int32."""
+    batch = params.shape[0]
+    dev = params.device
+    if hp is None:
+        hp = torch.empty((batch, plan.n_bins, 2), dtype=torch.float32, device=dev)
+    if hc is None:
+        hc = torch.empty((batch, plan.n_bins, 2), dtype=torch.float32, device=dev)
+    if flags is None:
+        flags = torch.empty((batch,), dtype=torch.int32, device=dev)
+    _check(_lib.amplfi_waveform_fd(plan._h, int(approximant), int(batch), _ptr(params, torch.float64, "params"),
+                                   float(f_lo), float(f_hi), _ptr(hp, torch.float32, "hp"),
+                                   _ptr(hc, torch.float32, "hc"), _ptr(flags, torch.int32, "flags"), _stream(stream)))
+    return hp, hc, flags
+
+
+def amplfi_project(plan, params, gmst, hp=None, hc=None, h_det=None, resp=None, want_resp=True, stream=None):
+    """-> (h_det [B, D, K, 2] fp32 or None, resp [B, D, 3] fp64 or None)."""
+    batch = params.shape[0]
+    dev = params.device
+    if hp is not None and h_det is None:
+        h_det = torch.empty((batch, plan.n_det, plan.n_bins, 2), dtype=torch.float32, device=dev)
+    if want_resp and resp is None:
+        resp = torch.empty((batch, plan.n_det, 3), dtype=torch.float64, device=dev)
+    _check(_lib.amplfi_project(plan._h, int(batch), _ptr(params, torch.float64, "params"), float(gmst),
+                               _ptr(hp, torch.float32, "hp"), _ptr(hc, torch.float32, "hc"),
+                               _ptr(h_det, torch.float32, "h_det"), _ptr(resp, torch.float64, "resp"),
+                               _stream(stream)))
+    return h_det, resp
+
+
+def amplfi_psd_welch(plan, bg, noverlap=None, detrend=1, average=0, psd=None, stream=None):
+    """bg [D, n_bg] fp32 -> psd [D, nperseg/2+1] fp32 (S * 2^140)."""
+    if noverlap is None:
+        noverlap = plan.nperseg // 2
+    if psd is None:
+        psd = torch.empty((plan.n_det, plan.nperseg // 2 + 1), dtype=torch.float32, device=bg.device)
+    if bg.dim() != 2 or bg.shape[0] != plan.n_det:
+        raise ValueError("bg must be [n_det, n_bg]")
+    _check(_lib.amplfi_psd_welch(plan._h, _ptr(bg, torch.float32, "bg"), int(bg.shape[1]), int(noverlap), int(detrend),
+                                 int(average), _ptr(psd, torch.float32, "psd"), _stream(stream)))
+    return psd
+
+
+def amplfi_inject_whiten(plan, batch, noise, psd, f_lo, f_hi, offsets=None, h_det=None, approximant=IMRPHENOMD,
+                         params=None, gmst=0.0, out=None, stream=None):
+    """noise dense [B, D, N] (offsets None) or strip [D, L] with offsets [B, D] int64 -> out [B, D, N] fp32."""
+    if out is None:
+        out = torch.empty((batch, plan.n_det, plan.n), dtype=torch.float32, device=noise.device)
+    strip_len = int(noise.shape[-1]) if offsets is not None else 0
+    _check(_lib.amplfi_inject_whiten(plan._h, int(batch), _ptr(noise, torch.float32, "noise"),
+                                     _ptr(offsets, torch.int64, "offsets"), strip_len,
+                                     _ptr(h_det, torch.float32, "h_det"), int(approximant),
+                                     _ptr(params, torch.float64, "params"), float(gmst),
+                                     _ptr(psd, torch.float32, "psd"), int(psd.shape[-1]), float(f_lo), float(f_hi),
+                                     _ptr(out, torch.float32, "out"), _stream(stream)))
+    return out

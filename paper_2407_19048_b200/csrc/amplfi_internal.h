@@ -1,0 +1,62 @@
+// amplfi_internal.h -- plan layout and launch entry points shared by the library's translation units.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "../../include/amplfi.h"
+#include "phenomd_table.h"
+
+namespace amplfi {
+struct WfCoef;
+struct DetResp;
+}
+
+struct amplfi_plan {
+    int n;                 // samples per segment
+    int n_bins;            // n/2 + 1
+    int logm;              // log2(n/2)
+    double fs, t_seg;
+    int n_det;
+    int det_ids[3];
+    int max_batch;
+    int nperseg;           // 0: no Welch
+    int device;
+    int sm_count;
+    // device tables / workspace (owned)
+    double* tab_ci;        // [n_bins] k^(-1/3)   (tab_ci[0] = 0)
+    double* tab_lnk;       // [n_bins] ln k       (tab_lnk[0] = 0)
+    double* pd_table;      // [19*11]
+    amplfi::WfCoef* coef;  // [max_batch]
+    amplfi::DetResp* resp; // [max_batch * n_det]
+    float2* h0;            // [max_batch * n_bins]   fused path: 2 fs h0
+    float* filt;           // [n_det * n_bins]       whitening filter incl. 1/(2n)
+    float* welch_part;     // [n_det * max_seg * (nperseg/2+1)]
+    int welch_max_seg;
+    int* d_det_ids;        // [3]
+};
+
+namespace amplfi {
+
+void set_error(const char* fmt, ...);
+int check_launch(const char* what);
+void count_launch(int n = 1);
+
+// waveform.cu
+int launch_prepare(const amplfi_plan* p, int approximant, int batch, const double* params, double gmst,
+                   double f_lo, double f_hi, double amp_mul, int* flags, cudaStream_t st);
+int launch_waveform_pol(const amplfi_plan* p, int batch, float* hp, float* hc, cudaStream_t st);
+int launch_waveform_h0(const amplfi_plan* p, int batch, cudaStream_t st);
+int launch_project(const amplfi_plan* p, int batch, const float* hp, const float* hc, float* h_det,
+                   double* resp_out, cudaStream_t st);
+int launch_tables(amplfi_plan* p, cudaStream_t st);
+
+// welch.cu
+int launch_welch(const amplfi_plan* p, const float* bg, long n_bg, int noverlap, int detrend, float* psd,
+                 cudaStream_t st);
+
+// inject_whiten.cu
+int launch_filter(const amplfi_plan* p, const float* psd, int n_psd, double f_lo, double f_hi, cudaStream_t st);
+int launch_inject_whiten(const amplfi_plan* p, int batch, const float* noise, const long* offsets,
+                         long strip_len, const float* h_det, int fused, float* out, cudaStream_t st);
+int setup_inject_whiten_attrs();
+
+}  // namespace amplfi

@@ -1,0 +1,204 @@
+// api.cu -- the C ABI of libamplfi (include/amplfi.h): argument validation, plan management and the
+// sequencing of kernel launches.  No computation happens on the host.
+#include <atomic>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+
+#include "amplfi_internal.h"
+#include "fft_core.cuh"
+#include "waveform.cuh"
+
+namespace amplfi {
+
+static thread_local char g_err[512] = "";
+static std::atomic<long> g_launches{0};
+
+void set_error(const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
+
+void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+int check_launch(const char* what) {
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        set_error("%s: %s", what, cudaGetErrorString(e));
+        return AMPLFI_ERR_CUDA;
+    }
+    return AMPLFI_OK;
+}
+
+static bool is_pow2_in_range(long v) { return v >= 1024 && v <= 65536 && (v & (v - 1)) == 0; }
+
+static const double kPdTable[AMPLFI_PD_ROWS][AMPLFI_PD_COLS] = AMPLFI_PD_TABLE_INIT;
+
+template <class T>
+static int dev_alloc(T** ptr, size_t count) {
+    cudaError_t e = cudaMalloc(reinterpret_cast<void**>(ptr), count * sizeof(T));
+    if (e != cudaSuccess) {
+        set_error("cudaMalloc(%zu bytes): %s", count * sizeof(T), cudaGetErrorString(e));
+        return AMPLFI_ERR_CUDA;
+    }
+    return AMPLFI_OK;
+}
+
+static int validate_band(const amplfi_plan* p, double f_lo, double f_hi, const char* who) {
+    if (!(f_lo >= 0.0) || !(f_hi > f_lo) || !(f_hi <= 0.5 * p->fs)) {
+        set_error("%s: need 0 <= f_lo < f_hi <= fs/2 (got %g, %g, fs %g)", who, f_lo, f_hi, p->fs);
+        return AMPLFI_ERR_INVALID_ARG;
+    }
+    return AMPLFI_OK;
+}
+
+}  // namespace amplfi
+
+using namespace amplfi;
+
+extern "C" {
+
+const char* amplfi_last_error(void) { return g_err; }
+
+double amplfi_psd_scale(void) { return std::ldexp(1.0, 140); }
+
+const char* amplfi_version(void) { return "amplfi-b200 0.1 (sm_100a)"; }
+
+long amplfi_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+int amplfi_phenomd_table(double* out) {
+    if (out == nullptr) { set_error("amplfi_phenomd_table: null output"); return AMPLFI_ERR_INVALID_ARG; }
+    std::memcpy(out, kPdTable, sizeof(kPdTable));
+    return AMPLFI_OK;
+}
+
+int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_batch, int nperseg,
+                       amplfi_plan** out) {
+    if (out == nullptr || det_ids == nullptr) { set_error("amplfi_plan_create: null pointer"); return AMPLFI_ERR_INVALID_ARG; }
+    *out = nullptr;
+    if (n_det < 1 || n_det > 3 || max_batch < 1 || !(fs > 0.0) || !std::isfinite(fs)) {
+        set_error("amplfi_plan_create: need 1 <= n_det <= 3, max_batch >= 1, fs > 0");
+        return AMPLFI_ERR_INVALID_ARG;
+    }
+    for (int d = 0; d < n_det; ++d)
+        if (det_ids[d] < 0 || det_ids[d] > 2) { set_error("amplfi_plan_create: unknown detector id %d", det_ids[d]); return AMPLFI_ERR_INVALID_ARG; }
+    if (!is_pow2_in_range(n)) { set_error("amplfi_plan_create: n = %d is not a power of two in [2^10, 2^16]", n); return AMPLFI_ERR_UNSUPPORTED_SIZE; }
+    if (nperseg != 0 && (!is_pow2_in_range(nperseg) || nperseg > 32768)) {
+        set_error("amplfi_plan_create: nperseg = %d is not a power of two in [2^10, 2^15]", nperseg);
+        return AMPLFI_ERR_UNSUPPORTED_SIZE;
+    }
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    int sms = 0;
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) { set_error("amplfi_plan_create: no CUDA device (%s)", cudaGetErrorString(e)); return AMPLFI_ERR_CUDA; }
+
+    amplfi_plan* p = new amplfi_plan();
+    std::memset(p, 0, sizeof(*p));
+    p->n = n; p->n_bins = n / 2 + 1; p->logm = ilog2(n) - 1;
+    p->fs = fs; p->t_seg = (double)n / fs;
+    p->n_det = n_det;
+    for (int d = 0; d < n_det; ++d) p->det_ids[d] = det_ids[d];
+    p->max_batch = max_batch; p->nperseg = nperseg; p->device = dev; p->sm_count = sms;
+    p->welch_max_seg = 256;
+    int rc = AMPLFI_OK;
+    if (!rc) rc = dev_alloc(&p->tab_ci, (size_t)p->n_bins);
+    if (!rc) rc = dev_alloc(&p->tab_lnk, (size_t)p->n_bins);
+    if (!rc) rc = dev_alloc(&p->pd_table, (size_t)AMPLFI_PD_ROWS * AMPLFI_PD_COLS);
+    if (!rc) rc = dev_alloc(&p->coef, (size_t)max_batch);
+    if (!rc) rc = dev_alloc(&p->resp, (size_t)max_batch * n_det);
+    if (!rc) rc = dev_alloc(&p->h0, (size_t)max_batch * p->n_bins);
+    if (!rc) rc = dev_alloc(&p->filt, (size_t)n_det * p->n_bins);
+    if (!rc) rc = dev_alloc(&p->d_det_ids, (size_t)3);
+    if (!rc && nperseg) rc = dev_alloc(&p->welch_part, (size_t)n_det * p->welch_max_seg * (nperseg / 2 + 1));
+    if (!rc) {
+        e = cudaMemcpy(p->pd_table, kPdTable, sizeof(kPdTable), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMemcpy(p->d_det_ids, p->det_ids, sizeof(int) * 3, cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) { set_error("amplfi_plan_create: cudaMemcpy: %s", cudaGetErrorString(e)); rc = AMPLFI_ERR_CUDA; }
+    }
+    if (!rc) rc = launch_tables(p, nullptr);
+    if (!rc) {
+        e = cudaStreamSynchronize(nullptr);
+        if (e != cudaSuccess) { set_error("amplfi_plan_create: %s", cudaGetErrorString(e)); rc = AMPLFI_ERR_CUDA; }
+    }
+    if (rc) { amplfi_plan_destroy(p); return rc; }
+    *out = p;
+    return AMPLFI_OK;
+}
+
+void amplfi_plan_destroy(amplfi_plan* p) {
+    if (p == nullptr) return;
+    cudaFree(p->tab_ci); cudaFree(p->tab_lnk); cudaFree(p->pd_table); cudaFree(p->coef); cudaFree(p->resp);
+    cudaFree(p->h0); cudaFree(p->filt); cudaFree(p->welch_part); cudaFree(p->d_det_ids);
+    delete p;
+}
+
+int amplfi_waveform_fd(const amplfi_plan* p, int approximant, int batch, const double* params, double f_lo,
+                       double f_hi, float* hp, float* hc, int* flags, void* stream) {
+    if (p == nullptr || params == nullptr || hp == nullptr || hc == nullptr) { set_error("amplfi_waveform_fd: null pointer"); return AMPLFI_ERR_INVALID_ARG; }
+    if (batch < 1 || batch > p->max_batch) { set_error("amplfi_waveform_fd: batch %d outside [1, %d]", batch, p->max_batch); return AMPLFI_ERR_INVALID_ARG; }
+    if (approximant != AMPLFI_TAYLORF2 && approximant != AMPLFI_IMRPHENOMD) { set_error("amplfi_waveform_fd: unknown approximant %d", approximant); return AMPLFI_ERR_INVALID_ARG; }
+    int rc = validate_band(p, f_lo, f_hi, "amplfi_waveform_fd");
+    if (rc) return rc;
+    if ((reinterpret_cast<size_t>(hp) | reinterpret_cast<size_t>(hc)) & 7) { set_error("amplfi_waveform_fd: hp/hc must be 8-byte aligned"); return AMPLFI_ERR_ALIGNMENT; }
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    rc = launch_prepare(p, approximant, batch, params, 0.0, f_lo, f_hi, 1.0, flags, st);
+    if (rc) return rc;
+    return launch_waveform_pol(p, batch, hp, hc, st);
+}
+
+int amplfi_project(const amplfi_plan* p, int batch, const double* params, double gmst, const float* hp,
+                   const float* hc, float* h_det, double* resp, void* stream) {
+    if (p == nullptr || params == nullptr) { set_error("amplfi_project: null pointer"); return AMPLFI_ERR_INVALID_ARG; }
+    if (batch < 1 || batch > p->max_batch) { set_error("amplfi_project: batch %d outside [1, %d]", batch, p->max_batch); return AMPLFI_ERR_INVALID_ARG; }
+    const bool any = hp != nullptr || hc != nullptr || h_det != nullptr;
+    if (any && (hp == nullptr || hc == nullptr || h_det == nullptr)) { set_error("amplfi_project: hp, hc, h_det must be all given or all NULL"); return AMPLFI_ERR_INVALID_ARG; }
+    if (!any && resp == nullptr) { set_error("amplfi_project: nothing to compute"); return AMPLFI_ERR_INVALID_ARG; }
+    if (any && ((reinterpret_cast<size_t>(hp) | reinterpret_cast<size_t>(hc) | reinterpret_cast<size_t>(h_det)) & 7)) { set_error("amplfi_project: buffers must be 8-byte aligned"); return AMPLFI_ERR_ALIGNMENT; }
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    int rc = launch_prepare(p, -1, batch, params, gmst, 0.0, 0.0, 1.0, nullptr, st);
+    if (rc) return rc;
+    return launch_project(p, batch, hp, hc, h_det, resp, st);
+}
+
+int amplfi_psd_welch(const amplfi_plan* p, const float* bg, long n_bg, int noverlap, int detrend, int average,
+                     float* psd, void* stream) {
+    if (p == nullptr || bg == nullptr || psd == nullptr) { set_error("amplfi_psd_welch: null pointer"); return AMPLFI_ERR_INVALID_ARG; }
+    if (p->nperseg == 0) { set_error("amplfi_psd_welch: plan was created with nperseg = 0"); return AMPLFI_ERR_INVALID_ARG; }
+    if (n_bg < p->nperseg) { set_error("amplfi_psd_welch: nperseg %d > n_bg %ld", p->nperseg, n_bg); return AMPLFI_ERR_UNSUPPORTED_SIZE; }
+    if (noverlap < 0 || noverlap >= p->nperseg || (detrend != 0 && detrend != 1) || average != 0) {
+        set_error("amplfi_psd_welch: need 0 <= noverlap < nperseg, detrend in {0,1}, average = 0 (mean)");
+        return AMPLFI_ERR_INVALID_ARG;
+    }
+    return launch_welch(p, bg, n_bg, noverlap, detrend, psd, static_cast<cudaStream_t>(stream));
+}
+
+int amplfi_inject_whiten(const amplfi_plan* p, int batch, const float* noise, const long* offsets, long strip_len,
+                         const float* h_det, int approximant, const double* params, double gmst, const float* psd,
+                         int n_psd, double f_lo, double f_hi, float* out, void* stream) {
+    if (p == nullptr || noise == nullptr || psd == nullptr || out == nullptr) { set_error("amplfi_inject_whiten: null pointer"); return AMPLFI_ERR_INVALID_ARG; }
+    if (batch < 1 || batch > p->max_batch) { set_error("amplfi_inject_whiten: batch %d outside [1, %d]", batch, p->max_batch); return AMPLFI_ERR_INVALID_ARG; }
+    int rc = validate_band(p, f_lo, f_hi, "amplfi_inject_whiten");
+    if (rc) return rc;
+    if (offsets != nullptr && strip_len < p->n) { set_error("amplfi_inject_whiten: strip_len %ld < n %d", strip_len, p->n); return AMPLFI_ERR_INVALID_ARG; }
+    if (n_psd < 2 || ((p->n / 2) % (n_psd - 1)) != 0) { set_error("amplfi_inject_whiten: n_psd = %d does not divide the segment grid (n/2 = %d)", n_psd, p->n / 2); return AMPLFI_ERR_INVALID_ARG; }
+    const bool fused = (h_det == nullptr && params != nullptr);
+    if (fused && approximant != AMPLFI_TAYLORF2 && approximant != AMPLFI_IMRPHENOMD) { set_error("amplfi_inject_whiten: unknown approximant %d", approximant); return AMPLFI_ERR_INVALID_ARG; }
+    if ((reinterpret_cast<size_t>(out) & 7) || (reinterpret_cast<size_t>(noise) & 3) || (reinterpret_cast<size_t>(h_det) & 7)) { set_error("amplfi_inject_whiten: out/h_det must be 8-byte aligned, noise 4-byte aligned"); return AMPLFI_ERR_ALIGNMENT; }
+    if (p->logm > 14) { set_error("amplfi_inject_whiten: n = %d not supported by this build", p->n); return AMPLFI_ERR_UNSUPPORTED_SIZE; }
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    rc = launch_filter(p, psd, n_psd, f_lo, f_hi, st);
+    if (rc) return rc;
+    if (fused) {
+        rc = launch_prepare(p, approximant, batch, params, gmst, f_lo, f_hi, 2.0 * p->fs, nullptr, st);
+        if (rc) return rc;
+        rc = launch_waveform_h0(p, batch, st);
+        if (rc) return rc;
+    }
+    return launch_inject_whiten(p, batch, noise, offsets, strip_len, h_det, fused ? 1 : 0, out, st);
+}
+
+}  // extern "C"

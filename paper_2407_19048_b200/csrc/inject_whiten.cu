@@ -1,0 +1,254 @@
+// inject_whiten.cu -- the fused gather -> real FFT -> inject -> whiten/band-limit -> inverse real FFT kernel.
+// PAPER.md:103 (background chunks "lazily loaded" from the GPU-resident strip), PAPER.md:105 ("inject the
+// signals into the background chunks ... whiten the batch using the estimated power spectra").
+//
+// One CTA per (sample, detector) segment.  The segment lives in shared memory between the FFT passes and
+// in registers during the per-bin work; HBM sees 4 B/sample in and 4 B/sample out (plus the L2-resident
+// filter and, on the fused path, the per-sample h0 spectrum shared by the detectors of a sample).
+#include "amplfi_internal.h"
+#include "fft_core.cuh"
+#include "waveform.cuh"
+
+namespace amplfi {
+
+// ---- whitening filter on the segment grid: w[k] = sqrt(2/(fs S)) / (2N) inside the band, else 0 ----
+// psd holds S * 2^140, so sqrt(2/(fs S)) = 2^70 * rsqrt(fs * psd / 2).
+__global__ void filter_kernel(const float* __restrict__ psd, int n_psd, int n_bins, int ratio, float fs, float norm,
+                              int k_lo, int k_hi, float* __restrict__ filt) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const int d = blockIdx.y;
+    if (k >= n_bins) return;
+    float w = 0.f;
+    if (k >= k_lo && k <= k_hi) {
+        const float* s = psd + (size_t)d * n_psd;
+        float sv;
+        if (ratio == 1) {
+            sv = s[k];
+        } else {
+            int i0 = k / ratio;
+            if (i0 > n_psd - 2) i0 = n_psd - 2;
+            const float t = (float)(k - i0 * ratio) / (float)ratio;
+            sv = (1.0f - t) * s[i0] + t * s[i0 + 1];
+        }
+        w = rsqrtf(0.5f * fs * sv) * norm;
+    }
+    filt[(size_t)d * n_bins + k] = w;
+}
+
+int launch_filter(const amplfi_plan* p, const float* psd, int n_psd, double f_lo, double f_hi, cudaStream_t st) {
+    const int ratio = (p->n / 2) / (n_psd - 1);
+    long k_lo = (long)ceil(f_lo * p->t_seg);
+    while ((double)(k_lo - 1) / p->t_seg >= f_lo) --k_lo;
+    while ((double)k_lo / p->t_seg < f_lo) ++k_lo;
+    long k_hi = (long)floor(f_hi * p->t_seg);
+    while ((double)(k_hi + 1) / p->t_seg <= f_hi) ++k_hi;
+    while (k_hi >= 0 && (double)k_hi / p->t_seg > f_hi) --k_hi;
+    if (k_lo < 0) k_lo = 0;
+    if (k_hi > p->n_bins - 1) k_hi = p->n_bins - 1;
+    const float norm = (float)(1180591620717411303424.0 / (2.0 * (double)p->n));      // 2^70 / (2N)
+    dim3 grid((p->n_bins + 255) / 256, p->n_det);
+    filter_kernel<<<grid, 256, 0, st>>>(psd, n_psd, p->n_bins, ratio, (float)p->fs, norm, (int)k_lo, (int)k_hi, p->filt);
+    count_launch();
+    return check_launch("filter_kernel");
+}
+
+enum { MODE_NONE = 0, MODE_HDET = 1, MODE_FUSED = 2 };
+
+struct IwArgs {
+    const float* noise;       // dense [B, D, N] or strip [D, L]
+    const long* offsets;      // nullptr: dense
+    long strip_len;
+    const float2* h_det;      // MODE_HDET: [B, D, K]
+    const float2* h0;         // MODE_FUSED: [B, K] (2 fs h0)
+    const WfCoef* coef;
+    const DetResp* resp;
+    const float* filt;        // [D, K]
+    float* out;               // [B, D, N]
+    int n_det;
+    float two_fs;
+    float inv_tseg;
+};
+
+template <int LOGM, int MODE>
+__global__ void __launch_bounds__(Fft<LOGM>::T) inject_whiten_kernel(const IwArgs a) {
+    using F = Fft<LOGM>;
+    constexpr int M = F::M, N = 2 * M, K = M + 1, RA = F::RA, RC = F::RC, T = F::T, LB = F::LB;
+    extern __shared__ float2 sm[];
+    const int unit = blockIdx.x, tid = threadIdx.x;
+    const int b = unit / a.n_det, d = unit - b * a.n_det;
+
+    // ---- a-5 gather ----
+    const float* x;
+    float* out = a.out + (size_t)unit * N;
+    if (a.offsets != nullptr) {
+        const long off = a.offsets[unit];
+        if (off < 0 || off + N > a.strip_len) {            // never read out of bounds: poison the row instead
+            const float qnan = __int_as_float(0x7fc00000);
+            for (int i = tid; i < N; i += T) out[i] = qnan;
+            return;
+        }
+        x = a.noise + (size_t)d * a.strip_len + off;
+    } else {
+        x = a.noise + (size_t)unit * N;
+    }
+    const bool aligned8 = ((reinterpret_cast<size_t>(x) & 7) == 0);
+
+    // ---- a-6 forward real FFT (packed as M complex points) ----
+    {
+        float2 v[F::NA][RA];
+        if (aligned8) {
+            const float2* x2 = reinterpret_cast<const float2*>(x);
+#pragma unroll
+            for (int i = 0; i < F::NA; ++i)
+#pragma unroll
+                for (int nA = 0; nA < RA; ++nA) v[i][nA] = __ldcs(x2 + nA * LB + tid + i * T);
+        } else {
+#pragma unroll
+            for (int i = 0; i < F::NA; ++i)
+#pragma unroll
+                for (int nA = 0; nA < RA; ++nA) {
+                    const int m = nA * LB + tid + i * T;
+                    v[i][nA] = make_float2(__ldg(x + 2 * m), __ldg(x + 2 * m + 1));
+                }
+        }
+#pragma unroll
+        for (int i = 0; i < F::NA; ++i) F::pass_a_fwd(v[i], tid + i * T, sm);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < F::NB; ++i) F::pass_b_fwd(tid + i * T, sm);
+    __syncthreads();
+    int klow_a, klow_b;
+    pass_c_klow<LOGM>(tid, klow_a, klow_b);
+    float2 va[RC], vb[RC];
+    F::pass_c_fwd(klow_a, va, sm);
+    F::pass_c_fwd(klow_b, vb, sm);
+
+    // ---- a-7 inject, a-8 whiten + band-limit (registers) ----
+    const float* filt = a.filt + (size_t)d * K;
+    const float2* hsrc = nullptr;
+    int w_lo = 1, w_hi = 0;
+    float cre = 0.f, cim = 0.f, delta = 0.f;
+    if (MODE == MODE_HDET) hsrc = a.h_det + (size_t)unit * K;
+    if (MODE == MODE_FUSED) {
+        const WfCoef* c = a.coef + b;
+        hsrc = a.h0 + (size_t)b * K;
+        if (c->valid) { w_lo = c->k_lo; w_hi = c->k_hi; }
+        const DetResp r = a.resp[unit];
+        cre = (float)r.fp * c->pol_p;                       // C = F+ (1+cos^2 i)/2 - i Fx cos i
+        cim = -(float)r.fc * c->pol_c;
+        delta = (float)(r.dt * (double)a.inv_tseg);          // turns per bin
+    }
+    auto inject = [&](int k, float2& x2) {
+        if (MODE == MODE_HDET) {
+            const float2 h = __ldg(hsrc + k);
+            x2.x = fmaf(a.two_fs, h.x, x2.x);
+            x2.y = fmaf(a.two_fs, h.y, x2.y);
+        } else if (MODE == MODE_FUSED) {
+            if (k >= w_lo && k <= w_hi) {
+                const float2 h = __ldg(hsrc + k);
+                float turns = (float)k * delta;
+                turns -= rintf(turns);
+                float s, co;
+                __sincosf(turns * -6.283185307179586f, &s, &co);          // exp(-2 pi i k dt / T)
+                const float2 cp = make_float2(cre * co - cim * s, cre * s + cim * co);
+                x2.x += h.x * cp.x - h.y * cp.y;
+                x2.y += h.x * cp.y + h.y * cp.x;
+            }
+        }
+    };
+    for_each_bin_pair<LOGM>(
+        tid, va, vb,
+        [&](int k, float2& za, float2& zb) {
+            const float2 w = twiddle<N>(k);
+            float2 xa, xb;
+            split_pair(za, zb, w, xa, xb);
+            inject(k, xa);
+            inject(M - k, xb);
+            const float fa = __ldg(filt + k), fb = __ldg(filt + M - k);
+            xa.x *= fa; xa.y *= fa; xb.x *= fb; xb.y *= fb;
+            merge_pair(xa, xb, w, za, zb);
+        },
+        [&](int k, float2& z) {
+            const float2 w = twiddle<N>(k);
+            float2 xa, xb, z2;
+            split_pair(z, z, w, xa, xb);
+            inject(k, xa);
+            const float fa = __ldg(filt + k);
+            xa.x *= fa; xa.y *= fa;
+            merge_pair(xa, xa, w, z, z2);
+        },
+        [&](float2& z) {
+            float x0 = 2.0f * (z.x + z.y), xm = 2.0f * (z.x - z.y);       // 2 X[0], 2 X[M] (real)
+            if (MODE == MODE_HDET) {
+                x0 = fmaf(a.two_fs, __ldg(hsrc).x, x0);
+                xm = fmaf(a.two_fs, __ldg(hsrc + M).x, xm);
+            }
+            const float y0 = x0 * __ldg(filt), ym = xm * __ldg(filt + M);
+            z = make_float2(y0 + ym, y0 - ym);                            // 4 Z'[0]
+        });
+
+    // ---- a-9 inverse real FFT and store ----
+    F::pass_c_inv(klow_a, va, sm);
+    F::pass_c_inv(klow_b, vb, sm);
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < F::NB; ++i) F::pass_b_inv(tid + i * T, sm);
+    __syncthreads();
+    float2* out2 = reinterpret_cast<float2*>(out);
+#pragma unroll
+    for (int i = 0; i < F::NA; ++i) {
+        float2 v[RA];
+        F::pass_a_inv(v, tid + i * T, sm);
+#pragma unroll
+        for (int nA = 0; nA < RA; ++nA) __stcs(out2 + nA * LB + tid + i * T, v[nA]);
+    }
+}
+
+template <int LOGM, int MODE>
+static int launch_iw_t(const IwArgs& a, int units, cudaStream_t st) {
+    using F = Fft<LOGM>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(inject_whiten_kernel<LOGM, MODE>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F::SMEM_BYTES);
+        if (e != cudaSuccess) { set_error("cudaFuncSetAttribute: %s", cudaGetErrorString(e)); return AMPLFI_ERR_CUDA; }
+        attr_done = true;
+    }
+    inject_whiten_kernel<LOGM, MODE><<<units, F::T, F::SMEM_BYTES, st>>>(a);
+    count_launch();
+    return check_launch("inject_whiten_kernel");
+}
+
+template <int LOGM>
+static int launch_iw_mode(const IwArgs& a, int mode, int units, cudaStream_t st) {
+    switch (mode) {
+        case MODE_NONE: return launch_iw_t<LOGM, MODE_NONE>(a, units, st);
+        case MODE_HDET: return launch_iw_t<LOGM, MODE_HDET>(a, units, st);
+        default: return launch_iw_t<LOGM, MODE_FUSED>(a, units, st);
+    }
+}
+
+int launch_inject_whiten(const amplfi_plan* p, int batch, const float* noise, const long* offsets,
+                         long strip_len, const float* h_det, int fused, float* out, cudaStream_t st) {
+    IwArgs a;
+    a.noise = noise; a.offsets = offsets; a.strip_len = strip_len;
+    a.h_det = reinterpret_cast<const float2*>(h_det);
+    a.h0 = p->h0; a.coef = p->coef; a.resp = p->resp; a.filt = p->filt; a.out = out;
+    a.n_det = p->n_det; a.two_fs = (float)(2.0 * p->fs); a.inv_tseg = (float)(1.0 / p->t_seg);
+    const int mode = h_det != nullptr ? MODE_HDET : (fused ? MODE_FUSED : MODE_NONE);
+    const int units = batch * p->n_det;
+    switch (p->logm) {
+        case 9: return launch_iw_mode<9>(a, mode, units, st);
+        case 10: return launch_iw_mode<10>(a, mode, units, st);
+        case 11: return launch_iw_mode<11>(a, mode, units, st);
+        case 12: return launch_iw_mode<12>(a, mode, units, st);
+        case 13: return launch_iw_mode<13>(a, mode, units, st);
+        case 14: return launch_iw_mode<14>(a, mode, units, st);
+        default:
+            set_error("amplfi_inject_whiten: segment length %d not supported by this build", p->n);
+            return AMPLFI_ERR_UNSUPPORTED_SIZE;
+    }
+}
+
+}  // namespace amplfi

@@ -1,0 +1,143 @@
+// waveform.cu -- per-sample preparation, materialised waveform and projection kernels.
+// PAPER.md:87, :104 (waveform on the GPU), PAPER.md:190 (antenna response on the fly).
+#include "amplfi_internal.h"
+#include "waveform.cuh"
+
+namespace amplfi {
+
+// ---- plan tables: k^(-1/3) and ln k in fp64 ----
+__global__ void tables_kernel(double* __restrict__ ci, double* __restrict__ lnk, int n_bins) {
+    int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_bins) return;
+    if (k == 0) { ci[0] = 0.0; lnk[0] = 0.0; return; }
+    const double kd = (double)k;
+    ci[k] = 1.0 / cbrt(kd);
+    lnk[k] = log(kd);
+}
+
+int launch_tables(amplfi_plan* p, cudaStream_t st) {
+    tables_kernel<<<(p->n_bins + 255) / 256, 256, 0, st>>>(p->tab_ci, p->tab_lnk, p->n_bins);
+    count_launch();
+    return check_launch("tables_kernel");
+}
+
+// ---- one thread per sample: waveform coefficients + detector responses (fp64) ----
+__global__ void prepare_kernel(const double* __restrict__ params, int batch, int approx, double t_seg, int n_bins,
+                               double f_lo, double f_hi, double amp_mul, double gmst,
+                               const double* __restrict__ pd_table, const int* __restrict__ det_ids, int n_det,
+                               WfCoef* __restrict__ coef, DetResp* __restrict__ resp, int* __restrict__ flags) {
+    int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= batch) return;
+    const double* p = params + (size_t)b * AMPLFI_N_PARAMS;
+    if (coef != nullptr) {
+        WfCoef c;
+        prepare_sample(p, approx, t_seg, n_bins, f_lo, f_hi, amp_mul, pd_table, c);
+        coef[b] = c;
+        if (flags != nullptr) flags[b] = c.valid ? 0 : 1;
+    }
+    for (int d = 0; d < n_det; ++d) resp[(size_t)b * n_det + d] = detector_response(p[8], p[9], p[10], gmst, det_ids[d]);
+}
+
+int launch_prepare(const amplfi_plan* p, int approximant, int batch, const double* params, double gmst,
+                   double f_lo, double f_hi, double amp_mul, int* flags, cudaStream_t st) {
+    const int threads = 64;
+    prepare_kernel<<<(batch + threads - 1) / threads, threads, 0, st>>>(
+        params, batch, approximant, p->t_seg, p->n_bins, f_lo, f_hi, amp_mul, gmst, p->pd_table, p->d_det_ids,
+        p->n_det, approximant < 0 ? nullptr : p->coef, p->resp, flags);
+    count_launch();
+    return check_launch("prepare_kernel");
+}
+
+// ---- materialised polarisations: hp = (1+cos^2 i)/2 h0, hc = -i cos i h0 ----
+template <bool POL>
+__global__ void __launch_bounds__(256) waveform_kernel(const WfCoef* __restrict__ coef, const double* __restrict__ tab_ci,
+                                                       const double* __restrict__ tab_lnk, int n_bins,
+                                                       float2* __restrict__ out_a, float2* __restrict__ out_b) {
+    const int b = blockIdx.y;
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    __shared__ WfCoef c;
+    // every thread reads the same struct; stage it once per CTA
+    {
+        const int* src = reinterpret_cast<const int*>(coef + b);
+        int* dst = reinterpret_cast<int*>(&c);
+        for (int i = threadIdx.x; i < (int)(sizeof(WfCoef) / sizeof(int)); i += blockDim.x) dst[i] = src[i];
+    }
+    __syncthreads();
+    if (k >= n_bins) return;
+    float2 h = make_float2(0.f, 0.f);
+    if (c.valid && k >= c.k_lo && k <= c.k_hi) h = eval_h0(c, k, tab_ci[k], tab_lnk[k]);
+    const size_t idx = (size_t)b * n_bins + k;
+    if (POL) {
+        out_a[idx] = make_float2(c.pol_p * h.x, c.pol_p * h.y);
+        out_b[idx] = make_float2(c.pol_c * h.y, -c.pol_c * h.x);     // -i c (x + i y) = c y - i c x
+    } else {
+        out_a[idx] = h;
+    }
+}
+
+int launch_waveform_pol(const amplfi_plan* p, int batch, float* hp, float* hc, cudaStream_t st) {
+    dim3 grid((p->n_bins + 255) / 256, batch);
+    waveform_kernel<true><<<grid, 256, 0, st>>>(p->coef, p->tab_ci, p->tab_lnk, p->n_bins,
+                                                reinterpret_cast<float2*>(hp), reinterpret_cast<float2*>(hc));
+    count_launch();
+    return check_launch("waveform_kernel<pol>");
+}
+
+int launch_waveform_h0(const amplfi_plan* p, int batch, cudaStream_t st) {
+    dim3 grid((p->n_bins + 255) / 256, batch);
+    waveform_kernel<false><<<grid, 256, 0, st>>>(p->coef, p->tab_ci, p->tab_lnk, p->n_bins, p->h0, nullptr);
+    count_launch();
+    return check_launch("waveform_kernel<h0>");
+}
+
+// ---- projection: h_d = (F+ h+ + Fx hx) exp(-2 pi i f_k dt_d) ----
+__global__ void __launch_bounds__(256) project_kernel(const DetResp* __restrict__ resp, int n_det, int n_bins,
+                                                      double inv_tseg, const float2* __restrict__ hp,
+                                                      const float2* __restrict__ hc, float2* __restrict__ h_det) {
+    const int b = blockIdx.y;
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_bins) return;
+    const float2 p = hp[(size_t)b * n_bins + k];
+    const float2 c = hc[(size_t)b * n_bins + k];
+    for (int d = 0; d < n_det; ++d) {
+        const DetResp r = resp[(size_t)b * n_det + d];
+        const float fp = (float)r.fp, fc = (float)r.fc;
+        const float2 h = make_float2(fp * p.x + fc * c.x, fp * p.y + fc * c.y);
+        double turns = (double)k * (r.dt * inv_tseg);
+        turns -= rint(turns);
+        float s, co;
+        sincospif(2.0f * (float)turns, &s, &co);
+        // h * (cos - i sin)
+        h_det[((size_t)b * n_det + d) * n_bins + k] = make_float2(h.x * co + h.y * s, h.y * co - h.x * s);
+    }
+}
+
+__global__ void copy_resp_kernel(const DetResp* __restrict__ resp, double* __restrict__ out, int count) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    out[3 * i + 0] = resp[i].fp;
+    out[3 * i + 1] = resp[i].fc;
+    out[3 * i + 2] = resp[i].dt;
+}
+
+int launch_project(const amplfi_plan* p, int batch, const float* hp, const float* hc, float* h_det,
+                   double* resp_out, cudaStream_t st) {
+    if (h_det != nullptr) {
+        dim3 grid((p->n_bins + 255) / 256, batch);
+        project_kernel<<<grid, 256, 0, st>>>(p->resp, p->n_det, p->n_bins, 1.0 / p->t_seg,
+                                             reinterpret_cast<const float2*>(hp), reinterpret_cast<const float2*>(hc),
+                                             reinterpret_cast<float2*>(h_det));
+        count_launch();
+        int rc = check_launch("project_kernel");
+        if (rc) return rc;
+    }
+    if (resp_out != nullptr) {
+        const int count = batch * p->n_det;
+        copy_resp_kernel<<<(count + 127) / 128, 128, 0, st>>>(p->resp, resp_out, count);
+        count_launch();
+        return check_launch("copy_resp_kernel");
+    }
+    return AMPLFI_OK;
+}
+
+}  // namespace amplfi

@@ -1,0 +1,371 @@
+// waveform.cuh -- per-sample waveform coefficients and the per-bin evaluator (device code).
+//
+// PAPER.md:87 (IMRPhenomD [32], inspiral = TaylorF2 3.5PN [33]) and PAPER.md:104 (waveforms are generated
+// on the GPU).  The evaluation is split in two so that the hot loop is a handful of FMAs per bin:
+//   1. prepare_sample(): one thread per sample, fp64.  Turns the 11 physical parameters into
+//      coefficients of fixed powers of the BIN INDEX k (f_k = k/T): on a regular grid
+//      (pi M f)^(p/3) = const * k^(p/3), so every PN / phenomenological term is
+//      (per-sample constant) x (per-bin table value).
+//   2. eval_h0(): per bin, phase in fp64 "turns" from k^(-1/3) and ln k (plan tables), reduced
+//      modulo 1, then one fast sincos; amplitude in fp32.
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+
+namespace amplfi {
+
+struct WfCoef {
+    int valid, approx, k_lo, k_hi;           // k_lo > k_hi: empty band
+    double kp1, kp2;                         // phase region boundaries in bins
+    // region 1 (inspiral) phase / 2pi
+    double lin1, c01, a_m5, a_m3, a_m2, a_m1, a_ln, a_p1, a_p1ln, a_p2, s_p4, s_p5, s_p6;
+    // region 2 (intermediate)
+    double lin2, c02, b_ln, b_m9;
+    // region 3 (merger-ringdown)
+    double lin3, c03, r_m3, r_34;
+    float r_at, at_k0, at_invw;
+    // amplitude
+    float amp_scale, ka1, ka2;
+    float e[8];                              // inspiral bracket: 1 + sum_{i=2..9} e[i-2] (k^(1/3))^i
+    float q[5], q_mid, q_invh;               // intermediate quartic in u = (k - q_mid) * q_invh
+    float g0, g_krd, g_invw, g2;             // ringdown: g0 exp(-g2 y)/(1 + y^2), y = (k - g_krd) g_invw
+    float pol_p, pol_c;                      // (1 + cos^2 iota)/2, cos iota
+};
+
+struct DetResp { double fp, fc, dt; };
+
+struct DetGeom { double r[3], x[3], y[3]; };
+
+// Site constants (Earth-fixed, metres / unit vectors) for H1, L1, V1 (PAPER.md:13, :103 name the sites).
+__device__ __constant__ DetGeom kDet[3] = {
+    {{-2.16141492636e6, -3.83469517889e6, 4.60035022664e6},
+     {-0.22389266154, 0.79983062746, 0.55690487831},
+     {-0.91397818574, 0.02609403989, -0.40492342125}},
+    {{-7.42760447238e4, -5.49628371971e6, 3.22425701744e6},
+     {-0.95457412153, -0.14158077340, -0.26218911324},
+     {0.29774156894, -0.48791033647, -0.82054461286}},
+    {{4.54637409900e6, 8.42989697626e5, 4.37857696241e6},
+     {-0.70045821479, 0.20848948619, 0.68256166277},
+     {-0.05379255368, -0.96908180549, 0.24080451708}}};
+
+#define AMPLFI_C_SI 299792458.0
+#define AMPLFI_MTSUN 4.925490947641267e-06
+#define AMPLFI_MPC 3.085677581491367e22
+#define AMPLFI_GAMMA_E 0.5772156649015329
+#define AMPLFI_PI 3.141592653589793238
+
+// antenna patterns and geocentric delay of detector `det`
+__device__ inline DetResp detector_response(double ra, double dec, double psi, double gmst, int det) {
+    const DetGeom& g = kDet[det];
+    double sg, cg, sd, cd, sp, cp;
+    sincos(gmst - ra, &sg, &cg);
+    sincos(dec, &sd, &cd);
+    sincos(psi, &sp, &cp);
+    const double X[3] = {-cp * sg - sp * cg * sd, -cp * cg + sp * sg * sd, sp * cd};
+    const double Y[3] = {sp * sg - cp * cg * sd, sp * cg + cp * sg * sd, cp * cd};
+    const double n[3] = {cd * cg, -cd * sg, sd};
+    // D = (x x^T - y y^T)/2 contracted with X, Y via the projections on the arms
+    const double xX = g.x[0] * X[0] + g.x[1] * X[1] + g.x[2] * X[2];
+    const double xY = g.x[0] * Y[0] + g.x[1] * Y[1] + g.x[2] * Y[2];
+    const double yX = g.y[0] * X[0] + g.y[1] * X[1] + g.y[2] * X[2];
+    const double yY = g.y[0] * Y[0] + g.y[1] * Y[1] + g.y[2] * Y[2];
+    DetResp r;
+    r.fp = 0.5 * ((xX * xX - yX * yX) - (xY * xY - yY * yY));
+    r.fc = xX * xY - yX * yY;
+    r.dt = -(g.r[0] * n[0] + g.r[1] * n[1] + g.r[2] * n[2]) / AMPLFI_C_SI;
+    return r;
+}
+
+__device__ inline double pd_fit(const double* t, double eta, double xi) {
+    const double e2 = eta * eta;
+    return t[0] + t[1] * eta + xi * ((t[2] + t[3] * eta + t[4] * e2)
+           + xi * ((t[5] + t[6] * eta + t[7] * e2) + xi * (t[8] + t[9] * eta + t[10] * e2)));
+}
+
+// p: 11 parameters; t_seg = n/fs; amp_mul multiplies the strain amplitude (1 for the API in strain/Hz).
+// tab: [19][11] fit table in global/constant memory.
+__device__ inline void prepare_sample(const double* p, int approx, double t_seg, int n_bins, double f_lo,
+                                      double f_hi, double amp_mul, const double* tab, WfCoef& c) {
+    const double PI = AMPLFI_PI, TWO_PI = 2.0 * AMPLFI_PI;
+    const double mc = p[0], q = p[1], chi1 = p[2], chi2 = p[3], dist = p[4];
+    bool ok = (mc > 0.0) && (q > 0.0) && (q <= 1.0) && (fabs(chi1) < 1.0) && (fabs(chi2) < 1.0) && (dist > 0.0);
+    for (int i = 0; i < 11; ++i) ok = ok && isfinite(p[i]);
+    c.valid = ok ? 1 : 0;
+    c.approx = approx;
+    c.k_lo = 1;
+    c.k_hi = 0;
+    if (!ok) return;
+    const double eta = q / ((1.0 + q) * (1.0 + q));
+    const double mtot = mc * pow(eta, -0.6);
+    const double ms = mtot * AMPLFI_MTSUN;           // seconds
+    const double mu = ms / t_seg;                    // Mf = mu * k
+    const double v1 = cbrt(PI * mu);                 // v = v1 * k^(1/3)
+    const double lnv1 = log(v1);
+    const double cosi = cos(p[5]);
+    c.pol_p = (float)(0.5 * (1.0 + cosi * cosi));
+    c.pol_c = (float)cosi;
+
+    // ---- band (DESIGN.md R-W7): f_lo <= k/T <= f_top, 1 <= k <= n_bins-2 ----
+    const double f_top = fmin(approx == 0 ? 1.0 / (14.696938456699069 * PI * ms) : 0.2 / ms, f_hi);   // 6^(3/2)
+    long klo = (long)ceil(f_lo * t_seg);
+    while ((double)(klo - 1) / t_seg >= f_lo) --klo;
+    while ((double)klo / t_seg < f_lo) ++klo;
+    long khi = (long)floor(f_top * t_seg);
+    while ((double)(khi + 1) / t_seg <= f_top) ++khi;
+    while (khi >= 0 && (double)khi / t_seg > f_top) --khi;
+    if (klo < 1) klo = 1;
+    if (khi > n_bins - 2) khi = n_bins - 2;
+    c.k_lo = (int)klo;
+    c.k_hi = (int)khi;
+
+    // ---- TaylorF2 phasing series (aligned spins for IMRPhenomD, none for TaylorF2) ----
+    const double s1 = (approx == 0) ? 0.0 : chi1, s2 = (approx == 0) ? 0.0 : chi2;
+    const double seta = sqrt(fmax(1.0 - 4.0 * eta, 0.0));
+    const double m1 = 0.5 * (1.0 + seta), m2 = 0.5 * (1.0 - seta);
+    const double SL = m1 * m1 * s1 + m2 * m2 * s2;
+    const double dSL = (m1 - m2) * (m2 * s2 - m1 * s1);
+    const double e2 = eta * eta, e3 = e2 * eta;
+    double pv2 = 5.0 * (743.0 / 84.0 + 11.0 * eta) / 9.0;
+    double pv3 = -16.0 * PI + 188.0 * SL / 3.0 + 25.0 * dSL;
+    const double sig = eta * (721.0 / 48.0 - 247.0 / 48.0) * s1 * s2
+                       + (719.0 / 96.0 - 233.0 / 96.0) * (m1 * m1 * s1 * s1 + m2 * m2 * s2 * s2);
+    double pv4 = 5.0 * (3058.673 / 7.056 + 5429.0 / 7.0 * eta + 617.0 * e2) / 72.0 - 10.0 * sig;
+    const double gam = (554345.0 / 1134.0 + 110.0 * eta / 9.0) * SL + (13915.0 / 84.0 - 10.0 * eta / 3.0) * dSL;
+    double pv5 = 5.0 / 9.0 * (7729.0 / 84.0 - 13.0 * eta) * PI - gam;
+    double pl5 = 5.0 / 3.0 * (7729.0 / 84.0 - 13.0 * eta) * PI - 3.0 * gam;
+    double pv6 = 11583.231236531 / 4.694215680 - 640.0 / 3.0 * PI * PI - 6848.0 / 21.0 * AMPLFI_GAMMA_E
+                 + eta * (-15737.765635 / 3.048192 + 2255.0 / 12.0 * PI * PI) + e2 * 76055.0 / 1728.0
+                 - e3 * 127825.0 / 1296.0 - 6848.0 / 21.0 * log(4.0)
+                 + PI * (3760.0 * SL + 1490.0 * dSL) / 3.0;
+    double pl6 = -6848.0 / 21.0;
+    double pv7 = PI * (77096675.0 / 254016.0 + 378515.0 / 1512.0 * eta - 74045.0 / 756.0 * e2)
+                 + (-8980424995.0 / 762048.0 + 6586595.0 * eta / 756.0 - 305.0 * e2 / 36.0) * SL
+                 - (170978035.0 / 48384.0 - 2876425.0 * eta / 672.0 - 4735.0 * e2 / 144.0) * dSL;
+    const double pfa = 3.0 / (128.0 * eta) / TWO_PI;          // everything below is in turns
+    const double iv = 1.0 / v1;
+    c.a_m5 = pfa * iv * iv * iv * iv * iv;
+    c.a_m3 = pfa * pv2 * iv * iv * iv;
+    c.a_m2 = pfa * pv3 * iv * iv;
+    c.a_m1 = pfa * pv4 * iv;
+    c.a_ln = pfa * pl5 / 3.0;
+    c.a_p1 = pfa * (pv6 + pl6 * lnv1) * v1;
+    c.a_p1ln = pfa * pl6 / 3.0 * v1;
+    c.a_p2 = pfa * pv7 * v1 * v1;
+    const double tc_turns = p[7] / t_seg;                     // 2 pi f t_c / 2 pi = k t_c / T
+    const double phic_turns = -2.0 * p[6] / TWO_PI;
+    double const1 = pfa * (pv5 + pl5 * lnv1) - 0.125 + phic_turns;      // -pi/4 -> -1/8 turn
+
+    if (approx == 0) {
+        c.kp1 = 1e300; c.kp2 = 1e300;
+        c.lin1 = tc_turns; c.c01 = const1;
+        c.s_p4 = c.s_p5 = c.s_p6 = 0.0;
+        c.lin2 = c.c02 = c.b_ln = c.b_m9 = 0.0;
+        c.lin3 = c.c03 = c.r_m3 = c.r_34 = 0.0;
+        c.r_at = 0.f; c.at_k0 = 0.f; c.at_invw = 0.f;
+        // A0 f^(-7/6), A0 = sqrt(5/24) pi^(-2/3) (G Mc/c^3)^(5/6) c / D
+        const double a0 = sqrt(5.0 / 24.0) * pow(PI, -2.0 / 3.0) * pow(mc * AMPLFI_MTSUN, 5.0 / 6.0)
+                          * AMPLFI_C_SI / (dist * AMPLFI_MPC);
+        c.amp_scale = (float)(a0 * pow(t_seg, 7.0 / 6.0) * amp_mul);
+        c.ka1 = 3.0e38f; c.ka2 = 3.0e38f;
+        for (int i = 0; i < 8; ++i) c.e[i] = 0.f;
+        for (int i = 0; i < 5; ++i) c.q[i] = 0.f;
+        c.q_mid = 0.f; c.q_invh = 0.f; c.g0 = 0.f; c.g_krd = 0.f; c.g_invw = 0.f; c.g2 = 0.f;
+        return;
+    }
+
+    // ---- IMRPhenomD ----
+    const double xi = (m1 * chi1 + m2 * chi2 - 38.0 * eta / 113.0 * (chi1 + chi2)) - 1.0;
+    double fit[AMPLFI_PD_ROWS];
+    for (int r = 0; r < AMPLFI_PD_ROWS; ++r) fit[r] = pd_fit(tab + r * AMPLFI_PD_COLS, eta, xi);
+    // remnant: final spin, radiated energy, ringdown / damping frequency (Kerr 220 closed-form fit)
+    const double stot = m1 * m1 * chi1 + m2 * m2 * chi2;
+    const double e4 = e2 * e2;
+    double af = 3.4641016151377544 * eta - 4.399247300629289 * e2 + 9.397292189321194 * e3 - 13.180949901606242 * e4
+                + (1.0 - 0.0850917821418767 * eta - 5.837029316602263 * e2) * stot
+                + (0.1014665242971878 * eta - 2.0967746996832157 * e2) * stot * stot
+                + (-1.3546806617824356 * eta + 4.108962025369336 * e2) * stot * stot * stot
+                + (-0.8676969352555539 * eta + 2.064046835273906 * e2) * stot * stot * stot * stot;
+    af = fmin(fmax(af, -0.999999), 0.999999);
+    const double sn = stot / (m1 * m1 + m2 * m2);
+    const double erad = (eta * (0.055974469826360077 + 0.5809510763115132 * eta - 0.9606726679372312 * e2
+                                + 3.352411249771192 * e3)
+                         * (1.0 + (-0.0030302335878845507 - 2.0066110851351073 * eta + 7.7050567802399215 * e2) * sn))
+                        / (1.0 + (-0.6714403054720589 - 1.4756929437702908 * eta + 7.304676214885011 * e2) * sn);
+    const double fring0 = (1.5251 - 1.1568 * pow(1.0 - af, 0.1292)) / TWO_PI;
+    const double qual = 0.7 + 1.4187 * pow(1.0 - af, -0.4990);
+    const double f_rd = fring0 / (1.0 - erad);
+    const double f_dm = fring0 / (2.0 * qual) / (1.0 - erad);
+
+    const double sg1 = fit[PD_SIGMA1], sg2 = fit[PD_SIGMA2], sg3 = fit[PD_SIGMA3], sg4 = fit[PD_SIGMA4];
+    const double be1 = fit[PD_BETA1], be2 = fit[PD_BETA2], be3 = fit[PD_BETA3];
+    const double al1 = fit[PD_ALPHA1], al2 = fit[PD_ALPHA2], al3 = fit[PD_ALPHA3], al4 = fit[PD_ALPHA4],
+                 al5 = fit[PD_ALPHA5];
+    // phases in radians as functions of Mf (value, derivative) at the two junctions
+    const double pn[8] = {1.0, 0.0, pv2, pv3, pv4, pv5, pv6, pv7};
+    const double pl[8] = {0.0, 0.0, 0.0, 0.0, 0.0, pl5, pl6, 0.0};
+    const double pfar = 3.0 / (128.0 * eta);
+    const double f1 = 0.018, f2 = 0.5 * f_rd;
+    double phi_ins, dphi_ins;
+    {
+        const double v = cbrt(PI * f1), lv = log(v);
+        double s = 0.0, ds = 0.0, vp = 1.0 / (v * v * v * v * v * v);      // v^(i-6)
+        for (int i = 0; i < 8; ++i) {
+            s += (pn[i] + pl[i] * lv) * vp * v;                            // v^(i-5)
+            ds += ((i - 5) * (pn[i] + pl[i] * lv) + pl[i]) * vp;
+            vp *= v;
+        }
+        const double c13 = cbrt(f1);
+        phi_ins = pfar * s - PI / 4.0
+                  + (sg1 * f1 + 0.75 * sg2 * f1 * c13 + 0.6 * sg3 * f1 * c13 * c13 + 0.5 * sg4 * f1 * f1) / eta;
+        dphi_ins = pfar * ds * v / (3.0 * f1) + (sg1 + sg2 * c13 + sg3 * c13 * c13 + sg4 * f1) / eta;
+    }
+    const double int1 = (be1 * f1 + be2 * log(f1) - be3 / (3.0 * f1 * f1 * f1)) / eta;
+    const double dint1 = (be1 + be2 / f1 + be3 / (f1 * f1 * f1 * f1)) / eta;
+    const double c2int = dphi_ins - dint1;
+    const double c1int = phi_ins - int1 - c2int * f1;
+    const double int2 = (be1 * f2 + be2 * log(f2) - be3 / (3.0 * f2 * f2 * f2)) / eta + c1int + c2int * f2;
+    const double dint2 = (be1 + be2 / f2 + be3 / (f2 * f2 * f2 * f2)) / eta + c2int;
+    const double x2 = (f2 - al5 * f_rd) / f_dm;
+    const double mr2 = (al1 * f2 - al2 / f2 + 4.0 / 3.0 * al3 * pow(f2, 0.75) + al4 * atan(x2)) / eta;
+    const double dmr2 = (al1 + al2 / (f2 * f2) + al3 * pow(f2, -0.25) + al4 / (f_dm * (1.0 + x2 * x2))) / eta;
+    const double c2mr = dint2 - dmr2;
+    const double c1mr = int2 - mr2 - c2mr * f2;
+    // amplitude peak and time alignment
+    const double g1 = fit[PD_GAMMA1], g2 = fit[PD_GAMMA2], g3 = fit[PD_GAMMA3];
+    const double f_peak = (g2 > 1.0) ? fabs(f_rd - f_dm * g3 / g2)
+                                     : fabs(f_rd + f_dm * (sqrt(1.0 - g2 * g2) - 1.0) * g3 / g2);
+    const double xp = (f_peak - al5 * f_rd) / f_dm;
+    const double t0 = (al1 + al2 / (f_peak * f_peak) + al3 * pow(f_peak, -0.25) + al4 / (f_dm * (1.0 + xp * xp))) / eta
+                      + c2mr;
+
+    c.kp1 = f1 / mu;
+    c.kp2 = f2 / mu;
+    const double mu13 = cbrt(mu);
+    c.lin1 = tc_turns + (sg1 / eta - t0) * mu / TWO_PI;
+    c.c01 = const1;
+    c.s_p4 = 0.75 * sg2 / eta * mu * mu13 / TWO_PI;
+    c.s_p5 = 0.6 * sg3 / eta * mu * mu13 * mu13 / TWO_PI;
+    c.s_p6 = 0.5 * sg4 / eta * mu * mu / TWO_PI;
+    c.lin2 = tc_turns + (be1 / eta + c2int - t0) * mu / TWO_PI;
+    c.c02 = (c1int + be2 / eta * log(mu)) / TWO_PI + phic_turns;
+    c.b_ln = be2 / eta / TWO_PI;
+    c.b_m9 = -be3 / (3.0 * eta * mu * mu * mu) / TWO_PI;
+    c.lin3 = tc_turns + (al1 / eta + c2mr - t0) * mu / TWO_PI;
+    c.c03 = c1mr / TWO_PI + phic_turns;
+    c.r_m3 = -al2 / (eta * mu) / TWO_PI;
+    c.r_34 = 4.0 / 3.0 * al3 / eta * pow(mu, 0.75) / TWO_PI;
+    c.r_at = (float)(al4 / eta / TWO_PI);
+    c.at_k0 = (float)(al5 * f_rd / mu);
+    c.at_invw = (float)(mu / f_dm);
+
+    // ---- amplitude ----
+    const double amp0 = 2.0 * sqrt(5.0 / (64.0 * PI)) * mtot * mtot * AMPLFI_MTSUN * (AMPLFI_MTSUN * AMPLFI_C_SI)
+                        / (dist * AMPLFI_MPC);
+    c.amp_scale = (float)(amp0 * sqrt(2.0 * eta / 3.0) * pow(PI, -1.0 / 6.0) * pow(mu, -7.0 / 6.0) * amp_mul);
+    const double c12 = chi1 * chi1, c22 = chi2 * chi2;
+    double A[7];
+    A[2] = (-969.0 + 1804.0 * eta) / 672.0;
+    A[3] = (chi1 * (81.0 * (1.0 + seta) - 44.0 * eta) + chi2 * (81.0 - 81.0 * seta - 44.0 * eta)) / 48.0;
+    A[4] = (-27312085.0 - 10287648.0 * c22 - 10287648.0 * c12 * (1.0 + seta) + 10287648.0 * c22 * seta
+            + 24.0 * (-1975055.0 + 857304.0 * c12 - 994896.0 * chi1 * chi2 + 857304.0 * c22) * eta
+            + 35371056.0 * e2) / 8128512.0;
+    A[5] = (chi2 * (-285197.0 * (-1.0 + seta) + 4.0 * (-91902.0 + 1579.0 * seta) * eta - 35632.0 * e2)
+            + chi1 * (285197.0 * (1.0 + seta) - 4.0 * (91902.0 + 1579.0 * seta) * eta - 35632.0 * e2)
+            + 42840.0 * (-1.0 + 4.0 * eta) * PI) / 32256.0;
+    A[6] = -(-336.0 * (-3248849057.0 + 2943675504.0 * c12 - 3339284256.0 * chi1 * chi2 + 2943675504.0 * c22) * e2
+             - 324322727232.0 * e3
+             - 7.0 * (-177520268561.0 + 107414046432.0 * c22 + 107414046432.0 * c12 * (1.0 + seta)
+                      - 107414046432.0 * c22 * seta + 11087290368.0 * (chi1 + chi2 + chi1 * seta - chi2 * seta) * PI)
+             + 12.0 * eta * (-545384828789.0 - 176491177632.0 * chi1 * chi2 + 202603761360.0 * c22
+                             + 77616.0 * c12 * (2610335.0 + 995766.0 * seta) - 77287373856.0 * c22 * seta
+                             + 5841690624.0 * (chi1 + chi2) * PI + 21384760320.0 * PI * PI)) / 60085960704.0;
+    const double rho1 = fit[PD_RHO1], rho2 = fit[PD_RHO2], rho3 = fit[PD_RHO3];
+    {
+        double vp = v1 * v1;
+        for (int i = 2; i <= 6; ++i) { c.e[i - 2] = (float)(A[i] * vp); vp *= v1; }
+        c.e[5] = (float)(rho1 * mu * mu * mu13);                // Mf^(7/3) = mu^(7/3) k^(7/3)
+        c.e[6] = (float)(rho2 * mu * mu * mu13 * mu13);
+        c.e[7] = (float)(rho3 * mu * mu * mu);
+    }
+    // inspiral bracket and slope at Mf = 0.014; ringdown ansatz value and slope at f_peak
+    const double fa = 0.014, fc = f_peak;
+    double va, da;
+    {
+        const double x = cbrt(PI * fa), dx = x / (3.0 * fa), c13 = cbrt(fa);
+        va = 1.0 + x * x * (A[2] + x * (A[3] + x * (A[4] + x * (A[5] + x * A[6]))))
+             + fa * fa * c13 * (rho1 + c13 * (rho2 + c13 * rho3));
+        da = (2.0 * A[2] * x + 3.0 * A[3] * x * x + 4.0 * A[4] * x * x * x + 5.0 * A[5] * x * x * x * x
+              + 6.0 * A[6] * x * x * x * x * x) * dx
+             + 7.0 / 3.0 * rho1 * fa * c13 + 8.0 / 3.0 * rho2 * fa * c13 * c13 + 3.0 * rho3 * fa * fa;
+    }
+    const double w = f_dm * g3;
+    double vc, dc;
+    {
+        const double d = fc - f_rd;
+        const double lor = w * g1 / (d * d + w * w);
+        const double ex = exp(-d * g2 / w);
+        vc = ex * lor;
+        dc = ex * lor * (-g2 / w - 2.0 * d / (d * d + w * w));
+    }
+    // quartic through (fa: value, slope), (midpoint: v2), (fc: value, slope) in u = (f - fm)/h in [-1, 1]
+    const double h = 0.5 * (fc - fa), fm = 0.5 * (fc + fa), vm = fit[PD_V2];
+    const double S = 0.5 * (vc + va) - vm, Aodd = 0.5 * (vc - va);
+    const double Dp = 0.5 * (dc + da) * h, Dm = 0.5 * (dc - da) * h;
+    const double q3 = 0.5 * (Dp - Aodd), q1 = Aodd - q3, q4 = 0.5 * (Dm - 2.0 * S), q2 = S - q4;
+    c.q[0] = (float)vm; c.q[1] = (float)q1; c.q[2] = (float)q2; c.q[3] = (float)q3; c.q[4] = (float)q4;
+    c.q_mid = (float)(fm / mu);
+    c.q_invh = (float)(mu / h);
+    c.ka1 = (float)(fa / mu);
+    c.ka2 = (float)(fc / mu);
+    c.g0 = (float)(g1 / w);
+    c.g_krd = (float)(f_rd / mu);
+    c.g_invw = (float)(mu / w);
+    c.g2 = (float)g2;
+}
+
+// h0 at bin k (k_lo <= k <= k_hi assumed).  ci = k^(-1/3), lnk = ln k (fp64 tables of the plan).
+__device__ __forceinline__ float2 eval_h0(const WfCoef& c, int k, double ci, double lnk) {
+    const double kd = (double)k;
+    const double ci2 = ci * ci;
+    const double c1 = kd * ci2;                       // k^(1/3)
+    double ph;
+    if (kd < c.kp1) {
+        ph = fma(c.lin1, kd, c.c01);
+        ph = fma(c.a_ln, lnk, ph);
+        ph = fma(ci, fma(ci, fma(ci, fma(ci2, c.a_m5, c.a_m3), c.a_m2), c.a_m1), ph);
+        ph = fma(c1, fma(c1, c.a_p2, fma(c.a_p1ln, lnk, c.a_p1)), ph);
+        if (c.approx != 0) ph = fma(kd * c1, fma(c1, fma(c1, c.s_p6, c.s_p5), c.s_p4), ph);
+    } else if (kd < c.kp2) {
+        const double ci3 = ci2 * ci;
+        ph = fma(c.lin2, kd, c.c02);
+        ph = fma(c.b_ln, lnk, ph);
+        ph = fma(c.b_m9, ci3 * ci3 * ci3, ph);
+    } else {
+        const double q4 = sqrt(sqrt(kd));             // k^(1/4)
+        ph = fma(c.lin3, kd, c.c03);
+        ph = fma(c.r_m3, ci2 * ci, ph);
+        ph = fma(c.r_34, q4 * q4 * q4, ph);
+        ph += (double)(c.r_at * atanf(((float)k - c.at_k0) * c.at_invw));
+    }
+    ph -= rint(ph);                                   // turns in [-1/2, 1/2]
+    float s, co;
+    __sincosf((float)ph * 6.283185307179586f, &s, &co);
+
+    const float kf = (float)k, cf = (float)ci, c1f = (float)c1;
+    float amp = c.amp_scale * cf * cf * cf * sqrtf(cf);          // k^(-7/6)
+    if (kf < c.ka1) {
+        float br = c.e[7];
+#pragma unroll
+        for (int i = 6; i >= 0; --i) br = fmaf(br, c1f, c.e[i]);
+        amp *= fmaf(br, c1f * c1f, 1.0f);
+    } else if (kf < c.ka2) {
+        const float u = (kf - c.q_mid) * c.q_invh;
+        amp *= fmaf(u, fmaf(u, fmaf(u, fmaf(u, c.q[4], c.q[3]), c.q[2]), c.q[1]), c.q[0]);
+    } else {
+        const float y = (kf - c.g_krd) * c.g_invw;
+        amp *= c.g0 * __expf(-c.g2 * y) / fmaf(y, y, 1.0f);
+    }
+    return make_float2(amp * co, -amp * s);           // A exp(-i Psi)
+}
+
+}  // namespace amplfi

@@ -1,0 +1,150 @@
+// welch.cu -- segmented Welch PSD: detrend, Hann window, real FFT, |X|^2 in one pass per segment, then
+// a fixed-order mean over segments (deterministic; no atomics).
+// PAPER.md:101 "power spectra estimation ... carried out on the GPU"; "The power spectra is
+// fit to this background chunk".  Estimator parameters: BASELINE.json configs (Hann, 50 % overlap, mean).
+#include "amplfi_internal.h"
+#include "fft_core.cuh"
+
+namespace amplfi {
+
+constexpr float kStrainScale = 1180591620717411303424.0f;   // 2^70: strain -> O(1); |X|^2 then carries 2^140
+
+// One CTA per (detector, segment).  part[d][seg][k] = |FFT(w (x - mean))[k]|^2 (scaled by 2^140).
+template <int LOGM>
+__global__ void __launch_bounds__(Fft<LOGM>::T) welch_segment_kernel(const float* __restrict__ bg, long n_bg, int step,
+                                                                     int nseg, int detrend, float* __restrict__ part) {
+    using F = Fft<LOGM>;
+    constexpr int M = F::M, NPS = 2 * M, RA = F::RA, RC = F::RC, T = F::T, LB = F::LB;
+    extern __shared__ float2 sm[];
+    __shared__ float red[32];
+    const int seg = blockIdx.x, d = blockIdx.y, tid = threadIdx.x;
+    const float* x = bg + (size_t)d * n_bg + (size_t)seg * step;
+
+    float2 v[F::NA][RA];
+    float sum = 0.f;
+#pragma unroll
+    for (int a = 0; a < F::NA; ++a) {
+        const int jA = tid + a * T;
+#pragma unroll
+        for (int nA = 0; nA < RA; ++nA) {
+            const int m = nA * LB + jA;
+            float2 z = make_float2(x[2 * m] * kStrainScale, x[2 * m + 1] * kStrainScale);
+            v[a][nA] = z;
+            sum += z.x + z.y;
+        }
+    }
+    float mean = 0.f;
+    if (detrend) {
+        // fixed-order block reduction: warp shuffles, then warp 0 over the per-warp sums
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+        if ((tid & 31) == 0) red[tid >> 5] = sum;
+        __syncthreads();
+        float tot = 0.f;
+        for (int w = 0; w < (T + 31) / 32; ++w) tot += red[w];
+        mean = tot * (1.0f / (float)NPS);
+    }
+#pragma unroll
+    for (int a = 0; a < F::NA; ++a) {
+        const int jA = tid + a * T;
+#pragma unroll
+        for (int nA = 0; nA < RA; ++nA) {
+            const int m = nA * LB + jA;
+            // periodic Hann at samples 2m, 2m+1: w[n] = (1 - cos(2 pi n / NPS)) / 2
+            const float w0 = 0.5f - 0.5f * cospif((float)(2 * m) * (2.0f / (float)NPS));
+            const float w1 = 0.5f - 0.5f * cospif((float)(2 * m + 1) * (2.0f / (float)NPS));
+            v[a][nA].x = (v[a][nA].x - mean) * w0;
+            v[a][nA].y = (v[a][nA].y - mean) * w1;
+        }
+        F::pass_a_fwd(v[a], jA, sm);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < F::NB; ++i) F::pass_b_fwd(tid + i * T, sm);
+    __syncthreads();
+    int klow_a, klow_b;
+    pass_c_klow<LOGM>(tid, klow_a, klow_b);
+    float2 va[RC], vb[RC];
+    F::pass_c_fwd(klow_a, va, sm);
+    F::pass_c_fwd(klow_b, vb, sm);
+
+    float* out = part + ((size_t)d * nseg + seg) * (M + 1);
+    for_each_bin_pair<LOGM>(
+        tid, va, vb,
+        [&](int k, float2& za, float2& zb) {
+            float2 xa, xb;
+            split_pair(za, zb, twiddle<2 * M>(k), xa, xb);
+            out[k] = 0.25f * (xa.x * xa.x + xa.y * xa.y);
+            out[M - k] = 0.25f * (xb.x * xb.x + xb.y * xb.y);
+        },
+        [&](int k, float2& z) {
+            float2 xa, xb;
+            split_pair(z, z, twiddle<2 * M>(k), xa, xb);
+            out[k] = 0.25f * (xa.x * xa.x + xa.y * xa.y);
+        },
+        [&](float2& z) {
+            const float dc = z.x + z.y, ny = z.x - z.y;
+            out[0] = dc * dc;
+            out[M] = ny * ny;
+        });
+}
+
+// psd[d][k] = c_k * (sum_seg part) / (nseg * fs * sum w^2), c_k = 2 except DC/Nyquist; sum w^2 = 3 NPS / 8.
+__global__ void welch_mean_kernel(const float* __restrict__ part, int nseg, int n_w, float scale,
+                                  float* __restrict__ psd) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const int d = blockIdx.y;
+    if (k >= n_w) return;
+    const float* p = part + (size_t)d * nseg * n_w + k;
+    float acc = 0.f;
+    for (int s = 0; s < nseg; ++s) acc += p[(size_t)s * n_w];
+    const float ck = (k == 0 || k == n_w - 1) ? 1.0f : 2.0f;
+    psd[(size_t)d * n_w + k] = acc * scale * ck;
+}
+
+template <int LOGM>
+static int launch_welch_t(const amplfi_plan* p, const float* bg, long n_bg, int step, int nseg, int detrend,
+                          cudaStream_t st) {
+    using F = Fft<LOGM>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaFuncSetAttribute(welch_segment_kernel<LOGM>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)F::SMEM_BYTES);
+        attr_done = true;
+    }
+    dim3 grid(nseg, p->n_det);
+    welch_segment_kernel<LOGM><<<grid, F::T, F::SMEM_BYTES, st>>>(bg, n_bg, step, nseg, detrend, p->welch_part);
+    count_launch();
+    return check_launch("welch_segment_kernel");
+}
+
+int launch_welch(const amplfi_plan* p, const float* bg, long n_bg, int noverlap, int detrend, float* psd,
+                 cudaStream_t st) {
+    const int nps = p->nperseg;
+    const int step = nps - noverlap;
+    const long nseg_l = (n_bg - nps) / step + 1;
+    if (nseg_l > p->welch_max_seg) {
+        set_error("amplfi_psd_welch: %ld segments exceed the plan's workspace (%d)", nseg_l, p->welch_max_seg);
+        return AMPLFI_ERR_UNSUPPORTED_SIZE;
+    }
+    const int nseg = (int)nseg_l;
+    int rc;
+    switch (ilog2(nps) - 1) {
+        case 9: rc = launch_welch_t<9>(p, bg, n_bg, step, nseg, detrend, st); break;
+        case 10: rc = launch_welch_t<10>(p, bg, n_bg, step, nseg, detrend, st); break;
+        case 11: rc = launch_welch_t<11>(p, bg, n_bg, step, nseg, detrend, st); break;
+        case 12: rc = launch_welch_t<12>(p, bg, n_bg, step, nseg, detrend, st); break;
+        case 13: rc = launch_welch_t<13>(p, bg, n_bg, step, nseg, detrend, st); break;
+        case 14: rc = launch_welch_t<14>(p, bg, n_bg, step, nseg, detrend, st); break;
+        default: set_error("amplfi_psd_welch: unsupported nperseg %d", nps); return AMPLFI_ERR_UNSUPPORTED_SIZE;
+    }
+    if (rc) return rc;
+    const int n_w = nps / 2 + 1;
+    const float scale = (float)(1.0 / ((double)nseg * p->fs * 0.375 * (double)nps));
+    dim3 grid((n_w + 255) / 256, p->n_det);
+    welch_mean_kernel<<<grid, 256, 0, st>>>(p->welch_part, nseg, n_w, scale, psd);
+    count_launch();
+    return check_launch("welch_mean_kernel");
+}
+
+}  // namespace amplfi
