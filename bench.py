@@ -1,0 +1,318 @@
+#!/usr/bin/env python
+"""bench.py -- whitened injected samples/s of the AMPLFI data-generation hot path on B200.
+
+One "step" = one pass of the whole hot path over one batch of BASELINE.json configs[2]
+(training-throughput shape): Welch PSD of a 64 s window of the GPU-resident strip + fused
+gather / waveform / projection / injection / whitening of batch 2048 x 3 detectors x 16384 samples.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+
+Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for every field.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "whitened injected samples/sec (3-det, 2048 Hz)"
+UNIT = "samples/s"
+WORKLOAD = ("c2 training-throughput: batch 2048 x H1+L1+V1, fs 2048 Hz, 8 s segments (16384), noise gathered "
+            "from a resident quarter-day strip [3, 44236800] at random per-(sample,detector) offsets, Welch PSD "
+            "(64 s, 2 s Hann, 50% overlap, mean) re-estimated every step, IMRPhenomD + aligned spins, Table-1 priors")
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--batch", type=int, default=2048)
+    ap.add_argument("--strip-len", type=int, default=44236800)
+    ap.add_argument("--cpu-sample", type=int, default=256, help="samples of the batch the CPU oracle is timed on")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# ------------------------------------------------------------------------------------------------
+# CPU oracle leg (cpu_baseline and --impl reference)
+# ------------------------------------------------------------------------------------------------
+
+def oracle_step(wl, rows):
+    """The whole hot path for `rows` samples of the workload, in the oracle (fp64, host)."""
+    from oracle import project as OP, waveform as OW, welch as OWE, whiten as OWH
+    o, nb = wl.extra["bg_offset"], wl.extra["n_bg"]
+    psd = OWE.welch(wl.strip[:, o:o + nb].astype(np.float64), wl.fs, wl.nperseg)
+    params = wl.params[rows]
+    noise = OWH.gather(wl.strip, wl.offsets[rows], wl.n)
+    hp, hc, _ = OW.waveform_fd(wl.approximant, params, wl.n, wl.fs, wl.f_lo, wl.f_hi)
+    h_det, _ = OP.project(hp, hc, params, wl.gmst, wl.det_ids, wl.n, wl.fs)
+    return OWH.inject_whiten(noise, h_det, psd, wl.fs, wl.f_lo, wl.f_hi)
+
+
+def threads_used():
+    try:
+        from threadpoolctl import threadpool_info
+        n = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
+        return int(n)
+    except Exception:
+        return 1
+
+
+def time_oracle(wl, n_rows, steps=1, warmup=0):
+    rows = np.arange(n_rows) % wl.batch
+    for _ in range(warmup):
+        oracle_step(wl, rows)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        oracle_step(wl, rows)
+    dt = (time.perf_counter() - t0) / steps
+    return n_rows * wl.n_det * wl.n / dt, dt
+
+
+def run_reference(args):
+    import workloads as WL
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    wl = WL.make_c2(batch=max(args.cpu_sample, 4), strip_len=min(args.strip_len, 1 << 24))
+    n_rows = args.cpu_sample
+    steps = max(1, min(args.steps, 3))
+    warm = min(args.warmup, 1)
+    value, dt = time_oracle(wl, n_rows, steps=steps, warmup=warm)
+    sample = "%d of 2048 samples (x3 detectors x 16384) + the full 64 s Welch per step; strip shortened to %d" % (
+        n_rows, wl.strip.shape[1])
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": warm, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": {"workload": WORKLOAD, "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads_used(), "kind": "oracle", "sample": sample,
+                             "host_cores": os.cpu_count()},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------
+# B200 arm
+# ------------------------------------------------------------------------------------------------
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 100 ms while the timed region runs."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.FIELDS,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            parts = [p.strip() for p in ln.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1])); power.append(float(parts[2]))
+            except ValueError:
+                continue
+            for name, val in zip(names, parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def run_b200(args):
+    import torch
+    import paper_2407_19048_b200 as A      # raises if libamplfi.so is missing: no fallback
+    import workloads as WL
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the B200 arm has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    # ---- synthetic workload (host, seeded), uploaded once: "before commencing training" ----
+    wl = WL.make_c2(batch=args.batch, seed=0xA3D30002 + rank, strip_len=args.strip_len)
+    B, D, N = wl.batch, wl.n_det, wl.n
+    plan = A.Plan(N, wl.fs, wl.det_ids, B, nperseg=wl.nperseg)
+    strip = torch.from_numpy(wl.strip).to(dev)
+    params_h = torch.from_numpy(wl.params).pin_memory()
+    offsets_h = torch.from_numpy(wl.offsets).pin_memory()
+    params = params_h.to(dev)
+    offsets = offsets_h.to(dev)
+    o, nb = wl.extra["bg_offset"], wl.extra["n_bg"]
+    bg = strip[:, o:o + nb]                                     # strided view: rows are L apart
+    psd = torch.empty((D, wl.nperseg // 2 + 1), dtype=torch.float32, device=dev)
+    out = torch.empty((B, D, N), dtype=torch.float32, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def step(p=params, off=offsets):
+        A.amplfi_psd_welch(plan, bg, psd=psd, stream=stream)
+        A.amplfi_inject_whiten(plan, B, strip, psd, wl.f_lo, wl.f_hi, offsets=off, approximant=wl.approximant,
+                               params=p, gmst=wl.gmst, out=out, stream=stream)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+
+    # ---- device-resident timing: exactly K steps, CUDA events on the launching stream ----
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    plan.set_timing(True)
+    launches0 = A.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    barrier()
+    total_ms = e0.elapsed_time(e1)
+    launches = A.launch_count() - launches0
+    kernel_ms = plan.kernel_times_ms()
+    plan.set_timing(False)
+    clocks = sampler.stop() if rank == 0 else None
+    if dist is not None:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = world * B * D * N / (ms_per_step * 1e-3)
+
+    # ---- end to end: per-step inputs from pinned host memory, result read back to the host ----
+    e2e = None
+    if not args.no_e2e:
+        out_h = torch.empty((B, D, N), dtype=torch.float32).pin_memory()
+        k2 = max(3, min(args.steps, 10))
+        p_d, off_d = torch.empty_like(params), torch.empty_like(offsets)
+
+        def step_e2e():
+            p_d.copy_(params_h, non_blocking=True)
+            off_d.copy_(offsets_h, non_blocking=True)
+            step(p_d, off_d)
+            out_h.copy_(out, non_blocking=True)
+
+        for _ in range(2):
+            step_e2e()
+        barrier()
+        e0.record(stream)
+        for _ in range(k2):
+            step_e2e()
+        e1.record(stream)
+        barrier()
+        ms2 = e0.elapsed_time(e1)
+        if dist is not None:
+            t = torch.tensor([ms2], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms2 = float(t.item())
+        e2e = {"value": world * B * D * N / (ms2 / k2 * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": int(params_h.numel() * 8 + offsets_h.numel() * 8),
+               "d2h_bytes_per_step": int(out_h.numel() * 4), "steps": k2, "ms_per_step": ms2 / k2}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (fused inject+whiten): 8 algorithmic bytes per output sample ----
+    peak, peak_src = peaks()
+    k_ms = float(np.mean(kernel_ms)) if kernel_ms else None
+    alg_bytes = 8.0 * B * D * N
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    if os.path.exists(tpath):
+        try:
+            with open(tpath) as fh:
+                traffic = json.load(fh).get("inject_whiten_kernel_dram_bytes_per_launch")
+        except Exception:
+            traffic = None
+    roofline = None
+    if k_ms:
+        ach = alg_bytes / (k_ms * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "kernel": "inject_whiten_kernel<13,fused>", "achieved": ach, "peak": peak,
+                    "unit": "GB/s", "frac": ach / peak, "frac_of_nominal_8TBps": ach / 8000.0, "peak_source": peak_src,
+                    "traffic": traffic, "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": k_ms,
+                    "kernel_share_of_step": k_ms / ms_per_step, "launches_timed": len(kernel_ms)}
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        v, dt = time_oracle(wl, args.cpu_sample)
+        cpu = {"value": v, "unit": UNIT, "cores": threads_used(), "host_cores": os.cpu_count(), "kind": "oracle",
+               "seconds": dt, "sample": "%d of %d samples (x%d detectors x %d) + the full 64 s Welch, one pass"
+               % (args.cpu_sample, B, D, N)}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "batch_per_gpu": B, "n_det": D, "n": N, "strip_len": int(wl.strip.shape[1]),
+                       "l2_policy": "inputs larger than L2 (random 64 KB gathers from a %.0f MB strip + %.0f MB output per step)"
+                       % (wl.strip.nbytes / 1e6, out.numel() * 4 / 1e6),
+                       "parallelism": "batch sharded, no collective" if world > 1 else "single GPU"},
+            "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
+            "hbm_gbs_step": 8.0 * B * D * N / (ms_per_step * 1e-3) / 1e9}
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_b200(a)

@@ -104,11 +104,13 @@ int amplfi_project(const amplfi_plan* plan, int batch, const double* params, dou
  * this background chunk"): per detector, segments of nperseg samples stepping by nperseg - noverlap
  * (full segments only), optional mean removal, periodic Hann window, |FFT|^2, mean over segments,
  * one-sided density.
- *   bg [n_det, n_bg] fp32 strain, row stride n_bg;  noverlap in [0, nperseg);  detrend 0 none / 1 constant;
+ *   bg fp32 strain: detector d's n_bg samples start at bg + d * row_stride (row_stride in elements,
+ *   >= n_bg; pass n_bg for a dense [n_det, n_bg] array, or the strip length to use a window of the
+ *   GPU-resident strip in place);  noverlap in [0, nperseg);  detrend 0 none / 1 constant;
  *   average must be 0 (mean);  psd [n_det, nperseg/2+1] fp32 receives S * 2^140.
  * Deterministic (fixed summation order). */
-int amplfi_psd_welch(const amplfi_plan* plan, const float* bg, long n_bg, int noverlap, int detrend,
-                     int average, float* psd, void* stream);
+int amplfi_psd_welch(const amplfi_plan* plan, const float* bg, long n_bg, long row_stride, int noverlap,
+                     int detrend, int average, float* psd, void* stream);
 
 /* a-5 .. a-9 Gather + inject + whiten ("N small background chunks ... are lazily loaded";
  * PAPER.md:105 "We then inject the signals into the background chunks ... We whiten the batch using the
@@ -131,6 +133,14 @@ int amplfi_inject_whiten(const amplfi_plan* plan, int batch, const float* noise,
                          long strip_len, const float* h_det, int approximant, const double* params,
                          double gmst, const float* psd, int n_psd, double f_lo, double f_hi,
                          float* out, void* stream);
+
+/* Device timing of the dominant kernel (the fused inject+whiten kernel).  With timing enabled every
+ * amplfi_inject_whiten call brackets that kernel with CUDA events recorded on the caller's stream (up to
+ * 512 calls are kept; enabling resets the list).  amplfi_plan_kernel_times waits for the recorded events
+ * and writes up to `max` durations in milliseconds to the HOST array ms; returns the number written, or a
+ * negative error. */
+int amplfi_plan_set_timing(amplfi_plan* plan, int enable);
+int amplfi_plan_kernel_times(amplfi_plan* plan, float* ms, int max);
 
 /* Number of kernel launches the library has enqueued since it was loaded (all plans, all threads).
  * bench.py reports the difference across its timed region as "gpu_launches". */

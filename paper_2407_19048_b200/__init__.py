@@ -22,7 +22,8 @@ N_PARAMS = 11
 
 EXPORTS = ("amplfi_last_error", "amplfi_psd_scale", "amplfi_version", "amplfi_phenomd_table",
            "amplfi_plan_create", "amplfi_plan_destroy", "amplfi_waveform_fd", "amplfi_project",
-           "amplfi_psd_welch", "amplfi_inject_whiten", "amplfi_launch_count")
+           "amplfi_psd_welch", "amplfi_inject_whiten", "amplfi_launch_count", "amplfi_plan_set_timing",
+           "amplfi_plan_kernel_times")
 
 
 class AmplfiError(RuntimeError):
@@ -52,12 +53,16 @@ def _load():
     lib.amplfi_plan_create.argtypes = [i32, dbl, i32, c.POINTER(i32), i32, i32, c.POINTER(vp)]
     lib.amplfi_plan_destroy.restype = None
     lib.amplfi_plan_destroy.argtypes = [vp]
+    lib.amplfi_plan_set_timing.restype = i32
+    lib.amplfi_plan_set_timing.argtypes = [vp, i32]
+    lib.amplfi_plan_kernel_times.restype = i32
+    lib.amplfi_plan_kernel_times.argtypes = [vp, vp, i32]
     lib.amplfi_waveform_fd.restype = i32
     lib.amplfi_waveform_fd.argtypes = [vp, i32, i32, vp, dbl, dbl, vp, vp, vp, vp]
     lib.amplfi_project.restype = i32
     lib.amplfi_project.argtypes = [vp, i32, vp, dbl, vp, vp, vp, vp, vp]
     lib.amplfi_psd_welch.restype = i32
-    lib.amplfi_psd_welch.argtypes = [vp, vp, i64, i32, i32, i32, vp, vp]
+    lib.amplfi_psd_welch.argtypes = [vp, vp, i64, i64, i32, i32, i32, vp, vp]
     lib.amplfi_inject_whiten.restype = i32
     lib.amplfi_inject_whiten.argtypes = [vp, i32, vp, vp, i64, vp, i32, vp, dbl, vp, i32, dbl, dbl, vp, vp]
     return lib
@@ -125,6 +130,17 @@ class Plan:
         self.n_det = len(det_ids)
         self.n_bins = self.n // 2 + 1
 
+    def set_timing(self, enable=True):
+        _check(_lib.amplfi_plan_set_timing(self._h, 1 if enable else 0))
+
+    def kernel_times_ms(self, max_count=512):
+        """Durations (ms) of the fused inject+whiten kernel of the calls made since set_timing(True)."""
+        buf = (ctypes.c_float * max_count)()
+        n = _lib.amplfi_plan_kernel_times(self._h, ctypes.cast(buf, ctypes.c_void_p), max_count)
+        if n < 0:
+            _check(n)
+        return [float(buf[i]) for i in range(n)]
+
     def close(self):
         if getattr(self, "_h", None):
             _lib.amplfi_plan_destroy(self._h)
@@ -174,9 +190,12 @@ def amplfi_psd_welch(plan, bg, noverlap=None, detrend=1, average=0, psd=None, st
         noverlap = plan.nperseg // 2
     if psd is None:
         psd = torch.empty((plan.n_det, plan.nperseg // 2 + 1), dtype=torch.float32, device=bg.device)
-    if bg.dim() != 2 or bg.shape[0] != plan.n_det:
-        raise ValueError("bg must be [n_det, n_bg]")
-    _check(_lib.amplfi_psd_welch(plan._h, _ptr(bg, torch.float32, "bg"), int(bg.shape[1]), int(noverlap), int(detrend),
+    if bg.dim() != 2 or bg.shape[0] != plan.n_det or bg.stride(1) != 1:
+        raise ValueError("bg must be [n_det, n_bg] with unit stride along time (rows may be a window of a strip)")
+    if not bg.is_cuda or bg.dtype != torch.float32:
+        raise TypeError("bg must be a CUDA float32 tensor (no CPU fallback)")
+    row_stride = int(bg.stride(0)) if plan.n_det > 1 else int(bg.shape[1])
+    _check(_lib.amplfi_psd_welch(plan._h, ctypes.c_void_p(bg.data_ptr()), int(bg.shape[1]), row_stride, int(noverlap), int(detrend),
                                  int(average), _ptr(psd, torch.float32, "psd"), _stream(stream)))
     return psd
 

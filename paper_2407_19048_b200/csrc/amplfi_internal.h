@@ -5,6 +5,8 @@
 #include "../../include/amplfi.h"
 #include "phenomd_table.h"
 
+#define AMPLFI_TIMING_RING 512
+
 namespace amplfi {
 struct WfCoef;
 struct DetResp;
@@ -32,6 +34,10 @@ struct amplfi_plan {
     float* welch_part;     // [n_det * max_seg * (nperseg/2+1)]
     int welch_max_seg;
     int* d_det_ids;        // [3]
+    // optional device timing of the dominant kernel (amplfi_plan_set_timing)
+    int timing;
+    int ev_count;
+    cudaEvent_t ev_start[AMPLFI_TIMING_RING], ev_stop[AMPLFI_TIMING_RING];
 };
 
 namespace amplfi {
@@ -50,7 +56,7 @@ int launch_project(const amplfi_plan* p, int batch, const float* hp, const float
 int launch_tables(amplfi_plan* p, cudaStream_t st);
 
 // welch.cu
-int launch_welch(const amplfi_plan* p, const float* bg, long n_bg, int noverlap, int detrend, float* psd,
+int launch_welch(const amplfi_plan* p, const float* bg, long n_bg, long row_stride, int noverlap, int detrend, float* psd,
                  cudaStream_t st);
 
 // inject_whiten.cu

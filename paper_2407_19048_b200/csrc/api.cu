@@ -129,8 +129,36 @@ int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_
     return AMPLFI_OK;
 }
 
+int amplfi_plan_set_timing(amplfi_plan* p, int enable) {
+    if (p == nullptr) { set_error("amplfi_plan_set_timing: null plan"); return AMPLFI_ERR_INVALID_ARG; }
+    if (enable && p->ev_start[0] == nullptr) {
+        for (int i = 0; i < AMPLFI_TIMING_RING; ++i) {
+            if (cudaEventCreate(&p->ev_start[i]) != cudaSuccess || cudaEventCreate(&p->ev_stop[i]) != cudaSuccess) {
+                set_error("amplfi_plan_set_timing: cudaEventCreate failed");
+                return AMPLFI_ERR_CUDA;
+            }
+        }
+    }
+    p->timing = enable ? 1 : 0;
+    p->ev_count = 0;
+    return AMPLFI_OK;
+}
+
+int amplfi_plan_kernel_times(amplfi_plan* p, float* ms, int max) {
+    if (p == nullptr || ms == nullptr) { set_error("amplfi_plan_kernel_times: null pointer"); return AMPLFI_ERR_INVALID_ARG; }
+    int n = p->ev_count < max ? p->ev_count : max;
+    for (int i = 0; i < n; ++i) {
+        cudaError_t e = cudaEventSynchronize(p->ev_stop[i]);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms[i], p->ev_start[i], p->ev_stop[i]);
+        if (e != cudaSuccess) { set_error("amplfi_plan_kernel_times: %s", cudaGetErrorString(e)); return AMPLFI_ERR_CUDA; }
+    }
+    return n;
+}
+
 void amplfi_plan_destroy(amplfi_plan* p) {
     if (p == nullptr) return;
+    if (p->ev_start[0] != nullptr)
+        for (int i = 0; i < AMPLFI_TIMING_RING; ++i) { cudaEventDestroy(p->ev_start[i]); cudaEventDestroy(p->ev_stop[i]); }
     cudaFree(p->tab_ci); cudaFree(p->tab_lnk); cudaFree(p->pd_table); cudaFree(p->coef); cudaFree(p->resp);
     cudaFree(p->h0); cudaFree(p->filt); cudaFree(p->welch_part); cudaFree(p->d_det_ids);
     delete p;
@@ -164,8 +192,8 @@ int amplfi_project(const amplfi_plan* p, int batch, const double* params, double
     return launch_project(p, batch, hp, hc, h_det, resp, st);
 }
 
-int amplfi_psd_welch(const amplfi_plan* p, const float* bg, long n_bg, int noverlap, int detrend, int average,
-                     float* psd, void* stream) {
+int amplfi_psd_welch(const amplfi_plan* p, const float* bg, long n_bg, long row_stride, int noverlap, int detrend,
+                     int average, float* psd, void* stream) {
     if (p == nullptr || bg == nullptr || psd == nullptr) { set_error("amplfi_psd_welch: null pointer"); return AMPLFI_ERR_INVALID_ARG; }
     if (p->nperseg == 0) { set_error("amplfi_psd_welch: plan was created with nperseg = 0"); return AMPLFI_ERR_INVALID_ARG; }
     if (n_bg < p->nperseg) { set_error("amplfi_psd_welch: nperseg %d > n_bg %ld", p->nperseg, n_bg); return AMPLFI_ERR_UNSUPPORTED_SIZE; }
@@ -173,7 +201,8 @@ int amplfi_psd_welch(const amplfi_plan* p, const float* bg, long n_bg, int nover
         set_error("amplfi_psd_welch: need 0 <= noverlap < nperseg, detrend in {0,1}, average = 0 (mean)");
         return AMPLFI_ERR_INVALID_ARG;
     }
-    return launch_welch(p, bg, n_bg, noverlap, detrend, psd, static_cast<cudaStream_t>(stream));
+    if (row_stride < n_bg) { set_error("amplfi_psd_welch: row_stride %ld < n_bg %ld", row_stride, n_bg); return AMPLFI_ERR_INVALID_ARG; }
+    return launch_welch(p, bg, n_bg, row_stride, noverlap, detrend, psd, static_cast<cudaStream_t>(stream));
 }
 
 int amplfi_inject_whiten(const amplfi_plan* p, int batch, const float* noise, const long* offsets, long strip_len,
@@ -198,7 +227,12 @@ int amplfi_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
         rc = launch_waveform_h0(p, batch, st);
         if (rc) return rc;
     }
-    return launch_inject_whiten(p, batch, noise, offsets, strip_len, h_det, fused ? 1 : 0, out, st);
+    amplfi_plan* mp = const_cast<amplfi_plan*>(p);
+    const bool timed = p->timing && p->ev_count < AMPLFI_TIMING_RING;
+    if (timed) cudaEventRecord(mp->ev_start[p->ev_count], st);
+    rc = launch_inject_whiten(p, batch, noise, offsets, strip_len, h_det, fused ? 1 : 0, out, st);
+    if (timed) { cudaEventRecord(mp->ev_stop[p->ev_count], st); mp->ev_count++; }
+    return rc;
 }
 
 }  // extern "C"

@@ -11,14 +11,14 @@ constexpr float kStrainScale = 1180591620717411303424.0f;   // 2^70: strain -> O
 
 // One CTA per (detector, segment).  part[d][seg][k] = |FFT(w (x - mean))[k]|^2 (scaled by 2^140).
 template <int LOGM>
-__global__ void __launch_bounds__(Fft<LOGM>::T) welch_segment_kernel(const float* __restrict__ bg, long n_bg, int step,
+__global__ void __launch_bounds__(Fft<LOGM>::T) welch_segment_kernel(const float* __restrict__ bg, long row_stride, int step,
                                                                      int nseg, int detrend, float* __restrict__ part) {
     using F = Fft<LOGM>;
     constexpr int M = F::M, NPS = 2 * M, RA = F::RA, RC = F::RC, T = F::T, LB = F::LB;
     extern __shared__ float2 sm[];
     __shared__ float red[32];
     const int seg = blockIdx.x, d = blockIdx.y, tid = threadIdx.x;
-    const float* x = bg + (size_t)d * n_bg + (size_t)seg * step;
+    const float* x = bg + (size_t)d * row_stride + (size_t)seg * step;
 
     float2 v[F::NA][RA];
     float sum = 0.f;
@@ -103,7 +103,7 @@ __global__ void welch_mean_kernel(const float* __restrict__ part, int nseg, int 
 }
 
 template <int LOGM>
-static int launch_welch_t(const amplfi_plan* p, const float* bg, long n_bg, int step, int nseg, int detrend,
+static int launch_welch_t(const amplfi_plan* p, const float* bg, long row_stride, int step, int nseg, int detrend,
                           cudaStream_t st) {
     using F = Fft<LOGM>;
     static bool attr_done = false;
@@ -113,12 +113,12 @@ static int launch_welch_t(const amplfi_plan* p, const float* bg, long n_bg, int 
         attr_done = true;
     }
     dim3 grid(nseg, p->n_det);
-    welch_segment_kernel<LOGM><<<grid, F::T, F::SMEM_BYTES, st>>>(bg, n_bg, step, nseg, detrend, p->welch_part);
+    welch_segment_kernel<LOGM><<<grid, F::T, F::SMEM_BYTES, st>>>(bg, row_stride, step, nseg, detrend, p->welch_part);
     count_launch();
     return check_launch("welch_segment_kernel");
 }
 
-int launch_welch(const amplfi_plan* p, const float* bg, long n_bg, int noverlap, int detrend, float* psd,
+int launch_welch(const amplfi_plan* p, const float* bg, long n_bg, long row_stride, int noverlap, int detrend, float* psd,
                  cudaStream_t st) {
     const int nps = p->nperseg;
     const int step = nps - noverlap;
@@ -130,12 +130,12 @@ int launch_welch(const amplfi_plan* p, const float* bg, long n_bg, int noverlap,
     const int nseg = (int)nseg_l;
     int rc;
     switch (ilog2(nps) - 1) {
-        case 9: rc = launch_welch_t<9>(p, bg, n_bg, step, nseg, detrend, st); break;
-        case 10: rc = launch_welch_t<10>(p, bg, n_bg, step, nseg, detrend, st); break;
-        case 11: rc = launch_welch_t<11>(p, bg, n_bg, step, nseg, detrend, st); break;
-        case 12: rc = launch_welch_t<12>(p, bg, n_bg, step, nseg, detrend, st); break;
-        case 13: rc = launch_welch_t<13>(p, bg, n_bg, step, nseg, detrend, st); break;
-        case 14: rc = launch_welch_t<14>(p, bg, n_bg, step, nseg, detrend, st); break;
+        case 9: rc = launch_welch_t<9>(p, bg, row_stride, step, nseg, detrend, st); break;
+        case 10: rc = launch_welch_t<10>(p, bg, row_stride, step, nseg, detrend, st); break;
+        case 11: rc = launch_welch_t<11>(p, bg, row_stride, step, nseg, detrend, st); break;
+        case 12: rc = launch_welch_t<12>(p, bg, row_stride, step, nseg, detrend, st); break;
+        case 13: rc = launch_welch_t<13>(p, bg, row_stride, step, nseg, detrend, st); break;
+        case 14: rc = launch_welch_t<14>(p, bg, row_stride, step, nseg, detrend, st); break;
         default: set_error("amplfi_psd_welch: unsupported nperseg %d", nps); return AMPLFI_ERR_UNSUPPORTED_SIZE;
     }
     if (rc) return rc;
