@@ -59,6 +59,26 @@ int launch_tables(amplfi_plan* p, cudaStream_t st);
 int launch_welch(const amplfi_plan* p, const float* bg, long n_bg, long row_stride, int noverlap, int detrend, float* psd,
                  cudaStream_t st);
 
+enum { MODE_NONE = 0, MODE_HDET = 1, MODE_FUSED = 2 };
+
+struct IwArgs {
+    const float* noise;       // dense [B, D, N] or strip [D, L]
+    const long* offsets;      // nullptr: dense
+    long strip_len;
+    const float2* h_det;      // MODE_HDET: [B, D, K]
+    const float2* h0;         // MODE_FUSED: [B, K] (2 fs h0)
+    const WfCoef* coef;
+    const DetResp* resp;
+    const float* filt;        // [D, K]
+    float* out;               // [B, D, N]
+    int n_det;
+    float two_fs;
+    float inv_tseg;
+};
+
+// inject_whiten13.cu (packed 4-pass kernel for n = 16384)
+int launch_iw13(const IwArgs& a, int mode, int units, cudaStream_t st);
+
 // inject_whiten.cu
 int launch_filter(const amplfi_plan* p, const float* psd, int n_psd, double f_lo, double f_hi, cudaStream_t st);
 int launch_inject_whiten(const amplfi_plan* p, int batch, const float* noise, const long* offsets,

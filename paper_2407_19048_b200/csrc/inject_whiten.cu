@@ -52,23 +52,6 @@ int launch_filter(const amplfi_plan* p, const float* psd, int n_psd, double f_lo
     return check_launch("filter_kernel");
 }
 
-enum { MODE_NONE = 0, MODE_HDET = 1, MODE_FUSED = 2 };
-
-struct IwArgs {
-    const float* noise;       // dense [B, D, N] or strip [D, L]
-    const long* offsets;      // nullptr: dense
-    long strip_len;
-    const float2* h_det;      // MODE_HDET: [B, D, K]
-    const float2* h0;         // MODE_FUSED: [B, K] (2 fs h0)
-    const WfCoef* coef;
-    const DetResp* resp;
-    const float* filt;        // [D, K]
-    float* out;               // [B, D, N]
-    int n_det;
-    float two_fs;
-    float inv_tseg;
-};
-
 template <int LOGM, int MODE>
 __global__ void __launch_bounds__(Fft<LOGM>::T) inject_whiten_kernel(const IwArgs a) {
     using F = Fft<LOGM>;
@@ -243,7 +226,7 @@ int launch_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
         case 10: return launch_iw_mode<10>(a, mode, units, st);
         case 11: return launch_iw_mode<11>(a, mode, units, st);
         case 12: return launch_iw_mode<12>(a, mode, units, st);
-        case 13: return launch_iw_mode<13>(a, mode, units, st);
+        case 13: return launch_iw13(a, mode, units, st);
         case 14: return launch_iw_mode<14>(a, mode, units, st);
         default:
             set_error("amplfi_inject_whiten: segment length %d not supported by this build", p->n);

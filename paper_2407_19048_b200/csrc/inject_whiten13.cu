@@ -1,0 +1,178 @@
+// inject_whiten13.cu -- fused gather -> FFT -> inject -> whiten -> iFFT for n = 16384 (configs c1, c2, c3),
+// second generation: 4 passes (16*8*8*8), 16 points per thread, 512 threads per segment, packed fp32x2 math,
+// 2 CTAs (32 warps) per SM.  See inject_whiten_v2.cuh for the index algebra.  PAPER.md:103, :105.
+#include "amplfi_internal.h"
+#include "inject_whiten_v2.cuh"
+
+namespace amplfi {
+
+using namespace v2;
+
+template <int MODE>
+__global__ void __launch_bounds__(T13, 2) inject_whiten13_kernel(const IwArgs a, int units) {
+    constexpr int M = M13, N = N13, K = M13 + 1;
+    extern __shared__ float smem13[];
+    float* re = smem13;
+    float* im = smem13 + M;
+    const int unit = blockIdx.x, t = threadIdx.x;
+    const int b = unit / a.n_det, d = unit - b * a.n_det;
+
+    // ---- a-5 gather ----
+    const float* x;
+    float* out = a.out + (size_t)unit * N;
+    if (a.offsets != nullptr) {
+        const long off = a.offsets[unit];
+        if (off < 0 || off + N > a.strip_len) {            // never read out of bounds: poison the row instead
+            const float qnan = __int_as_float(0x7fc00000);
+            for (int i = t; i < N; i += T13) out[i] = qnan;
+            return;
+        }
+        x = a.noise + (size_t)d * a.strip_len + off;
+    } else {
+        x = a.noise + (size_t)unit * N;
+    }
+
+    // ---- a-6 forward real FFT of the packed sequence z[m] = x[2m] + i x[2m+1] ----
+    {
+        float2 z[16];
+        if ((reinterpret_cast<size_t>(x) & 7) == 0) {
+            const float2* x2 = reinterpret_cast<const float2*>(x);
+#pragma unroll
+            for (int n1 = 0; n1 < 16; ++n1) z[n1] = __ldcs(x2 + n1 * 512 + t);
+        } else {
+#pragma unroll
+            for (int n1 = 0; n1 < 16; ++n1) {
+                const int m = n1 * 512 + t;
+                z[n1] = make_float2(__ldg(x + 2 * m), __ldg(x + 2 * m + 1));
+            }
+        }
+        p1_fwd(z, t, re, im);
+    }
+    __syncthreads();
+    p2_fwd(t, re, im);
+    __syncthreads();
+    p3_fwd(t, re, im);
+    __syncthreads();
+    const int klow_a = t, klow_b = (t == 0) ? 512 : 1024 - t;
+    C2 v[8];
+    p4_fwd(klow_a, klow_b, v, re, im);
+
+    // ---- a-7 inject, a-8 whiten + band-limit (registers) ----
+    const float* filt = a.filt + (size_t)d * K;
+    const float2* hsrc = nullptr;
+    int w_lo = 1, w_hi = 0;
+    float cre = 0.f, cim = 0.f, delta = 0.f;
+    if (MODE == MODE_HDET) hsrc = a.h_det + (size_t)unit * K;
+    if (MODE == MODE_FUSED) {
+        const WfCoef* c = a.coef + b;
+        hsrc = a.h0 + (size_t)b * K;
+        if (c->valid) { w_lo = c->k_lo; w_hi = c->k_hi; }
+        const DetResp r = a.resp[unit];
+        cre = (float)r.fp * c->pol_p;                       // C = F+ (1+cos^2 i)/2 - i Fx cos i
+        cim = -(float)r.fc * c->pol_c;
+        delta = (float)(r.dt * (double)a.inv_tseg);          // turns per bin
+    }
+    auto inject = [&](int k, float2& x2) {
+        if (MODE == MODE_HDET) {
+            const float2 h = __ldg(hsrc + k);
+            x2.x = fmaf(a.two_fs, h.x, x2.x);
+            x2.y = fmaf(a.two_fs, h.y, x2.y);
+        } else if (MODE == MODE_FUSED) {
+            if (k >= w_lo && k <= w_hi) {
+                const float2 h = __ldg(hsrc + k);
+                float turns = (float)k * delta;
+                turns -= rintf(turns);
+                float s, co;
+                __sincosf(turns * -6.283185307179586f, &s, &co);          // exp(-2 pi i k dt / T)
+                const float2 cp = make_float2(cre * co - cim * s, cre * s + cim * co);
+                x2.x += h.x * cp.x - h.y * cp.y;
+                x2.y += h.x * cp.y + h.y * cp.x;
+            }
+        }
+    };
+    auto do_pair = [&](int k, float2& za, float2& zb) {       // za = Z[k], zb = Z[M-k], 0 < k < M/2
+        const float2 w = twiddle<N>(k);
+        float2 xa, xb;
+        split_pair(za, zb, w, xa, xb);
+        inject(k, xa);
+        inject(M - k, xb);
+        const float fa = __ldg(filt + k), fb = __ldg(filt + M - k);
+        xa.x *= fa; xa.y *= fa; xb.x *= fb; xb.y *= fb;
+        merge_pair(xa, xb, w, za, zb);
+    };
+    float2 za[8], zb[8];            // halves A, B; index r holds k4 = brev<8>(r)
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+        unpack(v[r].r, za[r].x, zb[r].x);
+        unpack(v[r].i, za[r].y, zb[r].y);
+    }
+    if (t != 0) {
+#pragma unroll
+        for (int r = 0; r < 8; ++r) do_pair(t + 1024 * brev<8>(r), za[r], zb[7 - r]);
+    } else {
+        {   // Z[0] carries the DC and Nyquist bins of the real transform
+            float x0 = 2.0f * (za[0].x + za[0].y), xm = 2.0f * (za[0].x - za[0].y);
+            if (MODE == MODE_HDET) {
+                x0 = fmaf(a.two_fs, __ldg(hsrc).x, x0);
+                xm = fmaf(a.two_fs, __ldg(hsrc + M).x, xm);
+            }
+            const float y0 = x0 * __ldg(filt), ym = xm * __ldg(filt + M);
+            za[0] = make_float2(y0 + ym, y0 - ym);
+        }
+        {   // k = M/2 pairs with itself (k4 = 4 -> register brev(4) = 1)
+            const int k = M / 2;
+            const float2 w = twiddle<N>(k);
+            float2 xa, xb, z2;
+            split_pair(za[1], za[1], w, xa, xb);
+            inject(k, xa);
+            const float fa = __ldg(filt + k);
+            xa.x *= fa; xa.y *= fa;
+            merge_pair(xa, xa, w, za[1], z2);
+        }
+#pragma unroll
+        for (int q = 1; q < 4; ++q) do_pair(1024 * q, za[brev<8>(q)], za[brev<8>(8 - q)]);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) do_pair(512 + 1024 * q, zb[brev<8>(q)], zb[brev<8>(7 - q)]);
+    }
+#pragma unroll
+    for (int r = 0; r < 8; ++r) v[r] = C2{pack(za[r].x, zb[r].x), pack(za[r].y, zb[r].y)};
+
+    // ---- a-9 inverse real FFT and store ----
+    p4_inv(klow_a, klow_b, v, re, im);
+    __syncthreads();
+    p3_inv(t, re, im);
+    __syncthreads();
+    p2_inv(t, re, im);
+    __syncthreads();
+    {
+        float2 z[16];
+        p1_inv(z, t, re, im);
+        float2* out2 = reinterpret_cast<float2*>(out);
+#pragma unroll
+        for (int n1 = 0; n1 < 16; ++n1) __stcs(out2 + n1 * 512 + t, z[n1]);
+    }
+}
+
+template <int MODE>
+static int launch_iw13_t(const IwArgs& a, int units, cudaStream_t st) {
+    static bool attr_done = false;
+    const int smem = 2 * M13 * (int)sizeof(float);
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(inject_whiten13_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) { set_error("cudaFuncSetAttribute: %s", cudaGetErrorString(e)); return AMPLFI_ERR_CUDA; }
+        attr_done = true;
+    }
+    inject_whiten13_kernel<MODE><<<units, T13, smem, st>>>(a, units);
+    count_launch();
+    return check_launch("inject_whiten13_kernel");
+}
+
+int launch_iw13(const IwArgs& a, int mode, int units, cudaStream_t st) {
+    switch (mode) {
+        case MODE_NONE: return launch_iw13_t<MODE_NONE>(a, units, st);
+        case MODE_HDET: return launch_iw13_t<MODE_HDET>(a, units, st);
+        default: return launch_iw13_t<MODE_FUSED>(a, units, st);
+    }
+}
+
+}  // namespace amplfi

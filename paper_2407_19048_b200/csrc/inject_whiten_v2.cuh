@@ -1,0 +1,205 @@
+// inject_whiten_v2.cuh -- second-generation fused kernel for N = 16384 (M = 8192 complex points):
+// four passes 16 * 8 * 8 * 8, 16 points per thread, 512 threads per segment, packed fp32x2 arithmetic.
+//
+// Index algebra.  Input index  n = n1*512 + n2*64 + n3*8 + n4   (n1 < 16, n2, n3, n4 < 8)
+//                 output bin   k = k1 + 16*k2 + 128*k3 + 1024*k4 (k1 < 16, k2, k3, k4 < 8)
+//   P1 (radix 16 over n1, operands from global memory): one scalar radix-2 stage over the top bit of n1
+//       splits the butterfly into the even-k1 and odd-k1 halves, which then run as ONE packed radix-8
+//       (half A = even k1 = 2*kap, half B = odd k1 = 2*kap + 1).  Twiddle w_M^(j1 k1), j1 = n2*64+n3*8+n4.
+//   P2 (packed radix 8 over n2), twiddle w_512^((n3*8+n4) k2); both halves share it.
+//   P3 (packed radix 8 over n3), twiddle w_64^(n4 k3).
+//   P4 (packed radix 8 over n4): half A is the butterfly with klow = k1+16k2+128k3 = t, half B the one with
+//       klow' = 1024 - t, so bins k and M - k meet in one thread: split / inject / whiten / merge in registers.
+//   The inverse runs P4' P3' P2' P1' with conjugate twiddles and stores natural-order samples.
+//
+// Shared memory: two float planes (re, im) of M floats.  Float index of element (kap, pi, d2, d3, d4) is
+//   pi + 2*slot,  slot = kap<<9 | d2<<6 | (d3>>1)<<4 | ((d4 ^ kap) & 7)<<1 | ((d3 ^ d2) & 1)
+// so that the 64-bit (A, B) accesses of P1..P3 and the 32-bit accesses of P4 are all bank-conflict free.
+#pragma once
+#include "fft_packed.cuh"
+#include "waveform.cuh"
+
+namespace amplfi {
+namespace v2 {
+
+using namespace pk;
+
+constexpr int M13 = 8192, N13 = 16384, T13 = 512;
+
+__device__ __forceinline__ int slot13(int kap, int d2, int d3, int d4) {
+    return (kap << 9) | (d2 << 6) | ((d3 >> 1) << 4) | (((d4 ^ kap) & 7) << 1) | ((d3 ^ d2) & 1);
+}
+__device__ __forceinline__ C2 lds2(const float* re, const float* im, int slot) {
+    return C2{*reinterpret_cast<const u64*>(re + 2 * slot), *reinterpret_cast<const u64*>(im + 2 * slot)};
+}
+__device__ __forceinline__ void sts2(float* re, float* im, int slot, C2 v) {
+    *reinterpret_cast<u64*>(re + 2 * slot) = v.r;
+    *reinterpret_cast<u64*>(im + 2 * slot) = v.i;
+}
+
+// ---- forward passes ----
+// x[n1] = z[n1*512 + t] (natural complex, from global).  Leaves the spectrum digits (k1; n2 n3 n4) in smem.
+__device__ __forceinline__ void p1_fwd(const float2 (&x)[16], int t, float* re, float* im) {
+    C2 v[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const float2 s = amplfi::cadd(x[i], x[i + 8]);
+        float2 d = amplfi::csub(x[i], x[i + 8]);
+        switch (i) {      // d *= w16^i
+            case 0: break;
+            case 1: d = mul_w32<2, false>(d); break;
+            case 2: d = mul_w32<4, false>(d); break;
+            case 3: d = mul_w32<6, false>(d); break;
+            case 4: d = mul_w32<8, false>(d); break;
+            case 5: d = mul_w32<10, false>(d); break;
+            case 6: d = mul_w32<12, false>(d); break;
+            default: d = mul_w32<14, false>(d); break;
+        }
+        v[i] = C2{pack(s.x, d.x), pack(s.y, d.y)};
+    }
+    dif8(v);
+    // twiddles (w^(j1 2kap), w^(j1 (2kap+1))) = (1, u) * (u^2)^kap,  u = w_M^j1
+    const float2 u = twiddle<M13>(t);
+    const float2 u2 = twiddle<M13>(2 * t);
+    C2 tw[8];
+    powers8(C2{pack(1.0f, u.x), pack(0.0f, u.y)}, C2{bcast(u2.x), bcast(u2.y)}, tw);
+    const int n2 = t >> 6, n3 = (t >> 3) & 7, n4 = t & 7;
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+        const int kap = brev<8>(r);
+        sts2(re, im, slot13(kap, n2, n3, n4), cmul(v[r], tw[kap]));
+    }
+}
+
+__device__ __forceinline__ void p2_fwd(int t, float* re, float* im) {
+    const int kap = t >> 6, n3 = (t >> 3) & 7, n4 = t & 7;
+    C2 v[8];
+#pragma unroll
+    for (int n2 = 0; n2 < 8; ++n2) v[n2] = lds2(re, im, slot13(kap, n2, n3, n4));
+    dif8(v);
+    float2 g[8];
+    powers8(make_float2(1.0f, 0.0f), twiddle<512>(n3 * 8 + n4), g);
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+        const int k2 = brev<8>(r);
+        sts2(re, im, slot13(kap, k2, n3, n4), k2 == 0 ? v[r] : cmul_s(v[r], g[k2]));
+    }
+}
+
+__device__ __forceinline__ void p3_fwd(int t, float* re, float* im) {
+    const int kap = t >> 6, k2 = (t >> 3) & 7, n4 = t & 7;
+    C2 v[8];
+#pragma unroll
+    for (int n3 = 0; n3 < 8; ++n3) v[n3] = lds2(re, im, slot13(kap, k2, n3, n4));
+    dif8(v);
+    float2 g[8];
+    powers8(make_float2(1.0f, 0.0f), twiddle<64>(n4), g);
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+        const int k3 = brev<8>(r);
+        sts2(re, im, slot13(kap, k2, k3, n4), k3 == 0 ? v[r] : cmul_s(v[r], g[k3]));
+    }
+}
+
+struct P4Addr { int fa, fb, xa, xb; };     // float offsets of halves A, B at d4 = 0 and their kap (xor masks)
+
+__device__ __forceinline__ void p4_addr(int klow, int& base, int& kap) {
+    const int k1 = klow & 15, k2 = (klow >> 4) & 7, k3 = klow >> 7;
+    kap = k1 >> 1;
+    base = (k1 & 1) + 2 * ((kap << 9) | (k2 << 6) | ((k3 >> 1) << 4) | ((k3 ^ k2) & 1));
+}
+// element d4 of the butterfly at (base, kap): float index base + 2*(((d4 ^ kap) & 7) << 1)
+__device__ __forceinline__ int p4_off(int base, int kap, int d4) { return base + (((d4 ^ kap) & 7) << 2); }
+
+__device__ __forceinline__ void p4_fwd(int klow_a, int klow_b, C2 (&v)[8], const float* re, const float* im) {
+    int ba, ka, bb, kb;
+    p4_addr(klow_a, ba, ka);
+    p4_addr(klow_b, bb, kb);
+#pragma unroll
+    for (int n4 = 0; n4 < 8; ++n4) {
+        const int oa = p4_off(ba, ka, n4), ob = p4_off(bb, kb, n4);
+        v[n4] = C2{pack(re[oa], re[ob]), pack(im[oa], im[ob])};
+    }
+    dif8(v);
+}
+
+// ---- inverse passes ----
+__device__ __forceinline__ void p4_inv(int klow_a, int klow_b, C2 (&v)[8], float* re, float* im) {
+    dit8(v);
+    int ba, ka, bb, kb;
+    p4_addr(klow_a, ba, ka);
+    p4_addr(klow_b, bb, kb);
+    // conj twiddle of P3: w_64^(-n4 k3) per half
+    const float2 ga = twiddle<64>(klow_a >> 7), gb = twiddle<64>(klow_b >> 7);
+    C2 tw[8];
+    powers8(C2{bcast(1.0f), bcast(0.0f)}, C2{pack(ga.x, gb.x), pack(ga.y, gb.y)}, tw);
+#pragma unroll
+    for (int n4 = 0; n4 < 8; ++n4) {
+        const C2 y = n4 == 0 ? v[0] : cmul_conj(v[n4], tw[n4]);
+        float ar, br, ai, bi;
+        unpack(y.r, ar, br);
+        unpack(y.i, ai, bi);
+        const int oa = p4_off(ba, ka, n4), ob = p4_off(bb, kb, n4);
+        re[oa] = ar; im[oa] = ai;
+        re[ob] = br; im[ob] = bi;
+    }
+}
+
+__device__ __forceinline__ void p3_inv(int t, float* re, float* im) {
+    const int kap = t >> 6, k2 = (t >> 3) & 7, n4 = t & 7;
+    C2 v[8];
+#pragma unroll
+    for (int r = 0; r < 8; ++r) v[r] = lds2(re, im, slot13(kap, k2, brev<8>(r), n4));
+    dit8(v);
+    // conj twiddle of P2: w_512^(-(n3*8 + n4) k2) = conj(c * s^n3), c = w_512^(n4 k2), s = w_64^k2
+    float2 g[8];
+    powers8(twiddle<512>(n4 * k2), twiddle<64>(k2), g);
+#pragma unroll
+    for (int n3 = 0; n3 < 8; ++n3) sts2(re, im, slot13(kap, k2, n3, n4), cmul_conj_s(v[n3], g[n3]));
+}
+
+__device__ __forceinline__ void p2_inv(int t, float* re, float* im) {
+    const int kap = t >> 6, n3 = (t >> 3) & 7, n4 = t & 7;
+    C2 v[8];
+#pragma unroll
+    for (int r = 0; r < 8; ++r) v[r] = lds2(re, im, slot13(kap, brev<8>(r), n3, n4));
+    dit8(v);
+    // conj twiddle of P1: w_M^(-(n2*64 + j0) k1), j0 = n3*8 + n4, k1 = 2kap (A), 2kap+1 (B)
+    const int j0 = n3 * 8 + n4;
+    const float2 ca = twiddle<M13>(j0 * 2 * kap), cb = twiddle<M13>(j0 * (2 * kap + 1));
+    const float2 sa = twiddle<64>(kap), sb = twiddle<128>(2 * kap + 1);
+    C2 tw[8];
+    powers8(C2{pack(ca.x, cb.x), pack(ca.y, cb.y)}, C2{pack(sa.x, sb.x), pack(sa.y, sb.y)}, tw);
+#pragma unroll
+    for (int n2 = 0; n2 < 8; ++n2) sts2(re, im, slot13(kap, n2, n3, n4), cmul_conj(v[n2], tw[n2]));
+}
+
+// x[n1] = unnormalised inverse at n = n1*512 + t
+__device__ __forceinline__ void p1_inv(float2 (&x)[16], int t, const float* re, const float* im) {
+    const int n2 = t >> 6, n3 = (t >> 3) & 7, n4 = t & 7;
+    C2 v[8];
+#pragma unroll
+    for (int r = 0; r < 8; ++r) v[r] = lds2(re, im, slot13(brev<8>(r), n2, n3, n4));
+    dit8(v);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        float2 s, d;
+        unpack(v[i].r, s.x, d.x);
+        unpack(v[i].i, s.y, d.y);
+        switch (i) {      // d *= conj(w16^i)
+            case 0: break;
+            case 1: d = mul_w32<2, true>(d); break;
+            case 2: d = mul_w32<4, true>(d); break;
+            case 3: d = mul_w32<6, true>(d); break;
+            case 4: d = mul_w32<8, true>(d); break;
+            case 5: d = mul_w32<10, true>(d); break;
+            case 6: d = mul_w32<12, true>(d); break;
+            default: d = mul_w32<14, true>(d); break;
+        }
+        x[i] = amplfi::cadd(s, d);
+        x[i + 8] = amplfi::csub(s, d);
+    }
+}
+
+}  // namespace v2
+}  // namespace amplfi
