@@ -74,6 +74,7 @@ struct IwArgs {
     int n_det;
     float two_fs;
     float inv_tseg;
+    int prefetch_ahead;       // units ahead whose noise segment is prefetched into L2 (packed kernel)
 };
 
 // inject_whiten13.cu (packed 4-pass kernel for n = 16384)

@@ -21,7 +21,9 @@ __device__ __forceinline__ u64 add2(u64 a, u64 b) { u64 r; asm("add.rn.f32x2 %0,
 __device__ __forceinline__ u64 sub2(u64 a, u64 b) { u64 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ u64 mul2(u64 a, u64 b) { u64 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
 __device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c) { u64 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
-__device__ __forceinline__ u64 neg2(u64 a) { return a ^ 0x8000000080000000ull; }
+// negation written per half so that ptxas folds it into the consumer's operand modifier (-R.F32x2) instead of
+// two LOP3 on the 64-bit pair
+__device__ __forceinline__ u64 neg2(u64 a) { float lo, hi; unpack(a, lo, hi); return pack(-lo, -hi); }
 __device__ __forceinline__ u64 bcast(float s) { return pack(s, s); }
 
 struct C2 { u64 r, i; };          // two complex numbers: (A.re, B.re), (A.im, B.im)

@@ -219,6 +219,7 @@ int launch_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
     a.h_det = reinterpret_cast<const float2*>(h_det);
     a.h0 = p->h0; a.coef = p->coef; a.resp = p->resp; a.filt = p->filt; a.out = out;
     a.n_det = p->n_det; a.two_fs = (float)(2.0 * p->fs); a.inv_tseg = (float)(1.0 / p->t_seg);
+    a.prefetch_ahead = 2 * p->sm_count;
     const int mode = h_det != nullptr ? MODE_HDET : (fused ? MODE_FUSED : MODE_NONE);
     const int units = batch * p->n_det;
     switch (p->logm) {

@@ -32,6 +32,27 @@ __global__ void __launch_bounds__(T13, 2) inject_whiten13_kernel(const IwArgs a,
         x = a.noise + (size_t)unit * N;
     }
 
+    // L2 prefetch of the segment a CTA one wave later will gather (one bulk instruction for the whole 64 KB):
+    // the head-of-CTA loads then hit L2 instead of waiting on HBM.
+    if (t == 0) {
+        const int nu = unit + a.prefetch_ahead;
+        if (nu < units) {
+            const float* nx;
+            bool ok = true;
+            if (a.offsets != nullptr) {
+                const long noff = a.offsets[nu];
+                ok = noff >= 0 && noff + N <= a.strip_len;
+                nx = a.noise + (size_t)(nu % a.n_det) * a.strip_len + noff;
+            } else {
+                nx = a.noise + (size_t)nu * N;
+            }
+            if (ok) {
+                const size_t p0 = reinterpret_cast<size_t>(nx) & ~(size_t)15;
+                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p0), "r"(N * 4) : "memory");
+            }
+        }
+    }
+
     // ---- a-6 forward real FFT of the packed sequence z[m] = x[2m] + i x[2m+1] ----
     {
         float2 z[16];
@@ -107,8 +128,61 @@ __global__ void __launch_bounds__(T13, 2) inject_whiten13_kernel(const IwArgs a,
         unpack(v[r].i, za[r].y, zb[r].y);
     }
     if (t != 0) {
+        // bins k = t + 1024 k4 (half A) and M - k (half B), k4 = 0..7.
+        // split twiddle w_N^k = w_N^t * w_16^k4: one sincos and compile-time rotations.
+        const float2 wt = twiddle<N>(t);
+        float2 wk[8];
+        wk[0] = wt;
+        wk[1] = mul_w32<2, false>(wt);
+        wk[2] = mul_w32<4, false>(wt);
+        wk[3] = mul_w32<6, false>(wt);
+        wk[4] = mul_w32<8, false>(wt);
+        wk[5] = mul_w32<10, false>(wt);
+        wk[6] = mul_w32<12, false>(wt);
+        wk[7] = mul_w32<14, false>(wt);
+        // projection factors C exp(-2 pi i k dt/T) by recurrence over k4 (both halves in one packed chain):
+        //   A: C e(t) e(1024)^k4,  B: C e(M) conj(e(t)) conj(e(1024))^k4,  e(j) = exp(-2 pi i j delta)
+        C2 ph[8];
+        if (MODE == MODE_FUSED) {
+            auto unit_phase = [&](float turns) {
+                turns -= rintf(turns);
+                float s, co;
+                __sincosf(turns * -6.283185307179586f, &s, &co);
+                return make_float2(co, s);
+            };
+            const float2 et = unit_phase((float)t * delta);
+            const float2 es = unit_phase(1024.0f * delta);
+            const float2 em = unit_phase((float)M * delta);
+            const float2 cc = make_float2(cre, cim);
+            const float2 ca = amplfi::cmul(cc, et);
+            const float2 cb = amplfi::cmul_conj(amplfi::cmul(cc, em), et);
+            powers8(C2{pack(ca.x, cb.x), pack(ca.y, cb.y)}, C2{pack(es.x, es.x), pack(es.y, -es.y)}, ph);
+        }
 #pragma unroll
-        for (int r = 0; r < 8; ++r) do_pair(t + 1024 * brev<8>(r), za[r], zb[7 - r]);
+        for (int r = 0; r < 8; ++r) {
+            const int k4 = brev<8>(r);
+            const int k = t + 1024 * k4;
+            float2& pa = za[r];
+            float2& pb = zb[7 - r];
+            float2 xa, xb;
+            split_pair(pa, pb, wk[k4], xa, xb);
+            if (MODE == MODE_HDET) {
+                inject(k, xa);
+                inject(M - k, xb);
+            } else if (MODE == MODE_FUSED) {
+                const float2 ha = __ldg(hsrc + k), hb = __ldg(hsrc + M - k);
+                float ar, br, ai, bi;
+                unpack(ph[k4].r, ar, br);
+                unpack(ph[k4].i, ai, bi);
+                xa.x = fmaf(ha.x, ar, fmaf(-ha.y, ai, xa.x));
+                xa.y = fmaf(ha.x, ai, fmaf(ha.y, ar, xa.y));
+                xb.x = fmaf(hb.x, br, fmaf(-hb.y, bi, xb.x));
+                xb.y = fmaf(hb.x, bi, fmaf(hb.y, br, xb.y));
+            }
+            const float fa = __ldg(filt + k), fb = __ldg(filt + M - k);
+            xa.x *= fa; xa.y *= fa; xb.x *= fb; xb.y *= fb;
+            merge_pair(xa, xb, wk[k4], pa, pb);
+        }
     } else {
         {   // Z[0] carries the DC and Nyquist bins of the real transform
             float x0 = 2.0f * (za[0].x + za[0].y), xm = 2.0f * (za[0].x - za[0].y);
