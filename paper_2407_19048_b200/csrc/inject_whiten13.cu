@@ -127,22 +127,21 @@ __global__ void __launch_bounds__(T13, 2) inject_whiten13_kernel(const IwArgs a,
         unpack(v[r].r, za[r].x, zb[r].x);
         unpack(v[r].i, za[r].y, zb[r].y);
     }
-    if (t != 0) {
+    // Thread 0 holds the two self-paired butterflies (klow 0: bins 1024 q, with DC/Nyquist in Z[0]; klow 512: bins
+    // 512 + 1024 q).  It parks them in a scratch row; nine lanes of warp 0 process those bins after the generic
+    // section (which thread 0 executes on values that are then overwritten), so no warp runs a long divergent path.
+    __shared__ float2 sc[16];
+    if (t == 0) {
+#pragma unroll
+        for (int r = 0; r < 8; ++r) { sc[brev<8>(r)] = za[r]; sc[8 + brev<8>(r)] = zb[r]; }
+    }
+    {
         // bins k = t + 1024 k4 (half A) and M - k (half B), k4 = 0..7.
         // split twiddle w_N^k = w_N^t * w_16^k4: one sincos and compile-time rotations.
         const float2 wt = twiddle<N>(t);
-        float2 wk[8];
-        wk[0] = wt;
-        wk[1] = mul_w32<2, false>(wt);
-        wk[2] = mul_w32<4, false>(wt);
-        wk[3] = mul_w32<6, false>(wt);
-        wk[4] = mul_w32<8, false>(wt);
-        wk[5] = mul_w32<10, false>(wt);
-        wk[6] = mul_w32<12, false>(wt);
-        wk[7] = mul_w32<14, false>(wt);
         // projection factors C exp(-2 pi i k dt/T) by recurrence over k4 (both halves in one packed chain):
         //   A: C e(t) e(1024)^k4,  B: C e(M) conj(e(t)) conj(e(1024))^k4,  e(j) = exp(-2 pi i j delta)
-        C2 ph[8];
+        C2 ph, st;
         if (MODE == MODE_FUSED) {
             auto unit_phase = [&](float turns) {
                 turns -= rintf(turns);
@@ -156,57 +155,73 @@ __global__ void __launch_bounds__(T13, 2) inject_whiten13_kernel(const IwArgs a,
             const float2 cc = make_float2(cre, cim);
             const float2 ca = amplfi::cmul(cc, et);
             const float2 cb = amplfi::cmul_conj(amplfi::cmul(cc, em), et);
-            powers8(C2{pack(ca.x, cb.x), pack(ca.y, cb.y)}, C2{pack(es.x, es.x), pack(es.y, -es.y)}, ph);
+            ph = C2{pack(ca.x, cb.x), pack(ca.y, cb.y)};
+            st = C2{pack(es.x, es.x), pack(es.y, -es.y)};
         }
 #pragma unroll
-        for (int r = 0; r < 8; ++r) {
-            const int k4 = brev<8>(r);
+        for (int k4 = 0; k4 < 8; ++k4) {
+            const int r = brev<8>(k4);
             const int k = t + 1024 * k4;
+            float2 w = wt;
+            switch (k4) {
+                case 0: break;
+                case 1: w = mul_w32<2, false>(wt); break;
+                case 2: w = mul_w32<4, false>(wt); break;
+                case 3: w = mul_w32<6, false>(wt); break;
+                case 4: w = mul_w32<8, false>(wt); break;
+                case 5: w = mul_w32<10, false>(wt); break;
+                case 6: w = mul_w32<12, false>(wt); break;
+                default: w = mul_w32<14, false>(wt); break;
+            }
             float2& pa = za[r];
             float2& pb = zb[7 - r];
             float2 xa, xb;
-            split_pair(pa, pb, wk[k4], xa, xb);
+            split_pair(pa, pb, w, xa, xb);
             if (MODE == MODE_HDET) {
                 inject(k, xa);
                 inject(M - k, xb);
             } else if (MODE == MODE_FUSED) {
                 const float2 ha = __ldg(hsrc + k), hb = __ldg(hsrc + M - k);
                 float ar, br, ai, bi;
-                unpack(ph[k4].r, ar, br);
-                unpack(ph[k4].i, ai, bi);
+                unpack(ph.r, ar, br);
+                unpack(ph.i, ai, bi);
                 xa.x = fmaf(ha.x, ar, fmaf(-ha.y, ai, xa.x));
                 xa.y = fmaf(ha.x, ai, fmaf(ha.y, ar, xa.y));
                 xb.x = fmaf(hb.x, br, fmaf(-hb.y, bi, xb.x));
                 xb.y = fmaf(hb.x, bi, fmaf(hb.y, br, xb.y));
+                if (k4 < 7) ph = cmul(ph, st);
             }
             const float fa = __ldg(filt + k), fb = __ldg(filt + M - k);
             xa.x *= fa; xa.y *= fa; xb.x *= fb; xb.y *= fb;
-            merge_pair(xa, xb, wk[k4], pa, pb);
+            merge_pair(xa, xb, w, pa, pb);
         }
-    } else {
-        {   // Z[0] carries the DC and Nyquist bins of the real transform
-            float x0 = 2.0f * (za[0].x + za[0].y), xm = 2.0f * (za[0].x - za[0].y);
+    }
+    if (t < 32) {
+        __syncwarp();
+        if (t == 0) {       // Z[0] carries the DC and Nyquist bins of the real transform
+            const float2 z0 = sc[0];
+            float x0 = 2.0f * (z0.x + z0.y), xm = 2.0f * (z0.x - z0.y);
             if (MODE == MODE_HDET) {
                 x0 = fmaf(a.two_fs, __ldg(hsrc).x, x0);
                 xm = fmaf(a.two_fs, __ldg(hsrc + M).x, xm);
             }
             const float y0 = x0 * __ldg(filt), ym = xm * __ldg(filt + M);
-            za[0] = make_float2(y0 + ym, y0 - ym);
+            sc[0] = make_float2(y0 + ym, y0 - ym);
+        } else if (t < 9) {
+            // t = 1..3: (A[q], A[8-q]), k = 1024 q;  t = 4: A[4] with itself, k = M/2;
+            // t = 5..8: (B[q], B[7-q]), q = t - 5, k = 512 + 1024 q
+            const int ia = t <= 4 ? t : 3 + t, ib = t <= 4 ? 8 - t : 20 - t;
+            const int k = t <= 4 ? 1024 * t : 512 + 1024 * (t - 5);
+            float2 pa = sc[ia], pb = sc[ib];
+            do_pair(k, pa, pb);
+            sc[ia] = pa;
+            if (ib != ia) sc[ib] = pb;
         }
-        {   // k = M/2 pairs with itself (k4 = 4 -> register brev(4) = 1)
-            const int k = M / 2;
-            const float2 w = twiddle<N>(k);
-            float2 xa, xb, z2;
-            split_pair(za[1], za[1], w, xa, xb);
-            inject(k, xa);
-            const float fa = __ldg(filt + k);
-            xa.x *= fa; xa.y *= fa;
-            merge_pair(xa, xa, w, za[1], z2);
+        __syncwarp();
+        if (t == 0) {
+#pragma unroll
+            for (int r = 0; r < 8; ++r) { za[r] = sc[brev<8>(r)]; zb[r] = sc[8 + brev<8>(r)]; }
         }
-#pragma unroll
-        for (int q = 1; q < 4; ++q) do_pair(1024 * q, za[brev<8>(q)], za[brev<8>(8 - q)]);
-#pragma unroll
-        for (int q = 0; q < 4; ++q) do_pair(512 + 1024 * q, zb[brev<8>(q)], zb[brev<8>(7 - q)]);
     }
 #pragma unroll
     for (int r = 0; r < 8; ++r) v[r] = C2{pack(za[r].x, zb[r].x), pack(za[r].y, zb[r].y)};
