@@ -30,7 +30,8 @@ struct amplfi_plan {
     amplfi::WfCoef* coef;  // [max_batch]
     amplfi::DetResp* resp; // [max_batch * n_det]
     float2* h0;            // [max_batch * n_bins]   fused path: 2 fs h0
-    float* filt;           // [n_det * n_bins]       whitening filter incl. 1/(2n)
+    float* filt;           // [n_det * filt_stride]  whitening filter incl. 1/(2n); rows padded to 16 B
+    int filt_stride;       // n_bins rounded up to a multiple of 4
     float* welch_part;     // [n_det * max_seg * (nperseg/2+1)]
     int welch_max_seg;
     int* d_det_ids;        // [3]
@@ -69,7 +70,8 @@ struct IwArgs {
     const float2* h0;         // MODE_FUSED: [B, K] (2 fs h0)
     const WfCoef* coef;
     const DetResp* resp;
-    const float* filt;        // [D, K]
+    const float* filt;        // [D, filt_stride]
+    int filt_stride;
     float* out;               // [B, D, N]
     int n_det;
     float two_fs;

@@ -111,7 +111,8 @@ int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_
     if (!rc) rc = dev_alloc(&p->coef, (size_t)max_batch);
     if (!rc) rc = dev_alloc(&p->resp, (size_t)max_batch * n_det);
     if (!rc) rc = dev_alloc(&p->h0, (size_t)max_batch * p->n_bins);
-    if (!rc) rc = dev_alloc(&p->filt, (size_t)n_det * p->n_bins);
+    p->filt_stride = (p->n_bins + 3) & ~3;
+    if (!rc) rc = dev_alloc(&p->filt, (size_t)n_det * p->filt_stride);
     if (!rc) rc = dev_alloc(&p->d_det_ids, (size_t)3);
     if (!rc && nperseg) rc = dev_alloc(&p->welch_part, (size_t)n_det * p->welch_max_seg * (nperseg / 2 + 1));
     if (!rc) {

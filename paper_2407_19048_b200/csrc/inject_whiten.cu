@@ -14,12 +14,12 @@ namespace amplfi {
 // ---- whitening filter on the segment grid: w[k] = sqrt(2/(fs S)) / (2N) inside the band, else 0 ----
 // psd holds S * 2^140, so sqrt(2/(fs S)) = 2^70 * rsqrt(fs * psd / 2).
 __global__ void filter_kernel(const float* __restrict__ psd, int n_psd, int n_bins, int ratio, float fs, float norm,
-                              int k_lo, int k_hi, float* __restrict__ filt) {
+                              int k_lo, int k_hi, float* __restrict__ filt, int filt_stride) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     const int d = blockIdx.y;
-    if (k >= n_bins) return;
+    if (k >= filt_stride) return;
     float w = 0.f;
-    if (k >= k_lo && k <= k_hi) {
+    if (k >= k_lo && k <= k_hi && k < n_bins) {
         const float* s = psd + (size_t)d * n_psd;
         float sv;
         if (ratio == 1) {
@@ -32,7 +32,7 @@ __global__ void filter_kernel(const float* __restrict__ psd, int n_psd, int n_bi
         }
         w = rsqrtf(0.5f * fs * sv) * norm;
     }
-    filt[(size_t)d * n_bins + k] = w;
+    filt[(size_t)d * filt_stride + k] = w;
 }
 
 int launch_filter(const amplfi_plan* p, const float* psd, int n_psd, double f_lo, double f_hi, cudaStream_t st) {
@@ -46,8 +46,9 @@ int launch_filter(const amplfi_plan* p, const float* psd, int n_psd, double f_lo
     if (k_lo < 0) k_lo = 0;
     if (k_hi > p->n_bins - 1) k_hi = p->n_bins - 1;
     const float norm = (float)(1180591620717411303424.0 / (2.0 * (double)p->n));      // 2^70 / (2N)
-    dim3 grid((p->n_bins + 255) / 256, p->n_det);
-    filter_kernel<<<grid, 256, 0, st>>>(psd, n_psd, p->n_bins, ratio, (float)p->fs, norm, (int)k_lo, (int)k_hi, p->filt);
+    dim3 grid((p->filt_stride + 255) / 256, p->n_det);
+    filter_kernel<<<grid, 256, 0, st>>>(psd, n_psd, p->n_bins, ratio, (float)p->fs, norm, (int)k_lo, (int)k_hi, p->filt,
+                                        p->filt_stride);
     count_launch();
     return check_launch("filter_kernel");
 }
@@ -108,7 +109,7 @@ __global__ void __launch_bounds__(Fft<LOGM>::T) inject_whiten_kernel(const IwArg
     F::pass_c_fwd(klow_b, vb, sm);
 
     // ---- a-7 inject, a-8 whiten + band-limit (registers) ----
-    const float* filt = a.filt + (size_t)d * K;
+    const float* filt = a.filt + (size_t)d * a.filt_stride;
     const float2* hsrc = nullptr;
     int w_lo = 1, w_hi = 0;
     float cre = 0.f, cim = 0.f, delta = 0.f;
@@ -217,7 +218,7 @@ int launch_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
     IwArgs a;
     a.noise = noise; a.offsets = offsets; a.strip_len = strip_len;
     a.h_det = reinterpret_cast<const float2*>(h_det);
-    a.h0 = p->h0; a.coef = p->coef; a.resp = p->resp; a.filt = p->filt; a.out = out;
+    a.h0 = p->h0; a.coef = p->coef; a.resp = p->resp; a.filt = p->filt; a.filt_stride = p->filt_stride; a.out = out;
     a.n_det = p->n_det; a.two_fs = (float)(2.0 * p->fs); a.inv_tseg = (float)(1.0 / p->t_seg);
     a.prefetch_ahead = 2 * p->sm_count;
     const int mode = h_det != nullptr ? MODE_HDET : (fused ? MODE_FUSED : MODE_NONE);

@@ -79,7 +79,7 @@ __global__ void __launch_bounds__(T13, 2) inject_whiten13_kernel(const IwArgs a,
     p4_fwd(klow_a, klow_b, v, re, im);
 
     // ---- a-7 inject, a-8 whiten + band-limit (registers) ----
-    const float* filt = a.filt + (size_t)d * K;
+    const float* filt = a.filt + (size_t)d * a.filt_stride;
     const float2* hsrc = nullptr;
     int w_lo = 1, w_hi = 0;
     float cre = 0.f, cim = 0.f, delta = 0.f;

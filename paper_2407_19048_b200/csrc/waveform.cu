@@ -49,34 +49,41 @@ int launch_prepare(const amplfi_plan* p, int approximant, int batch, const doubl
 }
 
 // ---- materialised polarisations: hp = (1+cos^2 i)/2 h0, hc = -i cos i h0 ----
+// gridDim.x CTAs share one sample and take its 256-bin chunks round-robin; the coefficient struct is staged once
+// per CTA and chunks entirely outside the band [k_lo, k_hi] (common: heavy systems stop at a few hundred Hz) are
+// zero-filled without touching the tables.
+#define WF_SLICES 2
 template <bool POL>
-__global__ void __launch_bounds__(256) waveform_kernel(const WfCoef* __restrict__ coef, const double* __restrict__ tab_ci,
+__global__ void __launch_bounds__(256, 4) waveform_kernel(const WfCoef* __restrict__ coef, const double* __restrict__ tab_ci,
                                                        const double* __restrict__ tab_lnk, int n_bins,
                                                        float2* __restrict__ out_a, float2* __restrict__ out_b) {
     const int b = blockIdx.y;
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
     __shared__ WfCoef c;
-    // every thread reads the same struct; stage it once per CTA
     {
         const int* src = reinterpret_cast<const int*>(coef + b);
         int* dst = reinterpret_cast<int*>(&c);
-        for (int i = threadIdx.x; i < (int)(sizeof(WfCoef) / sizeof(int)); i += blockDim.x) dst[i] = src[i];
+        if (threadIdx.x < (int)(sizeof(WfCoef) / sizeof(int))) dst[threadIdx.x] = src[threadIdx.x];
     }
     __syncthreads();
-    if (k >= n_bins) return;
-    float2 h = make_float2(0.f, 0.f);
-    if (c.valid && k >= c.k_lo && k <= c.k_hi) h = eval_h0(c, k, tab_ci[k], tab_lnk[k]);
-    const size_t idx = (size_t)b * n_bins + k;
-    if (POL) {
-        out_a[idx] = make_float2(c.pol_p * h.x, c.pol_p * h.y);
-        out_b[idx] = make_float2(c.pol_c * h.y, -c.pol_c * h.x);     // -i c (x + i y) = c y - i c x
-    } else {
-        out_a[idx] = h;
+    const int k_lo = c.valid ? c.k_lo : 1, k_hi = c.valid ? c.k_hi : 0;
+    float2* oa = out_a + (size_t)b * n_bins;
+    float2* ob = POL ? out_b + (size_t)b * n_bins : nullptr;
+    for (int kc = blockIdx.x * 256; kc < n_bins; kc += 256 * gridDim.x) {
+        const int k = kc + threadIdx.x;
+        if (k >= n_bins) break;
+        float2 h = make_float2(0.f, 0.f);
+        if (k >= k_lo && k <= k_hi) h = eval_h0(c, k, tab_ci[k], tab_lnk[k]);
+        if (POL) {
+            oa[k] = make_float2(c.pol_p * h.x, c.pol_p * h.y);
+            ob[k] = make_float2(c.pol_c * h.y, -c.pol_c * h.x);     // -i c (x + i y) = c y - i c x
+        } else {
+            oa[k] = h;
+        }
     }
 }
 
 int launch_waveform_pol(const amplfi_plan* p, int batch, float* hp, float* hc, cudaStream_t st) {
-    dim3 grid((p->n_bins + 255) / 256, batch);
+    dim3 grid(WF_SLICES, batch);
     waveform_kernel<true><<<grid, 256, 0, st>>>(p->coef, p->tab_ci, p->tab_lnk, p->n_bins,
                                                 reinterpret_cast<float2*>(hp), reinterpret_cast<float2*>(hc));
     count_launch();
@@ -84,7 +91,7 @@ int launch_waveform_pol(const amplfi_plan* p, int batch, float* hp, float* hc, c
 }
 
 int launch_waveform_h0(const amplfi_plan* p, int batch, cudaStream_t st) {
-    dim3 grid((p->n_bins + 255) / 256, batch);
+    dim3 grid(WF_SLICES, batch);
     waveform_kernel<false><<<grid, 256, 0, st>>>(p->coef, p->tab_ci, p->tab_lnk, p->n_bins, p->h0, nullptr);
     count_launch();
     return check_launch("waveform_kernel<h0>");

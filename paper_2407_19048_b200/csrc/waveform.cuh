@@ -341,10 +341,14 @@ __device__ __forceinline__ float2 eval_h0(const WfCoef& c, int k, double ci, dou
         ph = fma(c.b_ln, lnk, ph);
         ph = fma(c.b_m9, ci3 * ci3 * ci3, ph);
     } else {
-        const double q4 = sqrt(sqrt(kd));             // k^(1/4)
+        // k^(3/4) = k * k^(-1/4): fp32 seed (two MUFU) and one Newton step in fp64 (relative error ~1e-13),
+        // instead of two software fp64 square roots
+        const double y0 = (double)rsqrtf(sqrtf((float)k));
+        const double y2 = y0 * y0;
+        const double y1 = fma(0.25 * y0, fma(-kd, y2 * y2, 1.0), y0);
         ph = fma(c.lin3, kd, c.c03);
         ph = fma(c.r_m3, ci2 * ci, ph);
-        ph = fma(c.r_34, q4 * q4 * q4, ph);
+        ph = fma(c.r_34, kd * y1, ph);
         ph += (double)(c.r_at * atanf(((float)k - c.at_k0) * c.at_invw));
     }
     ph -= rint(ph);                                   // turns in [-1/2, 1/2]
