@@ -35,6 +35,8 @@ struct amplfi_plan {
     float* welch_part;     // [n_det * max_seg * (nperseg/2+1)]
     int welch_max_seg;
     int* d_det_ids;        // [3]
+    float2* long_spec;     // n = 65536 only: sub-spectra of one chunk of units [long_chunk, 2, 16392] (L2-resident)
+    int long_chunk;        // units per chunk
     // optional device timing of the dominant kernel (amplfi_plan_set_timing)
     int timing;
     int ev_count;
@@ -87,5 +89,10 @@ int launch_filter(const amplfi_plan* p, const float* psd, int n_psd, double f_lo
 int launch_inject_whiten(const amplfi_plan* p, int batch, const float* noise, const long* offsets,
                          long strip_len, const float* h_det, int fused, float* out, cudaStream_t st);
 int setup_inject_whiten_attrs();
+
+// inject_whiten_long.cu (n = 65536: decimation by two around the 32768-sample transform)
+size_t long_scratch_floats2(int chunk_units);
+int launch_inject_whiten_long(const amplfi_plan* p, int batch, const float* noise, const long* offsets, long strip_len,
+                              const float* h_det, int fused, float* out, cudaStream_t st);
 
 }  // namespace amplfi

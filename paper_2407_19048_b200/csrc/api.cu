@@ -114,6 +114,10 @@ int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_
     p->filt_stride = (p->n_bins + 3) & ~3;
     if (!rc) rc = dev_alloc(&p->filt, (size_t)n_det * p->filt_stride);
     if (!rc) rc = dev_alloc(&p->d_det_ids, (size_t)3);
+    if (!rc && p->logm == 15) {
+        p->long_chunk = sms > 0 ? sms : 148;          // 2 CTAs per unit: two full waves of one CTA per SM; 39 MB of spectra
+        rc = dev_alloc(&p->long_spec, amplfi::long_scratch_floats2(p->long_chunk));
+    }
     if (!rc && nperseg) rc = dev_alloc(&p->welch_part, (size_t)n_det * p->welch_max_seg * (nperseg / 2 + 1));
     if (!rc) {
         e = cudaMemcpy(p->pd_table, kPdTable, sizeof(kPdTable), cudaMemcpyHostToDevice);
@@ -161,7 +165,7 @@ void amplfi_plan_destroy(amplfi_plan* p) {
     if (p->ev_start[0] != nullptr)
         for (int i = 0; i < AMPLFI_TIMING_RING; ++i) { cudaEventDestroy(p->ev_start[i]); cudaEventDestroy(p->ev_stop[i]); }
     cudaFree(p->tab_ci); cudaFree(p->tab_lnk); cudaFree(p->pd_table); cudaFree(p->coef); cudaFree(p->resp);
-    cudaFree(p->h0); cudaFree(p->filt); cudaFree(p->welch_part); cudaFree(p->d_det_ids);
+    cudaFree(p->h0); cudaFree(p->filt); cudaFree(p->welch_part); cudaFree(p->d_det_ids); cudaFree(p->long_spec);
     delete p;
 }
 
@@ -218,7 +222,7 @@ int amplfi_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
     const bool fused = (h_det == nullptr && params != nullptr);
     if (fused && approximant != AMPLFI_TAYLORF2 && approximant != AMPLFI_IMRPHENOMD) { set_error("amplfi_inject_whiten: unknown approximant %d", approximant); return AMPLFI_ERR_INVALID_ARG; }
     if ((reinterpret_cast<size_t>(out) & 7) || (reinterpret_cast<size_t>(noise) & 3) || (reinterpret_cast<size_t>(h_det) & 7)) { set_error("amplfi_inject_whiten: out/h_det must be 8-byte aligned, noise 4-byte aligned"); return AMPLFI_ERR_ALIGNMENT; }
-    if (p->logm > 14) { set_error("amplfi_inject_whiten: n = %d not supported by this build", p->n); return AMPLFI_ERR_UNSUPPORTED_SIZE; }
+    if (p->logm > 15) { set_error("amplfi_inject_whiten: n = %d not supported by this build", p->n); return AMPLFI_ERR_UNSUPPORTED_SIZE; }
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     rc = launch_filter(p, psd, n_psd, f_lo, f_hi, st);
     if (rc) return rc;

@@ -285,6 +285,31 @@ def test_c3_parity_snr12():
     assert row_err(got, ref).max() <= TOL
 
 
+@pytest.mark.parametrize("mode", ["fused", "hdet", "none"])
+def test_c4_parity(mode):
+    # configs[4] shape (fs 4096, 16 s = 65536 samples, Welch 4 s windows from 128 s, PSD grid ratio 4) at reduced
+    # batch and strip; n = 65536 runs the decimated three-kernel path.  One offset is odd (unaligned gather).
+    wl = WL.make_c4(batch=6, strip_len=1 << 22)
+    wl.offsets[1, 2] |= 1
+    wl.offsets[2, 0] = wl.strip.shape[1] - wl.n
+    got, psd = run_inject_whiten(wl, mode)
+    ref = oracle_inject_whiten(wl, mode)
+    assert row_err(got, ref).max() <= TOL
+    assert row_err(got, oracle_inject_whiten(wl, mode, psd=psd)).max() <= TOL
+
+
+def test_c4_many_chunks_sampled_rows():
+    # more units than one L2-resident chunk (148 units): every chunk boundary is crossed; sampled rows vs the oracle
+    wl = WL.make_c4(batch=120, strip_len=1 << 22)
+    got, psd = run_inject_whiten(wl, "fused")
+    assert got.shape == (120, 3, 65536) and np.all(np.isfinite(got))
+    rows = np.array([0, 49, 50, 98, 99, 119])
+    sub = WL.Workload("c4s", len(rows), wl.det_ids, wl.fs, wl.n, wl.approximant, nperseg=wl.nperseg,
+                      params=wl.params[rows], strip=wl.strip, offsets=wl.offsets[rows], extra=wl.extra)
+    ref = oracle_inject_whiten(sub, "fused")
+    assert row_err(got[rows], ref).max() <= TOL
+
+
 @pytest.mark.parametrize("n,fs", [(1024, 2048.0), (2048, 2048.0), (4096, 4096.0), (32768, 4096.0)])
 def test_other_segment_lengths(n, fs):
     rng = np.random.Generator(np.random.Philox(n))
