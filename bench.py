@@ -40,6 +40,10 @@ def parse():
     ap.add_argument("--cpu-sample", type=int, default=256, help="samples of the batch the CPU oracle is timed on")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--config", default="c2", choices=["c2", "c3", "c4", "sweep"],
+                    help="c2 (default): the contract line.  c3: online latency p50/p99 over --runs seeded runs.  "
+                         "c4: bandwidth stress (batch 8192 x 3 x 65536).  sweep: segment length 1-16 s at 4096 Hz.")
+    ap.add_argument("--runs", type=int, default=1000)
     return ap.parse_args()
 
 
@@ -310,9 +314,115 @@ def run_b200(args):
         dist.destroy_process_group()
 
 
+# ------------------------------------------------------------------------------------------------
+# Other BASELINE.json configs: not the contract line; one JSON line per measurement
+# ------------------------------------------------------------------------------------------------
+
+def run_extra(args):
+    import torch
+    import paper_2407_19048_b200 as A
+    import workloads as WL
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the B200 arm has no CPU fallback")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    stream = torch.cuda.current_stream()
+    peak, peak_src = peaks()
+
+    def throughput(wl, steps, warmup):
+        B, D, N = wl.batch, wl.n_det, wl.n
+        plan = A.Plan(N, wl.fs, wl.det_ids, B, nperseg=wl.nperseg)
+        strip = torch.from_numpy(wl.strip).to(dev)
+        params = torch.from_numpy(wl.params).to(dev)
+        offsets = torch.from_numpy(wl.offsets).to(dev)
+        o, nb = wl.extra["bg_offset"], wl.extra["n_bg"]
+        bg = strip[:, o:o + nb]
+        psd = torch.empty((D, wl.nperseg // 2 + 1), dtype=torch.float32, device=dev)
+        out = torch.empty((B, D, N), dtype=torch.float32, device=dev)
+
+        def step():
+            A.amplfi_psd_welch(plan, bg, psd=psd, stream=stream)
+            A.amplfi_inject_whiten(plan, B, strip, psd, wl.f_lo, wl.f_hi, offsets=offsets, approximant=wl.approximant,
+                                   params=params, gmst=wl.gmst, out=out, stream=stream)
+        for _ in range(warmup):
+            step()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = A.launch_count()
+        e0.record(stream)
+        for _ in range(steps):
+            step()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / steps
+        assert bool(torch.isfinite(out[:: max(1, B // 16)]).all())
+        sps = B * D * N / (ms * 1e-3)
+        n_l = (A.launch_count() - l0) // steps
+        del plan, strip, out
+        torch.cuda.empty_cache()
+        return ms, sps, n_l
+
+    if args.config == "c3":
+        lat, snr = [], []
+        plan = A.Plan(16384, 2048.0, (0, 1, 2), 1, nperseg=8192)
+        psd = torch.empty((3, 4097), dtype=torch.float32, device=dev)
+        out = torch.empty((1, 3, 16384), dtype=torch.float32, device=dev)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for r in range(-3, args.runs):                               # three untimed warm-up runs
+            wl = WL.make_c3(run=max(r, 0))
+            bg = torch.from_numpy(wl.bg).to(dev)
+            noise = torch.from_numpy(wl.noise).to(dev)
+            params = torch.from_numpy(wl.params).to(dev)
+            torch.cuda.synchronize()
+            e0.record(stream)
+            A.amplfi_psd_welch(plan, bg, psd=psd, stream=stream)
+            A.amplfi_inject_whiten(plan, 1, noise, psd, wl.f_lo, wl.f_hi, approximant=wl.approximant, params=params,
+                                   gmst=wl.gmst, out=out, stream=stream)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            if r >= 0:
+                lat.append(e0.elapsed_time(e1) * 1e3)
+        lat = np.array(lat)
+        print(json.dumps({"metric": "online PSD+whiten device latency", "unit": "us", "higher_is_better": False,
+                          "p50": float(np.percentile(lat, 50)), "p99": float(np.percentile(lat, 99)),
+                          "mean": float(lat.mean()), "min": float(lat.min()), "max": float(lat.max()), "runs": len(lat),
+                          "dtype": "f32", "data": "synthetic",
+                          "config": {"workload": "c3 online-latency: batch 1 x H1+L1+V1, 8 s at 2048 Hz, Welch from the 128 s "
+                                                 "preceding background (4 s Hann, 50% overlap), IMRPhenomD injection; run r "
+                                                 "uses seed 0xA3D30003 + r; CUDA events around amplfi_psd_welch + "
+                                                 "amplfi_inject_whiten on one stream, inputs resident"}}))
+        return
+
+    if args.config == "c4":
+        wl = WL.make_c4(batch=8192)
+        ms, sps, n_l = throughput(wl, max(3, min(args.steps, 10)), 3)
+        print(json.dumps({"metric": METRIC.replace("2048 Hz", "4096 Hz"), "value": sps, "unit": UNIT, "ms_per_step": ms,
+                          "higher_is_better": True, "dtype": "f32", "data": "synthetic", "gpu_launches_per_step": int(n_l),
+                          "hbm_gbs_step": 8.0 * sps / 1e9, "frac_of_measured_hbm": 8.0 * sps / 1e9 / peak,
+                          "peak_source": peak_src,
+                          "config": {"workload": "c4 bandwidth stress: batch 8192 x H1+L1+V1, fs 4096 Hz, 16 s segments (65536), "
+                                                 "gathered from a [3, 2^26] strip, Welch from 128 s (4 s Hann), IMRPhenomD"}}))
+        return
+
+    # sweep: fixed total samples (2^27 per detector), segment length 1..16 s at 4096 Hz
+    for t_seg in (1.0, 2.0, 4.0, 8.0, 16.0):
+        n = int(t_seg * 4096)
+        batch = (1 << 27) // n
+        wl = WL.make_c4(batch=batch, t_seg=t_seg)
+        wl.nperseg = min(wl.nperseg, n)                              # Welch window no longer than the segment
+        ms, sps, n_l = throughput(wl, max(3, min(args.steps, 10)), 3)
+        flops = 2 * 2.5 * n * np.log2(n) * batch * 3                  # forward + inverse real transforms
+        print(json.dumps({"metric": "segment-length sweep", "t_seg": t_seg, "n": n, "batch": batch, "value": sps, "unit": UNIT,
+                          "ms_per_step": ms, "hbm_gbs_step": 8.0 * sps / 1e9, "frac_of_measured_hbm": 8.0 * sps / 1e9 / peak,
+                          "fft_gflops": flops / (ms * 1e-3) / 1e9, "gpu_launches_per_step": int(n_l), "dtype": "f32",
+                          "data": "synthetic"}))
+
+
 if __name__ == "__main__":
     a = parse()
     if a.impl == "reference":
         run_reference(a)
+    elif a.config != "c2":
+        run_extra(a)
     else:
         run_b200(a)
