@@ -199,9 +199,10 @@ def run_b200(args):
     stream = torch.cuda.current_stream()
 
     def step(p=params, off=offsets):
-        A.amplfi_psd_welch(plan, bg, psd=psd, stream=stream)
-        A.amplfi_inject_whiten(plan, B, strip, psd, wl.f_lo, wl.f_hi, offsets=off, approximant=wl.approximant,
-                               params=p, gmst=wl.gmst, out=out, stream=stream)
+        # one data-generation step = Welch PSD + waveform/projection/injection/whitening (one C-ABI call; the
+        # two-call form amplfi_psd_welch + amplfi_inject_whiten gives identical results, tests/test_gpu_parity.py)
+        A.amplfi_assemble_batch(plan, B, bg, strip, p, wl.f_lo, wl.f_hi, offsets=off, approximant=wl.approximant,
+                                gmst=wl.gmst, psd=psd, out=out, stream=stream)
 
     def barrier():
         torch.cuda.synchronize()

@@ -128,11 +128,27 @@ int amplfi_psd_welch(const amplfi_plan* plan, const float* bg, long n_bg, long r
  *   psd      [n_det, n_psd] fp32, S * 2^140; n_psd == K, or n_psd == (n/r)/2+1 for an integer r >= 1, in
  *            which case S is linearly interpolated in frequency onto the segment grid.
  *   out      [batch, n_det, n] fp32.
- * batch <= the plan's max_batch.  n = 2^16 needs a 2-CTA thread-block cluster per segment. */
+ * batch <= the plan's max_batch.  n = 2^16 is decimated by two around the 2^15-sample transform, the
+ * intermediate spectra of a chunk of segments staying in L2. */
 int amplfi_inject_whiten(const amplfi_plan* plan, int batch, const float* noise, const long* offsets,
                          long strip_len, const float* h_det, int approximant, const double* params,
                          double gmst, const float* psd, int n_psd, double f_lo, double f_hi,
                          float* out, void* stream);
+
+/* One whole data-generation step (PSD fit to the background, waveforms generated on the
+ * GPU, projected, injected into lazily loaded background chunks, batch whitened) = amplfi_psd_welch followed
+ * by the fused amplfi_inject_whiten (h_det == NULL, params != NULL), with identical results.  The PSD chain
+ * (Welch, filter) and the waveform chain (per-sample coefficients, h0 spectra) do not depend on each other, so
+ * they run concurrently: the PSD chain on a stream owned by the plan, forked from and joined back into
+ * `stream` with events; everything is ordered after prior work on `stream` and complete (in stream order)
+ * when the call's last kernel on `stream` is.
+ *   bg, n_bg, row_stride, noverlap, detrend as in amplfi_psd_welch;  psd [n_det, nperseg/2+1] receives the
+ *   estimate;  noise, offsets, strip_len, approximant, params (not NULL), gmst, f_lo, f_hi, out as in
+ *   amplfi_inject_whiten. */
+int amplfi_assemble_batch(const amplfi_plan* plan, int batch, const float* bg, long n_bg, long row_stride,
+                          int noverlap, int detrend, float* psd, const float* noise, const long* offsets,
+                          long strip_len, int approximant, const double* params, double gmst, double f_lo,
+                          double f_hi, float* out, void* stream);
 
 /* Device timing of the dominant kernel (the fused inject+whiten kernel).  With timing enabled every
  * amplfi_inject_whiten call brackets that kernel with CUDA events recorded on the caller's stream (up to

@@ -23,7 +23,7 @@ N_PARAMS = 11
 EXPORTS = ("amplfi_last_error", "amplfi_psd_scale", "amplfi_version", "amplfi_phenomd_table",
            "amplfi_plan_create", "amplfi_plan_destroy", "amplfi_waveform_fd", "amplfi_project",
            "amplfi_psd_welch", "amplfi_inject_whiten", "amplfi_launch_count", "amplfi_plan_set_timing",
-           "amplfi_plan_kernel_times")
+           "amplfi_plan_kernel_times", "amplfi_assemble_batch")
 
 
 class AmplfiError(RuntimeError):
@@ -65,6 +65,8 @@ def _load():
     lib.amplfi_psd_welch.argtypes = [vp, vp, i64, i64, i32, i32, i32, vp, vp]
     lib.amplfi_inject_whiten.restype = i32
     lib.amplfi_inject_whiten.argtypes = [vp, i32, vp, vp, i64, vp, i32, vp, dbl, vp, i32, dbl, dbl, vp, vp]
+    lib.amplfi_assemble_batch.restype = i32
+    lib.amplfi_assemble_batch.argtypes = [vp, i32, vp, i64, i64, i32, i32, vp, vp, vp, i64, i32, vp, dbl, dbl, dbl, vp, vp]
     return lib
 
 
@@ -213,3 +215,27 @@ def amplfi_inject_whiten(plan, batch, noise, psd, f_lo, f_hi, offsets=None, h_de
                                      _ptr(psd, torch.float32, "psd"), int(psd.shape[-1]), float(f_lo), float(f_hi),
                                      _ptr(out, torch.float32, "out"), _stream(stream)))
     return out
+
+
+def amplfi_assemble_batch(plan, batch, bg, noise, params, f_lo, f_hi, offsets=None, approximant=IMRPHENOMD, gmst=0.0,
+                          noverlap=None, detrend=1, psd=None, out=None, stream=None):
+    """One data-generation step: Welch PSD of bg [D, n_bg], then waveform generation, projection, injection into
+    noise (dense [B, D, N], or strip [D, L] with offsets [B, D]) and whitening -> (out [B, D, N], psd)."""
+    if noverlap is None:
+        noverlap = plan.nperseg // 2
+    if psd is None:
+        psd = torch.empty((plan.n_det, plan.nperseg // 2 + 1), dtype=torch.float32, device=bg.device)
+    if out is None:
+        out = torch.empty((batch, plan.n_det, plan.n), dtype=torch.float32, device=noise.device)
+    if bg.dim() != 2 or bg.shape[0] != plan.n_det or bg.stride(1) != 1:
+        raise ValueError("bg must be [n_det, n_bg] with unit stride along time (rows may be a window of a strip)")
+    if not bg.is_cuda or bg.dtype != torch.float32:
+        raise TypeError("bg must be a CUDA float32 tensor (no CPU fallback)")
+    row_stride = int(bg.stride(0)) if plan.n_det > 1 else int(bg.shape[1])
+    strip_len = int(noise.shape[-1]) if offsets is not None else 0
+    _check(_lib.amplfi_assemble_batch(plan._h, int(batch), ctypes.c_void_p(bg.data_ptr()), int(bg.shape[1]), row_stride,
+                                      int(noverlap), int(detrend), _ptr(psd, torch.float32, "psd"),
+                                      _ptr(noise, torch.float32, "noise"), _ptr(offsets, torch.int64, "offsets"),
+                                      strip_len, int(approximant), _ptr(params, torch.float64, "params"), float(gmst),
+                                      float(f_lo), float(f_hi), _ptr(out, torch.float32, "out"), _stream(stream)))
+    return out, psd

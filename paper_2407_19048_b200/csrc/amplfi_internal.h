@@ -37,6 +37,9 @@ struct amplfi_plan {
     int* d_det_ids;        // [3]
     float2* long_spec;     // n = 65536 only: sub-spectra of one chunk of units [long_chunk, 2, 16392] (L2-resident)
     int long_chunk;        // units per chunk
+    // amplfi_assemble_batch: PSD chain runs on `side`, forked from / joined into the caller's stream
+    cudaStream_t side;
+    cudaEvent_t ev_fork, ev_join;
     // optional device timing of the dominant kernel (amplfi_plan_set_timing)
     int timing;
     int ev_count;

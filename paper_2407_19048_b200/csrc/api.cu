@@ -124,6 +124,12 @@ int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_
         if (e == cudaSuccess) e = cudaMemcpy(p->d_det_ids, p->det_ids, sizeof(int) * 3, cudaMemcpyHostToDevice);
         if (e != cudaSuccess) { set_error("amplfi_plan_create: cudaMemcpy: %s", cudaGetErrorString(e)); rc = AMPLFI_ERR_CUDA; }
     }
+    if (!rc) {
+        e = cudaStreamCreateWithFlags(&p->side, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p->ev_join, cudaEventDisableTiming);
+        if (e != cudaSuccess) { set_error("amplfi_plan_create: stream/event: %s", cudaGetErrorString(e)); rc = AMPLFI_ERR_CUDA; }
+    }
     if (!rc) rc = launch_tables(p, nullptr);
     if (!rc) {
         e = cudaStreamSynchronize(nullptr);
@@ -164,6 +170,9 @@ void amplfi_plan_destroy(amplfi_plan* p) {
     if (p == nullptr) return;
     if (p->ev_start[0] != nullptr)
         for (int i = 0; i < AMPLFI_TIMING_RING; ++i) { cudaEventDestroy(p->ev_start[i]); cudaEventDestroy(p->ev_stop[i]); }
+    if (p->side) cudaStreamDestroy(p->side);
+    if (p->ev_fork) cudaEventDestroy(p->ev_fork);
+    if (p->ev_join) cudaEventDestroy(p->ev_join);
     cudaFree(p->tab_ci); cudaFree(p->tab_lnk); cudaFree(p->pd_table); cudaFree(p->coef); cudaFree(p->resp);
     cudaFree(p->h0); cudaFree(p->filt); cudaFree(p->welch_part); cudaFree(p->d_det_ids); cudaFree(p->long_spec);
     delete p;
@@ -236,6 +245,48 @@ int amplfi_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
     const bool timed = p->timing && p->ev_count < AMPLFI_TIMING_RING;
     if (timed) cudaEventRecord(mp->ev_start[p->ev_count], st);
     rc = launch_inject_whiten(p, batch, noise, offsets, strip_len, h_det, fused ? 1 : 0, out, st);
+    if (timed) { cudaEventRecord(mp->ev_stop[p->ev_count], st); mp->ev_count++; }
+    return rc;
+}
+
+int amplfi_assemble_batch(const amplfi_plan* p, int batch, const float* bg, long n_bg, long row_stride, int noverlap,
+                          int detrend, float* psd, const float* noise, const long* offsets, long strip_len,
+                          int approximant, const double* params, double gmst, double f_lo, double f_hi, float* out,
+                          void* stream) {
+    if (p == nullptr || bg == nullptr || psd == nullptr || noise == nullptr || params == nullptr || out == nullptr) {
+        set_error("amplfi_assemble_batch: null pointer");
+        return AMPLFI_ERR_INVALID_ARG;
+    }
+    if (p->nperseg == 0) { set_error("amplfi_assemble_batch: plan was created with nperseg = 0"); return AMPLFI_ERR_INVALID_ARG; }
+    if (batch < 1 || batch > p->max_batch) { set_error("amplfi_assemble_batch: batch %d outside [1, %d]", batch, p->max_batch); return AMPLFI_ERR_INVALID_ARG; }
+    if (n_bg < p->nperseg) { set_error("amplfi_assemble_batch: nperseg %d > n_bg %ld", p->nperseg, n_bg); return AMPLFI_ERR_UNSUPPORTED_SIZE; }
+    if (noverlap < 0 || noverlap >= p->nperseg || (detrend != 0 && detrend != 1)) { set_error("amplfi_assemble_batch: need 0 <= noverlap < nperseg, detrend in {0,1}"); return AMPLFI_ERR_INVALID_ARG; }
+    if (row_stride < n_bg) { set_error("amplfi_assemble_batch: row_stride %ld < n_bg %ld", row_stride, n_bg); return AMPLFI_ERR_INVALID_ARG; }
+    int rc = validate_band(p, f_lo, f_hi, "amplfi_assemble_batch");
+    if (rc) return rc;
+    if (offsets != nullptr && strip_len < p->n) { set_error("amplfi_assemble_batch: strip_len %ld < n %d", strip_len, p->n); return AMPLFI_ERR_INVALID_ARG; }
+    if (approximant != AMPLFI_TAYLORF2 && approximant != AMPLFI_IMRPHENOMD) { set_error("amplfi_assemble_batch: unknown approximant %d", approximant); return AMPLFI_ERR_INVALID_ARG; }
+    if ((reinterpret_cast<size_t>(out) & 7) || (reinterpret_cast<size_t>(noise) & 3)) { set_error("amplfi_assemble_batch: out must be 8-byte aligned, noise 4-byte aligned"); return AMPLFI_ERR_ALIGNMENT; }
+    const int n_psd = p->nperseg / 2 + 1;
+    if (((p->n / 2) % (n_psd - 1)) != 0) { set_error("amplfi_assemble_batch: nperseg %d does not divide n %d", p->nperseg, p->n); return AMPLFI_ERR_INVALID_ARG; }
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    amplfi_plan* mp = const_cast<amplfi_plan*>(p);
+    // fork: PSD chain on the plan's stream, waveform chain on the caller's
+    cudaError_t e = cudaEventRecord(mp->ev_fork, st);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(mp->side, mp->ev_fork, 0);
+    if (e != cudaSuccess) { set_error("amplfi_assemble_batch: fork: %s", cudaGetErrorString(e)); return AMPLFI_ERR_CUDA; }
+    rc = launch_welch(p, bg, n_bg, row_stride, noverlap, detrend, psd, mp->side);
+    if (!rc) rc = launch_filter(p, psd, n_psd, f_lo, f_hi, mp->side);
+    e = cudaEventRecord(mp->ev_join, mp->side);
+    if (!rc) rc = launch_prepare(p, approximant, batch, params, gmst, f_lo, f_hi, 2.0 * p->fs, nullptr, st);
+    if (!rc) rc = launch_waveform_h0(p, batch, st);
+    // join (always, so the side stream never runs past the call unobserved)
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(st, mp->ev_join, 0);
+    if (e != cudaSuccess) { set_error("amplfi_assemble_batch: join: %s", cudaGetErrorString(e)); return AMPLFI_ERR_CUDA; }
+    if (rc) return rc;
+    const bool timed = p->timing && p->ev_count < AMPLFI_TIMING_RING;
+    if (timed) cudaEventRecord(mp->ev_start[p->ev_count], st);
+    rc = launch_inject_whiten(p, batch, noise, offsets, strip_len, nullptr, 1, out, st);
     if (timed) { cudaEventRecord(mp->ev_stop[p->ev_count], st); mp->ev_count++; }
     return rc;
 }

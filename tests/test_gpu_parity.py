@@ -262,6 +262,23 @@ def test_c2_gather_parity_unaligned_offsets():
     assert row_err(got, ref).max() <= TOL
 
 
+def test_assemble_batch_equals_two_call_path():
+    # amplfi_assemble_batch overlaps the PSD chain and the waveform chain on two streams; results must be
+    # identical to amplfi_psd_welch followed by the fused amplfi_inject_whiten, and match the oracle
+    wl = WL.make_c2(batch=16, strip_len=1 << 20)
+    ref_gpu, psd_ref = run_inject_whiten(wl, "fused")
+    plan = A.Plan(wl.n, wl.fs, wl.det_ids, wl.batch, nperseg=wl.nperseg)
+    strip = dev(wl.strip)
+    o, nb = wl.extra["bg_offset"], wl.extra["n_bg"]
+    for _ in range(3):                                     # repeated calls reuse the plan's side stream and events
+        out, psd = A.amplfi_assemble_batch(plan, wl.batch, strip[:, o:o + nb], strip, dev(wl.params), wl.f_lo, wl.f_hi,
+                                           offsets=dev(wl.offsets), approximant=wl.approximant, gmst=wl.gmst)
+        torch.cuda.synchronize()
+        assert np.array_equal(out.cpu().numpy().astype(np.float64), ref_gpu)
+        assert np.array_equal(psd.cpu().numpy().astype(np.float64) / PSD_SCALE, psd_ref)
+    assert row_err(ref_gpu, oracle_inject_whiten(wl, "fused")).max() <= TOL
+
+
 def test_gather_out_of_range_offset_poisons_row_only():
     wl = WL.make_c2(batch=4, strip_len=1 << 18)
     wl.offsets[1, 0] = wl.strip.shape[1] - wl.n + 1
