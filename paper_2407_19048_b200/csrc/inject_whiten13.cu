@@ -8,13 +8,17 @@ namespace amplfi {
 
 using namespace v2;
 
-template <int MODE>
-__global__ void __launch_bounds__(T13, 2) inject_whiten13_kernel(const IwArgs a, int units) {
+// VT virtual threads (of the 512 the index algebra is written for) per physical thread: VT = 2 runs 256 threads with
+// 128 registers, trading thread-level for instruction-level parallelism (loads of one virtual thread overlap the
+// arithmetic of the other).
+template <int MODE, int VT>
+__global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwArgs a, int units) {
+    constexpr int TT = T13 / VT;
     constexpr int M = M13, N = N13, K = M13 + 1;
     extern __shared__ float smem13[];
     float* re = smem13;
     float* im = smem13 + M;
-    const int unit = blockIdx.x, t = threadIdx.x;
+    const int unit = blockIdx.x, tt = threadIdx.x;
     const int b = unit / a.n_det, d = unit - b * a.n_det;
 
     // ---- a-5 gather ----
@@ -24,7 +28,7 @@ __global__ void __launch_bounds__(T13, 2) inject_whiten13_kernel(const IwArgs a,
         const long off = a.offsets[unit];
         if (off < 0 || off + N > a.strip_len) {            // never read out of bounds: poison the row instead
             const float qnan = __int_as_float(0x7fc00000);
-            for (int i = t; i < N; i += T13) out[i] = qnan;
+            for (int i = tt; i < N; i += TT) out[i] = qnan;
             return;
         }
         x = a.noise + (size_t)d * a.strip_len + off;
@@ -34,7 +38,7 @@ __global__ void __launch_bounds__(T13, 2) inject_whiten13_kernel(const IwArgs a,
 
     // L2 prefetch of the segment a CTA one wave later will gather (one bulk instruction for the whole 64 KB):
     // the head-of-CTA loads then hit L2 instead of waiting on HBM.
-    if (t == 0) {
+    if (tt == 0) {
         const int nu = unit + a.prefetch_ahead;
         if (nu < units) {
             const float* nx;
@@ -55,25 +59,36 @@ __global__ void __launch_bounds__(T13, 2) inject_whiten13_kernel(const IwArgs a,
 
     // ---- a-6 forward real FFT of the packed sequence z[m] = x[2m] + i x[2m+1] ----
     {
-        float2 z[16];
+        float2 z[VT][16];
         if ((reinterpret_cast<size_t>(x) & 7) == 0) {
             const float2* x2 = reinterpret_cast<const float2*>(x);
 #pragma unroll
-            for (int n1 = 0; n1 < 16; ++n1) z[n1] = __ldcs(x2 + n1 * 512 + t);
+            for (int vt = 0; vt < VT; ++vt)
+#pragma unroll
+                for (int n1 = 0; n1 < 16; ++n1) z[vt][n1] = __ldcs(x2 + n1 * 512 + tt + vt * TT);
         } else {
 #pragma unroll
-            for (int n1 = 0; n1 < 16; ++n1) {
-                const int m = n1 * 512 + t;
-                z[n1] = make_float2(__ldg(x + 2 * m), __ldg(x + 2 * m + 1));
-            }
+            for (int vt = 0; vt < VT; ++vt)
+#pragma unroll
+                for (int n1 = 0; n1 < 16; ++n1) {
+                    const int m = n1 * 512 + tt + vt * TT;
+                    z[vt][n1] = make_float2(__ldg(x + 2 * m), __ldg(x + 2 * m + 1));
+                }
         }
-        p1_fwd(z, t, re, im);
+#pragma unroll
+        for (int vt = 0; vt < VT; ++vt) p1_fwd(z[vt], tt + vt * TT, re, im);
     }
     __syncthreads();
-    p2_fwd(t, re, im);
+#pragma unroll
+    for (int vt = 0; vt < VT; ++vt) p2_fwd(tt + vt * TT, re, im);
     __syncthreads();
-    p3_fwd(t, re, im);
+#pragma unroll
+    for (int vt = 0; vt < VT; ++vt) p3_fwd(tt + vt * TT, re, im);
     __syncthreads();
+    __shared__ float2 sc[16];
+#pragma unroll
+    for (int vt = 0; vt < VT; ++vt) {
+    const int t = tt + vt * TT;
     const int klow_a = t, klow_b = (t == 0) ? 512 : 1024 - t;
     C2 v[8];
     p4_fwd(klow_a, klow_b, v, re, im);
@@ -130,7 +145,6 @@ __global__ void __launch_bounds__(T13, 2) inject_whiten13_kernel(const IwArgs a,
     // Thread 0 holds the two self-paired butterflies (klow 0: bins 1024 q, with DC/Nyquist in Z[0]; klow 512: bins
     // 512 + 1024 q).  It parks them in a scratch row; nine lanes of warp 0 process those bins after the generic
     // section (which thread 0 executes on values that are then overwritten), so no warp runs a long divergent path.
-    __shared__ float2 sc[16];
     if (t == 0) {
 #pragma unroll
         for (int r = 0; r < 8; ++r) { sc[brev<8>(r)] = za[r]; sc[8 + brev<8>(r)] = zb[r]; }
@@ -228,30 +242,39 @@ __global__ void __launch_bounds__(T13, 2) inject_whiten13_kernel(const IwArgs a,
 
     // ---- a-9 inverse real FFT and store ----
     p4_inv(klow_a, klow_b, v, re, im);
+    }
     __syncthreads();
-    p3_inv(t, re, im);
+#pragma unroll
+    for (int vt = 0; vt < VT; ++vt) p3_inv(tt + vt * TT, re, im);
     __syncthreads();
-    p2_inv(t, re, im);
+#pragma unroll
+    for (int vt = 0; vt < VT; ++vt) p2_inv(tt + vt * TT, re, im);
     __syncthreads();
     {
-        float2 z[16];
-        p1_inv(z, t, re, im);
         float2* out2 = reinterpret_cast<float2*>(out);
 #pragma unroll
-        for (int n1 = 0; n1 < 16; ++n1) __stcs(out2 + n1 * 512 + t, z[n1]);
+        for (int vt = 0; vt < VT; ++vt) {
+            float2 z[16];
+            p1_inv(z, tt + vt * TT, re, im);
+#pragma unroll
+            for (int n1 = 0; n1 < 16; ++n1) __stcs(out2 + n1 * 512 + tt + vt * TT, z[n1]);
+        }
     }
 }
 
+#ifndef IW13_VT
+#define IW13_VT 2
+#endif
 template <int MODE>
 static int launch_iw13_t(const IwArgs& a, int units, cudaStream_t st) {
     static bool attr_done = false;
     const int smem = 2 * M13 * (int)sizeof(float);
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(inject_whiten13_kernel<MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        cudaError_t e = cudaFuncSetAttribute(inject_whiten13_kernel<MODE, IW13_VT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) { set_error("cudaFuncSetAttribute: %s", cudaGetErrorString(e)); return AMPLFI_ERR_CUDA; }
         attr_done = true;
     }
-    inject_whiten13_kernel<MODE><<<units, T13, smem, st>>>(a, units);
+    inject_whiten13_kernel<MODE, IW13_VT><<<units, T13 / IW13_VT, smem, st>>>(a, units);
     count_launch();
     return check_launch("inject_whiten13_kernel");
 }
