@@ -81,19 +81,7 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
     __syncthreads();
 #pragma unroll
     for (int vt = 0; vt < VT; ++vt) p2_fwd(tt + vt * TT, re, im);
-    __syncthreads();
-#pragma unroll
-    for (int vt = 0; vt < VT; ++vt) p3_fwd(tt + vt * TT, re, im);
-    __syncthreads();
-    __shared__ float2 sc[16];
-#pragma unroll
-    for (int vt = 0; vt < VT; ++vt) {
-    const int t = tt + vt * TT;
-    const int klow_a = t, klow_b = (t == 0) ? 512 : 1024 - t;
-    C2 v[8];
-    p4_fwd(klow_a, klow_b, v, re, im);
-
-    // ---- a-7 inject, a-8 whiten + band-limit (registers) ----
+    // ---- per-unit constants of the pointwise stage ----
     const float* filt = a.filt + (size_t)d * a.filt_stride;
     const float2* hsrc = nullptr;
     int w_lo = 1, w_hi = 0;
@@ -108,7 +96,31 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
         cim = -(float)r.fc * c->pol_c;
         delta = (float)(r.dt * (double)a.inv_tseg);          // turns per bin
     }
-    auto inject = [&](int k, float2& x2) {
+    // Operands of the pointwise stage for virtual thread t: bins k = t + 1024 k4 (half A) and M - k (half B).
+    // They are requested one phase ahead of their use so that L2 latency is covered by butterfly work.  h0 is zero
+    // outside [w_lo, w_hi]: a warp none of whose 32 bins of a half is inside skips the load (warp-uniform test;
+    // heavy systems stop at a few hundred Hz).
+    struct PwOps { float2 ha[8], hb[8]; float fa[8], fb[8]; };
+    auto pw_load = [&](int t, PwOps& L) {
+        const int wbase = t & ~31;
+#pragma unroll
+        for (int k4 = 0; k4 < 8; ++k4) {
+            const int k = t + 1024 * k4;
+            L.fa[k4] = __ldg(filt + k);
+            L.fb[k4] = __ldg(filt + M - k);
+            if (MODE == MODE_HDET) {
+                L.ha[k4] = __ldg(hsrc + k);
+                L.hb[k4] = __ldg(hsrc + M - k);
+            } else if (MODE == MODE_FUSED) {
+                const int ka_lo = wbase + 1024 * k4, ka_hi = ka_lo + 31;
+                L.ha[k4] = make_float2(0.f, 0.f);
+                L.hb[k4] = make_float2(0.f, 0.f);
+                if (ka_hi >= w_lo && ka_lo <= w_hi) L.ha[k4] = __ldg(hsrc + k);
+                if (M - ka_lo >= w_lo && M - ka_hi <= w_hi) L.hb[k4] = __ldg(hsrc + M - k);
+            }
+        }
+    };
+    auto inject = [&](int k, float2& x2) {                   // slow path (self-paired bins only)
         if (MODE == MODE_HDET) {
             const float2 h = __ldg(hsrc + k);
             x2.x = fmaf(a.two_fs, h.x, x2.x);
@@ -126,7 +138,7 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
             }
         }
     };
-    auto do_pair = [&](int k, float2& za, float2& zb) {       // za = Z[k], zb = Z[M-k], 0 < k < M/2
+    auto do_pair = [&](int k, float2& za, float2& zb) {       // za = Z[k], zb = Z[M-k], 0 < k <= M/2
         const float2 w = twiddle<N>(k);
         float2 xa, xb;
         split_pair(za, zb, w, xa, xb);
@@ -136,21 +148,23 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
         xa.x *= fa; xa.y *= fa; xb.x *= fb; xb.y *= fb;
         merge_pair(xa, xb, w, za, zb);
     };
-    float2 za[8], zb[8];            // halves A, B; index r holds k4 = brev<8>(r)
+    __shared__ float2 sc[16];
+    // a-7 inject, a-8 whiten + band-limit on the registers of virtual thread t (v[r]: k4 = brev(r); halves A, B)
+    auto pointwise = [&](int t, C2 (&v)[8], const PwOps& L) {
+        float2 za[8], zb[8];
 #pragma unroll
-    for (int r = 0; r < 8; ++r) {
-        unpack(v[r].r, za[r].x, zb[r].x);
-        unpack(v[r].i, za[r].y, zb[r].y);
-    }
-    // Thread 0 holds the two self-paired butterflies (klow 0: bins 1024 q, with DC/Nyquist in Z[0]; klow 512: bins
-    // 512 + 1024 q).  It parks them in a scratch row; nine lanes of warp 0 process those bins after the generic
-    // section (which thread 0 executes on values that are then overwritten), so no warp runs a long divergent path.
-    if (t == 0) {
+        for (int r = 0; r < 8; ++r) {
+            unpack(v[r].r, za[r].x, zb[r].x);
+            unpack(v[r].i, za[r].y, zb[r].y);
+        }
+        // Thread 0 holds the two self-paired butterflies (klow 0: bins 1024 q, with DC/Nyquist in Z[0]; klow 512:
+        // bins 512 + 1024 q).  It parks them in a scratch row; nine lanes of warp 0 process those bins after the
+        // generic section (which thread 0 executes on values that are then overwritten), so no warp runs a long
+        // divergent path.
+        if (t == 0) {
 #pragma unroll
-        for (int r = 0; r < 8; ++r) { sc[brev<8>(r)] = za[r]; sc[8 + brev<8>(r)] = zb[r]; }
-    }
-    {
-        // bins k = t + 1024 k4 (half A) and M - k (half B), k4 = 0..7.
+            for (int r = 0; r < 8; ++r) { sc[brev<8>(r)] = za[r]; sc[8 + brev<8>(r)] = zb[r]; }
+        }
         // split twiddle w_N^k = w_N^t * w_16^k4: one sincos and compile-time rotations.
         const float2 wt = twiddle<N>(t);
         // projection factors C exp(-2 pi i k dt/T) by recurrence over k4 (both halves in one packed chain):
@@ -175,7 +189,6 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
 #pragma unroll
         for (int k4 = 0; k4 < 8; ++k4) {
             const int r = brev<8>(k4);
-            const int k = t + 1024 * k4;
             float2 w = wt;
             switch (k4) {
                 case 0: break;
@@ -191,11 +204,11 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
             float2& pb = zb[7 - r];
             float2 xa, xb;
             split_pair(pa, pb, w, xa, xb);
+            const float2 ha = L.ha[k4], hb = L.hb[k4];
             if (MODE == MODE_HDET) {
-                inject(k, xa);
-                inject(M - k, xb);
+                xa.x = fmaf(a.two_fs, ha.x, xa.x); xa.y = fmaf(a.two_fs, ha.y, xa.y);
+                xb.x = fmaf(a.two_fs, hb.x, xb.x); xb.y = fmaf(a.two_fs, hb.y, xb.y);
             } else if (MODE == MODE_FUSED) {
-                const float2 ha = __ldg(hsrc + k), hb = __ldg(hsrc + M - k);
                 float ar, br, ai, bi;
                 unpack(ph.r, ar, br);
                 unpack(ph.i, ai, bi);
@@ -205,43 +218,57 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
                 xb.y = fmaf(hb.x, bi, fmaf(hb.y, br, xb.y));
                 if (k4 < 7) ph = cmul(ph, st);
             }
-            const float fa = __ldg(filt + k), fb = __ldg(filt + M - k);
+            const float fa = L.fa[k4], fb = L.fb[k4];
             xa.x *= fa; xa.y *= fa; xb.x *= fb; xb.y *= fb;
             merge_pair(xa, xb, w, pa, pb);
         }
-    }
-    if (t < 32) {
-        __syncwarp();
-        if (t == 0) {       // Z[0] carries the DC and Nyquist bins of the real transform
-            const float2 z0 = sc[0];
-            float x0 = 2.0f * (z0.x + z0.y), xm = 2.0f * (z0.x - z0.y);
-            if (MODE == MODE_HDET) {
-                x0 = fmaf(a.two_fs, __ldg(hsrc).x, x0);
-                xm = fmaf(a.two_fs, __ldg(hsrc + M).x, xm);
+        if (t < 32) {
+            __syncwarp();
+            if (t == 0) {       // Z[0] carries the DC and Nyquist bins of the real transform
+                const float2 z0 = sc[0];
+                float x0 = 2.0f * (z0.x + z0.y), xm = 2.0f * (z0.x - z0.y);
+                if (MODE == MODE_HDET) {
+                    x0 = fmaf(a.two_fs, __ldg(hsrc).x, x0);
+                    xm = fmaf(a.two_fs, __ldg(hsrc + M).x, xm);
+                }
+                const float y0 = x0 * __ldg(filt), ym = xm * __ldg(filt + M);
+                sc[0] = make_float2(y0 + ym, y0 - ym);
+            } else if (t < 9) {
+                // t = 1..3: (A[q], A[8-q]), k = 1024 q;  t = 4: A[4] with itself, k = M/2;
+                // t = 5..8: (B[q], B[7-q]), q = t - 5, k = 512 + 1024 q
+                const int ia = t <= 4 ? t : 3 + t, ib = t <= 4 ? 8 - t : 20 - t;
+                const int k = t <= 4 ? 1024 * t : 512 + 1024 * (t - 5);
+                float2 pa = sc[ia], pb = sc[ib];
+                do_pair(k, pa, pb);
+                sc[ia] = pa;
+                if (ib != ia) sc[ib] = pb;
             }
-            const float y0 = x0 * __ldg(filt), ym = xm * __ldg(filt + M);
-            sc[0] = make_float2(y0 + ym, y0 - ym);
-        } else if (t < 9) {
-            // t = 1..3: (A[q], A[8-q]), k = 1024 q;  t = 4: A[4] with itself, k = M/2;
-            // t = 5..8: (B[q], B[7-q]), q = t - 5, k = 512 + 1024 q
-            const int ia = t <= 4 ? t : 3 + t, ib = t <= 4 ? 8 - t : 20 - t;
-            const int k = t <= 4 ? 1024 * t : 512 + 1024 * (t - 5);
-            float2 pa = sc[ia], pb = sc[ib];
-            do_pair(k, pa, pb);
-            sc[ia] = pa;
-            if (ib != ia) sc[ib] = pb;
-        }
-        __syncwarp();
-        if (t == 0) {
+            __syncwarp();
+            if (t == 0) {
 #pragma unroll
-            for (int r = 0; r < 8; ++r) { za[r] = sc[brev<8>(r)]; zb[r] = sc[8 + brev<8>(r)]; }
+                for (int r = 0; r < 8; ++r) { za[r] = sc[brev<8>(r)]; zb[r] = sc[8 + brev<8>(r)]; }
+            }
         }
-    }
 #pragma unroll
-    for (int r = 0; r < 8; ++r) v[r] = C2{pack(za[r].x, zb[r].x), pack(za[r].y, zb[r].y)};
+        for (int r = 0; r < 8; ++r) v[r] = C2{pack(za[r].x, zb[r].x), pack(za[r].y, zb[r].y)};
+    };
 
-    // ---- a-9 inverse real FFT and store ----
-    p4_inv(klow_a, klow_b, v, re, im);
+    __syncthreads();
+    PwOps ops[VT];
+    pw_load(tt, ops[0]);                                     // in flight during P3 and the barrier
+#pragma unroll
+    for (int vt = 0; vt < VT; ++vt) p3_fwd(tt + vt * TT, re, im);
+    __syncthreads();
+#pragma unroll
+    for (int vt = 0; vt < VT; ++vt) {
+        const int t = tt + vt * TT;
+        const int klow_a = t, klow_b = (t == 0) ? 512 : 1024 - t;
+        C2 v[8];
+        p4_fwd(klow_a, klow_b, v, re, im);
+        pointwise(t, v, ops[vt]);
+        if (vt + 1 < VT) pw_load(t + TT, ops[vt + 1]);      // in flight during this P4' and the next P4
+        // ---- a-9 inverse real FFT ----
+        p4_inv(klow_a, klow_b, v, re, im);
     }
     __syncthreads();
 #pragma unroll
