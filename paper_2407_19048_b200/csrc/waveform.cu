@@ -21,27 +21,33 @@ int launch_tables(amplfi_plan* p, cudaStream_t st) {
     return check_launch("tables_kernel");
 }
 
-// ---- one thread per sample: waveform coefficients + detector responses (fp64) ----
-__global__ void prepare_kernel(const double* __restrict__ params, int batch, int approx, double t_seg, int n_bins,
-                               double f_lo, double f_hi, double amp_mul, double gmst,
-                               const double* __restrict__ pd_table, const int* __restrict__ det_ids, int n_det,
-                               WfCoef* __restrict__ coef, DetResp* __restrict__ resp, int* __restrict__ flags) {
-    int b = blockIdx.x * blockDim.x + threadIdx.x;
+// ---- per sample: waveform coefficients (one warp role) and detector responses (the other), fp64 ----
+// Both are long dependent chains of fp64 library calls; a CTA of 64 threads serves 32 samples, warp 0 computing the
+// coefficients and warp 1 the responses, so the two chains run side by side on different schedulers.
+__global__ void __launch_bounds__(64) prepare_kernel(const double* __restrict__ params, int batch, int approx, double t_seg,
+                                                     int n_bins, double f_lo, double f_hi, double amp_mul, double gmst,
+                                                     const double* __restrict__ pd_table, const int* __restrict__ det_ids,
+                                                     int n_det, WfCoef* __restrict__ coef, DetResp* __restrict__ resp,
+                                                     int* __restrict__ flags) {
+    const int b = blockIdx.x * 32 + (threadIdx.x & 31);
     if (b >= batch) return;
     const double* p = params + (size_t)b * AMPLFI_N_PARAMS;
-    if (coef != nullptr) {
-        WfCoef c;
-        prepare_sample(p, approx, t_seg, n_bins, f_lo, f_hi, amp_mul, pd_table, c);
-        coef[b] = c;
-        if (flags != nullptr) flags[b] = c.valid ? 0 : 1;
+    if (threadIdx.x < 32) {
+        if (coef != nullptr) {
+            WfCoef c;
+            prepare_sample(p, approx, t_seg, n_bins, f_lo, f_hi, amp_mul, pd_table, c);
+            coef[b] = c;
+            if (flags != nullptr) flags[b] = c.valid ? 0 : 1;
+        }
+    } else {
+        const SkyFrame f = sky_frame(p[8], p[9], p[10], gmst);
+        for (int d = 0; d < n_det; ++d) resp[(size_t)b * n_det + d] = detector_response(f, det_ids[d]);
     }
-    for (int d = 0; d < n_det; ++d) resp[(size_t)b * n_det + d] = detector_response(p[8], p[9], p[10], gmst, det_ids[d]);
 }
 
 int launch_prepare(const amplfi_plan* p, int approximant, int batch, const double* params, double gmst,
                    double f_lo, double f_hi, double amp_mul, int* flags, cudaStream_t st) {
-    const int threads = 64;
-    prepare_kernel<<<(batch + threads - 1) / threads, threads, 0, st>>>(
+    prepare_kernel<<<(batch + 31) / 32, 64, 0, st>>>(
         params, batch, approximant, p->t_seg, p->n_bins, f_lo, f_hi, amp_mul, gmst, p->pd_table, p->d_det_ids,
         p->n_det, approximant < 0 ? nullptr : p->coef, p->resp, flags);
     count_launch();

@@ -55,15 +55,26 @@ __device__ __constant__ DetGeom kDet[3] = {
 #define AMPLFI_PI 3.141592653589793238
 
 // antenna patterns and geocentric delay of detector `det`
-__device__ inline DetResp detector_response(double ra, double dec, double psi, double gmst, int det) {
-    const DetGeom& g = kDet[det];
+struct SkyFrame { double X[3], Y[3], n[3]; };
+
+// polarisation axes X, Y and direction n toward the source in the Earth-fixed frame (shared by all detectors)
+__device__ inline SkyFrame sky_frame(double ra, double dec, double psi, double gmst) {
     double sg, cg, sd, cd, sp, cp;
     sincos(gmst - ra, &sg, &cg);
     sincos(dec, &sd, &cd);
     sincos(psi, &sp, &cp);
-    const double X[3] = {-cp * sg - sp * cg * sd, -cp * cg + sp * sg * sd, sp * cd};
-    const double Y[3] = {sp * sg - cp * cg * sd, sp * cg + cp * sg * sd, cp * cd};
-    const double n[3] = {cd * cg, -cd * sg, sd};
+    SkyFrame f;
+    f.X[0] = -cp * sg - sp * cg * sd; f.X[1] = -cp * cg + sp * sg * sd; f.X[2] = sp * cd;
+    f.Y[0] = sp * sg - cp * cg * sd;  f.Y[1] = sp * cg + cp * sg * sd;  f.Y[2] = cp * cd;
+    f.n[0] = cd * cg; f.n[1] = -cd * sg; f.n[2] = sd;
+    return f;
+}
+
+__device__ inline DetResp detector_response(const SkyFrame& f, int det) {
+    const DetGeom& g = kDet[det];
+    const double* X = f.X;
+    const double* Y = f.Y;
+    const double* n = f.n;
     // D = (x x^T - y y^T)/2 contracted with X, Y via the projections on the arms
     const double xX = g.x[0] * X[0] + g.x[1] * X[1] + g.x[2] * X[2];
     const double xY = g.x[0] * Y[0] + g.x[1] * Y[1] + g.x[2] * Y[2];
@@ -96,11 +107,12 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     c.k_hi = 0;
     if (!ok) return;
     const double eta = q / ((1.0 + q) * (1.0 + q));
-    const double mtot = mc * pow(eta, -0.6);
+    const double mtot = mc * exp(-0.6 * log(eta));
     const double ms = mtot * AMPLFI_MTSUN;           // seconds
     const double mu = ms / t_seg;                    // Mf = mu * k
-    const double v1 = cbrt(PI * mu);                 // v = v1 * k^(1/3)
-    const double lnv1 = log(v1);
+    const double lnmu = log(mu);
+    const double lnv1 = (lnmu + 1.1447298858494002) / 3.0;     // ln(pi) = 1.14472988584940017...
+    const double v1 = exp(lnv1);                     // (pi mu)^(1/3): v = v1 * k^(1/3)
     const double cosi = cos(p[5]);
     c.pol_p = (float)(0.5 * (1.0 + cosi * cosi));
     c.pol_c = (float)cosi;
@@ -191,8 +203,9 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
                                 + 3.352411249771192 * e3)
                          * (1.0 + (-0.0030302335878845507 - 2.0066110851351073 * eta + 7.7050567802399215 * e2) * sn))
                         / (1.0 + (-0.6714403054720589 - 1.4756929437702908 * eta + 7.304676214885011 * e2) * sn);
-    const double fring0 = (1.5251 - 1.1568 * pow(1.0 - af, 0.1292)) / TWO_PI;
-    const double qual = 0.7 + 1.4187 * pow(1.0 - af, -0.4990);
+    const double ln1maf = log(1.0 - af);
+    const double fring0 = (1.5251 - 1.1568 * exp(0.1292 * ln1maf)) / TWO_PI;
+    const double qual = 0.7 + 1.4187 * exp(-0.4990 * ln1maf);
     const double f_rd = fring0 / (1.0 - erad);
     const double f_dm = fring0 / (2.0 * qual) / (1.0 - erad);
 
@@ -223,11 +236,12 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     const double dint1 = (be1 + be2 / f1 + be3 / (f1 * f1 * f1 * f1)) / eta;
     const double c2int = dphi_ins - dint1;
     const double c1int = phi_ins - int1 - c2int * f1;
-    const double int2 = (be1 * f2 + be2 * log(f2) - be3 / (3.0 * f2 * f2 * f2)) / eta + c1int + c2int * f2;
+    const double lnf2 = log(f2), f2m14 = exp(-0.25 * lnf2);                 // f2^(-1/4)
+    const double int2 = (be1 * f2 + be2 * lnf2 - be3 / (3.0 * f2 * f2 * f2)) / eta + c1int + c2int * f2;
     const double dint2 = (be1 + be2 / f2 + be3 / (f2 * f2 * f2 * f2)) / eta + c2int;
     const double x2 = (f2 - al5 * f_rd) / f_dm;
-    const double mr2 = (al1 * f2 - al2 / f2 + 4.0 / 3.0 * al3 * pow(f2, 0.75) + al4 * atan(x2)) / eta;
-    const double dmr2 = (al1 + al2 / (f2 * f2) + al3 * pow(f2, -0.25) + al4 / (f_dm * (1.0 + x2 * x2))) / eta;
+    const double mr2 = (al1 * f2 - al2 / f2 + 4.0 / 3.0 * al3 * (f2 * f2m14) + al4 * atan(x2)) / eta;
+    const double dmr2 = (al1 + al2 / (f2 * f2) + al3 * f2m14 + al4 / (f_dm * (1.0 + x2 * x2))) / eta;
     const double c2mr = dint2 - dmr2;
     const double c1mr = int2 - mr2 - c2mr * f2;
     // amplitude peak and time alignment
@@ -235,25 +249,25 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     const double f_peak = (g2 > 1.0) ? fabs(f_rd - f_dm * g3 / g2)
                                      : fabs(f_rd + f_dm * (sqrt(1.0 - g2 * g2) - 1.0) * g3 / g2);
     const double xp = (f_peak - al5 * f_rd) / f_dm;
-    const double t0 = (al1 + al2 / (f_peak * f_peak) + al3 * pow(f_peak, -0.25) + al4 / (f_dm * (1.0 + xp * xp))) / eta
+    const double t0 = (al1 + al2 / (f_peak * f_peak) + al3 * rsqrt(sqrt(f_peak)) + al4 / (f_dm * (1.0 + xp * xp))) / eta
                       + c2mr;
 
     c.kp1 = f1 / mu;
     c.kp2 = f2 / mu;
-    const double mu13 = cbrt(mu);
+    const double mu13 = exp(lnmu / 3.0);
     c.lin1 = tc_turns + (sg1 / eta - t0) * mu / TWO_PI;
     c.c01 = const1;
     c.s_p4 = 0.75 * sg2 / eta * mu * mu13 / TWO_PI;
     c.s_p5 = 0.6 * sg3 / eta * mu * mu13 * mu13 / TWO_PI;
     c.s_p6 = 0.5 * sg4 / eta * mu * mu / TWO_PI;
     c.lin2 = tc_turns + (be1 / eta + c2int - t0) * mu / TWO_PI;
-    c.c02 = (c1int + be2 / eta * log(mu)) / TWO_PI + phic_turns;
+    c.c02 = (c1int + be2 / eta * lnmu) / TWO_PI + phic_turns;
     c.b_ln = be2 / eta / TWO_PI;
     c.b_m9 = -be3 / (3.0 * eta * mu * mu * mu) / TWO_PI;
     c.lin3 = tc_turns + (al1 / eta + c2mr - t0) * mu / TWO_PI;
     c.c03 = c1mr / TWO_PI + phic_turns;
     c.r_m3 = -al2 / (eta * mu) / TWO_PI;
-    c.r_34 = 4.0 / 3.0 * al3 / eta * pow(mu, 0.75) / TWO_PI;
+    c.r_34 = 4.0 / 3.0 * al3 / eta * exp(0.75 * lnmu) / TWO_PI;
     c.r_at = (float)(al4 / eta / TWO_PI);
     c.at_k0 = (float)(al5 * f_rd / mu);
     c.at_invw = (float)(mu / f_dm);
@@ -261,7 +275,7 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     // ---- amplitude ----
     const double amp0 = 2.0 * sqrt(5.0 / (64.0 * PI)) * mtot * mtot * AMPLFI_MTSUN * (AMPLFI_MTSUN * AMPLFI_C_SI)
                         / (dist * AMPLFI_MPC);
-    c.amp_scale = (float)(amp0 * sqrt(2.0 * eta / 3.0) * pow(PI, -1.0 / 6.0) * pow(mu, -7.0 / 6.0) * amp_mul);
+    c.amp_scale = (float)(amp0 * sqrt(2.0 * eta / 3.0) * 0.8263074871107581 * exp(-7.0 / 6.0 * lnmu) * amp_mul);   // pi^(-1/6)
     const double c12 = chi1 * chi1, c22 = chi2 * chi2;
     double A[7];
     A[2] = (-969.0 + 1804.0 * eta) / 672.0;
