@@ -60,7 +60,7 @@ int launch_prepare(const amplfi_plan* p, int approximant, int batch, const doubl
 // zero-filled without touching the tables.
 #define WF_SLICES 2
 template <bool POL>
-__global__ void __launch_bounds__(256, 4) waveform_kernel(const WfCoef* __restrict__ coef, const double* __restrict__ tab_ci,
+__global__ void __launch_bounds__(256, 3) waveform_kernel(const WfCoef* __restrict__ coef, const double* __restrict__ tab_ci,
                                                        const double* __restrict__ tab_lnk, int n_bins,
                                                        float2* __restrict__ out_a, float2* __restrict__ out_b) {
     const int b = blockIdx.y;
@@ -74,9 +74,17 @@ __global__ void __launch_bounds__(256, 4) waveform_kernel(const WfCoef* __restri
     const int k_lo = c.valid ? c.k_lo : 1, k_hi = c.valid ? c.k_hi : 0;
     float2* oa = out_a + (size_t)b * n_bins;
     float2* ob = POL ? out_b + (size_t)b * n_bins : nullptr;
-    for (int kc = blockIdx.x * 256; kc < n_bins; kc += 256 * gridDim.x) {
+    // The plan's h0 workspace (POL == false) is only ever read inside the band, widened to the 32-bin windows of
+    // the consumers' warp-uniform band test (inject_whiten13.cu): bins further than 64 from the band are not written.
+    int k_first = 0, k_last = n_bins - 1;
+    if (!POL) {
+        if (k_lo > k_hi) return;
+        k_first = k_lo > 64 ? ((k_lo - 64) & ~255) : 0;
+        k_last = k_hi + 64 < n_bins - 1 ? k_hi + 64 : n_bins - 1;
+    }
+    for (int kc = k_first + blockIdx.x * 256; kc <= k_last; kc += 256 * gridDim.x) {
         const int k = kc + threadIdx.x;
-        if (k >= n_bins) break;
+        if (k > k_last) break;
         float2 h = make_float2(0.f, 0.f);
         if (k >= k_lo && k <= k_hi) h = eval_h0(c, k, tab_ci[k], tab_lnk[k]);
         if (POL) {
