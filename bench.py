@@ -32,12 +32,12 @@ WORKLOAD = ("c2 training-throughput: batch 2048 x H1+L1+V1, fs 2048 Hz, 8 s segm
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--batch", type=int, default=2048)
     ap.add_argument("--strip-len", type=int, default=44236800)
-    ap.add_argument("--cpu-sample", type=int, default=256, help="samples of the batch the CPU oracle is timed on")
+    ap.add_argument("--cpu-sample", type=int, default=1024, help="samples of the batch the CPU oracle is timed on")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--config", default="c2", choices=["c2", "c3", "c4", "sweep"],
@@ -118,7 +118,7 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------------
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 100 ms while the timed region runs."""
+    """nvidia-smi clocks / throttle reasons sampled every 20 ms while the timed region runs."""
     FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
               "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
               "clocks_event_reasons.sw_power_cap")
@@ -129,7 +129,7 @@ class ClockSampler:
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.FIELDS,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -289,10 +289,17 @@ def run_b200(args):
     roofline = None
     if k_ms:
         ach = alg_bytes / (k_ms * 1e-3) / 1e9
-        roofline = {"bound": "hbm", "kernel": "inject_whiten_kernel<13,fused>", "achieved": ach, "peak": peak,
+        # secondary ceiling: fp32 lane-operations on the FMA pipe, 128 lanes/clk/SM (measured with
+        # FADD2/FFMA2 microbenchmarks), counted from the kernel's SASS: 2140 per 16 complex points = 66.9 per sample
+        sm_clk = (clocks or {}).get("sm_mhz") or 1965.0
+        alu_peak = 148 * 128 * sm_clk * 1e6 / 1e12
+        alu_ach = 66.9 * B * D * N / (k_ms * 1e-3) / 1e12
+        roofline = {"bound": "hbm", "kernel": "inject_whiten13_kernel<fused, VT=2>", "achieved": ach, "peak": peak,
                     "unit": "GB/s", "frac": ach / peak, "frac_of_nominal_8TBps": ach / 8000.0, "peak_source": peak_src,
                     "traffic": traffic, "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": k_ms,
-                    "kernel_share_of_step": k_ms / ms_per_step, "launches_timed": len(kernel_ms)}
+                    "kernel_share_of_step": k_ms / ms_per_step, "launches_timed": len(kernel_ms),
+                    "alu": {"bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "T fp32 lane-op/s",
+                            "frac": alu_ach / alu_peak, "lane_ops_per_sample": 66.9, "sm_mhz": sm_clk}}
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
