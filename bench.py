@@ -371,34 +371,56 @@ def run_extra(args):
         return ms, sps, n_l
 
     if args.config == "c3":
-        lat, snr = [], []
+        # one amplfi_assemble_batch call per candidate, inputs resident; measured both as plain stream launches and as a
+        # replayed CUDA graph of the same call (the online service keeps its buffers in place)
         plan = A.Plan(16384, 2048.0, (0, 1, 2), 1, nperseg=8192)
+        bg = torch.empty((3, 262144), dtype=torch.float32, device=dev)
+        noise = torch.empty((1, 3, 16384), dtype=torch.float32, device=dev)
+        params = torch.empty((1, 11), dtype=torch.float64, device=dev)
         psd = torch.empty((3, 4097), dtype=torch.float32, device=dev)
         out = torch.empty((1, 3, 16384), dtype=torch.float32, device=dev)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        for r in range(-3, args.runs):                               # three untimed warm-up runs
-            wl = WL.make_c3(run=max(r, 0))
-            bg = torch.from_numpy(wl.bg).to(dev)
-            noise = torch.from_numpy(wl.noise).to(dev)
-            params = torch.from_numpy(wl.params).to(dev)
+
+        def call(st):
+            A.amplfi_assemble_batch(plan, 1, bg, noise, params, 20.0, 1000.0, approximant=A.IMRPHENOMD, gmst=0.0,
+                                    psd=psd, out=out, stream=st)
+
+        def load(r):
+            wl = WL.make_c3(run=r)
+            bg.copy_(torch.from_numpy(wl.bg)); noise.copy_(torch.from_numpy(wl.noise)); params.copy_(torch.from_numpy(wl.params))
+
+        load(0)
+        for _ in range(3):
+            call(stream)
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        cs = torch.cuda.Stream()
+        cs.wait_stream(stream)
+        with torch.cuda.graph(graph, stream=cs):
+            call(torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        lat, lat_g = [], []
+        ref = None
+        for r in range(args.runs):
+            load(r)
             torch.cuda.synchronize()
-            e0.record(stream)
-            A.amplfi_psd_welch(plan, bg, psd=psd, stream=stream)
-            A.amplfi_inject_whiten(plan, 1, noise, psd, wl.f_lo, wl.f_hi, approximant=wl.approximant, params=params,
-                                   gmst=wl.gmst, out=out, stream=stream)
-            e1.record(stream)
+            e0.record(stream); call(stream); e1.record(stream)
             torch.cuda.synchronize()
-            if r >= 0:
-                lat.append(e0.elapsed_time(e1) * 1e3)
-        lat = np.array(lat)
-        print(json.dumps({"metric": "online PSD+whiten device latency", "unit": "us", "higher_is_better": False,
-                          "p50": float(np.percentile(lat, 50)), "p99": float(np.percentile(lat, 99)),
-                          "mean": float(lat.mean()), "min": float(lat.min()), "max": float(lat.max()), "runs": len(lat),
-                          "dtype": "f32", "data": "synthetic",
-                          "config": {"workload": "c3 online-latency: batch 1 x H1+L1+V1, 8 s at 2048 Hz, Welch from the 128 s "
-                                                 "preceding background (4 s Hann, 50% overlap), IMRPhenomD injection; run r "
-                                                 "uses seed 0xA3D30003 + r; CUDA events around amplfi_psd_welch + "
-                                                 "amplfi_inject_whiten on one stream, inputs resident"}}))
+            lat.append(e0.elapsed_time(e1) * 1e3)
+            ref = out.clone()
+            e0.record(stream); graph.replay(); e1.record(stream)
+            torch.cuda.synchronize()
+            lat_g.append(e0.elapsed_time(e1) * 1e3)
+            assert torch.equal(ref, out)
+        for name, v in (("stream launches", np.array(lat)), ("CUDA graph replay", np.array(lat_g))):
+            print(json.dumps({"metric": "online PSD+whiten device latency", "unit": "us", "higher_is_better": False,
+                              "launch": name, "p50": float(np.percentile(v, 50)), "p99": float(np.percentile(v, 99)),
+                              "mean": float(v.mean()), "min": float(v.min()), "max": float(v.max()), "runs": len(v),
+                              "dtype": "f32", "data": "synthetic",
+                              "config": {"workload": "c3 online-latency: batch 1 x H1+L1+V1, 8 s at 2048 Hz, Welch from the 128 s "
+                                                     "preceding background (4 s Hann, 50% overlap), IMRPhenomD injection; run r "
+                                                     "uses seed 0xA3D30003 + r; CUDA events around one amplfi_assemble_batch "
+                                                     "call, inputs resident"}}))
         return
 
     if args.config == "c4":
