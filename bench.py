@@ -184,7 +184,8 @@ def run_b200(args):
         dist.init_process_group("nccl", device_id=dev)
 
     # ---- synthetic workload (host, seeded), uploaded once: "before commencing training" ----
-    wl = WL.make_c2(batch=args.batch, seed=0xA3D30002 + rank, strip_len=args.strip_len)
+    from workloads import sharding as SH
+    wl = WL.make_c2(batch=args.batch, seed=SH.rank_seed(0xA3D30002, rank), strip_len=args.strip_len)
     B, D, N = wl.batch, wl.n_det, wl.n
     plan = A.Plan(N, wl.fs, wl.det_ids, B, nperseg=wl.nperseg)
     strip = torch.from_numpy(wl.strip).to(dev)
@@ -232,12 +233,9 @@ def run_b200(args):
     kernel_ms = plan.kernel_times_ms()
     plan.set_timing(False)
     clocks = sampler.stop() if rank == 0 else None
-    if dist is not None:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = SH.max_over_ranks(total_ms, dist, dev)
     ms_per_step = total_ms / args.steps
-    value = world * B * D * N / (ms_per_step * 1e-3)
+    value = SH.aggregate_throughput(B * D * N, world, ms_per_step)
 
     # ---- end to end: per-step inputs from pinned host memory, result read back to the host ----
     e2e = None
@@ -261,11 +259,8 @@ def run_b200(args):
         e1.record(stream)
         barrier()
         ms2 = e0.elapsed_time(e1)
-        if dist is not None:
-            t = torch.tensor([ms2], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms2 = float(t.item())
-        e2e = {"value": world * B * D * N / (ms2 / k2 * 1e-3), "unit": UNIT,
+        ms2 = SH.max_over_ranks(ms2, dist, dev)
+        e2e = {"value": SH.aggregate_throughput(B * D * N, world, ms2 / k2), "unit": UNIT,
                "h2d_bytes_per_step": int(params_h.numel() * 8 + offsets_h.numel() * 8),
                "d2h_bytes_per_step": int(out_h.numel() * 4), "steps": k2, "ms_per_step": ms2 / k2}
 
