@@ -60,7 +60,7 @@ int launch_prepare(const amplfi_plan* p, int approximant, int batch, const doubl
 // zero-filled without touching the tables.
 #define WF_SLICES 2
 template <bool POL>
-__global__ void __launch_bounds__(256, 3) waveform_kernel(const WfCoef* __restrict__ coef, const double* __restrict__ tab_ci,
+__global__ void __launch_bounds__(256, 4) waveform_kernel(const WfCoef* __restrict__ coef, const double* __restrict__ tab_ci,
                                                        const double* __restrict__ tab_lnk, int n_bins,
                                                        float2* __restrict__ out_a, float2* __restrict__ out_b) {
     const int b = blockIdx.y;
@@ -82,17 +82,24 @@ __global__ void __launch_bounds__(256, 3) waveform_kernel(const WfCoef* __restri
         k_first = k_lo > 64 ? ((k_lo - 64) & ~255) : 0;
         k_last = k_hi + 64 < n_bins - 1 ? k_hi + 64 : n_bins - 1;
     }
-    for (int kc = k_first + blockIdx.x * 256; kc <= k_last; kc += 256 * gridDim.x) {
-        const int k = kc + threadIdx.x;
-        if (k > k_last) break;
+    // the table values of the next chunk are requested before the current chunk is evaluated (L2 latency off the chain)
+    const int kstep = 256 * gridDim.x;
+    int k = k_first + blockIdx.x * 256 + threadIdx.x;
+    bool in = k >= k_lo && k <= k_hi;
+    double ci = in ? tab_ci[k] : 1.0, lnk = in ? tab_lnk[k] : 0.0;
+    for (; k <= k_last; k += kstep) {
+        const int kn = k + kstep;
+        const bool in_n = kn >= k_lo && kn <= k_hi;
+        const double ci_n = in_n ? tab_ci[kn] : 1.0, lnk_n = in_n ? tab_lnk[kn] : 0.0;
         float2 h = make_float2(0.f, 0.f);
-        if (k >= k_lo && k <= k_hi) h = eval_h0(c, k, tab_ci[k], tab_lnk[k]);
+        if (in) h = eval_h0(c, k, ci, lnk);
         if (POL) {
             oa[k] = make_float2(c.pol_p * h.x, c.pol_p * h.y);
             ob[k] = make_float2(c.pol_c * h.y, -c.pol_c * h.x);     // -i c (x + i y) = c y - i c x
         } else {
             oa[k] = h;
         }
+        in = in_n; ci = ci_n; lnk = lnk_n;
     }
 }
 

@@ -357,7 +357,8 @@ __device__ __forceinline__ float2 eval_h0(const WfCoef& c, int k, double ci, dou
     } else {
         // k^(3/4) = k * k^(-1/4): fp32 seed (two MUFU) and one Newton step in fp64 (relative error ~1e-13),
         // instead of two software fp64 square roots
-        const double y0 = (double)rsqrtf(sqrtf((float)k));
+        const float kq = (float)k;
+        const double y0 = (double)rsqrtf(kq * rsqrtf(kq));      // ~k^(-1/4), two MUFU, no slow paths
         const double y2 = y0 * y0;
         const double y1 = fma(0.25 * y0, fma(-kd, y2 * y2, 1.0), y0);
         ph = fma(c.lin3, kd, c.c03);
@@ -370,7 +371,8 @@ __device__ __forceinline__ float2 eval_h0(const WfCoef& c, int k, double ci, dou
     __sincosf((float)ph * 6.283185307179586f, &s, &co);
 
     const float kf = (float)k, cf = (float)ci, c1f = (float)c1;
-    float amp = c.amp_scale * cf * cf * cf * sqrtf(cf);          // k^(-7/6)
+    const float cf2 = cf * cf;
+    float amp = c.amp_scale * cf2 * cf2 * rsqrtf(cf);        // k^(-7/6) = cf^(7/2), cf = k^(-1/3)
     if (kf < c.ka1) {
         float br = c.e[7];
 #pragma unroll
@@ -381,7 +383,7 @@ __device__ __forceinline__ float2 eval_h0(const WfCoef& c, int k, double ci, dou
         amp *= fmaf(u, fmaf(u, fmaf(u, fmaf(u, c.q[4], c.q[3]), c.q[2]), c.q[1]), c.q[0]);
     } else {
         const float y = (kf - c.g_krd) * c.g_invw;
-        amp *= c.g0 * __expf(-c.g2 * y) / fmaf(y, y, 1.0f);
+        amp *= __fdividef(c.g0 * __expf(-c.g2 * y), fmaf(y, y, 1.0f));
     }
     return make_float2(amp * co, -amp * s);           // A exp(-i Psi)
 }
