@@ -158,6 +158,13 @@ int amplfi_assemble_batch(const amplfi_plan* plan, int batch, const float* bg, l
 int amplfi_plan_set_timing(amplfi_plan* plan, int enable);
 int amplfi_plan_kernel_times(amplfi_plan* plan, float* ms, int max);
 
+/* Measured fp32 arithmetic ceiling of the current device: runs a register-resident loop of packed fp32x2 FMAs
+ * (2 lane-operations per thread-instruction) on every SM and writes the achieved fp32 lane-operations per second
+ * to the HOST double *lane_ops_per_s.  This is the denominator of the second roofline bench.py reports for the
+ * fused kernel, whose FFT butterflies are bound by the fp32 pipe rather than by HBM.
+ * Synchronises the device; not part of the hot path. */
+int amplfi_probe_fp32_pipe(double* lane_ops_per_s);
+
 /* Number of kernel launches the library has enqueued since it was loaded (all plans, all threads).
  * bench.py reports the difference across its timed region as "gpu_launches". */
 long amplfi_launch_count(void);

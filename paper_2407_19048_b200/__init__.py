@@ -23,7 +23,7 @@ N_PARAMS = 11
 EXPORTS = ("amplfi_last_error", "amplfi_psd_scale", "amplfi_version", "amplfi_phenomd_table",
            "amplfi_plan_create", "amplfi_plan_destroy", "amplfi_waveform_fd", "amplfi_project",
            "amplfi_psd_welch", "amplfi_inject_whiten", "amplfi_launch_count", "amplfi_plan_set_timing",
-           "amplfi_plan_kernel_times", "amplfi_assemble_batch")
+           "amplfi_plan_kernel_times", "amplfi_assemble_batch", "amplfi_probe_fp32_pipe")
 
 
 class AmplfiError(RuntimeError):
@@ -65,6 +65,8 @@ def _load():
     lib.amplfi_psd_welch.argtypes = [vp, vp, i64, i64, i32, i32, i32, vp, vp]
     lib.amplfi_inject_whiten.restype = i32
     lib.amplfi_inject_whiten.argtypes = [vp, i32, vp, vp, i64, vp, i32, vp, dbl, vp, i32, dbl, dbl, vp, vp]
+    lib.amplfi_probe_fp32_pipe.restype = i32
+    lib.amplfi_probe_fp32_pipe.argtypes = [c.POINTER(dbl)]
     lib.amplfi_assemble_batch.restype = i32
     lib.amplfi_assemble_batch.argtypes = [vp, i32, vp, i64, i64, i32, i32, vp, vp, vp, i64, i32, vp, dbl, dbl, dbl, vp, vp]
     return lib
@@ -239,3 +241,10 @@ def amplfi_assemble_batch(plan, batch, bg, noise, params, f_lo, f_hi, offsets=No
                                       strip_len, int(approximant), _ptr(params, torch.float64, "params"), float(gmst),
                                       float(f_lo), float(f_hi), _ptr(out, torch.float32, "out"), _stream(stream)))
     return out, psd
+
+
+def probe_fp32_pipe():
+    """Measured fp32 lane-operations per second of the current device (packed FMA loop on every SM)."""
+    v = ctypes.c_double(0.0)
+    _check(_lib.amplfi_probe_fp32_pipe(ctypes.byref(v)))
+    return float(v.value)

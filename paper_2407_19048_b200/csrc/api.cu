@@ -59,6 +59,55 @@ static int validate_band(const amplfi_plan* p, double f_lo, double f_hi, const c
 
 using namespace amplfi;
 
+// ---- fp32 pipe probe (amplfi_probe_fp32_pipe) ----
+__global__ void __launch_bounds__(256) fp32_probe_kernel(unsigned long long* out, unsigned long long a, unsigned long long b,
+                                                         int iters) {
+    unsigned long long x[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) x[i] = (unsigned long long)(threadIdx.x + i);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(x[i]) : "l"(a), "l"(b));
+    }
+    unsigned long long s = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += x[i];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
+extern "C" int amplfi_probe_fp32_pipe(double* lane_ops_per_s) {
+    if (lane_ops_per_s == nullptr) { set_error("amplfi_probe_fp32_pipe: null pointer"); return AMPLFI_ERR_INVALID_ARG; }
+    int dev = 0, sms = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    unsigned long long* buf = nullptr;
+    const int ctas = sms * 8, iters = 4096;
+    if (e == cudaSuccess) e = cudaMalloc(&buf, (size_t)ctas * 256 * sizeof(unsigned long long));
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (e == cudaSuccess) e = cudaEventCreate(&e0);
+    if (e == cudaSuccess) e = cudaEventCreate(&e1);
+    float best = 0.f;
+    if (e == cudaSuccess) {
+        const unsigned long long a = 0x3f8000013f800001ull, b = 0x3089705f3089705full;     // (1 + 2^-23, ~1e-9) x 2
+        for (int rep = 0; rep < 4 && e == cudaSuccess; ++rep) {                             // first pass warms up
+            cudaEventRecord(e0, nullptr);
+            fp32_probe_kernel<<<ctas, 256>>>(buf, a, b, iters);
+            cudaEventRecord(e1, nullptr);
+            e = cudaEventSynchronize(e1);
+            float ms = 0.f;
+            if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+            if (rep > 0 && ms > 0.f && (best == 0.f || ms < best)) best = ms;
+        }
+        count_launch(4);
+    }
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(buf);
+    if (e != cudaSuccess || best <= 0.f) { set_error("amplfi_probe_fp32_pipe: %s", cudaGetErrorString(e)); return AMPLFI_ERR_CUDA; }
+    *lane_ops_per_s = (double)ctas * 256.0 * 8.0 * iters * 2.0 / ((double)best * 1e-3);
+    return AMPLFI_OK;
+}
+
 extern "C" {
 
 const char* amplfi_last_error(void) { return g_err; }
