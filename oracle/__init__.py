@@ -12,6 +12,7 @@ statement of the steps (section 3.2):
     detector projection -> oracle.project
     power-spectrum estimate -> oracle.welch
     injection + whitening (PAPER.md:105) -> oracle.whiten
+    two data views d, d' -> oracle.views
     Fourier transforms -> oracle.fft  (naive O(N^2) DFT for N <= 64,
                                           plain recursive radix-2 FFT above that)
 

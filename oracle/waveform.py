@@ -421,3 +421,14 @@ def waveform_fd(approximant, params, n, fs, f_lo, f_hi):
     hp, hc = polarisations(h0, params[:, 5])
     flags = np.array([0 if params_valid(p) else 1 for p in params], dtype=np.int32)
     return hp, hc, flags
+
+
+def waveform_td(approximant, params, n, fs, f_lo, f_hi):
+    """Time-domain polarisations on the segment grid t_j = j/fs (Figure 1 compares the
+    "time-domain IMRPhenomD").  The frequency-domain model is the definition; its time series is
+    the inverse Fourier integral sampled on the grid, h(t_j) = df * sum over the two-sided spectrum of
+    h~(f_k) exp(+2 pi i f_k t_j) = fs * irfft(h~)[j]  (circular on the segment: reading R-W9).
+    Returns (hp_t, hc_t, flags): [B, n] float64 each."""
+    from .fft import irfft
+    hp, hc, flags = waveform_fd(approximant, params, n, fs, f_lo, f_hi)
+    return fs * irfft(hp, n), fs * irfft(hc, n), flags

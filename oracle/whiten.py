@@ -72,3 +72,47 @@ def optimal_snr(h_det, psd, n, fs, f_lo, f_hi):
     h_det = np.asarray(h_det)
     rho2 = 4.0 * (fs / n) * np.sum(np.abs(h_det[..., band]) ** 2 / s[..., band], axis=(-1, -2))
     return np.sqrt(rho2)
+
+
+# ----------------------------------------------------------------------------------------
+# whitening with a time-truncated filter (the practice of the library the paper
+# delegates to; the paper itself prints nothing).  DESIGN.md reading R-I8.
+# ----------------------------------------------------------------------------------------
+
+def fir_truncated_filter(psd, n, fs, f_lo, f_hi, fduration):
+    """Frequency response W'[k], k = 0..n/2, of the whitening filter truncated in time to fduration seconds.
+
+    Step by step (R-I8):
+      1. w[k] = sqrt(2 / (fs S[k])) inside [f_lo, f_hi], 0 outside      (whitening_filter above)
+      2. q = irfft(w): the zero-phase impulse response, real and even, q[j] = q[n - j]
+      3. taper to ntaps = fduration * fs samples around lag 0 with a Hann window centred on lag 0:
+             q'[j] = q[j] * (1 + cos(2 pi m / ntaps)) / 2   for m = min(j, n - j) < ntaps / 2,   0 otherwise
+      4. W' = rfft(q')   (real, because q' is even; the imaginary rounding residue is dropped)
+    The response no longer vanishes exactly outside the band and no mask is re-applied.
+    """
+    w = whitening_filter(psd, n, fs, f_lo, f_hi)
+    ntaps = int(round(fduration * fs))
+    assert 2 <= ntaps <= n and ntaps % 2 == 0
+    q = irfft(w.astype(np.complex128), n)
+    j = np.arange(n)
+    m = np.minimum(j, n - j)
+    taper = np.where(m < ntaps // 2, 0.5 * (1.0 + np.cos(2.0 * np.pi * m / ntaps)), 0.0)
+    return rfft(q * taper).real
+
+
+def inject_whiten_fir(noise, h_det, psd, fs, f_lo, f_hi, fduration, crop=True):
+    """out = irfft( (rfft(noise) + fs h_det) * W' ), W' = fir_truncated_filter; with crop the first and last
+    fduration/2 seconds, which the circular convolution contaminates with samples from the other end of the
+    segment, are removed: out has n - ntaps samples.  Inside the crop the result equals the LINEAR convolution
+    of the data with the ntaps-long filter (pinned against numpy.convolve)."""
+    noise = np.asarray(noise, dtype=np.float64)
+    n = noise.shape[-1]
+    wf = fir_truncated_filter(psd, n, fs, f_lo, f_hi, fduration)
+    xk = rfft(noise)
+    if h_det is not None:
+        xk = xk + fs * np.asarray(h_det, dtype=np.complex128)
+    y = irfft(xk * wf[None, :, :], n)
+    if not crop:
+        return y
+    pad = int(round(fduration * fs)) // 2
+    return y[..., pad: n - pad]
