@@ -107,8 +107,11 @@ int amplfi_project(const amplfi_plan* plan, int batch, const double* params, dou
  *   bg fp32 strain: detector d's n_bg samples start at bg + d * row_stride (row_stride in elements,
  *   >= n_bg; pass n_bg for a dense [n_det, n_bg] array, or the strip length to use a window of the
  *   GPU-resident strip in place);  noverlap in [0, nperseg);  detrend 0 none / 1 constant;
- *   average must be 0 (mean);  psd [n_det, nperseg/2+1] fp32 receives S * 2^140.
- * Deterministic (fixed summation order). */
+ *   average 0: mean over segments.  average 1: per-bin median over segments divided by the
+ *   median-to-mean ratio of nseg exponentially distributed values (the middle order statistic of n unit
+ *   exponentials has expectation sum_{j=n-k+1}^{n} 1/j; two middle ones averaged for even nseg), which is
+ *   robust against loud transients in the background;  psd [n_det, nperseg/2+1] fp32 receives S * 2^140.
+ * Deterministic (fixed summation order; ties in the median broken by segment index). */
 int amplfi_psd_welch(const amplfi_plan* plan, const float* bg, long n_bg, long row_stride, int noverlap,
                      int detrend, int average, float* psd, void* stream);
 
@@ -134,6 +137,43 @@ int amplfi_inject_whiten(const amplfi_plan* plan, int batch, const float* noise,
                          long strip_len, const float* h_det, int approximant, const double* params,
                          double gmst, const float* psd, int n_psd, double f_lo, double f_hi,
                          float* out, void* stream);
+
+/* Two data views (d, d') of the self-supervised pre-training (Figure 2: "the same background strain
+ * with a time-shifted signal injected, the parameters of which are otherwise the same ... random up to 1s";
+ * PAPER.md:117 "all signal parameters being the same except the time of arrival"):
+ *     out  = amplfi_inject_whiten(fused) with params,
+ *     out2 = the same with t_c replaced by t_c + t_shift[b]  (same noise segment, same PSD).
+ * The per-sample coefficients and the h0 spectrum are computed once; the second view only changes the
+ * linear phase exp(-2 pi i f_k (dt_d + t_shift[b])), accumulated in fp64.
+ *   t_shift [batch] fp64 seconds;  out, out2 [batch, n_det, n] fp32;  other arguments as amplfi_inject_whiten
+ *   (fused form: params must not be NULL). */
+int amplfi_inject_whiten_views(const amplfi_plan* plan, int batch, const float* noise, const long* offsets,
+                               long strip_len, int approximant, const double* params, const double* t_shift,
+                               double gmst, const float* psd, int n_psd, double f_lo, double f_hi, float* out,
+                               float* out2, void* stream);
+
+/* Time-domain polarisations on the segment grid t_j = j / fs (Figure 1 shows the "time-domain
+ * IMRPhenomD"): the inverse Fourier integral of the frequency-domain model sampled on the grid,
+ *     h(t_j) = fs * irfft(h~)[j]      (circular on the segment; the band is cut sharply at f_lo and f_top),
+ * computed by the inverse half of the segment transform without materialising h+~, hx~.
+ *   params [batch, 11] fp64;  h_t [batch, 2, n] fp32 strain: row 0 = h+, row 1 = hx;  flags [batch] or NULL. */
+int amplfi_waveform_td(const amplfi_plan* plan, int approximant, int batch, const double* params, double f_lo,
+                       double f_hi, float* h_t, int* flags, void* stream);
+
+/* amplfi_inject_whiten with the whitening filter truncated in time (the practice of the
+ * library the paper delegates whitening to; reading R-I8):
+ *   1. w[k] = sqrt(2/(fs S(f_k))) in [f_lo, f_hi], 0 outside;  2. q = irfft(w) (real, even);
+ *   3. q'[j] = q[j] (1 + cos(2 pi m / ntaps))/2 for m = min(j, n-j) < ntaps/2, else 0, ntaps = fduration * fs;
+ *   4. W' = rfft(q');  out = irfft((rfft(x) + fs h_d) W').
+ * With crop = 1 the first and last ntaps/2 samples of every row, which the circular convolution contaminates
+ * with data from the other end of the segment, are not written: out is [batch, n_det, n - ntaps] and equals
+ * the linear convolution of the data with the ntaps-long filter.  crop = 0: out is [batch, n_det, n].
+ *   fduration * fs must be a multiple of 4 in [4, n] (n - ntaps > 0 with crop);  other arguments as
+ *   amplfi_inject_whiten. */
+int amplfi_inject_whiten_fir(const amplfi_plan* plan, int batch, const float* noise, const long* offsets,
+                             long strip_len, const float* h_det, int approximant, const double* params,
+                             double gmst, const float* psd, int n_psd, double f_lo, double f_hi, double fduration,
+                             int crop, float* out, void* stream);
 
 /* One whole data-generation step (PSD fit to the background, waveforms generated on the
  * GPU, projected, injected into lazily loaded background chunks, batch whitened) = amplfi_psd_welch followed

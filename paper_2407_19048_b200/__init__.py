@@ -23,7 +23,8 @@ N_PARAMS = 11
 EXPORTS = ("amplfi_last_error", "amplfi_psd_scale", "amplfi_version", "amplfi_phenomd_table",
            "amplfi_plan_create", "amplfi_plan_destroy", "amplfi_waveform_fd", "amplfi_project",
            "amplfi_psd_welch", "amplfi_inject_whiten", "amplfi_launch_count", "amplfi_plan_set_timing",
-           "amplfi_plan_kernel_times", "amplfi_assemble_batch", "amplfi_probe_fp32_pipe")
+           "amplfi_plan_kernel_times", "amplfi_assemble_batch", "amplfi_probe_fp32_pipe",
+           "amplfi_inject_whiten_views", "amplfi_waveform_td", "amplfi_inject_whiten_fir")
 
 
 class AmplfiError(RuntimeError):
@@ -34,7 +35,7 @@ class AmplfiError(RuntimeError):
 
 def _load():
     if not os.path.exists(LIB_PATH):
-        raise ImportError("libamplfi.so not found at %s: build it with `python -m paper_2407_19048_b200.build` "
+        raise ImportError("libamplfi.so not found at %s: build it with `python paper_2407_19048_b200/build.py` "
                           "(there is no CPU fallback)" % LIB_PATH)
     lib = ctypes.CDLL(LIB_PATH)
     c = ctypes
@@ -69,10 +70,19 @@ def _load():
     lib.amplfi_probe_fp32_pipe.argtypes = [c.POINTER(dbl)]
     lib.amplfi_assemble_batch.restype = i32
     lib.amplfi_assemble_batch.argtypes = [vp, i32, vp, i64, i64, i32, i32, vp, vp, vp, i64, i32, vp, dbl, dbl, dbl, vp, vp]
+    lib.amplfi_inject_whiten_views.restype = i32
+    lib.amplfi_inject_whiten_views.argtypes = [vp, i32, vp, vp, i64, i32, vp, vp, dbl, vp, i32, dbl, dbl, vp, vp, vp]
+    lib.amplfi_waveform_td.restype = i32
+    lib.amplfi_waveform_td.argtypes = [vp, i32, i32, vp, dbl, dbl, vp, vp, vp]
+    lib.amplfi_inject_whiten_fir.restype = i32
+    lib.amplfi_inject_whiten_fir.argtypes = [vp, i32, vp, vp, i64, vp, i32, vp, dbl, vp, i32, dbl, dbl, dbl, i32, vp, vp]
     return lib
 
 
-_lib = _load()
+try:
+    _lib = _load()
+except AttributeError as exc:      # a symbol of include/amplfi.h is missing: the .so predates the sources
+    raise ImportError("libamplfi.so is stale (%s): rebuild it with `python paper_2407_19048_b200/build.py --force`" % exc)
 
 
 def _check(rc):
@@ -216,6 +226,55 @@ def amplfi_inject_whiten(plan, batch, noise, psd, f_lo, f_hi, offsets=None, h_de
                                      _ptr(params, torch.float64, "params"), float(gmst),
                                      _ptr(psd, torch.float32, "psd"), int(psd.shape[-1]), float(f_lo), float(f_hi),
                                      _ptr(out, torch.float32, "out"), _stream(stream)))
+    return out
+
+
+def amplfi_inject_whiten_views(plan, batch, noise, psd, f_lo, f_hi, params, t_shift, offsets=None, approximant=IMRPHENOMD,
+                               gmst=0.0, out=None, out2=None, stream=None):
+    """Two views (d, d') of PAPER.md:93, :117: out2 repeats out with t_c + t_shift[b].  -> (out, out2) [B, D, N] fp32."""
+    if out is None:
+        out = torch.empty((batch, plan.n_det, plan.n), dtype=torch.float32, device=noise.device)
+    if out2 is None:
+        out2 = torch.empty((batch, plan.n_det, plan.n), dtype=torch.float32, device=noise.device)
+    strip_len = int(noise.shape[-1]) if offsets is not None else 0
+    _check(_lib.amplfi_inject_whiten_views(plan._h, int(batch), _ptr(noise, torch.float32, "noise"),
+                                           _ptr(offsets, torch.int64, "offsets"), strip_len, int(approximant),
+                                           _ptr(params, torch.float64, "params"), _ptr(t_shift, torch.float64, "t_shift"),
+                                           float(gmst), _ptr(psd, torch.float32, "psd"), int(psd.shape[-1]), float(f_lo),
+                                           float(f_hi), _ptr(out, torch.float32, "out"), _ptr(out2, torch.float32, "out2"),
+                                           _stream(stream)))
+    return out, out2
+
+
+def amplfi_waveform_td(plan, approximant, params, f_lo, f_hi, h_t=None, flags=None, stream=None):
+    """params [B, 11] fp64 cuda -> h_t [B, 2, N] fp32 (row 0 h+(t), row 1 hx(t)), flags [B] int32."""
+    batch = params.shape[0]
+    if h_t is None:
+        h_t = torch.empty((batch, 2, plan.n), dtype=torch.float32, device=params.device)
+    if flags is None:
+        flags = torch.empty((batch,), dtype=torch.int32, device=params.device)
+    _check(_lib.amplfi_waveform_td(plan._h, int(approximant), int(batch), _ptr(params, torch.float64, "params"), float(f_lo),
+                                   float(f_hi), _ptr(h_t, torch.float32, "h_t"), _ptr(flags, torch.int32, "flags"),
+                                   _stream(stream)))
+    return h_t, flags
+
+
+def amplfi_inject_whiten_fir(plan, batch, noise, psd, f_lo, f_hi, fduration, crop=True, offsets=None, h_det=None,
+                             approximant=IMRPHENOMD, params=None, gmst=0.0, out=None, stream=None):
+    """amplfi_inject_whiten with the whitening filter truncated to fduration seconds; crop drops fduration/2 at each
+    end -> out [B, D, N - fduration*fs] (crop) or [B, D, N]."""
+    ntaps = int(round(fduration * plan.fs))
+    n_out = max(plan.n - ntaps, 2) if crop else plan.n      # invalid fduration: the library reports it
+    if out is None:
+        out = torch.empty((batch, plan.n_det, n_out), dtype=torch.float32, device=noise.device)
+    strip_len = int(noise.shape[-1]) if offsets is not None else 0
+    _check(_lib.amplfi_inject_whiten_fir(plan._h, int(batch), _ptr(noise, torch.float32, "noise"),
+                                         _ptr(offsets, torch.int64, "offsets"), strip_len,
+                                         _ptr(h_det, torch.float32, "h_det"), int(approximant),
+                                         _ptr(params, torch.float64, "params"), float(gmst),
+                                         _ptr(psd, torch.float32, "psd"), int(psd.shape[-1]), float(f_lo), float(f_hi),
+                                         float(fduration), 1 if crop else 0, _ptr(out, torch.float32, "out"),
+                                         _stream(stream)))
     return out
 
 

@@ -29,9 +29,14 @@ struct amplfi_plan {
     double* pd_table;      // [19*11]
     amplfi::WfCoef* coef;  // [max_batch]
     amplfi::DetResp* resp; // [max_batch * n_det]
+    amplfi::DetResp* resp2; // [max_batch * 3]  second view: resp with dt + t_shift[b]; also the two "polarisation detectors" of
+                           //                  amplfi_waveform_td ((F+, Fx, dt) = (1,0,0), (0,1,0) per sample)
     float2* h0;            // [max_batch * n_bins]   fused path: 2 fs h0
     float* filt;           // [n_det * filt_stride]  whitening filter incl. 1/(2n); rows padded to 16 B
     int filt_stride;       // n_bins rounded up to a multiple of 4
+    float* filt_flat;      // [filt_stride] constant 1/(2n): the "no filter" row of the inverse-only launches
+    float2* fir_spec;      // [n_det * n_bins]  truncated-filter construction: spectrum-side workspace
+    float* fir_time;       // [n_det * n]       truncated-filter construction: time-side workspace
     float* welch_part;     // [n_det * max_seg * (nperseg/2+1)]
     int welch_max_seg;
     int* d_det_ids;        // [3]
@@ -62,13 +67,14 @@ int launch_project(const amplfi_plan* p, int batch, const float* hp, const float
 int launch_tables(amplfi_plan* p, cudaStream_t st);
 
 // welch.cu
-int launch_welch(const amplfi_plan* p, const float* bg, long n_bg, long row_stride, int noverlap, int detrend, float* psd,
-                 cudaStream_t st);
+int launch_welch(const amplfi_plan* p, const float* bg, long n_bg, long row_stride, int noverlap, int detrend, int average,
+                 float* psd, cudaStream_t st);
 
 enum { MODE_NONE = 0, MODE_HDET = 1, MODE_FUSED = 2 };
 
 struct IwArgs {
-    const float* noise;       // dense [B, D, N] or strip [D, L]
+    const float* noise;       // dense [B, D, N] or strip [D, L]; nullptr: no data, the spectrum starts at zero and the
+                              // forward transform is skipped (inverse-only launches: time-domain waveform, filter design)
     const long* offsets;      // nullptr: dense
     long strip_len;
     const float2* h_det;      // MODE_HDET: [B, D, K]
@@ -77,11 +83,21 @@ struct IwArgs {
     const DetResp* resp;
     const float* filt;        // [D, filt_stride]
     int filt_stride;
-    float* out;               // [B, D, N]
+    float* out;               // [B, D, N - 2 crop]
+    int crop;                 // samples dropped at each end of every output row (even)
     int n_det;
     float two_fs;
     float inv_tseg;
     int prefetch_ahead;       // units ahead whose noise segment is prefetched into L2 (packed kernel)
+};
+
+// optional overrides of launch_inject_whiten (defaults: the plan's detectors, responses and filter, no crop)
+struct IwOpts {
+    int n_det;                // units per sample (2 for the polarisations of amplfi_waveform_td, 1 for filter design)
+    const DetResp* resp;      // nullptr: plan->resp
+    const float* filt;        // nullptr: plan->filt
+    int filt_stride;
+    int crop;
 };
 
 // inject_whiten13.cu (packed 4-pass kernel for n = 16384)
@@ -90,12 +106,15 @@ int launch_iw13(const IwArgs& a, int mode, int units, cudaStream_t st);
 // inject_whiten.cu
 int launch_filter(const amplfi_plan* p, const float* psd, int n_psd, double f_lo, double f_hi, cudaStream_t st);
 int launch_inject_whiten(const amplfi_plan* p, int batch, const float* noise, const long* offsets,
-                         long strip_len, const float* h_det, int fused, float* out, cudaStream_t st);
+                         long strip_len, const float* h_det, int fused, float* out, cudaStream_t st,
+                         const IwOpts* opts = nullptr);
+int launch_fir_truncate(const amplfi_plan* p, double fduration, cudaStream_t st);
+int launch_shift_resp(const amplfi_plan* p, int batch, const double* t_shift, cudaStream_t st);
+int launch_td_resp(const amplfi_plan* p, int batch, cudaStream_t st);
 int setup_inject_whiten_attrs();
 
 // inject_whiten_long.cu (n = 65536: decimation by two around the 32768-sample transform)
 size_t long_scratch_floats2(int chunk_units);
-int launch_inject_whiten_long(const amplfi_plan* p, int batch, const float* noise, const long* offsets, long strip_len,
-                              const float* h_det, int fused, float* out, cudaStream_t st);
+int launch_inject_whiten_long(const amplfi_plan* p, const IwArgs& a, int mode, int units, cudaStream_t st);
 
 }  // namespace amplfi

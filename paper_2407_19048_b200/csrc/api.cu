@@ -75,6 +75,11 @@ __global__ void __launch_bounds__(256) fp32_probe_kernel(unsigned long long* out
     out[blockIdx.x * blockDim.x + threadIdx.x] = s;
 }
 
+__global__ void fill_kernel(float* dst, int count, float v) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < count) dst[i] = v;
+}
+
 extern "C" int amplfi_probe_fp32_pipe(double* lane_ops_per_s) {
     if (lane_ops_per_s == nullptr) { set_error("amplfi_probe_fp32_pipe: null pointer"); return AMPLFI_ERR_INVALID_ARG; }
     int dev = 0, sms = 0;
@@ -159,9 +164,13 @@ int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_
     if (!rc) rc = dev_alloc(&p->pd_table, (size_t)AMPLFI_PD_ROWS * AMPLFI_PD_COLS);
     if (!rc) rc = dev_alloc(&p->coef, (size_t)max_batch);
     if (!rc) rc = dev_alloc(&p->resp, (size_t)max_batch * n_det);
+    if (!rc) rc = dev_alloc(&p->resp2, (size_t)max_batch * 3);
     if (!rc) rc = dev_alloc(&p->h0, (size_t)max_batch * p->n_bins);
     p->filt_stride = (p->n_bins + 3) & ~3;
     if (!rc) rc = dev_alloc(&p->filt, (size_t)n_det * p->filt_stride);
+    if (!rc) rc = dev_alloc(&p->filt_flat, (size_t)p->filt_stride);
+    if (!rc) rc = dev_alloc(&p->fir_spec, (size_t)n_det * p->n_bins);
+    if (!rc) rc = dev_alloc(&p->fir_time, (size_t)n_det * n);
     if (!rc) rc = dev_alloc(&p->d_det_ids, (size_t)3);
     if (!rc && p->logm == 15) {
         p->long_chunk = sms > 0 ? sms : 148;          // 2 CTAs per unit: two full waves of one CTA per SM; 39 MB of spectra
@@ -180,6 +189,11 @@ int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_
         if (e != cudaSuccess) { set_error("amplfi_plan_create: stream/event: %s", cudaGetErrorString(e)); rc = AMPLFI_ERR_CUDA; }
     }
     if (!rc) rc = launch_tables(p, nullptr);
+    if (!rc) {
+        fill_kernel<<<(p->filt_stride + 255) / 256, 256>>>(p->filt_flat, p->filt_stride, (float)(1.0 / (2.0 * (double)n)));
+        count_launch();
+        rc = check_launch("fill_kernel");
+    }
     if (!rc) {
         e = cudaStreamSynchronize(nullptr);
         if (e != cudaSuccess) { set_error("amplfi_plan_create: %s", cudaGetErrorString(e)); rc = AMPLFI_ERR_CUDA; }
@@ -223,6 +237,7 @@ void amplfi_plan_destroy(amplfi_plan* p) {
     if (p->ev_fork) cudaEventDestroy(p->ev_fork);
     if (p->ev_join) cudaEventDestroy(p->ev_join);
     cudaFree(p->tab_ci); cudaFree(p->tab_lnk); cudaFree(p->pd_table); cudaFree(p->coef); cudaFree(p->resp);
+    cudaFree(p->resp2); cudaFree(p->filt_flat); cudaFree(p->fir_spec); cudaFree(p->fir_time);
     cudaFree(p->h0); cudaFree(p->filt); cudaFree(p->welch_part); cudaFree(p->d_det_ids); cudaFree(p->long_spec);
     delete p;
 }
@@ -260,12 +275,12 @@ int amplfi_psd_welch(const amplfi_plan* p, const float* bg, long n_bg, long row_
     if (p == nullptr || bg == nullptr || psd == nullptr) { set_error("amplfi_psd_welch: null pointer"); return AMPLFI_ERR_INVALID_ARG; }
     if (p->nperseg == 0) { set_error("amplfi_psd_welch: plan was created with nperseg = 0"); return AMPLFI_ERR_INVALID_ARG; }
     if (n_bg < p->nperseg) { set_error("amplfi_psd_welch: nperseg %d > n_bg %ld", p->nperseg, n_bg); return AMPLFI_ERR_UNSUPPORTED_SIZE; }
-    if (noverlap < 0 || noverlap >= p->nperseg || (detrend != 0 && detrend != 1) || average != 0) {
-        set_error("amplfi_psd_welch: need 0 <= noverlap < nperseg, detrend in {0,1}, average = 0 (mean)");
+    if (noverlap < 0 || noverlap >= p->nperseg || (detrend != 0 && detrend != 1) || (average != 0 && average != 1)) {
+        set_error("amplfi_psd_welch: need 0 <= noverlap < nperseg, detrend in {0,1}, average in {0 mean, 1 median}");
         return AMPLFI_ERR_INVALID_ARG;
     }
     if (row_stride < n_bg) { set_error("amplfi_psd_welch: row_stride %ld < n_bg %ld", row_stride, n_bg); return AMPLFI_ERR_INVALID_ARG; }
-    return launch_welch(p, bg, n_bg, row_stride, noverlap, detrend, psd, static_cast<cudaStream_t>(stream));
+    return launch_welch(p, bg, n_bg, row_stride, noverlap, detrend, average, psd, static_cast<cudaStream_t>(stream));
 }
 
 int amplfi_inject_whiten(const amplfi_plan* p, int batch, const float* noise, const long* offsets, long strip_len,
@@ -324,7 +339,7 @@ int amplfi_assemble_batch(const amplfi_plan* p, int batch, const float* bg, long
     cudaError_t e = cudaEventRecord(mp->ev_fork, st);
     if (e == cudaSuccess) e = cudaStreamWaitEvent(mp->side, mp->ev_fork, 0);
     if (e != cudaSuccess) { set_error("amplfi_assemble_batch: fork: %s", cudaGetErrorString(e)); return AMPLFI_ERR_CUDA; }
-    rc = launch_welch(p, bg, n_bg, row_stride, noverlap, detrend, psd, mp->side);
+    rc = launch_welch(p, bg, n_bg, row_stride, noverlap, detrend, 0, psd, mp->side);
     if (!rc) rc = launch_filter(p, psd, n_psd, f_lo, f_hi, mp->side);
     e = cudaEventRecord(mp->ev_join, mp->side);
     if (!rc) rc = launch_prepare(p, approximant, batch, params, gmst, f_lo, f_hi, 2.0 * p->fs, nullptr, st);
@@ -338,6 +353,86 @@ int amplfi_assemble_batch(const amplfi_plan* p, int batch, const float* bg, long
     rc = launch_inject_whiten(p, batch, noise, offsets, strip_len, nullptr, 1, out, st);
     if (timed) { cudaEventRecord(mp->ev_stop[p->ev_count], st); mp->ev_count++; }
     return rc;
+}
+
+// shared validation of the inject/whiten family
+static int validate_iw(const amplfi_plan* p, const char* who, int batch, const float* noise, const long* offsets, long strip_len,
+                       const float* psd, int n_psd, double f_lo, double f_hi, const float* out) {
+    if (p == nullptr || noise == nullptr || psd == nullptr || out == nullptr) { set_error("%s: null pointer", who); return AMPLFI_ERR_INVALID_ARG; }
+    if (batch < 1 || batch > p->max_batch) { set_error("%s: batch %d outside [1, %d]", who, batch, p->max_batch); return AMPLFI_ERR_INVALID_ARG; }
+    int rc = validate_band(p, f_lo, f_hi, who);
+    if (rc) return rc;
+    if (offsets != nullptr && strip_len < p->n) { set_error("%s: strip_len %ld < n %d", who, strip_len, p->n); return AMPLFI_ERR_INVALID_ARG; }
+    if (n_psd < 2 || ((p->n / 2) % (n_psd - 1)) != 0) { set_error("%s: n_psd = %d does not divide the segment grid (n/2 = %d)", who, n_psd, p->n / 2); return AMPLFI_ERR_INVALID_ARG; }
+    if ((reinterpret_cast<size_t>(out) & 7) || (reinterpret_cast<size_t>(noise) & 3)) { set_error("%s: out must be 8-byte aligned, noise 4-byte aligned", who); return AMPLFI_ERR_ALIGNMENT; }
+    return AMPLFI_OK;
+}
+
+int amplfi_inject_whiten_views(const amplfi_plan* p, int batch, const float* noise, const long* offsets, long strip_len,
+                               int approximant, const double* params, const double* t_shift, double gmst,
+                               const float* psd, int n_psd, double f_lo, double f_hi, float* out, float* out2,
+                               void* stream) {
+    int rc = validate_iw(p, "amplfi_inject_whiten_views", batch, noise, offsets, strip_len, psd, n_psd, f_lo, f_hi, out);
+    if (rc) return rc;
+    if (params == nullptr || t_shift == nullptr || out2 == nullptr) { set_error("amplfi_inject_whiten_views: null pointer"); return AMPLFI_ERR_INVALID_ARG; }
+    if (reinterpret_cast<size_t>(out2) & 7) { set_error("amplfi_inject_whiten_views: out2 must be 8-byte aligned"); return AMPLFI_ERR_ALIGNMENT; }
+    if (approximant != AMPLFI_TAYLORF2 && approximant != AMPLFI_IMRPHENOMD) { set_error("amplfi_inject_whiten_views: unknown approximant %d", approximant); return AMPLFI_ERR_INVALID_ARG; }
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    rc = launch_filter(p, psd, n_psd, f_lo, f_hi, st);
+    if (!rc) rc = launch_prepare(p, approximant, batch, params, gmst, f_lo, f_hi, 2.0 * p->fs, nullptr, st);
+    if (!rc) rc = launch_waveform_h0(p, batch, st);
+    if (!rc) rc = launch_shift_resp(p, batch, t_shift, st);
+    if (!rc) rc = launch_inject_whiten(p, batch, noise, offsets, strip_len, nullptr, 1, out, st);
+    if (rc) return rc;
+    IwOpts o;
+    o.n_det = p->n_det; o.resp = p->resp2; o.filt = nullptr; o.filt_stride = 0; o.crop = 0;
+    return launch_inject_whiten(p, batch, noise, offsets, strip_len, nullptr, 1, out2, st, &o);
+}
+
+int amplfi_waveform_td(const amplfi_plan* p, int approximant, int batch, const double* params, double f_lo, double f_hi,
+                       float* h_t, int* flags, void* stream) {
+    if (p == nullptr || params == nullptr || h_t == nullptr) { set_error("amplfi_waveform_td: null pointer"); return AMPLFI_ERR_INVALID_ARG; }
+    if (batch < 1 || batch > p->max_batch) { set_error("amplfi_waveform_td: batch %d outside [1, %d]", batch, p->max_batch); return AMPLFI_ERR_INVALID_ARG; }
+    if (approximant != AMPLFI_TAYLORF2 && approximant != AMPLFI_IMRPHENOMD) { set_error("amplfi_waveform_td: unknown approximant %d", approximant); return AMPLFI_ERR_INVALID_ARG; }
+    int rc = validate_band(p, f_lo, f_hi, "amplfi_waveform_td");
+    if (rc) return rc;
+    if (reinterpret_cast<size_t>(h_t) & 7) { set_error("amplfi_waveform_td: h_t must be 8-byte aligned"); return AMPLFI_ERR_ALIGNMENT; }
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    rc = launch_prepare(p, approximant, batch, params, 0.0, f_lo, f_hi, 2.0 * p->fs, flags, st);
+    if (!rc) rc = launch_waveform_h0(p, batch, st);
+    if (!rc) rc = launch_td_resp(p, batch, st);
+    if (rc) return rc;
+    IwOpts o;
+    o.n_det = 2; o.resp = p->resp2; o.filt = p->filt_flat; o.filt_stride = 0; o.crop = 0;
+    return launch_inject_whiten(p, batch, nullptr, nullptr, 0, nullptr, 1, h_t, st, &o);
+}
+
+int amplfi_inject_whiten_fir(const amplfi_plan* p, int batch, const float* noise, const long* offsets, long strip_len,
+                             const float* h_det, int approximant, const double* params, double gmst, const float* psd,
+                             int n_psd, double f_lo, double f_hi, double fduration, int crop, float* out, void* stream) {
+    int rc = validate_iw(p, "amplfi_inject_whiten_fir", batch, noise, offsets, strip_len, psd, n_psd, f_lo, f_hi, out);
+    if (rc) return rc;
+    const long ntaps = llrint(fduration * p->fs);
+    if (!(fduration > 0.0) || ntaps < 2 || ntaps > p->n || (ntaps & 3) || std::fabs((double)ntaps - fduration * p->fs) > 1e-6) {
+        set_error("amplfi_inject_whiten_fir: fduration * fs must be a multiple of 4 in [4, n] (got %g s)", fduration);
+        return AMPLFI_ERR_INVALID_ARG;
+    }
+    if (crop != 0 && crop != 1) { set_error("amplfi_inject_whiten_fir: crop must be 0 or 1"); return AMPLFI_ERR_INVALID_ARG; }
+    if (crop && ntaps >= p->n) { set_error("amplfi_inject_whiten_fir: nothing left after cropping"); return AMPLFI_ERR_INVALID_ARG; }
+    const bool fused = (h_det == nullptr && params != nullptr);
+    if (fused && approximant != AMPLFI_TAYLORF2 && approximant != AMPLFI_IMRPHENOMD) { set_error("amplfi_inject_whiten_fir: unknown approximant %d", approximant); return AMPLFI_ERR_INVALID_ARG; }
+    if (reinterpret_cast<size_t>(h_det) & 7) { set_error("amplfi_inject_whiten_fir: h_det must be 8-byte aligned"); return AMPLFI_ERR_ALIGNMENT; }
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    rc = launch_filter(p, psd, n_psd, f_lo, f_hi, st);
+    if (!rc) rc = launch_fir_truncate(p, fduration, st);
+    if (!rc && fused) {
+        rc = launch_prepare(p, approximant, batch, params, gmst, f_lo, f_hi, 2.0 * p->fs, nullptr, st);
+        if (!rc) rc = launch_waveform_h0(p, batch, st);
+    }
+    if (rc) return rc;
+    IwOpts o;
+    o.n_det = p->n_det; o.resp = nullptr; o.filt = nullptr; o.filt_stride = 0; o.crop = crop ? (int)(ntaps / 2) : 0;
+    return launch_inject_whiten(p, batch, noise, offsets, strip_len, h_det, fused ? 1 : 0, out, st, &o);
 }
 
 }  // extern "C"

@@ -53,6 +53,57 @@ int launch_filter(const amplfi_plan* p, const float* psd, int n_psd, double f_lo
     return check_launch("filter_kernel");
 }
 
+// ---- time-truncated whitening filter (reading R-I8) ----
+// The filter w (real, on the segment grid) has a real even impulse response q = irfft(w); q is tapered to ntaps samples
+// around lag 0 with a Hann window and transformed back.  Both transforms are INVERSE real transforms of a real "spectrum"
+// (for a real even sequence the forward transform equals n times the inverse one), so they run through the inverse half
+// of the segment kernel (noise == nullptr, MODE_HDET) with one unit per detector:
+//   time = fs * irfft(spec)   (two_fs * spec * 1/(2n), unnormalised inverse)
+__global__ void fir_real_to_spec_kernel(const float* __restrict__ src, int src_stride, int n_bins, float mul, int ntaps,
+                                        float2* __restrict__ spec) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const int d = blockIdx.y;
+    if (k >= n_bins) return;
+    float v = src[(size_t)d * src_stride + k] * mul;
+    if (ntaps > 0) {                                       // Hann taper centred on lag 0; lags k <= n/2 only (q is even)
+        v = (2 * k < ntaps) ? v * (0.5f + 0.5f * cospif(2.0f * (float)k / (float)ntaps)) : 0.f;
+    }
+    spec[(size_t)d * n_bins + k] = make_float2(v, 0.f);
+}
+
+__global__ void fir_time_to_filt_kernel(const float* __restrict__ time, int n, int n_bins, float mul, float* __restrict__ filt,
+                                        int filt_stride) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const int d = blockIdx.y;
+    if (k >= filt_stride) return;
+    filt[(size_t)d * filt_stride + k] = k < n_bins ? time[(size_t)d * n + k] * mul : 0.f;
+}
+
+// plan->filt (already holding the band-limited filter of launch_filter) is replaced by its time-truncated version.
+int launch_fir_truncate(const amplfi_plan* p, double fduration, cudaStream_t st) {
+    const int ntaps = (int)llrint(fduration * p->fs);
+    const int nb = p->n_bins;
+    const float inv_fs = (float)(1.0 / p->fs);
+    dim3 gb((nb + 255) / 256, p->n_det), gf((p->filt_stride + 255) / 256, p->n_det);
+    IwOpts o;
+    o.n_det = 1; o.resp = nullptr; o.filt = p->filt_flat; o.filt_stride = 0; o.crop = 0;
+    // q = irfft(w): time = fs q
+    fir_real_to_spec_kernel<<<gb, 256, 0, st>>>(p->filt, p->filt_stride, nb, 1.0f, 0, p->fir_spec);
+    count_launch();
+    int rc = launch_inject_whiten(p, p->n_det, nullptr, nullptr, 0, reinterpret_cast<const float*>(p->fir_spec), 0,
+                                  p->fir_time, st, &o);
+    if (rc) return rc;
+    // q' = taper(q) on lags 0 .. n/2; W' = rfft(q') = n irfft(q'[0 .. n/2]): time = fs W' / n
+    fir_real_to_spec_kernel<<<gb, 256, 0, st>>>(p->fir_time, p->n, nb, inv_fs, ntaps, p->fir_spec);
+    count_launch();
+    rc = launch_inject_whiten(p, p->n_det, nullptr, nullptr, 0, reinterpret_cast<const float*>(p->fir_spec), 0, p->fir_time,
+                              st, &o);
+    if (rc) return rc;
+    fir_time_to_filt_kernel<<<gf, 256, 0, st>>>(p->fir_time, p->n, nb, (float)((double)p->n / p->fs), p->filt, p->filt_stride);
+    count_launch();
+    return check_launch("fir_truncate");
+}
+
 template <int LOGM, int MODE>
 __global__ void __launch_bounds__(Fft<LOGM>::T) inject_whiten_kernel(const IwArgs a) {
     using F = Fft<LOGM>;
@@ -62,13 +113,16 @@ __global__ void __launch_bounds__(Fft<LOGM>::T) inject_whiten_kernel(const IwArg
     const int b = unit / a.n_det, d = unit - b * a.n_det;
 
     // ---- a-5 gather ----
-    const float* x;
-    float* out = a.out + (size_t)unit * N;
-    if (a.offsets != nullptr) {
+    const float* x = nullptr;
+    const int n_out = N - 2 * a.crop;
+    float* out = a.out + (size_t)unit * n_out;
+    if (a.noise == nullptr) {
+        // inverse-only launch: no data, the spectrum starts at zero
+    } else if (a.offsets != nullptr) {
         const long off = a.offsets[unit];
         if (off < 0 || off + N > a.strip_len) {            // never read out of bounds: poison the row instead
             const float qnan = __int_as_float(0x7fc00000);
-            for (int i = tid; i < N; i += T) out[i] = qnan;
+            for (int i = tid; i < n_out; i += T) out[i] = qnan;
             return;
         }
         x = a.noise + (size_t)d * a.strip_len + off;
@@ -76,9 +130,13 @@ __global__ void __launch_bounds__(Fft<LOGM>::T) inject_whiten_kernel(const IwArg
         x = a.noise + (size_t)unit * N;
     }
     const bool aligned8 = ((reinterpret_cast<size_t>(x) & 7) == 0);
+    int klow_a, klow_b;
+    pass_c_klow<LOGM>(tid, klow_a, klow_b);
+    float2 va[RC], vb[RC];
 
     // ---- a-6 forward real FFT (packed as M complex points) ----
-    {
+    if (x != nullptr) {
+      {
         float2 v[F::NA][RA];
         if (aligned8) {
             const float2* x2 = reinterpret_cast<const float2*>(x);
@@ -97,22 +155,24 @@ __global__ void __launch_bounds__(Fft<LOGM>::T) inject_whiten_kernel(const IwArg
         }
 #pragma unroll
         for (int i = 0; i < F::NA; ++i) F::pass_a_fwd(v[i], tid + i * T, sm);
-    }
-    __syncthreads();
+      }
+      __syncthreads();
 #pragma unroll
-    for (int i = 0; i < F::NB; ++i) F::pass_b_fwd(tid + i * T, sm);
-    __syncthreads();
-    int klow_a, klow_b;
-    pass_c_klow<LOGM>(tid, klow_a, klow_b);
-    float2 va[RC], vb[RC];
-    F::pass_c_fwd(klow_a, va, sm);
-    F::pass_c_fwd(klow_b, vb, sm);
+      for (int i = 0; i < F::NB; ++i) F::pass_b_fwd(tid + i * T, sm);
+      __syncthreads();
+      F::pass_c_fwd(klow_a, va, sm);
+      F::pass_c_fwd(klow_b, vb, sm);
+    } else {
+#pragma unroll
+      for (int i = 0; i < RC; ++i) va[i] = vb[i] = make_float2(0.f, 0.f);
+    }
 
     // ---- a-7 inject, a-8 whiten + band-limit (registers) ----
     const float* filt = a.filt + (size_t)d * a.filt_stride;
     const float2* hsrc = nullptr;
     int w_lo = 1, w_hi = 0;
-    float cre = 0.f, cim = 0.f, delta = 0.f;
+    float cre = 0.f, cim = 0.f;
+    double delta = 0.0;
     if (MODE == MODE_HDET) hsrc = a.h_det + (size_t)unit * K;
     if (MODE == MODE_FUSED) {
         const WfCoef* c = a.coef + b;
@@ -121,7 +181,7 @@ __global__ void __launch_bounds__(Fft<LOGM>::T) inject_whiten_kernel(const IwArg
         const DetResp r = a.resp[unit];
         cre = (float)r.fp * c->pol_p;                       // C = F+ (1+cos^2 i)/2 - i Fx cos i
         cim = -(float)r.fc * c->pol_c;
-        delta = (float)(r.dt * (double)a.inv_tseg);          // turns per bin
+        delta = r.dt * (double)a.inv_tseg;                   // turns per bin (fp64: the second view's dt reaches 1 s)
     }
     auto inject = [&](int k, float2& x2) {
         if (MODE == MODE_HDET) {
@@ -131,10 +191,10 @@ __global__ void __launch_bounds__(Fft<LOGM>::T) inject_whiten_kernel(const IwArg
         } else if (MODE == MODE_FUSED) {
             if (k >= w_lo && k <= w_hi) {
                 const float2 h = __ldg(hsrc + k);
-                float turns = (float)k * delta;
-                turns -= rintf(turns);
+                double td = (double)k * delta;
+                td -= rint(td);
                 float s, co;
-                __sincosf(turns * -6.283185307179586f, &s, &co);          // exp(-2 pi i k dt / T)
+                __sincosf((float)td * -6.283185307179586f, &s, &co);      // exp(-2 pi i k dt / T)
                 const float2 cp = make_float2(cre * co - cim * s, cre * s + cim * co);
                 x2.x += h.x * cp.x - h.y * cp.y;
                 x2.y += h.x * cp.y + h.y * cp.x;
@@ -184,8 +244,17 @@ __global__ void __launch_bounds__(Fft<LOGM>::T) inject_whiten_kernel(const IwArg
     for (int i = 0; i < F::NA; ++i) {
         float2 v[RA];
         F::pass_a_inv(v, tid + i * T, sm);
+        if (a.crop == 0) {
 #pragma unroll
-        for (int nA = 0; nA < RA; ++nA) __stcs(out2 + nA * LB + tid + i * T, v[nA]);
+            for (int nA = 0; nA < RA; ++nA) __stcs(out2 + nA * LB + tid + i * T, v[nA]);
+        } else {
+            const int c2 = a.crop >> 1;                      // crop is even: whole float2 pairs
+#pragma unroll
+            for (int nA = 0; nA < RA; ++nA) {
+                const int m = nA * LB + tid + i * T;
+                if (m >= c2 && m < M - c2) __stcs(out2 + m - c2, v[nA]);
+            }
+        }
     }
 }
 
@@ -214,15 +283,23 @@ static int launch_iw_mode(const IwArgs& a, int mode, int units, cudaStream_t st)
 }
 
 int launch_inject_whiten(const amplfi_plan* p, int batch, const float* noise, const long* offsets,
-                         long strip_len, const float* h_det, int fused, float* out, cudaStream_t st) {
+                         long strip_len, const float* h_det, int fused, float* out, cudaStream_t st,
+                         const IwOpts* opts) {
     IwArgs a;
     a.noise = noise; a.offsets = offsets; a.strip_len = strip_len;
     a.h_det = reinterpret_cast<const float2*>(h_det);
     a.h0 = p->h0; a.coef = p->coef; a.resp = p->resp; a.filt = p->filt; a.filt_stride = p->filt_stride; a.out = out;
+    a.crop = 0;
     a.n_det = p->n_det; a.two_fs = (float)(2.0 * p->fs); a.inv_tseg = (float)(1.0 / p->t_seg);
     a.prefetch_ahead = 2 * p->sm_count;
+    if (opts != nullptr) {
+        a.n_det = opts->n_det;
+        if (opts->resp != nullptr) a.resp = opts->resp;
+        if (opts->filt != nullptr) { a.filt = opts->filt; a.filt_stride = opts->filt_stride; }
+        a.crop = opts->crop;
+    }
     const int mode = h_det != nullptr ? MODE_HDET : (fused ? MODE_FUSED : MODE_NONE);
-    const int units = batch * p->n_det;
+    const int units = batch * a.n_det;
     switch (p->logm) {
         case 9: return launch_iw_mode<9>(a, mode, units, st);
         case 10: return launch_iw_mode<10>(a, mode, units, st);
@@ -230,7 +307,7 @@ int launch_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
         case 12: return launch_iw_mode<12>(a, mode, units, st);
         case 13: return launch_iw13(a, mode, units, st);
         case 14: return launch_iw_mode<14>(a, mode, units, st);
-        case 15: return launch_inject_whiten_long(p, batch, noise, offsets, strip_len, h_det, fused, out, st);
+        case 15: return launch_inject_whiten_long(p, a, mode, units, st);
         default:
             set_error("amplfi_inject_whiten: segment length %d not supported by this build", p->n);
             return AMPLFI_ERR_UNSUPPORTED_SIZE;

@@ -22,13 +22,16 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
     const int b = unit / a.n_det, d = unit - b * a.n_det;
 
     // ---- a-5 gather ----
-    const float* x;
-    float* out = a.out + (size_t)unit * N;
-    if (a.offsets != nullptr) {
+    const float* x = nullptr;
+    const int n_out = N - 2 * a.crop;
+    float* out = a.out + (size_t)unit * n_out;
+    const bool fwd = a.noise != nullptr;                   // false: inverse-only launch, the spectrum starts at zero
+    if (!fwd) {
+    } else if (a.offsets != nullptr) {
         const long off = a.offsets[unit];
         if (off < 0 || off + N > a.strip_len) {            // never read out of bounds: poison the row instead
             const float qnan = __int_as_float(0x7fc00000);
-            for (int i = tt; i < N; i += TT) out[i] = qnan;
+            for (int i = tt; i < n_out; i += TT) out[i] = qnan;
             return;
         }
         x = a.noise + (size_t)d * a.strip_len + off;
@@ -38,7 +41,7 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
 
     // L2 prefetch of the segment a CTA one wave later will gather (one bulk instruction for the whole 64 KB):
     // the head-of-CTA loads then hit L2 instead of waiting on HBM.
-    if (tt == 0) {
+    if (tt == 0 && fwd) {
         const int nu = unit + a.prefetch_ahead;
         if (nu < units) {
             const float* nx;
@@ -58,7 +61,7 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
     }
 
     // ---- a-6 forward real FFT of the packed sequence z[m] = x[2m] + i x[2m+1] ----
-    {
+    if (fwd) {
         float2 z[VT][16];
         if ((reinterpret_cast<size_t>(x) & 7) == 0) {
             const float2* x2 = reinterpret_cast<const float2*>(x);
@@ -79,13 +82,16 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
         for (int vt = 0; vt < VT; ++vt) p1_fwd(z[vt], tt + vt * TT, re, im);
     }
     __syncthreads();
+    if (fwd) {
 #pragma unroll
-    for (int vt = 0; vt < VT; ++vt) p2_fwd(tt + vt * TT, re, im);
+        for (int vt = 0; vt < VT; ++vt) p2_fwd(tt + vt * TT, re, im);
+    }
     // ---- per-unit constants of the pointwise stage ----
     const float* filt = a.filt + (size_t)d * a.filt_stride;
     const float2* hsrc = nullptr;
     int w_lo = 1, w_hi = 0;
-    float cre = 0.f, cim = 0.f, delta = 0.f;
+    float cre = 0.f, cim = 0.f;
+    double delta = 0.0;
     if (MODE == MODE_HDET) hsrc = a.h_det + (size_t)unit * K;
     if (MODE == MODE_FUSED) {
         const WfCoef* c = a.coef + b;
@@ -94,7 +100,7 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
         const DetResp r = a.resp[unit];
         cre = (float)r.fp * c->pol_p;                       // C = F+ (1+cos^2 i)/2 - i Fx cos i
         cim = -(float)r.fc * c->pol_c;
-        delta = (float)(r.dt * (double)a.inv_tseg);          // turns per bin
+        delta = r.dt * (double)a.inv_tseg;                   // turns per bin (fp64: the second view's dt reaches 1 s)
     }
     // Operands of the pointwise stage for virtual thread t: bins k = t + 1024 k4 (half A) and M - k (half B).
     // They are requested one phase ahead of their use so that L2 latency is covered by butterfly work.  h0 is zero
@@ -128,10 +134,10 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
         } else if (MODE == MODE_FUSED) {
             if (k >= w_lo && k <= w_hi) {
                 const float2 h = __ldg(hsrc + k);
-                float turns = (float)k * delta;
-                turns -= rintf(turns);
+                double td = (double)k * delta;
+                td -= rint(td);
                 float s, co;
-                __sincosf(turns * -6.283185307179586f, &s, &co);          // exp(-2 pi i k dt / T)
+                __sincosf((float)td * -6.283185307179586f, &s, &co);      // exp(-2 pi i k dt / T)
                 const float2 cp = make_float2(cre * co - cim * s, cre * s + cim * co);
                 x2.x += h.x * cp.x - h.y * cp.y;
                 x2.y += h.x * cp.y + h.y * cp.x;
@@ -171,15 +177,15 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
         //   A: C e(t) e(1024)^k4,  B: C e(M) conj(e(t)) conj(e(1024))^k4,  e(j) = exp(-2 pi i j delta)
         C2 ph, st;
         if (MODE == MODE_FUSED) {
-            auto unit_phase = [&](float turns) {
-                turns -= rintf(turns);
+            auto unit_phase = [&](double turns) {            // reduced in fp64, evaluated in fp32
+                turns -= rint(turns);
                 float s, co;
-                __sincosf(turns * -6.283185307179586f, &s, &co);
+                __sincosf((float)turns * -6.283185307179586f, &s, &co);
                 return make_float2(co, s);
             };
-            const float2 et = unit_phase((float)t * delta);
-            const float2 es = unit_phase(1024.0f * delta);
-            const float2 em = unit_phase((float)M * delta);
+            const float2 et = unit_phase((double)t * delta);
+            const float2 es = unit_phase(1024.0 * delta);
+            const float2 em = unit_phase((double)M * delta);
             const float2 cc = make_float2(cre, cim);
             const float2 ca = amplfi::cmul(cc, et);
             const float2 cb = amplfi::cmul_conj(amplfi::cmul(cc, em), et);
@@ -256,15 +262,22 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
     __syncthreads();
     PwOps ops[VT];
     pw_load(tt, ops[0]);                                     // in flight during P3 and the barrier
+    if (fwd) {
 #pragma unroll
-    for (int vt = 0; vt < VT; ++vt) p3_fwd(tt + vt * TT, re, im);
+        for (int vt = 0; vt < VT; ++vt) p3_fwd(tt + vt * TT, re, im);
+    }
     __syncthreads();
 #pragma unroll
     for (int vt = 0; vt < VT; ++vt) {
         const int t = tt + vt * TT;
         const int klow_a = t, klow_b = (t == 0) ? 512 : 1024 - t;
         C2 v[8];
-        p4_fwd(klow_a, klow_b, v, re, im);
+        if (fwd) {
+            p4_fwd(klow_a, klow_b, v, re, im);
+        } else {
+#pragma unroll
+            for (int r = 0; r < 8; ++r) v[r] = C2{0ull, 0ull};
+        }
         pointwise(t, v, ops[vt]);
         if (vt + 1 < VT) pw_load(t + TT, ops[vt + 1]);      // in flight during this P4' and the next P4
         // ---- a-9 inverse real FFT ----
@@ -283,8 +296,17 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
         for (int vt = 0; vt < VT; ++vt) {
             float2 z[16];
             p1_inv(z, tt + vt * TT, re, im);
+            if (a.crop == 0) {
 #pragma unroll
-            for (int n1 = 0; n1 < 16; ++n1) __stcs(out2 + n1 * 512 + tt + vt * TT, z[n1]);
+                for (int n1 = 0; n1 < 16; ++n1) __stcs(out2 + n1 * 512 + tt + vt * TT, z[n1]);
+            } else {
+                const int c2 = a.crop >> 1;                  // crop is even: whole float2 pairs
+#pragma unroll
+                for (int n1 = 0; n1 < 16; ++n1) {
+                    const int m = n1 * 512 + tt + vt * TT;
+                    if (m >= c2 && m < M - c2) __stcs(out2 + m - c2, z[n1]);
+                }
+            }
         }
     }
 }

@@ -29,6 +29,7 @@ struct LongArgs {
     int n_det;
     int unit0;                // first unit of the chunk
     int n_full;               // 65536
+    int crop;                 // samples dropped at each end of an output row (even)
 };
 
 // DIR = 0: x[2m+p] -> 2 Xp[k] (spectrum to scratch).  DIR = 1: spectrum from scratch -> y[2m+p].
@@ -44,7 +45,8 @@ __global__ void __launch_bounds__(Fft<LONG_LOGM>::T) long_sub_kernel(const LongA
     const int unit = a.unit0 + lu;
     const int d = unit % a.n_det;
     float2* spec = a.spec + ((size_t)lu * 2 + par) * LONG_KS_STRIDE;
-    float* out = a.out + (size_t)unit * a.n_full;
+    const int n_out = a.n_full - 2 * a.crop;
+    float* out = a.out + (size_t)unit * n_out;
 
     const float* x = nullptr;
     if (a.offsets != nullptr) {
@@ -52,7 +54,7 @@ __global__ void __launch_bounds__(Fft<LONG_LOGM>::T) long_sub_kernel(const LongA
         if (off < 0 || off + a.n_full > a.strip_len) {      // never read out of bounds: poison the row instead
             if (DIR == 1) {
                 const float qnan = __int_as_float(0x7fc00000);
-                for (int i = tid; i < N; i += T) out[2 * i + par] = qnan;
+                for (int i = tid; 2 * i + par < n_out; i += T) out[2 * i + par] = qnan;
             }
             return;
         }
@@ -124,8 +126,9 @@ __global__ void __launch_bounds__(Fft<LONG_LOGM>::T) long_sub_kernel(const LongA
 #pragma unroll
         for (int nA = 0; nA < RA; ++nA) {
             const int m = nA * LB + tid;
-            out[4 * m + par] = v[nA].x;
-            out[4 * m + 2 + par] = v[nA].y;
+            const int j0 = 4 * m + par - a.crop, j1 = j0 + 2;
+            if (j0 >= 0 && j0 < n_out) out[j0] = v[nA].x;
+            if (j1 >= 0 && j1 < n_out) out[j1] = v[nA].y;
         }
     }
 }
@@ -142,6 +145,7 @@ struct LongPwArgs {
     int unit0;
     float two_fs;
     double inv_tseg;
+    int nofwd;                // no data: the sub-spectra are taken as zero (inverse-only launches)
 };
 
 // One thread per k in [0, 16384]: bins k and 32768 - k of the full spectrum.
@@ -155,7 +159,8 @@ __global__ void __launch_bounds__(256) long_pointwise_kernel(const LongPwArgs a)
     const int b = unit / a.n_det, d = unit - b * a.n_det;
     float2* se = a.spec + ((size_t)lu * 2) * LONG_KS_STRIDE;
     float2* so = se + LONG_KS_STRIDE;
-    const float2 A = se[k], Bq = so[k];
+    float2 A = make_float2(0.f, 0.f), Bq = A;
+    if (!a.nofwd) { A = se[k]; Bq = so[k]; }
     const float2 w = twiddle<NF>(k);
     const float2 B = cmul(Bq, w);
     float2 x1 = make_float2(A.x + B.x, A.y + B.y);              // 2 X[k]
@@ -215,23 +220,21 @@ static int long_attr() {
 
 size_t long_scratch_floats2(int chunk_units) { return (size_t)chunk_units * 2 * LONG_KS_STRIDE; }
 
-int launch_inject_whiten_long(const amplfi_plan* p, int batch, const float* noise, const long* offsets, long strip_len,
-                              const float* h_det, int fused, float* out, cudaStream_t st) {
+int launch_inject_whiten_long(const amplfi_plan* p, const IwArgs& ia, int mode, int units, cudaStream_t st) {
     int rc = long_attr();
     if (rc) return rc;
-    const int units = batch * p->n_det;
-    const int mode = h_det != nullptr ? MODE_HDET : (fused ? MODE_FUSED : MODE_NONE);
     using F = Fft<LONG_LOGM>;
+    const bool nofwd = ia.noise == nullptr;
     for (int u0 = 0; u0 < units; u0 += p->long_chunk) {
         const int cu = units - u0 < p->long_chunk ? units - u0 : p->long_chunk;
         LongArgs a;
-        a.noise = noise; a.offsets = offsets; a.strip_len = strip_len; a.spec = p->long_spec; a.out = out;
-        a.n_det = p->n_det; a.unit0 = u0; a.n_full = p->n;
-        long_sub_kernel<0><<<2 * cu, F::T, F::SMEM_BYTES, st>>>(a);
+        a.noise = ia.noise; a.offsets = nofwd ? nullptr : ia.offsets; a.strip_len = ia.strip_len; a.spec = p->long_spec;
+        a.out = ia.out; a.n_det = ia.n_det; a.unit0 = u0; a.n_full = p->n; a.crop = ia.crop;
+        if (!nofwd) { long_sub_kernel<0><<<2 * cu, F::T, F::SMEM_BYTES, st>>>(a); count_launch(); }
         LongPwArgs w;
-        w.spec = p->long_spec; w.h_det = reinterpret_cast<const float2*>(h_det); w.h0 = p->h0; w.coef = p->coef;
-        w.resp = p->resp; w.filt = p->filt; w.filt_stride = p->filt_stride; w.n_det = p->n_det; w.unit0 = u0;
-        w.two_fs = (float)(2.0 * p->fs); w.inv_tseg = 1.0 / p->t_seg;
+        w.spec = p->long_spec; w.h_det = ia.h_det; w.h0 = ia.h0; w.coef = ia.coef;
+        w.resp = ia.resp; w.filt = ia.filt; w.filt_stride = ia.filt_stride; w.n_det = ia.n_det; w.unit0 = u0;
+        w.two_fs = ia.two_fs; w.inv_tseg = 1.0 / p->t_seg; w.nofwd = nofwd ? 1 : 0;
         dim3 grid((LONG_KS + 255) / 256, cu);
         switch (mode) {
             case MODE_NONE: long_pointwise_kernel<MODE_NONE><<<grid, 256, 0, st>>>(w); break;
@@ -239,7 +242,7 @@ int launch_inject_whiten_long(const amplfi_plan* p, int batch, const float* nois
             default: long_pointwise_kernel<MODE_FUSED><<<grid, 256, 0, st>>>(w); break;
         }
         long_sub_kernel<1><<<2 * cu, F::T, F::SMEM_BYTES, st>>>(a);
-        count_launch(3);
+        count_launch(2);
     }
     return check_launch("inject_whiten_long");
 }

@@ -140,6 +140,41 @@ __global__ void __launch_bounds__(256) project_kernel(const DetResp* __restrict_
     }
 }
 
+// ---- second data view: same responses, arrival time later by t_shift[b] ----
+__global__ void shift_resp_kernel(const DetResp* __restrict__ resp, const double* __restrict__ t_shift, int n_det, int count,
+                                  DetResp* __restrict__ resp2) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    DetResp r = resp[i];
+    r.dt += t_shift[i / n_det];
+    resp2[i] = r;
+}
+
+int launch_shift_resp(const amplfi_plan* p, int batch, const double* t_shift, cudaStream_t st) {
+    const int count = batch * p->n_det;
+    shift_resp_kernel<<<(count + 127) / 128, 128, 0, st>>>(p->resp, t_shift, p->n_det, count, p->resp2);
+    count_launch();
+    return check_launch("shift_resp_kernel");
+}
+
+// ---- the two polarisations as pseudo-detectors: (F+, Fx, dt) = (1, 0, 0) and (0, 1, 0) (amplfi_waveform_td) ----
+__global__ void td_resp_kernel(int count, DetResp* __restrict__ resp2) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    DetResp r;
+    r.fp = (i & 1) ? 0.0 : 1.0;
+    r.fc = (i & 1) ? 1.0 : 0.0;
+    r.dt = 0.0;
+    resp2[i] = r;
+}
+
+int launch_td_resp(const amplfi_plan* p, int batch, cudaStream_t st) {
+    const int count = batch * 2;
+    td_resp_kernel<<<(count + 127) / 128, 128, 0, st>>>(count, p->resp2);
+    count_launch();
+    return check_launch("td_resp_kernel");
+}
+
 __global__ void copy_resp_kernel(const DetResp* __restrict__ resp, double* __restrict__ out, int count) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= count) return;

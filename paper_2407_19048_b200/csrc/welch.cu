@@ -102,6 +102,34 @@ __global__ void welch_mean_kernel(const float* __restrict__ part, int nseg, int 
     psd[(size_t)d * n_w + k] = acc * scale * ck;
 }
 
+// Median over segments: per bin, the middle order statistic of the nseg periodogram values (the
+// mean of the two middle ones for even nseg), found by rank counting over a shared-memory column (nseg <= 256, so the
+// O(nseg^2) comparisons are a few thousand per bin); ties are broken by segment index, so ranks are a permutation.
+// `scale` carries 1 / (median_bias(nseg) fs sum w^2).
+__global__ void __launch_bounds__(64) welch_median_kernel(const float* __restrict__ part, int nseg, int n_w, float scale,
+                                                          float* __restrict__ psd) {
+    extern __shared__ float col[];                       // [nseg][64]
+    const int k = blockIdx.x * 64 + threadIdx.x;
+    const int d = blockIdx.y;
+    if (k >= n_w) return;
+    const float* p = part + (size_t)d * nseg * n_w + k;
+    for (int s = 0; s < nseg; ++s) col[s * 64 + threadIdx.x] = p[(size_t)s * n_w];
+    const int r_lo = (nseg - 1) >> 1, r_hi = nseg >> 1;   // equal for odd nseg
+    float v_lo = 0.f, v_hi = 0.f;
+    for (int i = 0; i < nseg; ++i) {
+        const float vi = col[i * 64 + threadIdx.x];
+        int rank = 0;
+        for (int j = 0; j < nseg; ++j) {
+            const float vj = col[j * 64 + threadIdx.x];
+            rank += (vj < vi || (vj == vi && j < i)) ? 1 : 0;
+        }
+        if (rank == r_lo) v_lo = vi;
+        if (rank == r_hi) v_hi = vi;
+    }
+    const float ck = (k == 0 || k == n_w - 1) ? 1.0f : 2.0f;
+    psd[(size_t)d * n_w + k] = 0.5f * (v_lo + v_hi) * scale * ck;
+}
+
 template <int LOGM>
 static int launch_welch_t(const amplfi_plan* p, const float* bg, long row_stride, int step, int nseg, int detrend,
                           cudaStream_t st) {
@@ -118,8 +146,15 @@ static int launch_welch_t(const amplfi_plan* p, const float* bg, long row_stride
     return check_launch("welch_segment_kernel");
 }
 
-int launch_welch(const amplfi_plan* p, const float* bg, long n_bg, long row_stride, int noverlap, int detrend, float* psd,
-                 cudaStream_t st) {
+// E[median] / E[mean] of nseg exponentially distributed periodogram values: the k-th smallest of n unit exponentials has
+// expectation sum_{j = n-k+1}^{n} 1/j (host arithmetic on a launch parameter, like the mean's 1/nseg).
+static double median_bias(int n) {
+    auto e_order = [n](int k) { double s = 0.0; for (int j = n - k + 1; j <= n; ++j) s += 1.0 / (double)j; return s; };
+    return (n & 1) ? e_order((n + 1) / 2) : 0.5 * (e_order(n / 2) + e_order(n / 2 + 1));
+}
+
+int launch_welch(const amplfi_plan* p, const float* bg, long n_bg, long row_stride, int noverlap, int detrend, int average,
+                 float* psd, cudaStream_t st) {
     const int nps = p->nperseg;
     const int step = nps - noverlap;
     const long nseg_l = (n_bg - nps) / step + 1;
@@ -140,6 +175,18 @@ int launch_welch(const amplfi_plan* p, const float* bg, long n_bg, long row_stri
     }
     if (rc) return rc;
     const int n_w = nps / 2 + 1;
+    if (average == 1) {
+        static bool attr_done = false;
+        if (!attr_done) {
+            cudaFuncSetAttribute(welch_median_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 256 * 64 * (int)sizeof(float));
+            attr_done = true;
+        }
+        const float mscale = (float)(1.0 / (median_bias(nseg) * p->fs * 0.375 * (double)nps));
+        dim3 mgrid((n_w + 63) / 64, p->n_det);
+        welch_median_kernel<<<mgrid, 64, (size_t)nseg * 64 * sizeof(float), st>>>(p->welch_part, nseg, n_w, mscale, psd);
+        count_launch();
+        return check_launch("welch_median_kernel");
+    }
     const float scale = (float)(1.0 / ((double)nseg * p->fs * 0.375 * (double)nps));
     dim3 grid((n_w + 255) / 256, p->n_det);
     welch_mean_kernel<<<grid, 256, 0, st>>>(p->welch_part, nseg, n_w, scale, psd);

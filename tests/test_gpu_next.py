@@ -1,0 +1,151 @@
+"""GPU parity of the SURVEY.md 8(f) calls against the oracle: two data views, time-domain waveform
+output, median-averaged Welch and the time-truncated whitening filter.  Same tolerances as
+tests/test_gpu_parity.py (BASELINE.json north_star): 1e-4 of the row RMS on strain, 1e-4 relative on the PSD in band."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+if not torch.cuda.is_available():
+    pytest.skip("needs a CUDA device", allow_module_level=True)
+
+import paper_2407_19048_b200 as A          # noqa: E402
+import workloads as WL                     # noqa: E402
+from oracle import project as OP           # noqa: E402
+from oracle import views as OV             # noqa: E402
+from oracle import waveform as OW          # noqa: E402
+from oracle import welch as OWE            # noqa: E402
+from oracle import whiten as OWH           # noqa: E402
+
+from test_gpu_parity import TOL, PSD_SCALE, dev, row_err, edge_params      # noqa: E402
+
+
+def _workload(n, fs, batch, dets, seed):
+    rng = np.random.Generator(np.random.Philox(seed))
+    t_seg = n / fs
+    par = WL.draw_params(rng, batch, t_c=(t_seg - 2.5, t_seg - 1.5) if t_seg >= 4 else (0.5 * t_seg, 0.6 * t_seg))
+    noise = WL.coloured_noise(rng, (batch, len(dets)), n, fs)
+    psd = np.stack([WL.aligo_psd(np.arange(n // 2 + 1) * fs / n) * (1.0 + 0.1 * d) for d in range(len(dets))])
+    return par, noise, psd
+
+
+# ------------------------------------------------------------------------------------------ two views
+@pytest.mark.parametrize("n,fs,approx", [(16384, 2048.0, A.IMRPHENOMD), (8192, 2048.0, A.TAYLORF2), (65536, 4096.0, A.IMRPHENOMD),
+                                         (2048, 2048.0, A.IMRPHENOMD)])
+def test_two_views_parity(n, fs, approx):
+    dets = [0, 1, 2]
+    batch = 6
+    par, noise, psd = _workload(n, fs, batch, dets, 1000 + n)
+    par[0, 4] = 100.0                                         # one very loud signal: phase errors would show
+    t_shift = np.array([1.0, 0.0, 0.37, 1.0 / fs, 0.999, 0.5])[:batch]
+    plan = A.Plan(n, fs, dets, batch)
+    out, out2 = A.amplfi_inject_whiten_views(plan, batch, dev(noise), dev((psd * PSD_SCALE).astype(np.float32)), 20.0, 1000.0,
+                                             dev(par), dev(t_shift), approximant=approx, gmst=0.3)
+    torch.cuda.synchronize()
+    psd32 = (psd * PSD_SCALE).astype(np.float32).astype(np.float64) / PSD_SCALE
+    d, d2 = OV.two_views(approx, par, t_shift, noise.astype(np.float64), psd32, 0.3, dets, fs, 20.0, 1000.0)
+    assert row_err(out.cpu().numpy().astype(np.float64), d).max() <= TOL
+    assert row_err(out2.cpu().numpy().astype(np.float64), d2).max() <= TOL
+    # the signal part alone (noise removed on both sides) to the same bar relative to ITS rms
+    bg = A.amplfi_inject_whiten(plan, batch, dev(noise), dev((psd * PSD_SCALE).astype(np.float32)), 20.0, 1000.0)
+    bg_ref = OWH.inject_whiten(noise.astype(np.float64), None, psd32, fs, 20.0, 1000.0)
+    s_gpu = (out2 - bg).cpu().numpy().astype(np.float64)
+    s_ref = d2 - bg_ref
+    assert row_err(s_gpu[0], s_ref[0]).max() <= 2e-3           # difference of two fp32 rows: noise rounding remains
+    # zero shift reproduces the first view bit for bit
+    assert torch.equal(out[1], out2[1])
+
+
+def test_two_views_from_strip_with_offsets():
+    wl = WL.make_c2(batch=8, strip_len=1 << 20)
+    plan = A.Plan(wl.n, wl.fs, wl.det_ids, 8, nperseg=wl.nperseg)
+    o, nb = wl.extra["bg_offset"], wl.extra["n_bg"]
+    psd = A.amplfi_psd_welch(plan, dev(np.ascontiguousarray(wl.strip[:, o:o + nb])))
+    t_shift = np.linspace(0.0, 1.0, 8)
+    out, out2 = A.amplfi_inject_whiten_views(plan, 8, dev(wl.strip), psd, wl.f_lo, wl.f_hi, dev(wl.params[:8]), dev(t_shift),
+                                             offsets=dev(wl.offsets[:8]), gmst=wl.gmst)
+    torch.cuda.synchronize()
+    psd_ref = psd.cpu().numpy().astype(np.float64) / PSD_SCALE
+    noise = OWH.gather(wl.strip, wl.offsets[:8], wl.n)
+    d, d2 = OV.two_views(wl.approximant, wl.params[:8], t_shift, noise, psd_ref, wl.gmst, wl.det_ids, wl.fs, wl.f_lo, wl.f_hi)
+    assert row_err(out.cpu().numpy().astype(np.float64), d).max() <= TOL
+    assert row_err(out2.cpu().numpy().astype(np.float64), d2).max() <= TOL
+
+
+# ------------------------------------------------------------------------------------------ time-domain waveform
+@pytest.mark.parametrize("approx", [A.TAYLORF2, A.IMRPHENOMD])
+@pytest.mark.parametrize("n,fs", [(8192, 2048.0), (16384, 2048.0), (65536, 4096.0), (1024, 2048.0)])
+def test_waveform_td_parity(approx, n, fs):
+    par = edge_params(0.6 * n / fs)
+    par = np.concatenate([par, par[:1]])
+    par[-1, 1] = 1.5                                          # invalid q: all-zero row and a flag
+    plan = A.Plan(n, fs, [0], len(par))
+    h_t, flags = A.amplfi_waveform_td(plan, approx, dev(par), 20.0, 1000.0)
+    torch.cuda.synchronize()
+    hp, hc, fl = OW.waveform_td(approx, par, n, fs, 20.0, 1000.0)
+    got = h_t.cpu().numpy().astype(np.float64)
+    assert np.array_equal(flags.cpu().numpy(), fl)
+    assert row_err(got[:, 0], hp).max() <= TOL
+    assert row_err(got[:, 1], hc).max() <= TOL
+    assert np.all(got[-1] == 0.0)
+
+
+# ------------------------------------------------------------------------------------------ median Welch
+@pytest.mark.parametrize("nperseg,n_bg,fs", [(4096, 131072, 2048.0), (8192, 262144, 2048.0), (1024, 1024 * 32 + 512, 2048.0),
+                                             (1024, 1024, 2048.0), (2048, 2048 * 128 + 1024, 4096.0)])
+def test_welch_median_parity(nperseg, n_bg, fs):
+    rng = np.random.Generator(np.random.Philox(nperseg + 7))
+    bg = WL.coloured_noise(rng, (3,), 1 << 19, fs)[:, :n_bg].copy()
+    bg[1, 5000:5040] += np.float32(4e-19)                      # a loud transient the median should ignore
+    plan = A.Plan(max(nperseg, 1024), fs, [0, 1, 2], 1, nperseg=nperseg)
+    psd = A.amplfi_psd_welch(plan, dev(bg), average=1)
+    assert torch.equal(psd, A.amplfi_psd_welch(plan, dev(bg), average=1))
+    ref = OWE.welch(bg.astype(np.float64), fs, nperseg, average="median") * PSD_SCALE
+    got = psd.cpu().numpy().astype(np.float64)
+    f = np.arange(nperseg // 2 + 1) * fs / nperseg
+    band = (f >= 20.0) & (f <= 1000.0)
+    level = WL.aligo_psd(f) * PSD_SCALE
+    assert (np.abs(got - ref)[:, band] / level[band]).max() <= TOL
+    nseg = (n_bg - nperseg) // (nperseg // 2) + 1
+    if nseg >= 8:
+        assert np.abs(got[:, band] / ref[:, band] - 1).max() <= TOL
+
+
+# ------------------------------------------------------------------------------------------ truncated whitening filter
+@pytest.mark.parametrize("n,fs,fdur", [(16384, 2048.0, 1.0), (8192, 2048.0, 0.5), (65536, 4096.0, 2.0), (2048, 2048.0, 0.25),
+                                       (16384, 2048.0, 8.0)])
+@pytest.mark.parametrize("crop", [True, False])
+def test_inject_whiten_fir_parity(n, fs, fdur, crop):
+    if crop and fdur * fs >= n:
+        pytest.skip("nothing left after cropping")
+    dets = [0, 1]
+    batch = 3
+    par, noise, psd = _workload(n, fs, batch, dets, 2000 + n)
+    psd = psd * (1.0 + 0.5 * np.sin(np.arange(n // 2 + 1) / 7.0) ** 2)      # a structured PSD: truncation matters
+    psd_s = (psd * PSD_SCALE).astype(np.float32)
+    plan = A.Plan(n, fs, dets, batch)
+    out = A.amplfi_inject_whiten_fir(plan, batch, dev(noise), dev(psd_s), 20.0, 1000.0, fdur, crop=crop, params=dev(par), gmst=0.1)
+    torch.cuda.synchronize()
+    psd64 = psd_s.astype(np.float64) / PSD_SCALE
+    hp, hc, _ = OW.waveform_fd(A.IMRPHENOMD, par, n, fs, 20.0, 1000.0)
+    h_det, _ = OP.project(hp, hc, par, 0.1, dets, n, fs)
+    ref = OWH.inject_whiten_fir(noise.astype(np.float64), h_det, psd64, fs, 20.0, 1000.0, fdur, crop=crop)
+    got = out.cpu().numpy().astype(np.float64)
+    assert got.shape == ref.shape
+    assert row_err(got, ref).max() <= TOL
+    # whiten only, h_det given: the other two modes of the call
+    out_n = A.amplfi_inject_whiten_fir(plan, batch, dev(noise), dev(psd_s), 20.0, 1000.0, fdur, crop=crop)
+    ref_n = OWH.inject_whiten_fir(noise.astype(np.float64), None, psd64, fs, 20.0, 1000.0, fdur, crop=crop)
+    assert row_err(out_n.cpu().numpy().astype(np.float64), ref_n).max() <= TOL
+
+
+def test_fir_argument_checks():
+    plan = A.Plan(4096, 2048.0, [0], 1)
+    noise = torch.zeros((1, 1, 4096), device="cuda")
+    psd = torch.ones((1, 2049), device="cuda")
+    for fdur in (0.0, 3.0, 0.5 + 1.0 / 2048.0):
+        with pytest.raises(A.AmplfiError):
+            A.amplfi_inject_whiten_fir(plan, 1, noise, psd, 20.0, 1000.0, fdur)
+    with pytest.raises(A.AmplfiError):
+        A.amplfi_inject_whiten_fir(plan, 1, noise, psd, 20.0, 1000.0, 2.0, crop=True)
