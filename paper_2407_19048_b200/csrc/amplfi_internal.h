@@ -85,6 +85,7 @@ struct IwArgs {
     int filt_stride;
     float* out;               // [B, D, N - 2 crop]
     int crop;                 // samples dropped at each end of every output row (even)
+    int phase64;              // packed kernel: reduce the projection phase in fp64 (needed when |dt| can reach ~1 s)
     int n_det;
     float two_fs;
     float inv_tseg;
@@ -98,6 +99,7 @@ struct IwOpts {
     const float* filt;        // nullptr: plan->filt
     int filt_stride;
     int crop;
+    int phase64;
 };
 
 // inject_whiten13.cu (packed 4-pass kernel for n = 16384)

@@ -11,7 +11,7 @@ using namespace v2;
 // VT virtual threads (of the 512 the index algebra is written for) per physical thread: VT = 2 runs 256 threads with
 // 128 registers, trading thread-level for instruction-level parallelism (loads of one virtual thread overlap the
 // arithmetic of the other).
-template <int MODE, int VT>
+template <int MODE, int VT, bool FWD>
 __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwArgs a, int units) {
     constexpr int TT = T13 / VT;
     constexpr int M = M13, N = N13, K = M13 + 1;
@@ -25,7 +25,7 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
     const float* x = nullptr;
     const int n_out = N - 2 * a.crop;
     float* out = a.out + (size_t)unit * n_out;
-    const bool fwd = a.noise != nullptr;                   // false: inverse-only launch, the spectrum starts at zero
+    constexpr bool fwd = FWD;                              // false: inverse-only launch, the spectrum starts at zero
     if (!fwd) {
     } else if (a.offsets != nullptr) {
         const long off = a.offsets[unit];
@@ -89,7 +89,7 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
     // ---- per-unit constants of the pointwise stage ----
     const float* filt = a.filt + (size_t)d * a.filt_stride;
     const float2* hsrc = nullptr;
-    int w_lo = 1, w_hi = 0;
+    int w_lo = 0x40000000, w_hi = -1;                      // empty band: no 32-bin window of pw_load overlaps it
     float cre = 0.f, cim = 0.f;
     double delta = 0.0;
     if (MODE == MODE_HDET) hsrc = a.h_det + (size_t)unit * K;
@@ -177,15 +177,24 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
         //   A: C e(t) e(1024)^k4,  B: C e(M) conj(e(t)) conj(e(1024))^k4,  e(j) = exp(-2 pi i j delta)
         C2 ph, st;
         if (MODE == MODE_FUSED) {
-            auto unit_phase = [&](double turns) {            // reduced in fp64, evaluated in fp32
-                turns -= rint(turns);
+            auto unit_phase = [&](float turns) {
+                turns -= rintf(turns);
                 float s, co;
-                __sincosf((float)turns * -6.283185307179586f, &s, &co);
+                __sincosf(turns * -6.283185307179586f, &s, &co);
                 return make_float2(co, s);
             };
-            const float2 et = unit_phase((double)t * delta);
-            const float2 es = unit_phase(1024.0 * delta);
-            const float2 em = unit_phase((double)M * delta);
+            float tt_, ts_, tm_;
+            if (a.phase64) {                                 // second data view: dt reaches 1 s, reduce in fp64
+                double x = (double)t * delta; tt_ = (float)(x - rint(x));
+                x = 1024.0 * delta; ts_ = (float)(x - rint(x));
+                x = (double)M * delta; tm_ = (float)(x - rint(x));
+            } else {                                         // |dt| <= 21 ms: fp32 is exact enough
+                const float df = (float)delta;
+                tt_ = (float)t * df; ts_ = 1024.0f * df; tm_ = (float)M * df;
+            }
+            const float2 et = unit_phase(tt_);
+            const float2 es = unit_phase(ts_);
+            const float2 em = unit_phase(tm_);
             const float2 cc = make_float2(cre, cim);
             const float2 ca = amplfi::cmul(cc, et);
             const float2 cb = amplfi::cmul_conj(amplfi::cmul(cc, em), et);
@@ -314,25 +323,31 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
 #ifndef IW13_VT
 #define IW13_VT 2
 #endif
-template <int MODE>
+template <int MODE, bool FWD>
 static int launch_iw13_t(const IwArgs& a, int units, cudaStream_t st) {
     static bool attr_done = false;
     const int smem = 2 * M13 * (int)sizeof(float);
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(inject_whiten13_kernel<MODE, IW13_VT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        cudaError_t e = cudaFuncSetAttribute(inject_whiten13_kernel<MODE, IW13_VT, FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) { set_error("cudaFuncSetAttribute: %s", cudaGetErrorString(e)); return AMPLFI_ERR_CUDA; }
         attr_done = true;
     }
-    inject_whiten13_kernel<MODE, IW13_VT><<<units, T13 / IW13_VT, smem, st>>>(a, units);
+    inject_whiten13_kernel<MODE, IW13_VT, FWD><<<units, T13 / IW13_VT, smem, st>>>(a, units);
     count_launch();
     return check_launch("inject_whiten13_kernel");
 }
 
 int launch_iw13(const IwArgs& a, int mode, int units, cudaStream_t st) {
+    if (a.noise == nullptr) {       // inverse-only launches (time-domain waveform, filter design)
+        if (mode == MODE_HDET) return launch_iw13_t<MODE_HDET, false>(a, units, st);
+        if (mode == MODE_FUSED) return launch_iw13_t<MODE_FUSED, false>(a, units, st);
+        set_error("inject_whiten13: no data and nothing to inject");
+        return AMPLFI_ERR_INVALID_ARG;
+    }
     switch (mode) {
-        case MODE_NONE: return launch_iw13_t<MODE_NONE>(a, units, st);
-        case MODE_HDET: return launch_iw13_t<MODE_HDET>(a, units, st);
-        default: return launch_iw13_t<MODE_FUSED>(a, units, st);
+        case MODE_NONE: return launch_iw13_t<MODE_NONE, true>(a, units, st);
+        case MODE_HDET: return launch_iw13_t<MODE_HDET, true>(a, units, st);
+        default: return launch_iw13_t<MODE_FUSED, true>(a, units, st);
     }
 }
 

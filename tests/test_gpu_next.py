@@ -149,3 +149,26 @@ def test_fir_argument_checks():
             A.amplfi_inject_whiten_fir(plan, 1, noise, psd, 20.0, 1000.0, fdur)
     with pytest.raises(A.AmplfiError):
         A.amplfi_inject_whiten_fir(plan, 1, noise, psd, 20.0, 1000.0, 2.0, crop=True)
+
+
+# ------------------------------------------------------------------------------------------ degenerate rows of the fused path
+@pytest.mark.parametrize("n,fs", [(16384, 2048.0), (8192, 2048.0), (65536, 4096.0)])
+def test_fused_invalid_and_empty_band_rows_inject_nothing(n, fs):
+    """A sample with invalid parameters, or whose band is empty (f_top < f_lo: reading R-W7), must come out exactly as
+    whitened noise, even when the plan's h0 workspace still holds a previous, loud batch."""
+    dets = [0, 1, 2]
+    batch = 4
+    par, noise, psd = _workload(n, fs, batch, dets, 3000 + n)
+    par[:, 4] = 50.0                                           # loud batch that fills the workspace
+    psd_s = dev((psd * PSD_SCALE).astype(np.float32))
+    plan = A.Plan(n, fs, dets, batch)
+    A.amplfi_inject_whiten(plan, batch, dev(noise), psd_s, 20.0, 1000.0, params=dev(par))
+    bad = par.copy()
+    bad[0, 1] = 1.5                                            # q > 1
+    bad[1, 2] = 1.0                                            # |chi1| = 1
+    bad[2, 0], bad[2, 1] = 100.0, 1.0                          # TaylorF2: f_ISCO = 19.1 Hz < f_lo -> empty band
+    bad[3, 4] = -1.0                                           # distance <= 0
+    out = A.amplfi_inject_whiten(plan, batch, dev(noise), psd_s, 20.0, 1000.0, approximant=A.TAYLORF2, params=dev(bad))
+    ref = A.amplfi_inject_whiten(plan, batch, dev(noise), psd_s, 20.0, 1000.0)
+    torch.cuda.synchronize()
+    assert torch.equal(out, ref)
