@@ -40,7 +40,7 @@ def parse():
     ap.add_argument("--cpu-sample", type=int, default=1024, help="samples of the batch the CPU oracle is timed on")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--config", default="c2", choices=["c2", "c3", "c4", "sweep"],
+    ap.add_argument("--config", default="c2", choices=["c2", "c3", "c4", "sweep", "next"],
                     help="c2 (default): the contract line.  c3: online latency p50/p99 over --runs seeded runs.  "
                          "c4: bandwidth stress (batch 8192 x 3 x 65536).  sweep: segment length 1-16 s at 4096 Hz.")
     ap.add_argument("--runs", type=int, default=1000)
@@ -419,6 +419,61 @@ def run_extra(args):
                                                      "preceding background (4 s Hann, 50% overlap), IMRPhenomD injection; run r "
                                                      "uses seed 0xA3D30003 + r; CUDA events around one amplfi_assemble_batch "
                                                      "call, inputs resident"}}))
+        return
+
+    if args.config == "next":
+        # SURVEY.md 8(f) rows on the c2 workload: two data views, time-domain waveforms, median Welch, truncated filter
+        wl = WL.make_c2(batch=args.batch, strip_len=args.strip_len)
+        B, D, N = wl.batch, wl.n_det, wl.n
+        plan = A.Plan(N, wl.fs, wl.det_ids, B, nperseg=wl.nperseg)
+        strip = torch.from_numpy(wl.strip).to(dev)
+        params = torch.from_numpy(wl.params).to(dev)
+        offsets = torch.from_numpy(wl.offsets).to(dev)
+        t_shift = torch.from_numpy(np.random.Generator(np.random.Philox(5)).uniform(0.0, 1.0, B)).to(dev)
+        o, nb = wl.extra["bg_offset"], wl.extra["n_bg"]
+        bg = strip[:, o:o + nb]
+        psd = torch.empty((D, wl.nperseg // 2 + 1), dtype=torch.float32, device=dev)
+        out = torch.empty((B, D, N), dtype=torch.float32, device=dev)
+        out2 = torch.empty((B, D, N), dtype=torch.float32, device=dev)
+        h_t = torch.empty((B, 2, N), dtype=torch.float32, device=dev)
+        fdur = 1.0
+        out_c = torch.empty((B, D, N - int(fdur * wl.fs)), dtype=torch.float32, device=dev)
+        A.amplfi_psd_welch(plan, bg, psd=psd, stream=stream)
+
+        def timed(fn, steps=max(5, min(args.steps, 50)), warmup=3):
+            for _ in range(warmup):
+                fn()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            l0 = A.launch_count()
+            e0.record(stream)
+            for _ in range(steps):
+                fn()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            return e0.elapsed_time(e1) / steps, (A.launch_count() - l0) // steps
+
+        rows = []
+        ms, nl = timed(lambda: A.amplfi_inject_whiten(plan, B, strip, psd, wl.f_lo, wl.f_hi, offsets=offsets, params=params,
+                                                      gmst=wl.gmst, out=out, stream=stream))
+        rows.append(("amplfi_inject_whiten (fused, one view; reference point)", ms, nl, B * D * N, 8.0 * B * D * N))
+        ms, nl = timed(lambda: A.amplfi_inject_whiten_views(plan, B, strip, psd, wl.f_lo, wl.f_hi, params, t_shift, offsets=offsets,
+                                                            gmst=wl.gmst, out=out, out2=out2, stream=stream))
+        rows.append(("amplfi_inject_whiten_views (two views d, d')", ms, nl, 2 * B * D * N, 12.0 * B * D * N))
+        ms, nl = timed(lambda: A.amplfi_waveform_td(plan, A.IMRPHENOMD, params, wl.f_lo, wl.f_hi, h_t=h_t, stream=stream))
+        rows.append(("amplfi_waveform_td (h+, hx time series)", ms, nl, 2 * B * N, 4.0 * 2 * B * N))
+        ms, nl = timed(lambda: A.amplfi_inject_whiten_fir(plan, B, strip, psd, wl.f_lo, wl.f_hi, fdur, crop=True, offsets=offsets,
+                                                          params=params, gmst=wl.gmst, out=out_c, stream=stream))
+        rows.append(("amplfi_inject_whiten_fir (1 s filter, cropped)", ms, nl, B * D * N, 4.0 * B * D * (2 * N - int(fdur * wl.fs))))
+        ms, nl = timed(lambda: A.amplfi_psd_welch(plan, bg, psd=psd, stream=stream))
+        rows.append(("amplfi_psd_welch average=mean (64 s, 63 segments x 3)", ms, nl, 3 * nb, 4.0 * 3 * nb))
+        ms, nl = timed(lambda: A.amplfi_psd_welch(plan, bg, average=1, psd=psd, stream=stream))
+        rows.append(("amplfi_psd_welch average=median", ms, nl, 3 * nb, 4.0 * 3 * nb))
+        for name, ms, nl, samples, alg_bytes in rows:
+            print(json.dumps({"metric": "8(f) rows on the c2 workload", "call": name, "ms_per_call": ms, "gpu_launches_per_call": int(nl),
+                              "samples_per_s": samples / (ms * 1e-3), "algorithmic_gbs": alg_bytes / (ms * 1e-3) / 1e9,
+                              "frac_of_measured_hbm": alg_bytes / (ms * 1e-3) / 1e9 / peak, "dtype": "f32", "data": "synthetic",
+                              "config": {"batch": B, "n_det": D, "n": N}}))
         return
 
     if args.config == "c4":

@@ -41,7 +41,7 @@ def build(force=False, verbose=False):
         fh.write("\n".join(log))
     if verbose:
         sys.stdout.write("\n".join(log))
-    subprocess.check_call([nvcc, "-shared", "-o", LIB] + objs + ["-lcudart"])
+    subprocess.check_call([nvcc, "-shared", "-Wno-deprecated-gpu-targets", "-o", LIB] + objs + ["-lcudart"])
     return LIB
 
 

@@ -104,30 +104,41 @@ __global__ void welch_mean_kernel(const float* __restrict__ part, int nseg, int 
 
 // Median over segments: per bin, the middle order statistic of the nseg periodogram values (the
 // mean of the two middle ones for even nseg), found by rank counting over a shared-memory column (nseg <= 256, so the
-// O(nseg^2) comparisons are a few thousand per bin); ties are broken by segment index, so ranks are a permutation.
-// `scale` carries 1 / (median_bias(nseg) fs sum w^2).
-__global__ void __launch_bounds__(64) welch_median_kernel(const float* __restrict__ part, int nseg, int n_w, float scale,
-                                                          float* __restrict__ psd) {
-    extern __shared__ float col[];                       // [nseg][64]
-    const int k = blockIdx.x * 64 + threadIdx.x;
+// O(nseg^2) comparisons are a few thousand per bin); ties are broken by segment index, so ranks are a permutation and
+// exactly one candidate has each of the two middle ranks.  A CTA serves 64 bins with MED_PARTS threads per bin, each
+// ranking every MED_PARTS-th candidate.  `scale` carries 1 / (median_bias(nseg) fs sum w^2).
+constexpr int MED_PARTS = 8;
+__global__ void __launch_bounds__(64 * MED_PARTS) welch_median_kernel(const float* __restrict__ part, int nseg, int n_w,
+                                                                      float scale, float* __restrict__ psd) {
+    extern __shared__ float col[];                       // [nseg][64], then the two middle values [2][64]
+    const int lane = threadIdx.x & 63, sub = threadIdx.x >> 6;
+    const int k = blockIdx.x * 64 + lane;
     const int d = blockIdx.y;
-    if (k >= n_w) return;
-    const float* p = part + (size_t)d * nseg * n_w + k;
-    for (int s = 0; s < nseg; ++s) col[s * 64 + threadIdx.x] = p[(size_t)s * n_w];
-    const int r_lo = (nseg - 1) >> 1, r_hi = nseg >> 1;   // equal for odd nseg
-    float v_lo = 0.f, v_hi = 0.f;
-    for (int i = 0; i < nseg; ++i) {
-        const float vi = col[i * 64 + threadIdx.x];
-        int rank = 0;
-        for (int j = 0; j < nseg; ++j) {
-            const float vj = col[j * 64 + threadIdx.x];
-            rank += (vj < vi || (vj == vi && j < i)) ? 1 : 0;
-        }
-        if (rank == r_lo) v_lo = vi;
-        if (rank == r_hi) v_hi = vi;
+    const bool live = k < n_w;
+    float* mid = col + nseg * 64;
+    if (live) {
+        const float* p = part + (size_t)d * nseg * n_w + k;
+        for (int s = sub; s < nseg; s += MED_PARTS) col[s * 64 + lane] = p[(size_t)s * n_w];
     }
-    const float ck = (k == 0 || k == n_w - 1) ? 1.0f : 2.0f;
-    psd[(size_t)d * n_w + k] = 0.5f * (v_lo + v_hi) * scale * ck;
+    __syncthreads();
+    if (live) {
+        const int r_lo = (nseg - 1) >> 1, r_hi = nseg >> 1;   // equal for odd nseg
+        for (int i = sub; i < nseg; i += MED_PARTS) {
+            const float vi = col[i * 64 + lane];
+            int rank = 0;
+            for (int j = 0; j < nseg; ++j) {
+                const float vj = col[j * 64 + lane];
+                rank += (vj < vi || (vj == vi && j < i)) ? 1 : 0;
+            }
+            if (rank == r_lo) mid[lane] = vi;
+            if (rank == r_hi) mid[64 + lane] = vi;
+        }
+    }
+    __syncthreads();
+    if (live && sub == 0) {
+        const float ck = (k == 0 || k == n_w - 1) ? 1.0f : 2.0f;
+        psd[(size_t)d * n_w + k] = 0.5f * (mid[lane] + mid[64 + lane]) * scale * ck;
+    }
 }
 
 template <int LOGM>
@@ -178,12 +189,12 @@ int launch_welch(const amplfi_plan* p, const float* bg, long n_bg, long row_stri
     if (average == 1) {
         static bool attr_done = false;
         if (!attr_done) {
-            cudaFuncSetAttribute(welch_median_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 256 * 64 * (int)sizeof(float));
+            cudaFuncSetAttribute(welch_median_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (256 + 2) * 64 * (int)sizeof(float));
             attr_done = true;
         }
         const float mscale = (float)(1.0 / (median_bias(nseg) * p->fs * 0.375 * (double)nps));
         dim3 mgrid((n_w + 63) / 64, p->n_det);
-        welch_median_kernel<<<mgrid, 64, (size_t)nseg * 64 * sizeof(float), st>>>(p->welch_part, nseg, n_w, mscale, psd);
+        welch_median_kernel<<<mgrid, 64 * MED_PARTS, (size_t)(nseg + 2) * 64 * sizeof(float), st>>>(p->welch_part, nseg, n_w, mscale, psd);
         count_launch();
         return check_launch("welch_median_kernel");
     }
