@@ -84,6 +84,8 @@ struct IwArgs {
     const float* filt;        // [D, filt_stride]
     int filt_stride;
     float* out;               // [B, D, N - 2 crop]
+    float* out2;              // packed kernel, two-view launch: second view [B, D, N] (16-byte aligned); else nullptr
+    const double* t_shift;    // two-view launch: [B] seconds added to the arrival time in the second view
     int crop;                 // samples dropped at each end of every output row (even)
     int phase64;              // packed kernel: reduce the projection phase in fp64 (needed when |dt| can reach ~1 s)
     int n_det;
@@ -100,6 +102,8 @@ struct IwOpts {
     int filt_stride;
     int crop;
     int phase64;
+    float* out2;              // with t_shift: both views in one launch (n = 16384 only)
+    const double* t_shift;
 };
 
 // inject_whiten13.cu (packed 4-pass kernel for n = 16384)

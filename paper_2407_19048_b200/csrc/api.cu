@@ -381,10 +381,16 @@ int amplfi_inject_whiten_views(const amplfi_plan* p, int batch, const float* noi
     rc = launch_filter(p, psd, n_psd, f_lo, f_hi, st);
     if (!rc) rc = launch_prepare(p, approximant, batch, params, gmst, f_lo, f_hi, 2.0 * p->fs, nullptr, st);
     if (!rc) rc = launch_waveform_h0(p, batch, st);
-    if (!rc) rc = launch_shift_resp(p, batch, t_shift, st);
     // both views with the fp64-reduced phase, so that a zero shift reproduces the first view bit for bit
     IwOpts o;
     o.n_det = p->n_det; o.resp = nullptr; o.filt = nullptr; o.filt_stride = 0; o.crop = 0; o.phase64 = 1;
+    o.out2 = nullptr; o.t_shift = nullptr;
+    if (!rc && p->logm == 13 && (reinterpret_cast<size_t>(out2) & 15) == 0) {
+        // n = 16384: one launch, one forward transform for both views (inject_whiten13.cu, VIEWS = 2)
+        o.out2 = out2; o.t_shift = t_shift;
+        return launch_inject_whiten(p, batch, noise, offsets, strip_len, nullptr, 1, out, st, &o);
+    }
+    if (!rc) rc = launch_shift_resp(p, batch, t_shift, st);
     if (!rc) rc = launch_inject_whiten(p, batch, noise, offsets, strip_len, nullptr, 1, out, st, &o);
     if (rc) return rc;
     o.resp = p->resp2;
@@ -406,6 +412,7 @@ int amplfi_waveform_td(const amplfi_plan* p, int approximant, int batch, const d
     if (rc) return rc;
     IwOpts o;
     o.n_det = 2; o.resp = p->resp2; o.filt = p->filt_flat; o.filt_stride = 0; o.crop = 0; o.phase64 = 0;
+    o.out2 = nullptr; o.t_shift = nullptr;
     return launch_inject_whiten(p, batch, nullptr, nullptr, 0, nullptr, 1, h_t, st, &o);
 }
 
@@ -434,6 +441,7 @@ int amplfi_inject_whiten_fir(const amplfi_plan* p, int batch, const float* noise
     if (rc) return rc;
     IwOpts o;
     o.n_det = p->n_det; o.resp = nullptr; o.filt = nullptr; o.filt_stride = 0; o.crop = crop ? (int)(ntaps / 2) : 0; o.phase64 = 0;
+    o.out2 = nullptr; o.t_shift = nullptr;
     return launch_inject_whiten(p, batch, noise, offsets, strip_len, h_det, fused ? 1 : 0, out, st, &o);
 }
 

@@ -86,7 +86,7 @@ int launch_fir_truncate(const amplfi_plan* p, double fduration, cudaStream_t st)
     const float inv_fs = (float)(1.0 / p->fs);
     dim3 gb((nb + 255) / 256, p->n_det), gf((p->filt_stride + 255) / 256, p->n_det);
     IwOpts o;
-    o.n_det = 1; o.resp = nullptr; o.filt = p->filt_flat; o.filt_stride = 0; o.crop = 0; o.phase64 = 0;
+    o.n_det = 1; o.resp = nullptr; o.filt = p->filt_flat; o.filt_stride = 0; o.crop = 0; o.phase64 = 0; o.out2 = nullptr; o.t_shift = nullptr;
     // q = irfft(w): time = fs q
     fir_real_to_spec_kernel<<<gb, 256, 0, st>>>(p->filt, p->filt_stride, nb, 1.0f, 0, p->fir_spec);
     count_launch();
@@ -289,7 +289,7 @@ int launch_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
     a.noise = noise; a.offsets = offsets; a.strip_len = strip_len;
     a.h_det = reinterpret_cast<const float2*>(h_det);
     a.h0 = p->h0; a.coef = p->coef; a.resp = p->resp; a.filt = p->filt; a.filt_stride = p->filt_stride; a.out = out;
-    a.crop = 0; a.phase64 = 0;
+    a.crop = 0; a.phase64 = 0; a.out2 = nullptr; a.t_shift = nullptr;
     a.n_det = p->n_det; a.two_fs = (float)(2.0 * p->fs); a.inv_tseg = (float)(1.0 / p->t_seg);
     a.prefetch_ahead = 2 * p->sm_count;
     if (opts != nullptr) {
@@ -297,6 +297,7 @@ int launch_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
         if (opts->resp != nullptr) a.resp = opts->resp;
         if (opts->filt != nullptr) { a.filt = opts->filt; a.filt_stride = opts->filt_stride; }
         a.crop = opts->crop; a.phase64 = opts->phase64;
+        if (p->logm == 13) { a.out2 = opts->out2; a.t_shift = opts->t_shift; }
     }
     const int mode = h_det != nullptr ? MODE_HDET : (fused ? MODE_FUSED : MODE_NONE);
     const int units = batch * a.n_det;

@@ -11,7 +11,10 @@ using namespace v2;
 // VT virtual threads (of the 512 the index algebra is written for) per physical thread: VT = 2 runs 256 threads with
 // 128 registers, trading thread-level for instruction-level parallelism (loads of one virtual thread overlap the
 // arithmetic of the other).
-template <int MODE, int VT, bool FWD>
+// VIEWS = 2 (MODE_FUSED only): the two data views d, d' of PAPER.md:93, :117 from ONE forward transform.  The forward
+// spectrum of every virtual thread is parked in the second view's own output row (64 KB, exactly the row size; it stays
+// in L2 until that view's samples overwrite it) and read back for the second pointwise stage + inverse transform.
+template <int MODE, int VT, bool FWD, int VIEWS>
 __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwArgs a, int units) {
     constexpr int TT = T13 / VT;
     constexpr int M = M13, N = N13, K = M13 + 1;
@@ -276,6 +279,52 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
         for (int vt = 0; vt < VT; ++vt) p3_fwd(tt + vt * TT, re, im);
     }
     __syncthreads();
+    if constexpr (VIEWS == 2) {
+        ulonglong2* stash = reinterpret_cast<ulonglong2*>(a.out2 + (size_t)unit * N);
+        const double delta0 = delta;
+        float2* outv = reinterpret_cast<float2*>(out);
+#pragma unroll 1
+        for (int view = 0; view < 2; ++view) {
+            if (view == 1) {
+                __syncthreads();                             // every thread is done reading smem for the first view
+                delta = delta0 + a.t_shift[b] * (double)a.inv_tseg;
+                outv = reinterpret_cast<float2*>(a.out2 + (size_t)unit * N);
+                pw_load(tt, ops[0]);
+            }
+#pragma unroll
+            for (int vt = 0; vt < VT; ++vt) {
+                const int t = tt + vt * TT;
+                const int klow_a = t, klow_b = (t == 0) ? 512 : 1024 - t;
+                C2 v[8];
+                if (view == 0) {
+                    p4_fwd(klow_a, klow_b, v, re, im);
+#pragma unroll
+                    for (int r = 0; r < 8; ++r) stash[r * T13 + t] = make_ulonglong2(v[r].r, v[r].i);
+                } else {
+#pragma unroll
+                    for (int r = 0; r < 8; ++r) { const ulonglong2 q = stash[r * T13 + t]; v[r] = C2{q.x, q.y}; }
+                }
+                pointwise(t, v, ops[vt]);
+                if (vt + 1 < VT) pw_load(t + TT, ops[vt + 1]);
+                p4_inv(klow_a, klow_b, v, re, im);
+            }
+            __syncthreads();
+#pragma unroll
+            for (int vt = 0; vt < VT; ++vt) p3_inv(tt + vt * TT, re, im);
+            __syncthreads();
+#pragma unroll
+            for (int vt = 0; vt < VT; ++vt) p2_inv(tt + vt * TT, re, im);
+            __syncthreads();
+#pragma unroll
+            for (int vt = 0; vt < VT; ++vt) {
+                float2 z[16];
+                p1_inv(z, tt + vt * TT, re, im);
+#pragma unroll
+                for (int n1 = 0; n1 < 16; ++n1) __stcs(outv + n1 * 512 + tt + vt * TT, z[n1]);
+            }
+        }
+        return;
+    }
 #pragma unroll
     for (int vt = 0; vt < VT; ++vt) {
         const int t = tt + vt * TT;
@@ -323,21 +372,28 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
 #ifndef IW13_VT
 #define IW13_VT 2
 #endif
-template <int MODE, bool FWD>
+template <int MODE, bool FWD, int VIEWS = 1>
 static int launch_iw13_t(const IwArgs& a, int units, cudaStream_t st) {
     static bool attr_done = false;
     const int smem = 2 * M13 * (int)sizeof(float);
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(inject_whiten13_kernel<MODE, IW13_VT, FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        cudaError_t e = cudaFuncSetAttribute(inject_whiten13_kernel<MODE, IW13_VT, FWD, VIEWS>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) { set_error("cudaFuncSetAttribute: %s", cudaGetErrorString(e)); return AMPLFI_ERR_CUDA; }
         attr_done = true;
     }
-    inject_whiten13_kernel<MODE, IW13_VT, FWD><<<units, T13 / IW13_VT, smem, st>>>(a, units);
+    inject_whiten13_kernel<MODE, IW13_VT, FWD, VIEWS><<<units, T13 / IW13_VT, smem, st>>>(a, units);
     count_launch();
     return check_launch("inject_whiten13_kernel");
 }
 
 int launch_iw13(const IwArgs& a, int mode, int units, cudaStream_t st) {
+    if (a.out2 != nullptr) {        // two data views from one forward transform
+        if (mode != MODE_FUSED || a.noise == nullptr || a.t_shift == nullptr || a.crop != 0) {
+            set_error("inject_whiten13: the two-view launch needs the fused mode");
+            return AMPLFI_ERR_INVALID_ARG;
+        }
+        return launch_iw13_t<MODE_FUSED, true, 2>(a, units, st);
+    }
     if (a.noise == nullptr) {       // inverse-only launches (time-domain waveform, filter design)
         if (mode == MODE_HDET) return launch_iw13_t<MODE_HDET, false>(a, units, st);
         if (mode == MODE_FUSED) return launch_iw13_t<MODE_FUSED, false>(a, units, st);
