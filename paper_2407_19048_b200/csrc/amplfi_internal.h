@@ -108,6 +108,7 @@ struct IwOpts {
 
 // inject_whiten13.cu (packed 4-pass kernel for n = 16384)
 int launch_iw13(const IwArgs& a, int mode, int units, cudaStream_t st);
+int init_iw13_tables(cudaStream_t st);      // fills the packed kernel's twiddle tables (idempotent; called by plan_create)
 
 // inject_whiten.cu
 int launch_filter(const amplfi_plan* p, const float* psd, int n_psd, double f_lo, double f_hi, cudaStream_t st);

@@ -189,6 +189,7 @@ int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_
         if (e != cudaSuccess) { set_error("amplfi_plan_create: stream/event: %s", cudaGetErrorString(e)); rc = AMPLFI_ERR_CUDA; }
     }
     if (!rc) rc = launch_tables(p, nullptr);
+    if (!rc && p->logm == 13) rc = init_iw13_tables(nullptr);
     if (!rc) {
         fill_kernel<<<(p->filt_stride + 255) / 256, 256>>>(p->filt_flat, p->filt_stride, (float)(1.0 / (2.0 * (double)n)));
         count_launch();

@@ -369,6 +369,39 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
     }
 }
 
+
+__global__ void init_tw13_kernel() {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;       // 0 .. 511
+    auto w = [](int num, int den) {                           // exp(-2 pi i num / den), fp64 -> fp32
+        double s, c;
+        sincospi(-2.0 * (double)(num % den) / (double)den, &s, &c);
+        return make_float2((float)c, (float)s);
+    };
+    auto put = [](float4& dst, int k, float2 v) { if (k & 1) { dst.z = v.x; dst.w = v.y; } else { dst.x = v.x; dst.y = v.y; } };
+    if (i < 512) {
+        const int s = i >> 3, k = i & 7;                       // p2: set s, power k
+        put(g_tw13.p2[k >> 1][s], k, w(s * k, 512));
+        const int k2 = s >> 3, n4 = s & 7, n3 = k;             // p3i: set s = k2*8 + n4, entry n3
+        put(g_tw13.p3i[n3 >> 1][s], n3, w((n3 * 8 + n4) * k2, 512));
+    }
+    if (i < 64) {
+        const int n4 = i >> 3, k = i & 7;
+        put(g_tw13.p3[k >> 1][n4], k, w(n4 * k, 64));
+        const int c = i >> 3, m4 = i & 7;                      // p4i: combination c, time digit m4
+        const int k3a = c >> 1;
+        const int t = (c & 1) ? 128 * k3a + 1 : 128 * k3a;     // a representative thread of the combination
+        const int klow_b = (t == 0) ? 512 : 1024 - t;
+        const float2 A = w(m4 * k3a, 64), B = w(m4 * (klow_b >> 7), 64);
+        g_tw13.p4i[c][m4] = make_ulonglong2(pack(A.x, B.x), pack(A.y, B.y));
+    }
+}
+
+int init_iw13_tables(cudaStream_t st) {
+    init_tw13_kernel<<<2, 256, 0, st>>>();
+    count_launch();
+    return check_launch("init_tw13_kernel");
+}
+
 #ifndef IW13_VT
 #define IW13_VT 2
 #endif

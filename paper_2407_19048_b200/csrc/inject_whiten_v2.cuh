@@ -37,6 +37,30 @@ __device__ __forceinline__ void sts2(float* re, float* im, int slot, C2 v) {
     *reinterpret_cast<u64*>(im + 2 * slot) = v.i;
 }
 
+// ---- twiddle tables of the passes whose twiddles depend on few index bits (filled once by init_tw13, fp64 -> fp32) ----
+//   p2[q][s]  = (g[2q], g[2q+1]),  g[k] = w_512^(s k),              s = n3*8 + n4      (P2 forward)
+//   p3[q][s]  = (g[2q], g[2q+1]),  g[k] = w_64^(s k),               s = n4             (P3 forward)
+//   p3i[q][s] = (g[2q], g[2q+1]),  g[n3] = w_512^((n3*8 + n4) k2),  s = k2*8 + n4      (P3 inverse: conj twiddle of P2)
+//   p4i[c][n4] = halves (w_64^(n4 k3a), w_64^(n4 k3b)) in the packed layout, c = the (k3a, k3b) combination of thread t
+// 9.5 KB, read through L1 by every CTA; the twiddles of P1 forward / P2 inverse depend on all nine bits of t (64 KB per
+// table) and stay computed.
+struct Tw13 {
+    float4 p2[4][64];
+    float4 p3[4][8];
+    float4 p3i[4][64];
+    ulonglong2 p4i[8][8];
+};
+static __device__ Tw13 g_tw13;       // this header is included by inject_whiten13.cu only
+
+__device__ __forceinline__ void tw_load8(const float4* col, int stride, float2 (&g)[8]) {
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const float4 f = __ldg(col + q * stride);
+        g[2 * q] = make_float2(f.x, f.y);
+        g[2 * q + 1] = make_float2(f.z, f.w);
+    }
+}
+
 // ---- forward passes ----
 // x[n1] = z[n1*512 + t] (natural complex, from global).  Leaves the spectrum digits (k1; n2 n3 n4) in smem.
 __device__ __forceinline__ void p1_fwd(const float2 (&x)[16], int t, float* re, float* im) {
@@ -73,12 +97,12 @@ __device__ __forceinline__ void p1_fwd(const float2 (&x)[16], int t, float* re, 
 
 __device__ __forceinline__ void p2_fwd(int t, float* re, float* im) {
     const int kap = t >> 6, n3 = (t >> 3) & 7, n4 = t & 7;
+    float2 g[8];
+    tw_load8(&g_tw13.p2[0][t & 63], 64, g);
     C2 v[8];
 #pragma unroll
     for (int n2 = 0; n2 < 8; ++n2) v[n2] = lds2(re, im, slot13(kap, n2, n3, n4));
     dif8(v);
-    float2 g[8];
-    powers8(make_float2(1.0f, 0.0f), twiddle<512>(n3 * 8 + n4), g);
 #pragma unroll
     for (int r = 0; r < 8; ++r) {
         const int k2 = brev<8>(r);
@@ -88,12 +112,12 @@ __device__ __forceinline__ void p2_fwd(int t, float* re, float* im) {
 
 __device__ __forceinline__ void p3_fwd(int t, float* re, float* im) {
     const int kap = t >> 6, k2 = (t >> 3) & 7, n4 = t & 7;
+    float2 g[8];
+    tw_load8(&g_tw13.p3[0][n4], 8, g);
     C2 v[8];
 #pragma unroll
     for (int n3 = 0; n3 < 8; ++n3) v[n3] = lds2(re, im, slot13(kap, k2, n3, n4));
     dif8(v);
-    float2 g[8];
-    powers8(make_float2(1.0f, 0.0f), twiddle<64>(n4), g);
 #pragma unroll
     for (int r = 0; r < 8; ++r) {
         const int k3 = brev<8>(r);
@@ -129,13 +153,15 @@ __device__ __forceinline__ void p4_inv(int klow_a, int klow_b, C2 (&v)[8], float
     int ba, ka, bb, kb;
     p4_addr(klow_a, ba, ka);
     p4_addr(klow_b, bb, kb);
-    // conj twiddle of P3: w_64^(-n4 k3) per half
-    const float2 ga = twiddle<64>(klow_a >> 7), gb = twiddle<64>(klow_b >> 7);
-    C2 tw[8];
-    powers8(C2{bcast(1.0f), bcast(0.0f)}, C2{pack(ga.x, gb.x), pack(ga.y, gb.y)}, tw);
+    // conj twiddle of P3: w_64^(-n4 k3) per half, from the table row of this thread's (k3a, k3b) combination
+    const ulonglong2* trow = g_tw13.p4i[2 * (klow_a >> 7) + ((klow_a & 127) != 0 ? 1 : 0)];
 #pragma unroll
     for (int n4 = 0; n4 < 8; ++n4) {
-        const C2 y = n4 == 0 ? v[0] : cmul_conj(v[n4], tw[n4]);
+        C2 y = v[0];
+        if (n4 != 0) {
+            const ulonglong2 w = __ldg(trow + n4);
+            y = cmul_conj(v[n4], C2{w.x, w.y});
+        }
         float ar, br, ai, bi;
         unpack(y.r, ar, br);
         unpack(y.i, ai, bi);
@@ -151,9 +177,9 @@ __device__ __forceinline__ void p3_inv(int t, float* re, float* im) {
 #pragma unroll
     for (int r = 0; r < 8; ++r) v[r] = lds2(re, im, slot13(kap, k2, brev<8>(r), n4));
     dit8(v);
-    // conj twiddle of P2: w_512^(-(n3*8 + n4) k2) = conj(c * s^n3), c = w_512^(n4 k2), s = w_64^k2
+    // conj twiddle of P2: w_512^(-(n3*8 + n4) k2)
     float2 g[8];
-    powers8(twiddle<512>(n4 * k2), twiddle<64>(k2), g);
+    tw_load8(&g_tw13.p3i[0][t & 63], 64, g);
 #pragma unroll
     for (int n3 = 0; n3 < 8; ++n3) sts2(re, im, slot13(kap, k2, n3, n4), cmul_conj_s(v[n3], g[n3]));
 }
