@@ -487,8 +487,8 @@ def run_extra(args):
                                                  "gathered from a [3, 2^26] strip, Welch from 128 s (4 s Hann), IMRPhenomD"}}))
         return
 
-    # sweep: fixed total samples (2^27 per detector), segment length 1..16 s at 4096 Hz
-    for t_seg in (1.0, 2.0, 4.0, 8.0, 16.0):
+    # sweep: fixed total samples (2^27 per detector), segment length 1..256 s at 4096 Hz (n = 2^12 .. 2^20)
+    for t_seg in (1.0, 2.0, 4.0, 8.0, 16.0, 32.0, 64.0, 128.0, 256.0):
         n = int(t_seg * 4096)
         batch = (1 << 27) // n
         wl = WL.make_c4(batch=batch, t_seg=t_seg)

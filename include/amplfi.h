@@ -33,7 +33,7 @@ extern "C" {
 
 #define AMPLFI_OK                    0
 #define AMPLFI_ERR_INVALID_ARG      (-1)  /* null pointer, batch/n_det <= 0, f_lo >= f_hi, f_hi > fs/2, bad ids */
-#define AMPLFI_ERR_UNSUPPORTED_SIZE (-2)  /* n or nperseg not a power of two in [2^10, 2^16]; nperseg > n_bg */
+#define AMPLFI_ERR_UNSUPPORTED_SIZE (-2)  /* n not a power of two in [2^10, 2^20], nperseg not one in [2^10, 2^15]; nperseg > n_bg */
 #define AMPLFI_ERR_CUDA             (-3)  /* CUDA runtime/launch error (message in amplfi_last_error) */
 #define AMPLFI_ERR_ALIGNMENT        (-4)  /* a buffer is not aligned as documented */
 
@@ -69,11 +69,12 @@ const char* amplfi_version(void);
 int amplfi_phenomd_table(double* out);
 
 /* Create a plan for segments of n samples at fs Hz seen by n_det detectors.
- *   n        power of two, 2^10 .. 2^16 (4 s at 2048 Hz = 8192)
+ *   n        power of two, 2^10 .. 2^20 (4 s at 2048 Hz = 8192; minutes-long
+ *            binary-neutron-star segments are "larger by an order of magnitude": 256 s at 4096 Hz = 2^20)
  *   det_ids  HOST array [n_det] of AMPLFI_H1/L1/V1 ("Hanford and Livingston"), n_det 1..3
  *   max_batch  largest batch later passed to the per-batch calls (sizes the coefficient workspace
  *              and, for the fused call, the [max_batch, K] complex h0 workspace)
- *   nperseg  Welch segment length, power of two 2^10 .. 2^16 with nperseg <= n, or 0 if
+ *   nperseg  Welch segment length, power of two 2^10 .. 2^15 with nperseg <= n, or 0 if
  *            amplfi_psd_welch will not be called
  * Allocates device tables on the current CUDA device.  *out receives the plan. */
 int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_batch, int nperseg,
@@ -131,7 +132,7 @@ int amplfi_psd_welch(const amplfi_plan* plan, const float* bg, long n_bg, long r
  *   psd      [n_det, n_psd] fp32, S * 2^140; n_psd == K, or n_psd == (n/r)/2+1 for an integer r >= 1, in
  *            which case S is linearly interpolated in frequency onto the segment grid.
  *   out      [batch, n_det, n] fp32.
- * batch <= the plan's max_batch.  n = 2^16 is decimated by two around the 2^15-sample transform, the
+ * batch <= the plan's max_batch.  n >= 2^16 is decimated by n / 2^15 around the 2^15-sample transform, the
  * intermediate spectra of a chunk of segments staying in L2. */
 int amplfi_inject_whiten(const amplfi_plan* plan, int batch, const float* noise, const long* offsets,
                          long strip_len, const float* h_det, int approximant, const double* params,

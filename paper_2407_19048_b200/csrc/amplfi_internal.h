@@ -40,7 +40,7 @@ struct amplfi_plan {
     float* welch_part;     // [n_det * max_seg * (nperseg/2+1)]
     int welch_max_seg;
     int* d_det_ids;        // [3]
-    float2* long_spec;     // n = 65536 only: sub-spectra of one chunk of units [long_chunk, 2, 16392] (L2-resident)
+    float2* long_spec;     // n >= 65536: sub-spectra of one chunk of units [long_chunk, n/32768, 16392] (L2-resident)
     int long_chunk;        // units per chunk
     // amplfi_assemble_batch: PSD chain runs on `side`, forked from / joined into the caller's stream
     cudaStream_t side;
@@ -120,8 +120,8 @@ int launch_shift_resp(const amplfi_plan* p, int batch, const double* t_shift, cu
 int launch_td_resp(const amplfi_plan* p, int batch, cudaStream_t st);
 int setup_inject_whiten_attrs();
 
-// inject_whiten_long.cu (n = 65536: decimation by two around the 32768-sample transform)
-size_t long_scratch_floats2(int chunk_units);
+// inject_whiten_long.cu (n = 2^16 .. 2^20: decimation by n/32768 around the 32768-sample transform)
+size_t long_scratch_floats2(int chunk_units, int rdec);
 int launch_inject_whiten_long(const amplfi_plan* p, const IwArgs& a, int mode, int units, cudaStream_t st);
 
 }  // namespace amplfi

@@ -33,7 +33,7 @@ int check_launch(const char* what) {
     return AMPLFI_OK;
 }
 
-static bool is_pow2_in_range(long v) { return v >= 1024 && v <= 65536 && (v & (v - 1)) == 0; }
+static bool is_pow2_in_range(long v, long hi = 65536) { return v >= 1024 && v <= hi && (v & (v - 1)) == 0; }
 
 static const double kPdTable[AMPLFI_PD_ROWS][AMPLFI_PD_COLS] = AMPLFI_PD_TABLE_INIT;
 
@@ -139,7 +139,7 @@ int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_
     }
     for (int d = 0; d < n_det; ++d)
         if (det_ids[d] < 0 || det_ids[d] > 2) { set_error("amplfi_plan_create: unknown detector id %d", det_ids[d]); return AMPLFI_ERR_INVALID_ARG; }
-    if (!is_pow2_in_range(n)) { set_error("amplfi_plan_create: n = %d is not a power of two in [2^10, 2^16]", n); return AMPLFI_ERR_UNSUPPORTED_SIZE; }
+    if (!is_pow2_in_range(n, 1L << 20)) { set_error("amplfi_plan_create: n = %d is not a power of two in [2^10, 2^20]", n); return AMPLFI_ERR_UNSUPPORTED_SIZE; }
     if (nperseg != 0 && (!is_pow2_in_range(nperseg) || nperseg > 32768)) {
         set_error("amplfi_plan_create: nperseg = %d is not a power of two in [2^10, 2^15]", nperseg);
         return AMPLFI_ERR_UNSUPPORTED_SIZE;
@@ -172,9 +172,12 @@ int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_
     if (!rc) rc = dev_alloc(&p->fir_spec, (size_t)n_det * p->n_bins);
     if (!rc) rc = dev_alloc(&p->fir_time, (size_t)n_det * n);
     if (!rc) rc = dev_alloc(&p->d_det_ids, (size_t)3);
-    if (!rc && p->logm == 15) {
-        p->long_chunk = sms > 0 ? sms : 148;          // 2 CTAs per unit: two full waves of one CTA per SM; 39 MB of spectra
-        rc = dev_alloc(&p->long_spec, amplfi::long_scratch_floats2(p->long_chunk));
+    if (!rc && p->logm >= 15) {
+        // n/32768 CTAs per unit, one CTA per SM: a chunk is two full waves and its spectra (39 MB) stay in L2
+        const int rdec = n / 32768;
+        p->long_chunk = (2 * (sms > 0 ? sms : 148)) / rdec;
+        if (p->long_chunk < 1) p->long_chunk = 1;
+        rc = dev_alloc(&p->long_spec, amplfi::long_scratch_floats2(p->long_chunk, rdec));
     }
     if (!rc && nperseg) rc = dev_alloc(&p->welch_part, (size_t)n_det * p->welch_max_seg * (nperseg / 2 + 1));
     if (!rc) {
@@ -296,7 +299,6 @@ int amplfi_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
     const bool fused = (h_det == nullptr && params != nullptr);
     if (fused && approximant != AMPLFI_TAYLORF2 && approximant != AMPLFI_IMRPHENOMD) { set_error("amplfi_inject_whiten: unknown approximant %d", approximant); return AMPLFI_ERR_INVALID_ARG; }
     if ((reinterpret_cast<size_t>(out) & 7) || (reinterpret_cast<size_t>(noise) & 3) || (reinterpret_cast<size_t>(h_det) & 7)) { set_error("amplfi_inject_whiten: out/h_det must be 8-byte aligned, noise 4-byte aligned"); return AMPLFI_ERR_ALIGNMENT; }
-    if (p->logm > 15) { set_error("amplfi_inject_whiten: n = %d not supported by this build", p->n); return AMPLFI_ERR_UNSUPPORTED_SIZE; }
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     rc = launch_filter(p, psd, n_psd, f_lo, f_hi, st);
     if (rc) return rc;

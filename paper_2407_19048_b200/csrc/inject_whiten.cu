@@ -308,7 +308,7 @@ int launch_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
         case 12: return launch_iw_mode<12>(a, mode, units, st);
         case 13: return launch_iw13(a, mode, units, st);
         case 14: return launch_iw_mode<14>(a, mode, units, st);
-        case 15: return launch_inject_whiten_long(p, a, mode, units, st);
+        case 15: case 16: case 17: case 18: case 19: return launch_inject_whiten_long(p, a, mode, units, st);
         default:
             set_error("amplfi_inject_whiten: segment length %d not supported by this build", p->n);
             return AMPLFI_ERR_UNSUPPORTED_SIZE;

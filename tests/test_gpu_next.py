@@ -172,3 +172,64 @@ def test_fused_invalid_and_empty_band_rows_inject_nothing(n, fs):
     ref = A.amplfi_inject_whiten(plan, batch, dev(noise), psd_s, 20.0, 1000.0)
     torch.cuda.synchronize()
     assert torch.equal(out, ref)
+
+
+# ------------------------------------------------------------------------------------------ long segments (8(f)-4)
+@pytest.mark.parametrize("n,fs,mode", [(1 << 17, 4096.0, "fused"), (1 << 17, 4096.0, "none"), (1 << 18, 4096.0, "fused"),
+                                       (1 << 18, 4096.0, "hdet"), (1 << 19, 4096.0, "fused"), (1 << 20, 4096.0, "fused")])
+def test_long_segments_parity(n, fs, mode):
+    """binary-neutron-star signals last minutes, "input arrays larger by an order of magnitude": segments of
+    32 .. 256 s at 4096 Hz, a low-mass TaylorF2 inspiral that spends the whole segment in band next to a heavy IMR system."""
+    dets = [0, 1]
+    batch = 2
+    t_seg = n / fs
+    rng = np.random.Generator(np.random.Philox(n))
+    par = WL.draw_params(rng, batch, t_c=(t_seg - 2.5, t_seg - 1.5))
+    par[0, :5] = [1.2, 0.9, 0.0, 0.0, 40.0]                    # a binary neutron star at 40 Mpc
+    approx = A.TAYLORF2
+    noise = WL.coloured_noise(rng, (batch, len(dets)), n, fs)
+    psd = np.stack([WL.aligo_psd(np.arange(n // 2 + 1) * fs / n)] * 2)
+    psd_s = (psd * PSD_SCALE).astype(np.float32)
+    plan = A.Plan(n, fs, dets, batch)
+    kw = {}
+    h_det_ref = None
+    if mode != "none":
+        hp, hc, _ = OW.waveform_fd(approx, par, n, fs, 20.0, 1000.0)
+        h_det_ref, _ = OP.project(hp, hc, par, 0.2, dets, n, fs)
+    if mode == "fused":
+        kw = dict(approximant=approx, params=dev(par), gmst=0.2)
+    elif mode == "hdet":
+        hp_g, hc_g, _ = A.amplfi_waveform_fd(plan, approx, dev(par), 20.0, 1000.0)
+        h_det, _ = A.amplfi_project(plan, dev(par), 0.2, hp_g, hc_g)
+        kw = dict(h_det=h_det)
+    out = A.amplfi_inject_whiten(plan, batch, dev(noise), dev(psd_s), 20.0, 1000.0, **kw)
+    torch.cuda.synchronize()
+    ref = OWH.inject_whiten(noise.astype(np.float64), h_det_ref, psd_s.astype(np.float64) / PSD_SCALE, fs, 20.0, 1000.0)
+    assert row_err(out.cpu().numpy().astype(np.float64), ref).max() <= TOL
+
+
+def test_long_segment_gather_views_and_td():
+    """n = 2^17 through the other entry points: strip gather with offsets, two views, time-domain output, cropped FIR."""
+    n, fs, dets, batch = 1 << 17, 4096.0, [0, 1, 2], 2
+    rng = np.random.Generator(np.random.Philox(17))
+    par = WL.draw_params(rng, batch, t_c=(29.0, 30.0))
+    strip = WL.coloured_noise(rng, (3,), 1 << 19, fs)
+    offsets = np.array([[5, 100001, 262144 + 3], [393216, 0, 77]], dtype=np.int64)
+    psd = np.stack([WL.aligo_psd(np.arange(n // 2 + 1) * fs / n)] * 3)
+    psd_s = (psd * PSD_SCALE).astype(np.float32)
+    psd64 = psd_s.astype(np.float64) / PSD_SCALE
+    plan = A.Plan(n, fs, dets, batch)
+    t_shift = np.array([0.75, 0.001])
+    out, out2 = A.amplfi_inject_whiten_views(plan, batch, dev(strip), dev(psd_s), 20.0, 1000.0, dev(par), dev(t_shift),
+                                             offsets=dev(offsets), gmst=0.4)
+    noise = OWH.gather(strip, offsets, n)
+    d, d2 = OV.two_views(A.IMRPHENOMD, par, t_shift, noise, psd64, 0.4, dets, fs, 20.0, 1000.0)
+    assert row_err(out.cpu().numpy().astype(np.float64), d).max() <= TOL
+    assert row_err(out2.cpu().numpy().astype(np.float64), d2).max() <= TOL
+    h_t, _ = A.amplfi_waveform_td(plan, A.IMRPHENOMD, dev(par), 20.0, 1000.0)
+    hp, hc, _ = OW.waveform_td(A.IMRPHENOMD, par, n, fs, 20.0, 1000.0)
+    got = h_t.cpu().numpy().astype(np.float64)
+    assert row_err(got[:, 0], hp).max() <= TOL and row_err(got[:, 1], hc).max() <= TOL
+    out_f = A.amplfi_inject_whiten_fir(plan, batch, dev(strip), dev(psd_s), 20.0, 1000.0, 2.0, crop=True, offsets=dev(offsets))
+    ref_f = OWH.inject_whiten_fir(noise, None, psd64, fs, 20.0, 1000.0, 2.0, crop=True)
+    assert row_err(out_f.cpu().numpy().astype(np.float64), ref_f).max() <= TOL
