@@ -77,7 +77,7 @@ def test_argument_validation_without_device(lib):
     assert L.amplfi_plan_create(8192, 2048.0, 3, ids, 0, 0, ctypes.byref(h)) == lib.ERR_INVALID_ARG
     assert L.amplfi_plan_create(8000, 2048.0, 3, ids, 4, 0, ctypes.byref(h)) == lib.ERR_UNSUPPORTED_SIZE
     assert L.amplfi_plan_create(512, 2048.0, 3, ids, 4, 0, ctypes.byref(h)) == lib.ERR_UNSUPPORTED_SIZE
-    assert L.amplfi_plan_create(1 << 17, 2048.0, 3, ids, 4, 0, ctypes.byref(h)) == lib.ERR_UNSUPPORTED_SIZE
+    assert L.amplfi_plan_create(1 << 21, 2048.0, 3, ids, 4, 0, ctypes.byref(h)) == lib.ERR_UNSUPPORTED_SIZE
     assert L.amplfi_plan_create(8192, 2048.0, 3, ids, 4, 3000, ctypes.byref(h)) == lib.ERR_UNSUPPORTED_SIZE
     assert h.value is None
     # null plan / null buffers
