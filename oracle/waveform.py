@@ -397,6 +397,49 @@ def imrphenomd_h0(p, n_bins, t_seg, f_lo, f_hi, tab=None, sigma_scale=1.0):
 
 
 # ----------------------------------------------------------------------------------------
+# Sine-Gaussian burst ("can be extended to burst signal morphologies like sine-Gaussians ...
+# central frequency or duration").  The paper gives no formula: DESIGN.md reading R-W12.
+# ----------------------------------------------------------------------------------------
+SINE_GAUSSIAN = 2
+
+
+def sg_params_valid(p):
+    """row layout for this family: 0 f0 [Hz], 1 Q, 2-3 unused, 4 peak amplitude A, 5 ellipticity angle iota,
+    6 phase phi, 7 central time t0 [s], 8 ra, 9 dec, 10 psi."""
+    return bool((p[0] > 0) and (p[1] > 0) and (p[4] > 0) and np.all(np.isfinite(p)))
+
+
+def sine_gaussian_td(p, t):
+    """Time-domain definition: h+(t) = (1 + cos^2 iota)/2 * A e^{-(t-t0)^2/tau^2} cos(2 pi f0 (t-t0) + phi),
+    hx(t) = cos iota * A e^{-(t-t0)^2/tau^2} sin(2 pi f0 (t-t0) + phi),  tau = Q / (sqrt 2 pi f0)."""
+    f0, q, amp, iota, phi, t0 = p[0], p[1], p[4], p[5], p[6], p[7]
+    tau = q / (np.sqrt(2.0) * np.pi * f0)
+    env = amp * np.exp(-((t - t0) / tau) ** 2)
+    arg = 2.0 * np.pi * f0 * (t - t0) + phi
+    ci = np.cos(iota)
+    return 0.5 * (1.0 + ci * ci) * env * np.cos(arg), ci * env * np.sin(arg)
+
+
+def sine_gaussian_h0(p, n_bins, t_seg, f_lo, f_hi):
+    """Frequency-domain model on the grid, positive-frequency Gaussian only (the mirror term centred on -f0 is dropped:
+    it is e^{-2 Q^2} of the peak at f0 and at most e^{-Q^2/2} of it anywhere, reached as f -> 0): h0(f) = A tau sqrt(pi)/2 * e^{-pi^2 tau^2 (f - f0)^2} * e^{-i (2 pi f t0 - phi)},
+    with h+ = (1 + cos^2 iota)/2 h0 and hx = -i cos iota h0 as for the binaries (R-W6); non-zero for
+    f_lo <= f_k <= f_hi, bins 0 and Nyquist always zero (R-W7)."""
+    h0 = np.zeros(n_bins, dtype=np.complex128)
+    if not sg_params_valid(p):
+        return h0
+    f0, q, amp, phi, t0 = p[0], p[1], p[4], p[6], p[7]
+    tau = q / (np.sqrt(2.0) * np.pi * f0)
+    k = np.arange(n_bins)
+    f = k / t_seg
+    band = (f >= f_lo) & (f <= f_hi) & (k > 0) & (k < n_bins - 1)
+    fb = f[band]
+    h0[band] = 0.5 * amp * tau * np.sqrt(np.pi) * np.exp(-(np.pi * tau * (fb - f0)) ** 2) \
+        * np.exp(-1j * (2.0 * np.pi * fb * t0 - phi))
+    return h0
+
+
+# ----------------------------------------------------------------------------------------
 # batch entry point mirroring amplfi_waveform_fd
 # ----------------------------------------------------------------------------------------
 
@@ -404,7 +447,7 @@ def h0_fd(approximant, params, n, fs, f_lo, f_hi):
     params = np.atleast_2d(np.asarray(params, dtype=np.float64))
     n_bins = n // 2 + 1
     t_seg = n / fs
-    fn = taylorf2_h0 if approximant == TAYLORF2 else imrphenomd_h0
+    fn = {TAYLORF2: taylorf2_h0, IMRPHENOMD: imrphenomd_h0, SINE_GAUSSIAN: sine_gaussian_h0}[approximant]
     return np.stack([fn(p, n_bins, t_seg, f_lo, f_hi) for p in params])
 
 
@@ -419,7 +462,8 @@ def waveform_fd(approximant, params, n, fs, f_lo, f_hi):
     params = np.atleast_2d(np.asarray(params, dtype=np.float64))
     h0 = h0_fd(approximant, params, n, fs, f_lo, f_hi)
     hp, hc = polarisations(h0, params[:, 5])
-    flags = np.array([0 if params_valid(p) else 1 for p in params], dtype=np.int32)
+    valid = sg_params_valid if approximant == SINE_GAUSSIAN else params_valid
+    flags = np.array([0 if valid(p) else 1 for p in params], dtype=np.int32)
     return hp, hc, flags
 
 

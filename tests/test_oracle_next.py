@@ -195,3 +195,46 @@ def test_fir_whitened_noise_variance_and_signal_linearity():
     a = WH.inject_whiten_fir(x[:1], h_det, psd, FS, 20.0, 1000.0, 1.0)
     s = WH.inject_whiten_fir(0 * x[:1], h_det, psd, FS, 20.0, 1000.0, 1.0)
     assert np.abs(a - (y[:1] + s)).max() < 1e-9 * np.abs(a).max()
+
+
+# ---------------------------------------------------------------- sine-Gaussian burst
+def _sg(f0=250.0, q=9.0, amp=1e-21, iota=0.6, phi=0.4, t0=2.0):
+    return np.array([f0, q, 0.0, 0.0, amp, iota, phi, t0, 1.0, -0.4, 0.9])
+
+
+@pytest.mark.parametrize("f0,q", [(250.0, 9.0), (80.0, 5.0), (600.0, 30.0)])
+def test_sine_gaussian_fd_model_is_the_fourier_transform_of_the_td_definition(f0, q):
+    # independent route: sample the time-domain closed form and take numpy's FFT; X[k]/fs approximates the continuous
+    # Fourier transform (the Gaussian is far from the segment edges and far below Nyquist)
+    p = _sg(f0=f0, q=q)
+    t = np.arange(N) / FS
+    hp_t, hc_t = OW.sine_gaussian_td(p, t)
+    hp, hc, flags = OW.waveform_fd(OW.SINE_GAUSSIAN, p[None], N, FS, 1.0, 1023.0)
+    assert flags[0] == 0
+    for ht, hf in ((hp_t, hp[0]), (hc_t, hc[0])):
+        ref = np.fft.rfft(ht) / FS
+        scale = np.abs(ref).max()
+        # the dropped mirror term is at most e^(-Q^2/2) of the peak (reached as f -> 0)
+        assert np.abs(hf[5:-5] - ref[5:-5]).max() < max(3.0 * np.exp(-0.5 * q * q), 1e-9) * scale
+    # duration and central frequency are what the parameters say ("central frequency or duration")
+    tau = q / (np.sqrt(2.0) * np.pi * f0)
+    env2 = hp_t ** 2 + (hc_t * (0.5 * (1 + np.cos(0.6) ** 2)) / np.cos(0.6)) ** 2
+    t_mean = np.sum(t * env2) / np.sum(env2)
+    assert abs(t_mean - 2.0) < 1e-6
+    assert abs(np.sqrt(np.sum((t - t_mean) ** 2 * env2) / np.sum(env2)) / (tau / 2.0) - 1) < 1e-6
+    kpk = np.argmax(np.abs(hp[0]))
+    assert abs(kpk * FS / N - f0) <= FS / N
+
+
+def test_sine_gaussian_band_flags_and_td_output():
+    p = np.stack([_sg(), _sg(q=-1.0), _sg(amp=0.0), _sg(f0=np.nan)])
+    hp, hc, flags = OW.waveform_fd(OW.SINE_GAUSSIAN, p, N, FS, 200.0, 300.0)
+    assert list(flags) == [0, 1, 1, 1]
+    assert np.all(hp[1:] == 0) and np.all(hc[1:] == 0)
+    f = np.arange(N // 2 + 1) * FS / N
+    assert np.all(hp[0][(f < 200.0) | (f > 300.0)] == 0) and hp[0][f == 200.0] != 0 and hp[0][f == 300.0] != 0
+    # the time-domain output call reproduces the closed form (full band)
+    hp_t, hc_t, _ = OW.waveform_td(OW.SINE_GAUSSIAN, _sg()[None], N, FS, 1.0, 1023.0)
+    a, b = OW.sine_gaussian_td(_sg(), np.arange(N) / FS)
+    assert np.abs(hp_t[0] - a).max() < 1e-9 * np.abs(a).max()
+    assert np.abs(hc_t[0] - b).max() < 1e-9 * np.abs(a).max()
