@@ -39,6 +39,7 @@ extern "C" {
 
 #define AMPLFI_TAYLORF2    0   /* 3.5PN non-spinning inspiral to f_ISCO (ref. [33]) */
 #define AMPLFI_IMRPHENOMD  1   /* the paper's approximant (ref. [32]), aligned spins */
+#define AMPLFI_SINE_GAUSSIAN 2 /* burst family the paper names as an extension; see the params note below */
 
 #define AMPLFI_H1 0
 #define AMPLFI_L1 1
@@ -50,7 +51,13 @@ extern "C" {
  * = Theta of PAPER.md:151 eq. (4) plus the aligned spins and the arrival time
  * (PAPER.md:93, :117).  A row with q outside (0,1], |chi| >= 1, dist <= 0, mchirp <= 0 or a
  * non-finite entry does not fail the call: that sample's waveform is identically zero and
- * flags[b] = 1 where a flags buffer is given. */
+ * flags[b] = 1 where a flags buffer is given.
+ * AMPLFI_SINE_GAUSSIAN reads the row as  0 f0 [Hz]  1 Q  2,3 unused  4 peak amplitude A  5 iota (ellipticity angle)
+ * 6 phi  7 t0 (central time)  8 ra  9 dec  10 psi  and evaluates, with tau = Q / (sqrt2 pi f0),
+ *     h0(f) = A tau sqrt(pi)/2 exp(-(pi tau (f - f0))^2) exp(-i (2 pi f t0 - phi)),  h+ = (1+cos^2 iota)/2 h0,  hx = -i cos iota h0,
+ * the Fourier transform of  h+(t) = (1+cos^2 iota)/2 A e^{-(t-t0)^2/tau^2} cos(2 pi f0 (t-t0) + phi),
+ * hx(t) = cos iota A e^{-(t-t0)^2/tau^2} sin(2 pi f0 (t-t0) + phi)  up to the mirror term at -f0 (<= e^{-Q^2/2} of the peak);
+ * invalid: f0 <= 0, Q <= 0, A <= 0 or a non-finite entry. */
 
 typedef struct amplfi_plan amplfi_plan;   /* opaque */
 

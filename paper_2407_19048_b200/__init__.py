@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libamplfi.so")
 
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED_SIZE, ERR_CUDA, ERR_ALIGNMENT = 0, -1, -2, -3, -4
-TAYLORF2, IMRPHENOMD = 0, 1
+TAYLORF2, IMRPHENOMD, SINE_GAUSSIAN = 0, 1, 2
 H1, L1, V1 = 0, 1, 2
 N_PARAMS = 11
 

@@ -21,6 +21,7 @@ struct amplfi_plan {
     int det_ids[3];
     int max_batch;
     int nperseg;           // 0: no Welch
+    int last_approx;       // approximant of the last launch_prepare (the waveform launch that follows evaluates that family)
     int device;
     int sm_count;
     // device tables / workspace (owned)

@@ -47,6 +47,8 @@ static int dev_alloc(T** ptr, size_t count) {
     return AMPLFI_OK;
 }
 
+static bool known_approximant(int a) { return a == AMPLFI_TAYLORF2 || a == AMPLFI_IMRPHENOMD || a == AMPLFI_SINE_GAUSSIAN; }
+
 static int validate_band(const amplfi_plan* p, double f_lo, double f_hi, const char* who) {
     if (!(f_lo >= 0.0) || !(f_hi > f_lo) || !(f_hi <= 0.5 * p->fs)) {
         set_error("%s: need 0 <= f_lo < f_hi <= fs/2 (got %g, %g, fs %g)", who, f_lo, f_hi, p->fs);
@@ -250,7 +252,7 @@ int amplfi_waveform_fd(const amplfi_plan* p, int approximant, int batch, const d
                        double f_hi, float* hp, float* hc, int* flags, void* stream) {
     if (p == nullptr || params == nullptr || hp == nullptr || hc == nullptr) { set_error("amplfi_waveform_fd: null pointer"); return AMPLFI_ERR_INVALID_ARG; }
     if (batch < 1 || batch > p->max_batch) { set_error("amplfi_waveform_fd: batch %d outside [1, %d]", batch, p->max_batch); return AMPLFI_ERR_INVALID_ARG; }
-    if (approximant != AMPLFI_TAYLORF2 && approximant != AMPLFI_IMRPHENOMD) { set_error("amplfi_waveform_fd: unknown approximant %d", approximant); return AMPLFI_ERR_INVALID_ARG; }
+    if (!known_approximant(approximant)) { set_error("amplfi_waveform_fd: unknown approximant %d", approximant); return AMPLFI_ERR_INVALID_ARG; }
     int rc = validate_band(p, f_lo, f_hi, "amplfi_waveform_fd");
     if (rc) return rc;
     if ((reinterpret_cast<size_t>(hp) | reinterpret_cast<size_t>(hc)) & 7) { set_error("amplfi_waveform_fd: hp/hc must be 8-byte aligned"); return AMPLFI_ERR_ALIGNMENT; }
@@ -297,7 +299,7 @@ int amplfi_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
     if (offsets != nullptr && strip_len < p->n) { set_error("amplfi_inject_whiten: strip_len %ld < n %d", strip_len, p->n); return AMPLFI_ERR_INVALID_ARG; }
     if (n_psd < 2 || ((p->n / 2) % (n_psd - 1)) != 0) { set_error("amplfi_inject_whiten: n_psd = %d does not divide the segment grid (n/2 = %d)", n_psd, p->n / 2); return AMPLFI_ERR_INVALID_ARG; }
     const bool fused = (h_det == nullptr && params != nullptr);
-    if (fused && approximant != AMPLFI_TAYLORF2 && approximant != AMPLFI_IMRPHENOMD) { set_error("amplfi_inject_whiten: unknown approximant %d", approximant); return AMPLFI_ERR_INVALID_ARG; }
+    if (fused && !known_approximant(approximant)) { set_error("amplfi_inject_whiten: unknown approximant %d", approximant); return AMPLFI_ERR_INVALID_ARG; }
     if ((reinterpret_cast<size_t>(out) & 7) || (reinterpret_cast<size_t>(noise) & 3) || (reinterpret_cast<size_t>(h_det) & 7)) { set_error("amplfi_inject_whiten: out/h_det must be 8-byte aligned, noise 4-byte aligned"); return AMPLFI_ERR_ALIGNMENT; }
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     rc = launch_filter(p, psd, n_psd, f_lo, f_hi, st);
@@ -332,7 +334,7 @@ int amplfi_assemble_batch(const amplfi_plan* p, int batch, const float* bg, long
     int rc = validate_band(p, f_lo, f_hi, "amplfi_assemble_batch");
     if (rc) return rc;
     if (offsets != nullptr && strip_len < p->n) { set_error("amplfi_assemble_batch: strip_len %ld < n %d", strip_len, p->n); return AMPLFI_ERR_INVALID_ARG; }
-    if (approximant != AMPLFI_TAYLORF2 && approximant != AMPLFI_IMRPHENOMD) { set_error("amplfi_assemble_batch: unknown approximant %d", approximant); return AMPLFI_ERR_INVALID_ARG; }
+    if (!known_approximant(approximant)) { set_error("amplfi_assemble_batch: unknown approximant %d", approximant); return AMPLFI_ERR_INVALID_ARG; }
     if ((reinterpret_cast<size_t>(out) & 7) || (reinterpret_cast<size_t>(noise) & 3)) { set_error("amplfi_assemble_batch: out must be 8-byte aligned, noise 4-byte aligned"); return AMPLFI_ERR_ALIGNMENT; }
     const int n_psd = p->nperseg / 2 + 1;
     if (((p->n / 2) % (n_psd - 1)) != 0) { set_error("amplfi_assemble_batch: nperseg %d does not divide n %d", p->nperseg, p->n); return AMPLFI_ERR_INVALID_ARG; }
@@ -379,7 +381,7 @@ int amplfi_inject_whiten_views(const amplfi_plan* p, int batch, const float* noi
     if (rc) return rc;
     if (params == nullptr || t_shift == nullptr || out2 == nullptr) { set_error("amplfi_inject_whiten_views: null pointer"); return AMPLFI_ERR_INVALID_ARG; }
     if (reinterpret_cast<size_t>(out2) & 7) { set_error("amplfi_inject_whiten_views: out2 must be 8-byte aligned"); return AMPLFI_ERR_ALIGNMENT; }
-    if (approximant != AMPLFI_TAYLORF2 && approximant != AMPLFI_IMRPHENOMD) { set_error("amplfi_inject_whiten_views: unknown approximant %d", approximant); return AMPLFI_ERR_INVALID_ARG; }
+    if (!known_approximant(approximant)) { set_error("amplfi_inject_whiten_views: unknown approximant %d", approximant); return AMPLFI_ERR_INVALID_ARG; }
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     rc = launch_filter(p, psd, n_psd, f_lo, f_hi, st);
     if (!rc) rc = launch_prepare(p, approximant, batch, params, gmst, f_lo, f_hi, 2.0 * p->fs, nullptr, st);
@@ -404,7 +406,7 @@ int amplfi_waveform_td(const amplfi_plan* p, int approximant, int batch, const d
                        float* h_t, int* flags, void* stream) {
     if (p == nullptr || params == nullptr || h_t == nullptr) { set_error("amplfi_waveform_td: null pointer"); return AMPLFI_ERR_INVALID_ARG; }
     if (batch < 1 || batch > p->max_batch) { set_error("amplfi_waveform_td: batch %d outside [1, %d]", batch, p->max_batch); return AMPLFI_ERR_INVALID_ARG; }
-    if (approximant != AMPLFI_TAYLORF2 && approximant != AMPLFI_IMRPHENOMD) { set_error("amplfi_waveform_td: unknown approximant %d", approximant); return AMPLFI_ERR_INVALID_ARG; }
+    if (!known_approximant(approximant)) { set_error("amplfi_waveform_td: unknown approximant %d", approximant); return AMPLFI_ERR_INVALID_ARG; }
     int rc = validate_band(p, f_lo, f_hi, "amplfi_waveform_td");
     if (rc) return rc;
     if (reinterpret_cast<size_t>(h_t) & 7) { set_error("amplfi_waveform_td: h_t must be 8-byte aligned"); return AMPLFI_ERR_ALIGNMENT; }
@@ -432,7 +434,7 @@ int amplfi_inject_whiten_fir(const amplfi_plan* p, int batch, const float* noise
     if (crop != 0 && crop != 1) { set_error("amplfi_inject_whiten_fir: crop must be 0 or 1"); return AMPLFI_ERR_INVALID_ARG; }
     if (crop && ntaps >= p->n) { set_error("amplfi_inject_whiten_fir: nothing left after cropping"); return AMPLFI_ERR_INVALID_ARG; }
     const bool fused = (h_det == nullptr && params != nullptr);
-    if (fused && approximant != AMPLFI_TAYLORF2 && approximant != AMPLFI_IMRPHENOMD) { set_error("amplfi_inject_whiten_fir: unknown approximant %d", approximant); return AMPLFI_ERR_INVALID_ARG; }
+    if (fused && !known_approximant(approximant)) { set_error("amplfi_inject_whiten_fir: unknown approximant %d", approximant); return AMPLFI_ERR_INVALID_ARG; }
     if (reinterpret_cast<size_t>(h_det) & 7) { set_error("amplfi_inject_whiten_fir: h_det must be 8-byte aligned"); return AMPLFI_ERR_ALIGNMENT; }
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     rc = launch_filter(p, psd, n_psd, f_lo, f_hi, st);

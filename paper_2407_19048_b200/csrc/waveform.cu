@@ -47,6 +47,7 @@ __global__ void __launch_bounds__(64) prepare_kernel(const double* __restrict__ 
 
 int launch_prepare(const amplfi_plan* p, int approximant, int batch, const double* params, double gmst,
                    double f_lo, double f_hi, double amp_mul, int* flags, cudaStream_t st) {
+    if (approximant >= 0) const_cast<amplfi_plan*>(p)->last_approx = approximant;     // selects the evaluation kernel that follows
     prepare_kernel<<<(batch + 31) / 32, 64, 0, st>>>(
         params, batch, approximant, p->t_seg, p->n_bins, f_lo, f_hi, amp_mul, gmst, p->pd_table, p->d_det_ids,
         p->n_det, approximant < 0 ? nullptr : p->coef, p->resp, flags);
@@ -103,7 +104,34 @@ __global__ void __launch_bounds__(256, 4) waveform_kernel(const WfCoef* __restri
     }
 }
 
+// ---- sine-Gaussian family: a closed form per bin, no tables (its own small kernel so that the tuned kernel above is
+// not touched); same outputs and the same "written only near the band" rule for the h0 workspace ----
+template <bool POL>
+__global__ void __launch_bounds__(256) sine_gaussian_kernel(const WfCoef* __restrict__ coef, int n_bins,
+                                                            float2* __restrict__ out_a, float2* __restrict__ out_b) {
+    const int b = blockIdx.y;
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_bins) return;
+    const WfCoef& c = coef[b];
+    const bool in = c.valid && k >= c.k_lo && k <= c.k_hi;
+    if (!POL && !in && (!c.valid || k < c.k_lo - 64 || k > c.k_hi + 64)) return;
+    const float2 h = in ? eval_sine_gaussian(c, k) : make_float2(0.f, 0.f);
+    if (POL) {
+        out_a[(size_t)b * n_bins + k] = make_float2(c.pol_p * h.x, c.pol_p * h.y);
+        out_b[(size_t)b * n_bins + k] = make_float2(c.pol_c * h.y, -c.pol_c * h.x);
+    } else {
+        out_a[(size_t)b * n_bins + k] = h;
+    }
+}
+
 int launch_waveform_pol(const amplfi_plan* p, int batch, float* hp, float* hc, cudaStream_t st) {
+    if (p->last_approx == 2) {
+        dim3 g((p->n_bins + 255) / 256, batch);
+        sine_gaussian_kernel<true><<<g, 256, 0, st>>>(p->coef, p->n_bins, reinterpret_cast<float2*>(hp),
+                                                      reinterpret_cast<float2*>(hc));
+        count_launch();
+        return check_launch("sine_gaussian_kernel<pol>");
+    }
     dim3 grid(WF_SLICES, batch);
     waveform_kernel<true><<<grid, 256, 0, st>>>(p->coef, p->tab_ci, p->tab_lnk, p->n_bins,
                                                 reinterpret_cast<float2*>(hp), reinterpret_cast<float2*>(hc));
@@ -112,6 +140,12 @@ int launch_waveform_pol(const amplfi_plan* p, int batch, float* hp, float* hc, c
 }
 
 int launch_waveform_h0(const amplfi_plan* p, int batch, cudaStream_t st) {
+    if (p->last_approx == 2) {
+        dim3 g((p->n_bins + 255) / 256, batch);
+        sine_gaussian_kernel<false><<<g, 256, 0, st>>>(p->coef, p->n_bins, p->h0, nullptr);
+        count_launch();
+        return check_launch("sine_gaussian_kernel<h0>");
+    }
     dim3 grid(WF_SLICES, batch);
     waveform_kernel<false><<<grid, 256, 0, st>>>(p->coef, p->tab_ci, p->tab_lnk, p->n_bins, p->h0, nullptr);
     count_launch();

@@ -95,8 +95,54 @@ __device__ inline double pd_fit(const double* t, double eta, double xi) {
 
 // p: 11 parameters; t_seg = n/fs; amp_mul multiplies the strain amplitude (1 for the API in strain/Hz).
 // tab: [19][11] fit table in global/constant memory.
+// Sine-Gaussian burst (reading R-W12): row = f0, Q, -, -, A, iota, phi, t0, ra, dec, psi.
+//   h0(f_k) = A tau sqrt(pi)/2 exp(-(pi tau (f_k - f0))^2) exp(-i (2 pi f_k t0 - phi)),  tau = Q / (sqrt2 pi f0)
+// Fields used: lin1 (t0/T, turns per bin), c01 (-phi / 2 pi), amp_scale, g_krd (f0 T), g_invw (pi tau / T), pol_p, pol_c.
+__device__ inline void prepare_sine_gaussian(const double* p, double t_seg, int n_bins, double f_lo, double f_hi,
+                                             double amp_mul, WfCoef& c) {
+    const double PI = AMPLFI_PI;
+    const double f0 = p[0], q = p[1], amp = p[4];
+    bool ok = (f0 > 0.0) && (q > 0.0) && (amp > 0.0);
+    for (int i = 0; i < 11; ++i) ok = ok && isfinite(p[i]);
+    c.valid = ok ? 1 : 0;
+    c.approx = 2;
+    c.k_lo = 1;
+    c.k_hi = 0;
+    if (!ok) return;
+    const double tau = q / (1.4142135623730951 * PI * f0);
+    const double cosi = cos(p[5]);
+    c.pol_p = (float)(0.5 * (1.0 + cosi * cosi));
+    c.pol_c = (float)cosi;
+    long klo = (long)ceil(f_lo * t_seg);
+    while ((double)(klo - 1) / t_seg >= f_lo) --klo;
+    while ((double)klo / t_seg < f_lo) ++klo;
+    long khi = (long)floor(f_hi * t_seg);
+    while ((double)(khi + 1) / t_seg <= f_hi) ++khi;
+    while (khi >= 0 && (double)khi / t_seg > f_hi) --khi;
+    if (klo < 1) klo = 1;
+    if (khi > n_bins - 2) khi = n_bins - 2;
+    c.k_lo = (int)klo;
+    c.k_hi = (int)khi;
+    c.lin1 = p[7] / t_seg;
+    c.c01 = -p[6] / (2.0 * PI);
+    c.amp_scale = (float)(amp_mul * 0.5 * amp * tau * 1.7724538509055159);      // sqrt(pi)
+    c.g_krd = (float)(f0 * t_seg);
+    c.g_invw = (float)(PI * tau / t_seg);
+}
+
+__device__ __forceinline__ float2 eval_sine_gaussian(const WfCoef& c, int k) {
+    double ph = fma(c.lin1, (double)k, c.c01);
+    ph -= rint(ph);
+    float s, co;
+    __sincosf((float)ph * 6.283185307179586f, &s, &co);
+    const float y = ((float)k - c.g_krd) * c.g_invw;
+    const float amp = c.amp_scale * __expf(-y * y);
+    return make_float2(amp * co, -amp * s);
+}
+
 __device__ inline void prepare_sample(const double* p, int approx, double t_seg, int n_bins, double f_lo,
                                       double f_hi, double amp_mul, const double* tab, WfCoef& c) {
+    if (approx == 2) { prepare_sine_gaussian(p, t_seg, n_bins, f_lo, f_hi, amp_mul, c); return; }
     const double PI = AMPLFI_PI, TWO_PI = 2.0 * AMPLFI_PI;
     const double mc = p[0], q = p[1], chi1 = p[2], chi2 = p[3], dist = p[4];
     bool ok = (mc > 0.0) && (q > 0.0) && (q <= 1.0) && (fabs(chi1) < 1.0) && (fabs(chi2) < 1.0) && (dist > 0.0);

@@ -233,3 +233,44 @@ def test_long_segment_gather_views_and_td():
     out_f = A.amplfi_inject_whiten_fir(plan, batch, dev(strip), dev(psd_s), 20.0, 1000.0, 2.0, crop=True, offsets=dev(offsets))
     ref_f = OWH.inject_whiten_fir(noise, None, psd64, fs, 20.0, 1000.0, 2.0, crop=True)
     assert row_err(out_f.cpu().numpy().astype(np.float64), ref_f).max() <= TOL
+
+
+# ------------------------------------------------------------------------------------------ sine-Gaussian family (8(f)-4)
+def _sg_params(n, fs):
+    t_seg = n / fs
+    rows = []
+    for f0, q, amp, iota in [(250.0, 9.0, 1e-21, 0.6), (60.0, 4.0, 5e-22, 0.0), (800.0, 100.0, 2e-21, 1.5707963),
+                             (35.0, 20.0, 1e-20, 2.5), (999.0, 3.0, 1e-21, 1.0), (250.0, -1.0, 1e-21, 0.3)]:
+        rows.append([f0, q, 0.0, 0.0, amp, iota, 1.3, 0.55 * t_seg, 1.0, 0.5, 0.7])
+    return np.array(rows, dtype=np.float64)
+
+
+@pytest.mark.parametrize("n,fs", [(16384, 2048.0), (8192, 2048.0), (65536, 4096.0)])
+def test_sine_gaussian_parity(n, fs):
+    par = _sg_params(n, fs)
+    dets = [0, 1, 2]
+    plan = A.Plan(n, fs, dets, len(par))
+    hp, hc, flags = A.amplfi_waveform_fd(plan, A.SINE_GAUSSIAN, dev(par), 20.0, 1000.0)
+    hp_r, hc_r, fl_r = OW.waveform_fd(OW.SINE_GAUSSIAN, par, n, fs, 20.0, 1000.0)
+    assert np.array_equal(flags.cpu().numpy(), fl_r)
+    from test_gpu_parity import cplx
+    assert row_err(cplx(hp), hp_r).max() <= TOL and row_err(cplx(hc), hc_r).max() <= TOL
+    f = np.arange(n // 2 + 1) * fs / n
+    outside = (f < 20.0) | (f > 1000.0)
+    assert np.all(cplx(hp)[:, outside] == 0) and np.all(cplx(hc)[:, outside] == 0)      # hard band edges (R-W7)
+    assert np.all(cplx(hp)[-1] == 0) and np.all(cplx(hc)[-1] == 0)                      # the invalid row
+    assert cplx(hp)[4][f == 1000.0] != 0                                                # upper edge inclusive (f0 = 999 Hz)
+    # injected and whitened through the fused call, and as a time series
+    rng = np.random.Generator(np.random.Philox(n + 5))
+    noise = WL.coloured_noise(rng, (len(par), 3), n, fs)
+    psd = np.stack([WL.aligo_psd(np.arange(n // 2 + 1) * fs / n)] * 3)
+    psd_s = (psd * PSD_SCALE).astype(np.float32)
+    out = A.amplfi_inject_whiten(plan, len(par), dev(noise), dev(psd_s), 20.0, 1000.0, approximant=A.SINE_GAUSSIAN,
+                                 params=dev(par), gmst=0.7)
+    h_det, _ = OP.project(hp_r, hc_r, par, 0.7, dets, n, fs)
+    ref = OWH.inject_whiten(noise.astype(np.float64), h_det, psd_s.astype(np.float64) / PSD_SCALE, fs, 20.0, 1000.0)
+    assert row_err(out.cpu().numpy().astype(np.float64), ref).max() <= TOL
+    h_t, _ = A.amplfi_waveform_td(plan, A.SINE_GAUSSIAN, dev(par), 20.0, 1000.0)
+    hp_t, hc_t, _ = OW.waveform_td(OW.SINE_GAUSSIAN, par, n, fs, 20.0, 1000.0)
+    got = h_t.cpu().numpy().astype(np.float64)
+    assert row_err(got[:, 0], hp_t).max() <= TOL and row_err(got[:, 1], hc_t).max() <= TOL
