@@ -14,10 +14,11 @@ using namespace v2;
 // VIEWS = 2 (MODE_FUSED only): the two data views d, d' of PAPER.md:93, :117 from ONE forward transform.  The forward
 // spectrum of every virtual thread is parked in the second view's own output row (64 KB, exactly the row size; it stays
 // in L2 until that view's samples overwrite it) and read back for the second pointwise stage + inverse transform.
-template <int MODE, int VT, bool FWD, int VIEWS>
-__global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwArgs a, int units) {
-    constexpr int TT = T13 / VT;
-    constexpr int M = M13, N = N13, K = M13 + 1;
+template <int LOGM, int MODE, int VT, bool FWD, int VIEWS>
+__global__ void __launch_bounds__(Geo<LOGM>::T / VT, LOGM == 13 ? 2 : 4) inject_whiten13_kernel(const IwArgs a, int units) {
+    using G = Geo<LOGM>;
+    constexpr int TT = G::T / VT;
+    constexpr int M = G::M, N = G::N, K = G::M + 1, KL = G::KL;
     extern __shared__ float smem13[];
     float* re = smem13;
     float* im = smem13 + M;
@@ -71,18 +72,21 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
 #pragma unroll
             for (int vt = 0; vt < VT; ++vt)
 #pragma unroll
-                for (int n1 = 0; n1 < 16; ++n1) z[vt][n1] = __ldcs(x2 + n1 * 512 + tt + vt * TT);
+                for (int n1 = 0; n1 < 16; ++n1) z[vt][n1] = __ldcs(x2 + sample_index<LOGM>(n1, tt + vt * TT));
         } else {
 #pragma unroll
             for (int vt = 0; vt < VT; ++vt)
 #pragma unroll
                 for (int n1 = 0; n1 < 16; ++n1) {
-                    const int m = n1 * 512 + tt + vt * TT;
+                    const int m = sample_index<LOGM>(n1, tt + vt * TT);
                     z[vt][n1] = make_float2(__ldg(x + 2 * m), __ldg(x + 2 * m + 1));
                 }
         }
 #pragma unroll
-        for (int vt = 0; vt < VT; ++vt) p1_fwd(z[vt], tt + vt * TT, re, im);
+        for (int vt = 0; vt < VT; ++vt) {
+            if constexpr (LOGM == 13) p1_fwd(z[vt], tt + vt * TT, re, im);
+            else p1_fwd12(z[vt], tt + vt * TT, re, im);
+        }
     }
     __syncthreads();
     if (fwd) {
@@ -99,13 +103,13 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
     if (MODE == MODE_FUSED) {
         const WfCoef* c = a.coef + b;
         hsrc = a.h0 + (size_t)b * K;
-        if (c->valid) { w_lo = c->k_lo; w_hi = c->k_hi; }
+        if (c->valid) { w_lo = c->k_lo; w_hi = c->k_hi; }       // an empty band is stored as (2^30, -1) by prepare_kernel
         const DetResp r = a.resp[unit];
         cre = (float)r.fp * c->pol_p;                       // C = F+ (1+cos^2 i)/2 - i Fx cos i
         cim = -(float)r.fc * c->pol_c;
         delta = r.dt * (double)a.inv_tseg;                   // turns per bin (fp64: the second view's dt reaches 1 s)
     }
-    // Operands of the pointwise stage for virtual thread t: bins k = t + 1024 k4 (half A) and M - k (half B).
+    // Operands of the pointwise stage for virtual thread t: bins k = t + KL k4 (half A) and M - k (half B), KL = 1024 (512).
     // They are requested one phase ahead of their use so that L2 latency is covered by butterfly work.  h0 is zero
     // outside [w_lo, w_hi]: a warp none of whose 32 bins of a half is inside skips the load (warp-uniform test;
     // heavy systems stop at a few hundred Hz).
@@ -114,14 +118,14 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
         const int wbase = t & ~31;
 #pragma unroll
         for (int k4 = 0; k4 < 8; ++k4) {
-            const int k = t + 1024 * k4;
+            const int k = t + KL * k4;
             L.fa[k4] = __ldg(filt + k);
             L.fb[k4] = __ldg(filt + M - k);
             if (MODE == MODE_HDET) {
                 L.ha[k4] = __ldg(hsrc + k);
                 L.hb[k4] = __ldg(hsrc + M - k);
             } else if (MODE == MODE_FUSED) {
-                const int ka_lo = wbase + 1024 * k4, ka_hi = ka_lo + 31;
+                const int ka_lo = wbase + KL * k4, ka_hi = ka_lo + 31;
                 L.ha[k4] = make_float2(0.f, 0.f);
                 L.hb[k4] = make_float2(0.f, 0.f);
                 if (ka_hi >= w_lo && ka_lo <= w_hi) L.ha[k4] = __ldg(hsrc + k);
@@ -189,11 +193,11 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
             float tt_, ts_, tm_;
             if (a.phase64) {                                 // second data view: dt reaches 1 s, reduce in fp64
                 double x = (double)t * delta; tt_ = (float)(x - rint(x));
-                x = 1024.0 * delta; ts_ = (float)(x - rint(x));
+                x = (double)KL * delta; ts_ = (float)(x - rint(x));
                 x = (double)M * delta; tm_ = (float)(x - rint(x));
             } else {                                         // |dt| <= 21 ms: fp32 is exact enough
                 const float df = (float)delta;
-                tt_ = (float)t * df; ts_ = 1024.0f * df; tm_ = (float)M * df;
+                tt_ = (float)t * df; ts_ = (float)KL * df; tm_ = (float)M * df;
             }
             const float2 et = unit_phase(tt_);
             const float2 es = unit_phase(ts_);
@@ -255,7 +259,7 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
                 // t = 1..3: (A[q], A[8-q]), k = 1024 q;  t = 4: A[4] with itself, k = M/2;
                 // t = 5..8: (B[q], B[7-q]), q = t - 5, k = 512 + 1024 q
                 const int ia = t <= 4 ? t : 3 + t, ib = t <= 4 ? 8 - t : 20 - t;
-                const int k = t <= 4 ? 1024 * t : 512 + 1024 * (t - 5);
+                const int k = t <= 4 ? KL * t : KL / 2 + KL * (t - 5);
                 float2 pa = sc[ia], pb = sc[ib];
                 do_pair(k, pa, pb);
                 sc[ia] = pa;
@@ -294,33 +298,34 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
 #pragma unroll
             for (int vt = 0; vt < VT; ++vt) {
                 const int t = tt + vt * TT;
-                const int klow_a = t, klow_b = (t == 0) ? 512 : 1024 - t;
+                const int klow_a = t, klow_b = (t == 0) ? KL / 2 : KL - t;
                 C2 v[8];
                 if (view == 0) {
-                    p4_fwd(klow_a, klow_b, v, re, im);
+                    p4_fwd<LOGM>(klow_a, klow_b, v, re, im);
 #pragma unroll
-                    for (int r = 0; r < 8; ++r) stash[r * T13 + t] = make_ulonglong2(v[r].r, v[r].i);
+                    for (int r = 0; r < 8; ++r) stash[r * G::T + t] = make_ulonglong2(v[r].r, v[r].i);
                 } else {
 #pragma unroll
-                    for (int r = 0; r < 8; ++r) { const ulonglong2 q = stash[r * T13 + t]; v[r] = C2{q.x, q.y}; }
+                    for (int r = 0; r < 8; ++r) { const ulonglong2 q = stash[r * G::T + t]; v[r] = C2{q.x, q.y}; }
                 }
                 pointwise(t, v, ops[vt]);
                 if (vt + 1 < VT) pw_load(t + TT, ops[vt + 1]);
-                p4_inv(klow_a, klow_b, v, re, im);
+                p4_inv<LOGM>(klow_a, klow_b, v, re, im);
             }
             __syncthreads();
 #pragma unroll
             for (int vt = 0; vt < VT; ++vt) p3_inv(tt + vt * TT, re, im);
             __syncthreads();
 #pragma unroll
-            for (int vt = 0; vt < VT; ++vt) p2_inv(tt + vt * TT, re, im);
+            for (int vt = 0; vt < VT; ++vt) p2_inv<LOGM>(tt + vt * TT, re, im);
             __syncthreads();
 #pragma unroll
             for (int vt = 0; vt < VT; ++vt) {
                 float2 z[16];
-                p1_inv(z, tt + vt * TT, re, im);
+                if constexpr (LOGM == 13) p1_inv(z, tt + vt * TT, re, im);
+                else p1_inv12(z, tt + vt * TT, re, im);
 #pragma unroll
-                for (int n1 = 0; n1 < 16; ++n1) __stcs(outv + n1 * 512 + tt + vt * TT, z[n1]);
+                for (int n1 = 0; n1 < 16; ++n1) __stcs(outv + sample_index<LOGM>(n1, tt + vt * TT), z[n1]);
             }
         }
         return;
@@ -328,10 +333,10 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
 #pragma unroll
     for (int vt = 0; vt < VT; ++vt) {
         const int t = tt + vt * TT;
-        const int klow_a = t, klow_b = (t == 0) ? 512 : 1024 - t;
+        const int klow_a = t, klow_b = (t == 0) ? KL / 2 : KL - t;
         C2 v[8];
         if (fwd) {
-            p4_fwd(klow_a, klow_b, v, re, im);
+            p4_fwd<LOGM>(klow_a, klow_b, v, re, im);
         } else {
 #pragma unroll
             for (int r = 0; r < 8; ++r) v[r] = C2{0ull, 0ull};
@@ -339,29 +344,30 @@ __global__ void __launch_bounds__(T13 / VT, 2) inject_whiten13_kernel(const IwAr
         pointwise(t, v, ops[vt]);
         if (vt + 1 < VT) pw_load(t + TT, ops[vt + 1]);      // in flight during this P4' and the next P4
         // ---- a-9 inverse real FFT ----
-        p4_inv(klow_a, klow_b, v, re, im);
+        p4_inv<LOGM>(klow_a, klow_b, v, re, im);
     }
     __syncthreads();
 #pragma unroll
     for (int vt = 0; vt < VT; ++vt) p3_inv(tt + vt * TT, re, im);
     __syncthreads();
 #pragma unroll
-    for (int vt = 0; vt < VT; ++vt) p2_inv(tt + vt * TT, re, im);
+    for (int vt = 0; vt < VT; ++vt) p2_inv<LOGM>(tt + vt * TT, re, im);
     __syncthreads();
     {
         float2* out2 = reinterpret_cast<float2*>(out);
 #pragma unroll
         for (int vt = 0; vt < VT; ++vt) {
             float2 z[16];
-            p1_inv(z, tt + vt * TT, re, im);
+            if constexpr (LOGM == 13) p1_inv(z, tt + vt * TT, re, im);
+            else p1_inv12(z, tt + vt * TT, re, im);
             if (a.crop == 0) {
 #pragma unroll
-                for (int n1 = 0; n1 < 16; ++n1) __stcs(out2 + n1 * 512 + tt + vt * TT, z[n1]);
+                for (int n1 = 0; n1 < 16; ++n1) __stcs(out2 + sample_index<LOGM>(n1, tt + vt * TT), z[n1]);
             } else {
                 const int c2 = a.crop >> 1;                  // crop is even: whole float2 pairs
 #pragma unroll
                 for (int n1 = 0; n1 < 16; ++n1) {
-                    const int m = n1 * 512 + tt + vt * TT;
+                    const int m = sample_index<LOGM>(n1, tt + vt * TT);
                     if (m >= c2 && m < M - c2) __stcs(out2 + m - c2, z[n1]);
                 }
             }
@@ -389,10 +395,13 @@ __global__ void init_tw13_kernel() {
         put(g_tw13.p3[k >> 1][n4], k, w(n4 * k, 64));
         const int c = i >> 3, m4 = i & 7;                      // p4i: combination c, time digit m4
         const int k3a = c >> 1;
-        const int t = (c & 1) ? 128 * k3a + 1 : 128 * k3a;     // a representative thread of the combination
-        const int klow_b = (t == 0) ? 512 : 1024 - t;
-        const float2 A = w(m4 * k3a, 64), B = w(m4 * (klow_b >> 7), 64);
-        g_tw13.p4i[c][m4] = make_ulonglong2(pack(A.x, B.x), pack(A.y, B.y));
+        for (int lg = 0; lg < 2; ++lg) {                       // LOGM = 12 + lg: klow >> s3 = k3, klow spans kl
+            const int s3 = 6 + lg, kl = 512 << lg;
+            const int t = (k3a << s3) + (c & 1);               // a representative thread of the combination
+            const int klow_b = (t == 0) ? kl / 2 : kl - t;
+            const float2 A = w(m4 * k3a, 64), B = w(m4 * (klow_b >> s3), 64);
+            g_tw13.p4i[lg][c][m4] = make_ulonglong2(pack(A.x, B.x), pack(A.y, B.y));
+        }
     }
 }
 
@@ -405,39 +414,45 @@ int init_iw13_tables(cudaStream_t st) {
 #ifndef IW13_VT
 #define IW13_VT 2
 #endif
-template <int MODE, bool FWD, int VIEWS = 1>
+template <int LOGM, int MODE, bool FWD, int VIEWS = 1>
 static int launch_iw13_t(const IwArgs& a, int units, cudaStream_t st) {
     static bool attr_done = false;
-    const int smem = 2 * M13 * (int)sizeof(float);
+    constexpr int T13 = Geo<LOGM>::T;
+    const int smem = 2 * Geo<LOGM>::M * (int)sizeof(float);
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(inject_whiten13_kernel<MODE, IW13_VT, FWD, VIEWS>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        cudaError_t e = cudaFuncSetAttribute(inject_whiten13_kernel<LOGM, MODE, IW13_VT, FWD, VIEWS>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) { set_error("cudaFuncSetAttribute: %s", cudaGetErrorString(e)); return AMPLFI_ERR_CUDA; }
         attr_done = true;
     }
-    inject_whiten13_kernel<MODE, IW13_VT, FWD, VIEWS><<<units, T13 / IW13_VT, smem, st>>>(a, units);
+    inject_whiten13_kernel<LOGM, MODE, IW13_VT, FWD, VIEWS><<<units, T13 / IW13_VT, smem, st>>>(a, units);
     count_launch();
     return check_launch("inject_whiten13_kernel");
 }
 
-int launch_iw13(const IwArgs& a, int mode, int units, cudaStream_t st) {
+template <int LOGM>
+static int launch_iw13_l(const IwArgs& a, int mode, int units, cudaStream_t st) {
     if (a.out2 != nullptr) {        // two data views from one forward transform
         if (mode != MODE_FUSED || a.noise == nullptr || a.t_shift == nullptr || a.crop != 0) {
             set_error("inject_whiten13: the two-view launch needs the fused mode");
             return AMPLFI_ERR_INVALID_ARG;
         }
-        return launch_iw13_t<MODE_FUSED, true, 2>(a, units, st);
+        return launch_iw13_t<LOGM, MODE_FUSED, true, 2>(a, units, st);
     }
     if (a.noise == nullptr) {       // inverse-only launches (time-domain waveform, filter design)
-        if (mode == MODE_HDET) return launch_iw13_t<MODE_HDET, false>(a, units, st);
-        if (mode == MODE_FUSED) return launch_iw13_t<MODE_FUSED, false>(a, units, st);
+        if (mode == MODE_HDET) return launch_iw13_t<LOGM, MODE_HDET, false>(a, units, st);
+        if (mode == MODE_FUSED) return launch_iw13_t<LOGM, MODE_FUSED, false>(a, units, st);
         set_error("inject_whiten13: no data and nothing to inject");
         return AMPLFI_ERR_INVALID_ARG;
     }
     switch (mode) {
-        case MODE_NONE: return launch_iw13_t<MODE_NONE, true>(a, units, st);
-        case MODE_HDET: return launch_iw13_t<MODE_HDET, true>(a, units, st);
-        default: return launch_iw13_t<MODE_FUSED, true>(a, units, st);
+        case MODE_NONE: return launch_iw13_t<LOGM, MODE_NONE, true>(a, units, st);
+        case MODE_HDET: return launch_iw13_t<LOGM, MODE_HDET, true>(a, units, st);
+        default: return launch_iw13_t<LOGM, MODE_FUSED, true>(a, units, st);
     }
+}
+
+int launch_iw13(const IwArgs& a, int logm, int mode, int units, cudaStream_t st) {
+    return logm == 13 ? launch_iw13_l<13>(a, mode, units, st) : launch_iw13_l<12>(a, mode, units, st);
 }
 
 }  // namespace amplfi

@@ -26,6 +26,25 @@ using namespace pk;
 
 constexpr int M13 = 8192, N13 = 16384, T13 = 512;
 
+// Geometry of the two supported lengths.  LOGM = 13: M = 8192 = 16*8*8*8 (N = 16384, the index algebra above).
+// LOGM = 12: M = 4096 = 8*8*8*8 (N = 8192, the paper's own 4 s at 2048 Hz): pass 1 is a radix 8 and every
+// virtual thread takes two of its butterflies (j1 = t and t + 256); passes 2-4 are unchanged with kap < 4.
+template <int LOGM>
+struct Geo {
+    static constexpr int M = 1 << LOGM, N = 2 * M;
+    static constexpr int R1 = M / 512;                 // radix of pass 1: 16 or 8
+    static constexpr int LR1 = LOGM - 9;               // log2 R1
+    static constexpr int T = M / 16;                   // virtual threads: 512 or 256
+    static constexpr int KL = 64 * R1;                 // span of klow = k1 + R1 k2 + 8 R1 k3: 1024 or 512
+    static constexpr int S3 = LR1 + 3;                 // klow >> S3 = k3
+};
+// complex index (in float2 units) of the i-th of the 16 samples of virtual thread t
+template <int LOGM>
+__device__ __forceinline__ int sample_index(int i, int t) {
+    if constexpr (LOGM == 13) return i * 512 + t;
+    else return (i & 7) * 512 + t + 256 * (i >> 3);
+}
+
 __device__ __forceinline__ int slot13(int kap, int d2, int d3, int d4) {
     return (kap << 9) | (d2 << 6) | ((d3 >> 1) << 4) | (((d4 ^ kap) & 7) << 1) | ((d3 ^ d2) & 1);
 }
@@ -48,7 +67,7 @@ struct Tw13 {
     float4 p2[4][64];
     float4 p3[4][8];
     float4 p3i[4][64];
-    ulonglong2 p4i[8][8];
+    ulonglong2 p4i[2][8][8];      // [LOGM - 12]
 };
 static __device__ Tw13 g_tw13;       // this header is included by inject_whiten13.cu only
 
@@ -63,6 +82,56 @@ __device__ __forceinline__ void tw_load8(const float4* col, int stride, float2 (
 
 // ---- forward passes ----
 // x[n1] = z[n1*512 + t] (natural complex, from global).  Leaves the spectrum digits (k1; n2 n3 n4) in smem.
+// dif4 / dit4: the last two stages of dif8 / the first two of dit8, on four packed elements
+__device__ __forceinline__ void dif4(C2 (&v)[4]) {
+    C2 d;
+    d = csub(v[0], v[2]); v[0] = cadd(v[0], v[2]); v[2] = d;
+    d = csub(v[1], v[3]); v[1] = cadd(v[1], v[3]); v[3] = mul_w8<2, false>(d);
+    d = csub(v[0], v[1]); v[0] = cadd(v[0], v[1]); v[1] = d;
+    d = csub(v[2], v[3]); v[2] = cadd(v[2], v[3]); v[3] = d;
+}
+__device__ __forceinline__ void dit4(C2 (&v)[4]) {
+    C2 b;
+    b = v[1]; v[1] = csub(v[0], b); v[0] = cadd(v[0], b);
+    b = v[3]; v[3] = csub(v[2], b); v[2] = cadd(v[2], b);
+    b = v[2]; v[2] = csub(v[0], b); v[0] = cadd(v[0], b);
+    b = mul_w8<2, true>(v[3]); v[3] = csub(v[1], b); v[1] = cadd(v[1], b);
+}
+
+// M = 4096: x[h*8 + n1] = z[n1*512 + j1], j1 = t + 256 h.  Per butterfly: scalar radix-2 stage over the top bit of n1, then one
+// packed radix 4 over the even-k1 / odd-k1 halves (k1 = 2 kap, 2 kap + 1, kap < 4); twiddle w_M^(j1 k1).
+__device__ __forceinline__ void p1_fwd12(const float2 (&x)[16], int t, float* re, float* im) {
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        const int j1 = t + 256 * h;
+        C2 v[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const float2 s = amplfi::cadd(x[h * 8 + i], x[h * 8 + i + 4]);
+            float2 d = amplfi::csub(x[h * 8 + i], x[h * 8 + i + 4]);
+            switch (i) {      // d *= w8^i
+                case 0: break;
+                case 1: d = mul_w32<4, false>(d); break;
+                case 2: d = mul_w32<8, false>(d); break;
+                default: d = mul_w32<12, false>(d); break;
+            }
+            v[i] = C2{pack(s.x, d.x), pack(s.y, d.y)};
+        }
+        dif4(v);
+        const float2 u = twiddle<4096>(j1);
+        const float2 u2 = twiddle<4096>(2 * j1);
+        const C2 base = C2{pack(1.0f, u.x), pack(0.0f, u.y)}, step = C2{bcast(u2.x), bcast(u2.y)};
+        const C2 s2 = cmul(step, step);
+        const C2 tw[4] = {base, cmul(base, step), cmul(base, s2), cmul(cmul(base, step), s2)};
+        const int n2 = j1 >> 6, n3 = (j1 >> 3) & 7, n4 = j1 & 7;
+#pragma unroll
+        for (int r = 0; r < 4; ++r) {
+            const int kap = brev<4>(r);
+            sts2(re, im, slot13(kap, n2, n3, n4), cmul(v[r], tw[kap]));
+        }
+    }
+}
+
 __device__ __forceinline__ void p1_fwd(const float2 (&x)[16], int t, float* re, float* im) {
     C2 v[8];
 #pragma unroll
@@ -127,18 +196,20 @@ __device__ __forceinline__ void p3_fwd(int t, float* re, float* im) {
 
 struct P4Addr { int fa, fb, xa, xb; };     // float offsets of halves A, B at d4 = 0 and their kap (xor masks)
 
+template <int LOGM>
 __device__ __forceinline__ void p4_addr(int klow, int& base, int& kap) {
-    const int k1 = klow & 15, k2 = (klow >> 4) & 7, k3 = klow >> 7;
+    const int k1 = klow & (Geo<LOGM>::R1 - 1), k2 = (klow >> Geo<LOGM>::LR1) & 7, k3 = klow >> Geo<LOGM>::S3;
     kap = k1 >> 1;
     base = (k1 & 1) + 2 * ((kap << 9) | (k2 << 6) | ((k3 >> 1) << 4) | ((k3 ^ k2) & 1));
 }
 // element d4 of the butterfly at (base, kap): float index base + 2*(((d4 ^ kap) & 7) << 1)
 __device__ __forceinline__ int p4_off(int base, int kap, int d4) { return base + (((d4 ^ kap) & 7) << 2); }
 
+template <int LOGM>
 __device__ __forceinline__ void p4_fwd(int klow_a, int klow_b, C2 (&v)[8], const float* re, const float* im) {
     int ba, ka, bb, kb;
-    p4_addr(klow_a, ba, ka);
-    p4_addr(klow_b, bb, kb);
+    p4_addr<LOGM>(klow_a, ba, ka);
+    p4_addr<LOGM>(klow_b, bb, kb);
 #pragma unroll
     for (int n4 = 0; n4 < 8; ++n4) {
         const int oa = p4_off(ba, ka, n4), ob = p4_off(bb, kb, n4);
@@ -148,13 +219,15 @@ __device__ __forceinline__ void p4_fwd(int klow_a, int klow_b, C2 (&v)[8], const
 }
 
 // ---- inverse passes ----
+template <int LOGM>
 __device__ __forceinline__ void p4_inv(int klow_a, int klow_b, C2 (&v)[8], float* re, float* im) {
     dit8(v);
     int ba, ka, bb, kb;
-    p4_addr(klow_a, ba, ka);
-    p4_addr(klow_b, bb, kb);
+    p4_addr<LOGM>(klow_a, ba, ka);
+    p4_addr<LOGM>(klow_b, bb, kb);
     // conj twiddle of P3: w_64^(-n4 k3) per half, from the table row of this thread's (k3a, k3b) combination
-    const ulonglong2* trow = g_tw13.p4i[2 * (klow_a >> 7) + ((klow_a & 127) != 0 ? 1 : 0)];
+    constexpr int S3 = Geo<LOGM>::S3;
+    const ulonglong2* trow = g_tw13.p4i[LOGM - 12][2 * (klow_a >> S3) + ((klow_a & ((1 << S3) - 1)) != 0 ? 1 : 0)];
 #pragma unroll
     for (int n4 = 0; n4 < 8; ++n4) {
         C2 y = v[0];
@@ -184,7 +257,9 @@ __device__ __forceinline__ void p3_inv(int t, float* re, float* im) {
     for (int n3 = 0; n3 < 8; ++n3) sts2(re, im, slot13(kap, k2, n3, n4), cmul_conj_s(v[n3], g[n3]));
 }
 
+template <int LOGM>
 __device__ __forceinline__ void p2_inv(int t, float* re, float* im) {
+    constexpr int M = Geo<LOGM>::M;
     const int kap = t >> 6, n3 = (t >> 3) & 7, n4 = t & 7;
     C2 v[8];
 #pragma unroll
@@ -192,12 +267,39 @@ __device__ __forceinline__ void p2_inv(int t, float* re, float* im) {
     dit8(v);
     // conj twiddle of P1: w_M^(-(n2*64 + j0) k1), j0 = n3*8 + n4, k1 = 2kap (A), 2kap+1 (B)
     const int j0 = n3 * 8 + n4;
-    const float2 ca = twiddle<M13>(j0 * 2 * kap), cb = twiddle<M13>(j0 * (2 * kap + 1));
-    const float2 sa = twiddle<64>(kap), sb = twiddle<128>(2 * kap + 1);
+    const float2 ca = twiddle<M>(j0 * 2 * kap), cb = twiddle<M>(j0 * (2 * kap + 1));
+    const float2 sa = twiddle<M / 128>(kap), sb = twiddle<M / 64>(2 * kap + 1);
     C2 tw[8];
     powers8(C2{pack(ca.x, cb.x), pack(ca.y, cb.y)}, C2{pack(sa.x, sb.x), pack(sa.y, sb.y)}, tw);
 #pragma unroll
     for (int n2 = 0; n2 < 8; ++n2) sts2(re, im, slot13(kap, n2, n3, n4), cmul_conj(v[n2], tw[n2]));
+}
+
+// M = 4096: x[h*8 + n1] = unnormalised inverse at n = n1*512 + t + 256 h
+__device__ __forceinline__ void p1_inv12(float2 (&x)[16], int t, const float* re, const float* im) {
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        const int j1 = t + 256 * h;
+        const int n2 = j1 >> 6, n3 = (j1 >> 3) & 7, n4 = j1 & 7;
+        C2 v[4];
+#pragma unroll
+        for (int r = 0; r < 4; ++r) v[r] = lds2(re, im, slot13(brev<4>(r), n2, n3, n4));
+        dit4(v);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            float2 s, d;
+            unpack(v[i].r, s.x, d.x);
+            unpack(v[i].i, s.y, d.y);
+            switch (i) {      // d *= conj(w8^i)
+                case 0: break;
+                case 1: d = mul_w32<4, true>(d); break;
+                case 2: d = mul_w32<8, true>(d); break;
+                default: d = mul_w32<12, true>(d); break;
+            }
+            x[h * 8 + i] = amplfi::cadd(s, d);
+            x[h * 8 + i + 4] = amplfi::csub(s, d);
+        }
+    }
 }
 
 // x[n1] = unnormalised inverse at n = n1*512 + t

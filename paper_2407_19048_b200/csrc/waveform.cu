@@ -36,6 +36,8 @@ __global__ void __launch_bounds__(64) prepare_kernel(const double* __restrict__ 
         if (coef != nullptr) {
             WfCoef c;
             prepare_sample(p, approx, t_seg, n_bins, f_lo, f_hi, amp_mul, pd_table, c);
+            // canonical empty band: no 32-bin window of the fused kernel's operand loads may overlap it
+            if (c.k_lo > c.k_hi) { c.k_lo = 0x40000000; c.k_hi = -1; }
             coef[b] = c;
             if (flags != nullptr) flags[b] = c.valid ? 0 : 1;
         }
