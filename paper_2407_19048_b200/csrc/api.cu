@@ -194,7 +194,7 @@ int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_
         if (e != cudaSuccess) { set_error("amplfi_plan_create: stream/event: %s", cudaGetErrorString(e)); rc = AMPLFI_ERR_CUDA; }
     }
     if (!rc) rc = launch_tables(p, nullptr);
-    if (!rc && (p->logm == 13 || p->logm == 12)) rc = init_iw13_tables(nullptr);
+    if (!rc && p->logm >= 11 && p->logm <= 13) rc = init_iw13_tables(nullptr);
     if (!rc) {
         fill_kernel<<<(p->filt_stride + 255) / 256, 256>>>(p->filt_flat, p->filt_stride, (float)(1.0 / (2.0 * (double)n)));
         count_launch();
@@ -390,7 +390,7 @@ int amplfi_inject_whiten_views(const amplfi_plan* p, int batch, const float* noi
     IwOpts o;
     o.n_det = p->n_det; o.resp = nullptr; o.filt = nullptr; o.filt_stride = 0; o.crop = 0; o.phase64 = 1;
     o.out2 = nullptr; o.t_shift = nullptr;
-    if (!rc && (p->logm == 13 || p->logm == 12) && (reinterpret_cast<size_t>(out2) & 15) == 0) {
+    if (!rc && p->logm >= 11 && p->logm <= 13 && (reinterpret_cast<size_t>(out2) & 15) == 0) {
         // n = 16384: one launch, one forward transform for both views (inject_whiten13.cu, VIEWS = 2)
         o.out2 = out2; o.t_shift = t_shift;
         return launch_inject_whiten(p, batch, noise, offsets, strip_len, nullptr, 1, out, st, &o);

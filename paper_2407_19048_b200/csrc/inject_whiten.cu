@@ -297,14 +297,14 @@ int launch_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
         if (opts->resp != nullptr) a.resp = opts->resp;
         if (opts->filt != nullptr) { a.filt = opts->filt; a.filt_stride = opts->filt_stride; }
         a.crop = opts->crop; a.phase64 = opts->phase64;
-        if (p->logm == 13 || p->logm == 12) { a.out2 = opts->out2; a.t_shift = opts->t_shift; }
+        if (p->logm >= 11 && p->logm <= 13) { a.out2 = opts->out2; a.t_shift = opts->t_shift; }
     }
     const int mode = h_det != nullptr ? MODE_HDET : (fused ? MODE_FUSED : MODE_NONE);
     const int units = batch * a.n_det;
     switch (p->logm) {
         case 9: return launch_iw_mode<9>(a, mode, units, st);
         case 10: return launch_iw_mode<10>(a, mode, units, st);
-        case 11: return launch_iw_mode<11>(a, mode, units, st);
+        case 11: return launch_iw13(a, 11, mode, units, st);
         case 12: return launch_iw13(a, 12, mode, units, st);
         case 13: return launch_iw13(a, 13, mode, units, st);
         case 14: return launch_iw_mode<14>(a, mode, units, st);

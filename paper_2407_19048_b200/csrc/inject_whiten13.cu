@@ -15,7 +15,7 @@ using namespace v2;
 // spectrum of every virtual thread is parked in the second view's own output row (64 KB, exactly the row size; it stays
 // in L2 until that view's samples overwrite it) and read back for the second pointwise stage + inverse transform.
 template <int LOGM, int MODE, int VT, bool FWD, int VIEWS>
-__global__ void __launch_bounds__(Geo<LOGM>::T / VT, LOGM == 13 ? 2 : 4) inject_whiten13_kernel(const IwArgs a, int units) {
+__global__ void __launch_bounds__(Geo<LOGM>::T / VT, LOGM == 13 ? 2 : (LOGM == 12 ? 4 : 8)) inject_whiten13_kernel(const IwArgs a, int units) {
     using G = Geo<LOGM>;
     constexpr int TT = G::T / VT;
     constexpr int M = G::M, N = G::N, K = G::M + 1, KL = G::KL;
@@ -85,7 +85,8 @@ __global__ void __launch_bounds__(Geo<LOGM>::T / VT, LOGM == 13 ? 2 : 4) inject_
 #pragma unroll
         for (int vt = 0; vt < VT; ++vt) {
             if constexpr (LOGM == 13) p1_fwd(z[vt], tt + vt * TT, re, im);
-            else p1_fwd12(z[vt], tt + vt * TT, re, im);
+            else if constexpr (LOGM == 12) p1_fwd12(z[vt], tt + vt * TT, re, im);
+            else p1_fwd11(z[vt], tt + vt * TT, re, im);
         }
     }
     __syncthreads();
@@ -323,7 +324,8 @@ __global__ void __launch_bounds__(Geo<LOGM>::T / VT, LOGM == 13 ? 2 : 4) inject_
             for (int vt = 0; vt < VT; ++vt) {
                 float2 z[16];
                 if constexpr (LOGM == 13) p1_inv(z, tt + vt * TT, re, im);
-                else p1_inv12(z, tt + vt * TT, re, im);
+                else if constexpr (LOGM == 12) p1_inv12(z, tt + vt * TT, re, im);
+                else p1_inv11(z, tt + vt * TT, re, im);
 #pragma unroll
                 for (int n1 = 0; n1 < 16; ++n1) __stcs(outv + sample_index<LOGM>(n1, tt + vt * TT), z[n1]);
             }
@@ -359,7 +361,8 @@ __global__ void __launch_bounds__(Geo<LOGM>::T / VT, LOGM == 13 ? 2 : 4) inject_
         for (int vt = 0; vt < VT; ++vt) {
             float2 z[16];
             if constexpr (LOGM == 13) p1_inv(z, tt + vt * TT, re, im);
-            else p1_inv12(z, tt + vt * TT, re, im);
+            else if constexpr (LOGM == 12) p1_inv12(z, tt + vt * TT, re, im);
+            else p1_inv11(z, tt + vt * TT, re, im);
             if (a.crop == 0) {
 #pragma unroll
                 for (int n1 = 0; n1 < 16; ++n1) __stcs(out2 + sample_index<LOGM>(n1, tt + vt * TT), z[n1]);
@@ -395,8 +398,8 @@ __global__ void init_tw13_kernel() {
         put(g_tw13.p3[k >> 1][n4], k, w(n4 * k, 64));
         const int c = i >> 3, m4 = i & 7;                      // p4i: combination c, time digit m4
         const int k3a = c >> 1;
-        for (int lg = 0; lg < 2; ++lg) {                       // LOGM = 12 + lg: klow >> s3 = k3, klow spans kl
-            const int s3 = 6 + lg, kl = 512 << lg;
+        for (int lg = 0; lg < 3; ++lg) {                       // LOGM = 11 + lg: klow >> s3 = k3, klow spans kl
+            const int s3 = 5 + lg, kl = 256 << lg;
             const int t = (k3a << s3) + (c & 1);               // a representative thread of the combination
             const int klow_b = (t == 0) ? kl / 2 : kl - t;
             const float2 A = w(m4 * k3a, 64), B = w(m4 * (klow_b >> s3), 64);
@@ -452,7 +455,9 @@ static int launch_iw13_l(const IwArgs& a, int mode, int units, cudaStream_t st) 
 }
 
 int launch_iw13(const IwArgs& a, int logm, int mode, int units, cudaStream_t st) {
-    return logm == 13 ? launch_iw13_l<13>(a, mode, units, st) : launch_iw13_l<12>(a, mode, units, st);
+    if (logm == 13) return launch_iw13_l<13>(a, mode, units, st);
+    if (logm == 12) return launch_iw13_l<12>(a, mode, units, st);
+    return launch_iw13_l<11>(a, mode, units, st);
 }
 
 }  // namespace amplfi

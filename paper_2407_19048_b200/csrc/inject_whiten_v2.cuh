@@ -29,6 +29,7 @@ constexpr int M13 = 8192, N13 = 16384, T13 = 512;
 // Geometry of the two supported lengths.  LOGM = 13: M = 8192 = 16*8*8*8 (N = 16384, the index algebra above).
 // LOGM = 12: M = 4096 = 8*8*8*8 (N = 8192, the paper's own 4 s at 2048 Hz): pass 1 is a radix 8 and every
 // virtual thread takes two of its butterflies (j1 = t and t + 256); passes 2-4 are unchanged with kap < 4.
+// LOGM = 11: M = 2048 = 4*8*8*8 (N = 4096): pass 1 is a radix 4, four butterflies per virtual thread (j1 = t + 128 h), kap < 2.
 template <int LOGM>
 struct Geo {
     static constexpr int M = 1 << LOGM, N = 2 * M;
@@ -42,7 +43,7 @@ struct Geo {
 template <int LOGM>
 __device__ __forceinline__ int sample_index(int i, int t) {
     if constexpr (LOGM == 13) return i * 512 + t;
-    else return (i & 7) * 512 + t + 256 * (i >> 3);
+    else return (i & (Geo<LOGM>::R1 - 1)) * 512 + t + Geo<LOGM>::T * (i >> Geo<LOGM>::LR1);
 }
 
 __device__ __forceinline__ int slot13(int kap, int d2, int d3, int d4) {
@@ -67,7 +68,7 @@ struct Tw13 {
     float4 p2[4][64];
     float4 p3[4][8];
     float4 p3i[4][64];
-    ulonglong2 p4i[2][8][8];      // [LOGM - 12]
+    ulonglong2 p4i[3][8][8];      // [LOGM - 11]
 };
 static __device__ Tw13 g_tw13;       // this header is included by inject_whiten13.cu only
 
@@ -129,6 +130,39 @@ __device__ __forceinline__ void p1_fwd12(const float2 (&x)[16], int t, float* re
             const int kap = brev<4>(r);
             sts2(re, im, slot13(kap, n2, n3, n4), cmul(v[r], tw[kap]));
         }
+    }
+}
+
+// M = 2048: x[h*4 + n1] = z[n1*512 + j1], j1 = t + 128 h, h < 4.  Radix 4 = scalar radix-2 stage + packed radix 2.
+__device__ __forceinline__ void p1_fwd11(const float2 (&x)[16], int t, float* re, float* im) {
+#pragma unroll
+    for (int h = 0; h < 4; ++h) {
+        const int j1 = t + 128 * h;
+        const float2 s0 = amplfi::cadd(x[h * 4], x[h * 4 + 2]), d0 = amplfi::csub(x[h * 4], x[h * 4 + 2]);
+        const float2 s1 = amplfi::cadd(x[h * 4 + 1], x[h * 4 + 3]);
+        const float2 d1 = mul_w32<8, false>(amplfi::csub(x[h * 4 + 1], x[h * 4 + 3]));       // * w4^1 = -i
+        const C2 v0 = C2{pack(s0.x, d0.x), pack(s0.y, d0.y)}, v1 = C2{pack(s1.x, d1.x), pack(s1.y, d1.y)};
+        const float2 u = twiddle<2048>(j1);
+        const float2 u2 = twiddle<2048>(2 * j1);
+        const C2 base = C2{pack(1.0f, u.x), pack(0.0f, u.y)}, step = C2{bcast(u2.x), bcast(u2.y)};
+        const int n2 = j1 >> 6, n3 = (j1 >> 3) & 7, n4 = j1 & 7;
+        sts2(re, im, slot13(0, n2, n3, n4), cmul(cadd(v0, v1), base));
+        sts2(re, im, slot13(1, n2, n3, n4), cmul(csub(v0, v1), cmul(base, step)));
+    }
+}
+__device__ __forceinline__ void p1_inv11(float2 (&x)[16], int t, const float* re, const float* im) {
+#pragma unroll
+    for (int h = 0; h < 4; ++h) {
+        const int j1 = t + 128 * h;
+        const int n2 = j1 >> 6, n3 = (j1 >> 3) & 7, n4 = j1 & 7;
+        const C2 a = lds2(re, im, slot13(0, n2, n3, n4)), b = lds2(re, im, slot13(1, n2, n3, n4));
+        const C2 v0 = cadd(a, b), v1 = csub(a, b);
+        float2 s0, d0, s1, d1;
+        unpack(v0.r, s0.x, d0.x); unpack(v0.i, s0.y, d0.y);
+        unpack(v1.r, s1.x, d1.x); unpack(v1.i, s1.y, d1.y);
+        d1 = mul_w32<8, true>(d1);                                                           // * conj(w4^1) = +i
+        x[h * 4] = amplfi::cadd(s0, d0); x[h * 4 + 2] = amplfi::csub(s0, d0);
+        x[h * 4 + 1] = amplfi::cadd(s1, d1); x[h * 4 + 3] = amplfi::csub(s1, d1);
     }
 }
 
@@ -227,7 +261,7 @@ __device__ __forceinline__ void p4_inv(int klow_a, int klow_b, C2 (&v)[8], float
     p4_addr<LOGM>(klow_b, bb, kb);
     // conj twiddle of P3: w_64^(-n4 k3) per half, from the table row of this thread's (k3a, k3b) combination
     constexpr int S3 = Geo<LOGM>::S3;
-    const ulonglong2* trow = g_tw13.p4i[LOGM - 12][2 * (klow_a >> S3) + ((klow_a & ((1 << S3) - 1)) != 0 ? 1 : 0)];
+    const ulonglong2* trow = g_tw13.p4i[LOGM - 11][2 * (klow_a >> S3) + ((klow_a & ((1 << S3) - 1)) != 0 ? 1 : 0)];
 #pragma unroll
     for (int n4 = 0; n4 < 8; ++n4) {
         C2 y = v[0];

@@ -251,9 +251,10 @@ def test_c1_parity(mode):
     assert row_err(got, ref2).max() <= TOL
 
 
-def test_c2_gather_parity_unaligned_offsets():
+@pytest.mark.parametrize("n", [16384, 8192, 4096])
+def test_c2_gather_parity_unaligned_offsets(n):
     # configs[2] shape at reduced batch / strip; arbitrary (odd) offsets exercise the unaligned path
-    wl = WL.make_c2(batch=16, strip_len=1 << 20)
+    wl = WL.make_c2(batch=16, strip_len=1 << 20, n=n)
     wl.offsets[0, 0] = 0
     wl.offsets[1, 1] = wl.strip.shape[1] - wl.n            # last valid offset
     wl.offsets[2, 2] |= 1
@@ -341,9 +342,10 @@ def test_other_segment_lengths(n, fs):
     assert row_err(got, ref).max() <= TOL
 
 
-def test_full_band_including_dc_and_nyquist():
-    # f_lo = 0, f_hi = fs/2: the DC and Nyquist bins take the special path of the packed real FFT
-    n, fs = 2048, 2048.0
+@pytest.mark.parametrize("n", [2048, 4096, 8192, 16384, 32768, 65536, 131072])
+def test_full_band_including_dc_and_nyquist(n):
+    # f_lo = 0, f_hi = fs/2: the DC and Nyquist bins take the special path of the packed real FFT (every kernel family)
+    fs = 2048.0
     rng = np.random.Generator(np.random.Philox(5))
     noise = rng.standard_normal((2, 1, n)).astype(np.float32) * np.float32(1e-21) + np.float32(2e-22)
     k = n // 2 + 1
