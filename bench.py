@@ -285,19 +285,21 @@ def run_b200(args):
     if k_ms:
         ach = alg_bytes / (k_ms * 1e-3) / 1e9
         # secondary ceiling: fp32 lane-operations on the FMA pipe, 128 lanes/clk/SM (measured with
-        # FADD2/FFMA2 microbenchmarks), counted from the kernel's SASS: 2140 per 16 complex points = 66.9 per sample
+        # FADD2/FFMA2 microbenchmarks); executed fp32 instructions of the kernel from the ncu source page
+        # (profiles/r01_ncu_inject_whiten_v4.md): 69.2 M packed (2 lanes each) + 43.3 M scalar warp-instructions per launch
+        # = 57.8 lane-operations per output sample
         sm_clk = (clocks or {}).get("sm_mhz") or 1965.0
         try:
             alu_peak, alu_src = A.probe_fp32_pipe() / 1e12, "measured in this run (amplfi_probe_fp32_pipe: packed FMA loop)"
         except Exception:
             alu_peak, alu_src = 148 * 128 * sm_clk * 1e6 / 1e12, "nominal 148 SMs x 128 lanes x SM clock"
-        alu_ach = 66.9 * B * D * N / (k_ms * 1e-3) / 1e12
+        alu_ach = 57.8 * B * D * N / (k_ms * 1e-3) / 1e12
         roofline = {"bound": "hbm", "kernel": "inject_whiten13_kernel<fused, VT=2>", "achieved": ach, "peak": peak,
                     "unit": "GB/s", "frac": ach / peak, "frac_of_nominal_8TBps": ach / 8000.0, "peak_source": peak_src,
                     "traffic": traffic, "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": k_ms,
                     "kernel_share_of_step": k_ms / ms_per_step, "launches_timed": len(kernel_ms),
                     "alu": {"bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "T fp32 lane-op/s",
-                            "frac": alu_ach / alu_peak, "lane_ops_per_sample": 66.9, "sm_mhz": sm_clk, "peak_source": alu_src}}
+                            "frac": alu_ach / alu_peak, "lane_ops_per_sample": 57.8, "sm_mhz": sm_clk, "peak_source": alu_src}}
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
