@@ -274,7 +274,7 @@ def run_b200(args):
     k_ms = float(np.mean(kernel_ms)) if kernel_ms else None
     alg_bytes = 8.0 * B * D * N
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    tpath = os.path.join(ROOT, "profiles", "ncu_traffic.txt")
     if os.path.exists(tpath):
         try:
             with open(tpath) as fh:
