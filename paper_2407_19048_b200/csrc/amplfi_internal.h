@@ -2,6 +2,8 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <atomic>
+
 #include "../../include/amplfi.h"
 #include "phenomd_table.h"
 
@@ -21,7 +23,7 @@ struct amplfi_plan {
     int det_ids[3];
     int max_batch;
     int nperseg;           // 0: no Welch
-    int last_approx;       // approximant of the last launch_prepare (the waveform launch that follows evaluates that family)
+    mutable int last_approx;       // approximant of the last launch_prepare (the waveform launch that follows evaluates that family)
     int device;
     int sm_count;
     // device tables / workspace (owned)
@@ -47,8 +49,9 @@ struct amplfi_plan {
     cudaStream_t side;
     cudaEvent_t ev_fork, ev_join;
     // optional device timing of the dominant kernel (amplfi_plan_set_timing)
+    // (mutable: the compute calls take a const plan; a plan is used by one host thread and one stream at a time)
     int timing;
-    int ev_count;
+    mutable int ev_count;
     cudaEvent_t ev_start[AMPLFI_TIMING_RING], ev_stop[AMPLFI_TIMING_RING];
 };
 
@@ -57,6 +60,20 @@ namespace amplfi {
 void set_error(const char* fmt, ...);
 int check_launch(const char* what);
 void count_launch(int n = 1);
+
+// Opt a kernel in to `bytes` of dynamic shared memory once per device (the attribute is per device; setting it twice is
+// harmless, so a racing second thread costs one redundant call).  `done` is a per-kernel bit mask of devices.
+template <class Kernel>
+inline int ensure_dynamic_smem(Kernel kernel, int bytes, std::atomic<unsigned>& done) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    const unsigned bit = 1u << (dev & 31);
+    if (done.load(std::memory_order_acquire) & bit) return AMPLFI_OK;
+    const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e != cudaSuccess) { set_error("cudaFuncSetAttribute: %s", cudaGetErrorString(e)); return AMPLFI_ERR_CUDA; }
+    done.fetch_or(bit, std::memory_order_release);
+    return AMPLFI_OK;
+}
 
 // waveform.cu
 int launch_prepare(const amplfi_plan* p, int approximant, int batch, const double* params, double gmst,

@@ -310,11 +310,10 @@ int amplfi_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
         rc = launch_waveform_h0(p, batch, st);
         if (rc) return rc;
     }
-    amplfi_plan* mp = const_cast<amplfi_plan*>(p);
     const bool timed = p->timing && p->ev_count < AMPLFI_TIMING_RING;
-    if (timed) cudaEventRecord(mp->ev_start[p->ev_count], st);
+    if (timed) cudaEventRecord(p->ev_start[p->ev_count], st);
     rc = launch_inject_whiten(p, batch, noise, offsets, strip_len, h_det, fused ? 1 : 0, out, st);
-    if (timed) { cudaEventRecord(mp->ev_stop[p->ev_count], st); mp->ev_count++; }
+    if (timed) { cudaEventRecord(p->ev_stop[p->ev_count], st); p->ev_count++; }
     return rc;
 }
 
@@ -339,7 +338,7 @@ int amplfi_assemble_batch(const amplfi_plan* p, int batch, const float* bg, long
     const int n_psd = p->nperseg / 2 + 1;
     if (((p->n / 2) % (n_psd - 1)) != 0) { set_error("amplfi_assemble_batch: nperseg %d does not divide n %d", p->nperseg, p->n); return AMPLFI_ERR_INVALID_ARG; }
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    amplfi_plan* mp = const_cast<amplfi_plan*>(p);
+    const amplfi_plan* mp = p;
     // fork: PSD chain on the plan's stream, waveform chain on the caller's
     cudaError_t e = cudaEventRecord(mp->ev_fork, st);
     if (e == cudaSuccess) e = cudaStreamWaitEvent(mp->side, mp->ev_fork, 0);
@@ -354,9 +353,9 @@ int amplfi_assemble_batch(const amplfi_plan* p, int batch, const float* bg, long
     if (e != cudaSuccess) { set_error("amplfi_assemble_batch: join: %s", cudaGetErrorString(e)); return AMPLFI_ERR_CUDA; }
     if (rc) return rc;
     const bool timed = p->timing && p->ev_count < AMPLFI_TIMING_RING;
-    if (timed) cudaEventRecord(mp->ev_start[p->ev_count], st);
+    if (timed) cudaEventRecord(p->ev_start[p->ev_count], st);
     rc = launch_inject_whiten(p, batch, noise, offsets, strip_len, nullptr, 1, out, st);
-    if (timed) { cudaEventRecord(mp->ev_stop[p->ev_count], st); mp->ev_count++; }
+    if (timed) { cudaEventRecord(p->ev_stop[p->ev_count], st); p->ev_count++; }
     return rc;
 }
 

@@ -261,13 +261,9 @@ __global__ void __launch_bounds__(Fft<LOGM>::T) inject_whiten_kernel(const IwArg
 template <int LOGM, int MODE>
 static int launch_iw_t(const IwArgs& a, int units, cudaStream_t st) {
     using F = Fft<LOGM>;
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(inject_whiten_kernel<LOGM, MODE>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)F::SMEM_BYTES);
-        if (e != cudaSuccess) { set_error("cudaFuncSetAttribute: %s", cudaGetErrorString(e)); return AMPLFI_ERR_CUDA; }
-        attr_done = true;
-    }
+    static std::atomic<unsigned> attr_done{0};
+    const int rc = ensure_dynamic_smem(inject_whiten_kernel<LOGM, MODE>, (int)F::SMEM_BYTES, attr_done);
+    if (rc) return rc;
     inject_whiten_kernel<LOGM, MODE><<<units, F::T, F::SMEM_BYTES, st>>>(a);
     count_launch();
     return check_launch("inject_whiten_kernel");

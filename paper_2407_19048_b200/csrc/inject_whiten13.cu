@@ -419,14 +419,11 @@ int init_iw13_tables(cudaStream_t st) {
 #endif
 template <int LOGM, int MODE, bool FWD, int VIEWS = 1>
 static int launch_iw13_t(const IwArgs& a, int units, cudaStream_t st) {
-    static bool attr_done = false;
+    static std::atomic<unsigned> attr_done{0};
     constexpr int T13 = Geo<LOGM>::T;
     const int smem = 2 * Geo<LOGM>::M * (int)sizeof(float);
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(inject_whiten13_kernel<LOGM, MODE, IW13_VT, FWD, VIEWS>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) { set_error("cudaFuncSetAttribute: %s", cudaGetErrorString(e)); return AMPLFI_ERR_CUDA; }
-        attr_done = true;
-    }
+    const int rc = ensure_dynamic_smem(inject_whiten13_kernel<LOGM, MODE, IW13_VT, FWD, VIEWS>, smem, attr_done);
+    if (rc) return rc;
     inject_whiten13_kernel<LOGM, MODE, IW13_VT, FWD, VIEWS><<<units, T13 / IW13_VT, smem, st>>>(a, units);
     count_launch();
     return check_launch("inject_whiten13_kernel");

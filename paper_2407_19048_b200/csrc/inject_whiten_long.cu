@@ -268,16 +268,9 @@ __global__ void __launch_bounds__(128) long_pointwise_kernel(const LongPwArgs a)
 }
 
 static int long_attr() {
-    static bool done = false;
-    if (done) return AMPLFI_OK;
-    cudaError_t e = cudaFuncSetAttribute(long_sub_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)Fft<LONG_LOGM>::SMEM_BYTES);
-    if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(long_sub_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)Fft<LONG_LOGM>::SMEM_BYTES);
-    if (e != cudaSuccess) { set_error("cudaFuncSetAttribute: %s", cudaGetErrorString(e)); return AMPLFI_ERR_CUDA; }
-    done = true;
-    return AMPLFI_OK;
+    static std::atomic<unsigned> done0{0}, done1{0};
+    const int rc = ensure_dynamic_smem(long_sub_kernel<0>, (int)Fft<LONG_LOGM>::SMEM_BYTES, done0);
+    return rc ? rc : ensure_dynamic_smem(long_sub_kernel<1>, (int)Fft<LONG_LOGM>::SMEM_BYTES, done1);
 }
 
 size_t long_scratch_floats2(int chunk_units, int rdec) { return (size_t)chunk_units * rdec * LONG_KS_STRIDE; }

@@ -49,7 +49,7 @@ __global__ void __launch_bounds__(64) prepare_kernel(const double* __restrict__ 
 
 int launch_prepare(const amplfi_plan* p, int approximant, int batch, const double* params, double gmst,
                    double f_lo, double f_hi, double amp_mul, int* flags, cudaStream_t st) {
-    if (approximant >= 0) const_cast<amplfi_plan*>(p)->last_approx = approximant;     // selects the evaluation kernel that follows
+    if (approximant >= 0) p->last_approx = approximant;     // selects the evaluation kernel that follows
     prepare_kernel<<<(batch + 31) / 32, 64, 0, st>>>(
         params, batch, approximant, p->t_seg, p->n_bins, f_lo, f_hi, amp_mul, gmst, p->pd_table, p->d_det_ids,
         p->n_det, approximant < 0 ? nullptr : p->coef, p->resp, flags);

@@ -145,12 +145,9 @@ template <int LOGM>
 static int launch_welch_t(const amplfi_plan* p, const float* bg, long row_stride, int step, int nseg, int detrend,
                           cudaStream_t st) {
     using F = Fft<LOGM>;
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaFuncSetAttribute(welch_segment_kernel<LOGM>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)F::SMEM_BYTES);
-        attr_done = true;
-    }
+    static std::atomic<unsigned> attr_done{0};
+    const int arc = ensure_dynamic_smem(welch_segment_kernel<LOGM>, (int)F::SMEM_BYTES, attr_done);
+    if (arc) return arc;
     dim3 grid(nseg, p->n_det);
     welch_segment_kernel<LOGM><<<grid, F::T, F::SMEM_BYTES, st>>>(bg, row_stride, step, nseg, detrend, p->welch_part);
     count_launch();
@@ -187,11 +184,9 @@ int launch_welch(const amplfi_plan* p, const float* bg, long n_bg, long row_stri
     if (rc) return rc;
     const int n_w = nps / 2 + 1;
     if (average == 1) {
-        static bool attr_done = false;
-        if (!attr_done) {
-            cudaFuncSetAttribute(welch_median_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (256 + 2) * 64 * (int)sizeof(float));
-            attr_done = true;
-        }
+        static std::atomic<unsigned> attr_done{0};
+        const int arc = ensure_dynamic_smem(welch_median_kernel, (256 + 2) * 64 * (int)sizeof(float), attr_done);
+        if (arc) return arc;
         const float mscale = (float)(1.0 / (median_bias(nseg) * p->fs * 0.375 * (double)nps));
         dim3 mgrid((n_w + 63) / 64, p->n_det);
         welch_median_kernel<<<mgrid, 64 * MED_PARTS, (size_t)(nseg + 2) * 64 * sizeof(float), st>>>(p->welch_part, nseg, n_w, mscale, psd);
