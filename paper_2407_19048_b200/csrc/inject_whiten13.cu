@@ -89,10 +89,13 @@ __global__ void __launch_bounds__(Geo<LOGM>::T / VT, LOGM == 13 ? 2 : (LOGM == 1
             else p1_fwd11(z[vt], tt + vt * TT, re, im);
         }
     }
+    // twiddle rows are requested ahead of each barrier; both virtual threads use the same row (TT is a multiple of 64)
+    float2 gtw[8];
+    if (fwd) tw_load8(&g_tw13.p2[0][tt & 63], 64, gtw);
     __syncthreads();
     if (fwd) {
 #pragma unroll
-        for (int vt = 0; vt < VT; ++vt) p2_fwd(tt + vt * TT, re, im);
+        for (int vt = 0; vt < VT; ++vt) p2_fwd(tt + vt * TT, re, im, gtw);
     }
     // ---- per-unit constants of the pointwise stage ----
     const float* filt = a.filt + (size_t)d * a.filt_stride;
@@ -276,12 +279,13 @@ __global__ void __launch_bounds__(Geo<LOGM>::T / VT, LOGM == 13 ? 2 : (LOGM == 1
         for (int r = 0; r < 8; ++r) v[r] = C2{pack(za[r].x, zb[r].x), pack(za[r].y, zb[r].y)};
     };
 
-    __syncthreads();
     PwOps ops[VT];
-    pw_load(tt, ops[0]);                                     // in flight during P3 and the barrier
+    pw_load(tt, ops[0]);                                     // in flight during the barrier and P3
+    if (fwd) tw_load8(&g_tw13.p3[0][tt & 7], 8, gtw);
+    __syncthreads();
     if (fwd) {
 #pragma unroll
-        for (int vt = 0; vt < VT; ++vt) p3_fwd(tt + vt * TT, re, im);
+        for (int vt = 0; vt < VT; ++vt) p3_fwd(tt + vt * TT, re, im, gtw);
     }
     __syncthreads();
     if constexpr (VIEWS == 2) {
@@ -313,12 +317,16 @@ __global__ void __launch_bounds__(Geo<LOGM>::T / VT, LOGM == 13 ? 2 : (LOGM == 1
                 if (vt + 1 < VT) pw_load(t + TT, ops[vt + 1]);
                 p4_inv<LOGM>(klow_a, klow_b, v, re, im);
             }
+            tw_load8(&g_tw13.p3i[0][tt & 63], 64, gtw);
             __syncthreads();
 #pragma unroll
-            for (int vt = 0; vt < VT; ++vt) p3_inv(tt + vt * TT, re, im);
+            for (int vt = 0; vt < VT; ++vt) p3_inv(tt + vt * TT, re, im, gtw);
+            C2 tw2[VT][8];
+#pragma unroll
+            for (int vt = 0; vt < VT; ++vt) p2_inv_twiddles<LOGM>(tt + vt * TT, tw2[vt]);
             __syncthreads();
 #pragma unroll
-            for (int vt = 0; vt < VT; ++vt) p2_inv<LOGM>(tt + vt * TT, re, im);
+            for (int vt = 0; vt < VT; ++vt) p2_inv(tt + vt * TT, re, im, tw2[vt]);
             __syncthreads();
 #pragma unroll
             for (int vt = 0; vt < VT; ++vt) {
@@ -348,12 +356,16 @@ __global__ void __launch_bounds__(Geo<LOGM>::T / VT, LOGM == 13 ? 2 : (LOGM == 1
         // ---- a-9 inverse real FFT ----
         p4_inv<LOGM>(klow_a, klow_b, v, re, im);
     }
+    tw_load8(&g_tw13.p3i[0][tt & 63], 64, gtw);
     __syncthreads();
 #pragma unroll
-    for (int vt = 0; vt < VT; ++vt) p3_inv(tt + vt * TT, re, im);
+    for (int vt = 0; vt < VT; ++vt) p3_inv(tt + vt * TT, re, im, gtw);
+    C2 tw2[VT][8];
+#pragma unroll
+    for (int vt = 0; vt < VT; ++vt) p2_inv_twiddles<LOGM>(tt + vt * TT, tw2[vt]);
     __syncthreads();
 #pragma unroll
-    for (int vt = 0; vt < VT; ++vt) p2_inv<LOGM>(tt + vt * TT, re, im);
+    for (int vt = 0; vt < VT; ++vt) p2_inv(tt + vt * TT, re, im, tw2[vt]);
     __syncthreads();
     {
         float2* out2 = reinterpret_cast<float2*>(out);

@@ -198,10 +198,9 @@ __device__ __forceinline__ void p1_fwd(const float2 (&x)[16], int t, float* re, 
     }
 }
 
-__device__ __forceinline__ void p2_fwd(int t, float* re, float* im) {
+// g: the twiddle row of set t & 63 (tw_load8 of g_tw13.p2), requested by the caller ahead of the barrier
+__device__ __forceinline__ void p2_fwd(int t, float* re, float* im, const float2 (&g)[8]) {
     const int kap = t >> 6, n3 = (t >> 3) & 7, n4 = t & 7;
-    float2 g[8];
-    tw_load8(&g_tw13.p2[0][t & 63], 64, g);
     C2 v[8];
 #pragma unroll
     for (int n2 = 0; n2 < 8; ++n2) v[n2] = lds2(re, im, slot13(kap, n2, n3, n4));
@@ -213,10 +212,8 @@ __device__ __forceinline__ void p2_fwd(int t, float* re, float* im) {
     }
 }
 
-__device__ __forceinline__ void p3_fwd(int t, float* re, float* im) {
+__device__ __forceinline__ void p3_fwd(int t, float* re, float* im, const float2 (&g)[8]) {
     const int kap = t >> 6, k2 = (t >> 3) & 7, n4 = t & 7;
-    float2 g[8];
-    tw_load8(&g_tw13.p3[0][n4], 8, g);
     C2 v[8];
 #pragma unroll
     for (int n3 = 0; n3 < 8; ++n3) v[n3] = lds2(re, im, slot13(kap, k2, n3, n4));
@@ -278,33 +275,33 @@ __device__ __forceinline__ void p4_inv(int klow_a, int klow_b, C2 (&v)[8], float
     }
 }
 
-__device__ __forceinline__ void p3_inv(int t, float* re, float* im) {
+__device__ __forceinline__ void p3_inv(int t, float* re, float* im, const float2 (&g)[8]) {
     const int kap = t >> 6, k2 = (t >> 3) & 7, n4 = t & 7;
     C2 v[8];
 #pragma unroll
     for (int r = 0; r < 8; ++r) v[r] = lds2(re, im, slot13(kap, k2, brev<8>(r), n4));
     dit8(v);
-    // conj twiddle of P2: w_512^(-(n3*8 + n4) k2)
-    float2 g[8];
-    tw_load8(&g_tw13.p3i[0][t & 63], 64, g);
+    // conj twiddle of P2: w_512^(-(n3*8 + n4) k2): g = row t & 63 of g_tw13.p3i
 #pragma unroll
     for (int n3 = 0; n3 < 8; ++n3) sts2(re, im, slot13(kap, k2, n3, n4), cmul_conj_s(v[n3], g[n3]));
 }
 
+// conj twiddles of P1 for virtual thread t: w_M^(-(n2*64 + j0) k1), j0 = n3*8 + n4, k1 = 2kap (A), 2kap+1 (B), n2 = 0..7.
+// Pure arithmetic (4 sincos + a packed power chain): the caller runs it ahead of the barrier that precedes p2_inv.
 template <int LOGM>
-__device__ __forceinline__ void p2_inv(int t, float* re, float* im) {
+__device__ __forceinline__ void p2_inv_twiddles(int t, C2 (&tw)[8]) {
     constexpr int M = Geo<LOGM>::M;
+    const int kap = t >> 6, j0 = t & 63;
+    const float2 ca = twiddle<M>(j0 * 2 * kap), cb = twiddle<M>(j0 * (2 * kap + 1));
+    const float2 sa = twiddle<M / 128>(kap), sb = twiddle<M / 64>(2 * kap + 1);
+    powers8(C2{pack(ca.x, cb.x), pack(ca.y, cb.y)}, C2{pack(sa.x, sb.x), pack(sa.y, sb.y)}, tw);
+}
+__device__ __forceinline__ void p2_inv(int t, float* re, float* im, const C2 (&tw)[8]) {
     const int kap = t >> 6, n3 = (t >> 3) & 7, n4 = t & 7;
     C2 v[8];
 #pragma unroll
     for (int r = 0; r < 8; ++r) v[r] = lds2(re, im, slot13(kap, brev<8>(r), n3, n4));
     dit8(v);
-    // conj twiddle of P1: w_M^(-(n2*64 + j0) k1), j0 = n3*8 + n4, k1 = 2kap (A), 2kap+1 (B)
-    const int j0 = n3 * 8 + n4;
-    const float2 ca = twiddle<M>(j0 * 2 * kap), cb = twiddle<M>(j0 * (2 * kap + 1));
-    const float2 sa = twiddle<M / 128>(kap), sb = twiddle<M / 64>(2 * kap + 1);
-    C2 tw[8];
-    powers8(C2{pack(ca.x, cb.x), pack(ca.y, cb.y)}, C2{pack(sa.x, sb.x), pack(sa.y, sb.y)}, tw);
 #pragma unroll
     for (int n2 = 0; n2 < 8; ++n2) sts2(re, im, slot13(kap, n2, n3, n4), cmul_conj(v[n2], tw[n2]));
 }
