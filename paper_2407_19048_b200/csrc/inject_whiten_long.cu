@@ -154,11 +154,13 @@ struct LongPwArgs {
     int nofwd;                // no data: the sub-spectra are taken as zero (inverse-only launches)
 };
 
-// exp(-2 pi i num / den) for a power-of-two den <= 2^21: the argument is reduced exactly in integers
+// exp(-2 pi i num / den) for a power-of-two den <= 2^21: the argument is reduced exactly in integers to [-pi, pi) and
+// evaluated with the fast sine/cosine (absolute error ~4e-7, as for the twiddles of the transforms themselves)
 __device__ __forceinline__ float2 long_w(long num, int den) {
-    const int m = (int)(num & (long)(den - 1));
+    int m = (int)(num & (long)(den - 1));
+    if (m >= den / 2) m -= den;
     float s, c;
-    sincospif(-2.0f * ((float)m / (float)den), &s, &c);       // m / den is exact in fp32
+    __sincosf((float)m * (-6.283185307179586f / (float)den), &s, &c);
     return make_float2(c, s);
 }
 
@@ -206,7 +208,7 @@ __global__ void __launch_bounds__(128) long_pointwise_kernel(const LongPwArgs a)
                 double turns = (double)k * delta;
                 turns -= rint(turns);
                 float s, co;
-                sincospif(-2.0f * (float)turns, &s, &co);   // exp(-2 pi i k dt / T)
+                __sincosf((float)turns * -6.283185307179586f, &s, &co);   // exp(-2 pi i k dt / T), |turns| <= 1/2
                 const float2 cp = make_float2(cre * co - cim * s, cre * s + cim * co);
                 x.x += hv.x * cp.x - hv.y * cp.y;
                 x.y += hv.x * cp.y + hv.y * cp.x;
