@@ -420,10 +420,21 @@ __global__ void init_tw13_kernel() {
     }
 }
 
+// Once per device: the tables are the same for every plan, and amplfi_plan_create synchronises before it returns, so a
+// later plan never rewrites them under a running kernel of an earlier one.
 int init_iw13_tables(cudaStream_t st) {
+    static std::atomic<unsigned> done{0};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    const unsigned bit = 1u << (dev & 31);
+    if (done.load(std::memory_order_acquire) & bit) return AMPLFI_OK;
     init_tw13_kernel<<<2, 256, 0, st>>>();
     count_launch();
-    return check_launch("init_tw13_kernel");
+    const int rc = check_launch("init_tw13_kernel");
+    if (rc) return rc;
+    if (cudaStreamSynchronize(st) != cudaSuccess) { set_error("init_tw13_kernel: synchronise failed"); return AMPLFI_ERR_CUDA; }
+    done.fetch_or(bit, std::memory_order_release);
+    return AMPLFI_OK;
 }
 
 #ifndef IW13_VT

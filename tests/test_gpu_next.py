@@ -274,3 +274,26 @@ def test_sine_gaussian_parity(n, fs):
     hp_t, hc_t, _ = OW.waveform_td(OW.SINE_GAUSSIAN, par, n, fs, 20.0, 1000.0)
     got = h_t.cpu().numpy().astype(np.float64)
     assert row_err(got[:, 0], hp_t).max() <= TOL and row_err(got[:, 1], hc_t).max() <= TOL
+
+
+# ------------------------------------------------------------------------------------------ plans side by side
+def test_two_plans_side_by_side_and_plan_reuse():
+    """Two plans of different lengths alive at once (they share the packed kernel's twiddle tables), one of them reused for
+    another batch size, approximant and mode: results equal those of fresh plans bit for bit."""
+    par16, noise16, psd16 = _workload(16384, 2048.0, 4, [0, 1], 4242)
+    par8, noise8, psd8 = _workload(8192, 2048.0, 3, [0, 1], 4243)
+    s16, s8 = dev((psd16 * PSD_SCALE).astype(np.float32)), dev((psd8 * PSD_SCALE).astype(np.float32))
+
+    def run(plan, par, noise, psd_s, batch, approx):
+        return A.amplfi_inject_whiten(plan, batch, dev(noise[:batch]), psd_s, 20.0, 1000.0, approximant=approx, params=dev(par[:batch]))
+
+    fresh16 = run(A.Plan(16384, 2048.0, [0, 1], 4), par16, noise16, s16, 4, A.IMRPHENOMD)
+    fresh8 = run(A.Plan(8192, 2048.0, [0, 1], 3), par8, noise8, s8, 3, A.TAYLORF2)
+    fresh16b = run(A.Plan(16384, 2048.0, [0, 1], 4), par16, noise16, s16, 2, A.TAYLORF2)
+    pa, pb = A.Plan(16384, 2048.0, [0, 1], 4), A.Plan(8192, 2048.0, [0, 1], 3)
+    a1 = run(pa, par16, noise16, s16, 4, A.IMRPHENOMD)
+    b1 = run(pb, par8, noise8, s8, 3, A.TAYLORF2)
+    a2 = run(pa, par16, noise16, s16, 2, A.TAYLORF2)            # same plan, smaller batch, other approximant
+    a3 = run(pa, par16, noise16, s16, 4, A.IMRPHENOMD)          # and back
+    torch.cuda.synchronize()
+    assert torch.equal(a1, fresh16) and torch.equal(b1, fresh8) and torch.equal(a2, fresh16b) and torch.equal(a3, fresh16)
