@@ -193,7 +193,7 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     double pl5 = 5.0 / 3.0 * (7729.0 / 84.0 - 13.0 * eta) * PI - 3.0 * gam;
     double pv6 = 11583.231236531 / 4.694215680 - 640.0 / 3.0 * PI * PI - 6848.0 / 21.0 * AMPLFI_GAMMA_E
                  + eta * (-15737.765635 / 3.048192 + 2255.0 / 12.0 * PI * PI) + e2 * 76055.0 / 1728.0
-                 - e3 * 127825.0 / 1296.0 - 6848.0 / 21.0 * log(4.0)
+                 - e3 * 127825.0 / 1296.0 - 6848.0 / 21.0 * 1.3862943611198906        /* ln 4 */
                  + PI * (3760.0 * SL + 1490.0 * dSL) / 3.0;
     double pl6 = -6848.0 / 21.0;
     double pv7 = PI * (77096675.0 / 254016.0 + 378515.0 / 1512.0 * eta - 74045.0 / 756.0 * e2)
@@ -266,19 +266,20 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     const double f1 = 0.018, f2 = 0.5 * f_rd;
     double phi_ins, dphi_ins;
     {
-        const double v = cbrt(PI * f1), lv = log(v);
+        // the junction frequencies are constants of the model: their roots and logarithms are written out
+        const double v = 0.3838316585355026 /* cbrt(pi 0.018) */, lv = -0.957551211745524 /* ln v */;
         double s = 0.0, ds = 0.0, vp = 1.0 / (v * v * v * v * v * v);      // v^(i-6)
         for (int i = 0; i < 8; ++i) {
             s += (pn[i] + pl[i] * lv) * vp * v;                            // v^(i-5)
             ds += ((i - 5) * (pn[i] + pl[i] * lv) + pl[i]) * vp;
             vp *= v;
         }
-        const double c13 = cbrt(f1);
+        const double c13 = 0.26207413942088964;   // cbrt(0.018)
         phi_ins = pfar * s - PI / 4.0
                   + (sg1 * f1 + 0.75 * sg2 * f1 * c13 + 0.6 * sg3 * f1 * c13 * c13 + 0.5 * sg4 * f1 * f1) / eta;
         dphi_ins = pfar * ds * v / (3.0 * f1) + (sg1 + sg2 * c13 + sg3 * c13 * c13 + sg4 * f1) / eta;
     }
-    const double int1 = (be1 * f1 + be2 * log(f1) - be3 / (3.0 * f1 * f1 * f1)) / eta;
+    const double int1 = (be1 * f1 + be2 * -4.017383521085972 /* ln 0.018 */ - be3 / (3.0 * f1 * f1 * f1)) / eta;
     const double dint1 = (be1 + be2 / f1 + be3 / (f1 * f1 * f1 * f1)) / eta;
     const double c2int = dphi_ins - dint1;
     const double c1int = phi_ins - int1 - c2int * f1;
@@ -351,7 +352,7 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     const double fa = 0.014, fc = f_peak;
     double va, da;
     {
-        const double x = cbrt(PI * fa), dx = x / (3.0 * fa), c13 = cbrt(fa);
+        const double x = 0.35298748079802034 /* cbrt(pi 0.014) */, dx = x / (3.0 * fa), c13 = 0.24101422641752301 /* cbrt(0.014) */;
         va = 1.0 + x * x * (A[2] + x * (A[3] + x * (A[4] + x * (A[5] + x * A[6]))))
              + fa * fa * c13 * (rho1 + c13 * (rho2 + c13 * rho3));
         da = (2.0 * A[2] * x + 3.0 * A[3] * x * x + 4.0 * A[4] * x * x * x + 5.0 * A[5] * x * x * x * x
