@@ -95,6 +95,13 @@ __device__ inline double pd_fit(const double* t, double eta, double xi) {
 
 // p: 11 parameters; t_seg = n/fs; amp_mul multiplies the strain amplitude (1 for the API in strain/Hz).
 // tab: [19][11] fit table in global/constant memory.
+// prepare_kernel runs one warp per SM through ~7000 straight-line instructions, so it is bound by instruction fetch
+// (ncu: 45 % of its stall samples are "no instruction").  The fp64 library routines and the division are therefore kept
+// out of line: one copy each, hit in the instruction cache from the second call on.
+static __device__ __noinline__ double pexp(double x) { return exp(x); }
+static __device__ __noinline__ double plog(double x) { return log(x); }
+static __device__ __noinline__ double pdiv(double a, double b) { return a / b; }
+
 // Sine-Gaussian burst (reading R-W12): row = f0, Q, -, -, A, iota, phi, t0, ra, dec, psi.
 //   h0(f_k) = A tau sqrt(pi)/2 exp(-(pi tau (f_k - f0))^2) exp(-i (2 pi f_k t0 - phi)),  tau = Q / (sqrt2 pi f0)
 // Fields used: lin1 (t0/T, turns per bin), c01 (-phi / 2 pi), amp_scale, g_krd (f0 T), g_invw (pi tau / T), pol_p, pol_c.
@@ -143,7 +150,7 @@ __device__ __forceinline__ float2 eval_sine_gaussian(const WfCoef& c, int k) {
 __device__ inline void prepare_sample(const double* p, int approx, double t_seg, int n_bins, double f_lo,
                                       double f_hi, double amp_mul, const double* tab, WfCoef& c) {
     if (approx == 2) { prepare_sine_gaussian(p, t_seg, n_bins, f_lo, f_hi, amp_mul, c); return; }
-    const double PI = AMPLFI_PI, TWO_PI = 2.0 * AMPLFI_PI;
+    const double PI = AMPLFI_PI, TWO_PI = 2.0 * AMPLFI_PI, I2PI = 0.15915494309189535;   // 1 / (2 pi)
     const double mc = p[0], q = p[1], chi1 = p[2], chi2 = p[3], dist = p[4];
     bool ok = (mc > 0.0) && (q > 0.0) && (q <= 1.0) && (fabs(chi1) < 1.0) && (fabs(chi2) < 1.0) && (dist > 0.0);
     for (int i = 0; i < 11; ++i) ok = ok && isfinite(p[i]);
@@ -153,12 +160,15 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     c.k_hi = 0;
     if (!ok) return;
     const double eta = q / ((1.0 + q) * (1.0 + q));
-    const double mtot = mc * exp(-0.6 * log(eta));
+    const double ieta = 1.0 / eta;                   // reciprocals once: every fp64 division is ~25 instructions of this
+                                                     // fetch-bound kernel
+    const double mtot = mc * pexp(-0.6 * plog(eta));
     const double ms = mtot * AMPLFI_MTSUN;           // seconds
     const double mu = ms / t_seg;                    // Mf = mu * k
-    const double lnmu = log(mu);
+    const double imu = 1.0 / mu;
+    const double lnmu = plog(mu);
     const double lnv1 = (lnmu + 1.1447298858494002) / 3.0;     // ln(pi) = 1.14472988584940017...
-    const double v1 = exp(lnv1);                     // (pi mu)^(1/3): v = v1 * k^(1/3)
+    const double v1 = pexp(lnv1);                     // (pi mu)^(1/3): v = v1 * k^(1/3)
     const double cosi = cos(p[5]);
     c.pol_p = (float)(0.5 * (1.0 + cosi * cosi));
     c.pol_c = (float)cosi;
@@ -199,7 +209,7 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     double pv7 = PI * (77096675.0 / 254016.0 + 378515.0 / 1512.0 * eta - 74045.0 / 756.0 * e2)
                  + (-8980424995.0 / 762048.0 + 6586595.0 * eta / 756.0 - 305.0 * e2 / 36.0) * SL
                  - (170978035.0 / 48384.0 - 2876425.0 * eta / 672.0 - 4735.0 * e2 / 144.0) * dSL;
-    const double pfa = 3.0 / (128.0 * eta) / TWO_PI;          // everything below is in turns
+    const double pfa = 3.0 / (128.0 * eta) * I2PI;          // everything below is in turns
     const double iv = 1.0 / v1;
     c.a_m5 = pfa * iv * iv * iv * iv * iv;
     c.a_m3 = pfa * pv2 * iv * iv * iv;
@@ -210,7 +220,7 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     c.a_p1ln = pfa * pl6 / 3.0 * v1;
     c.a_p2 = pfa * pv7 * v1 * v1;
     const double tc_turns = p[7] / t_seg;                     // 2 pi f t_c / 2 pi = k t_c / T
-    const double phic_turns = -2.0 * p[6] / TWO_PI;
+    const double phic_turns = -2.0 * p[6] * I2PI;
     double const1 = pfa * (pv5 + pl5 * lnv1) - 0.125 + phic_turns;      // -pi/4 -> -1/8 turn
 
     if (approx == 0) {
@@ -249,9 +259,9 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
                                 + 3.352411249771192 * e3)
                          * (1.0 + (-0.0030302335878845507 - 2.0066110851351073 * eta + 7.7050567802399215 * e2) * sn))
                         / (1.0 + (-0.6714403054720589 - 1.4756929437702908 * eta + 7.304676214885011 * e2) * sn);
-    const double ln1maf = log(1.0 - af);
-    const double fring0 = (1.5251 - 1.1568 * exp(0.1292 * ln1maf)) / TWO_PI;
-    const double qual = 0.7 + 1.4187 * exp(-0.4990 * ln1maf);
+    const double ln1maf = plog(1.0 - af);
+    const double fring0 = (1.5251 - 1.1568 * pexp(0.1292 * ln1maf)) * I2PI;
+    const double qual = 0.7 + 1.4187 * pexp(-0.4990 * ln1maf);
     const double f_rd = fring0 / (1.0 - erad);
     const double f_dm = fring0 / (2.0 * qual) / (1.0 - erad);
 
@@ -276,19 +286,19 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
         }
         const double c13 = 0.26207413942088964;   // cbrt(0.018)
         phi_ins = pfar * s - PI / 4.0
-                  + (sg1 * f1 + 0.75 * sg2 * f1 * c13 + 0.6 * sg3 * f1 * c13 * c13 + 0.5 * sg4 * f1 * f1) / eta;
-        dphi_ins = pfar * ds * v / (3.0 * f1) + (sg1 + sg2 * c13 + sg3 * c13 * c13 + sg4 * f1) / eta;
+                  + (sg1 * f1 + 0.75 * sg2 * f1 * c13 + 0.6 * sg3 * f1 * c13 * c13 + 0.5 * sg4 * f1 * f1) * ieta;
+        dphi_ins = pfar * ds * v / (3.0 * f1) + (sg1 + sg2 * c13 + sg3 * c13 * c13 + sg4 * f1) * ieta;
     }
-    const double int1 = (be1 * f1 + be2 * -4.017383521085972 /* ln 0.018 */ - be3 / (3.0 * f1 * f1 * f1)) / eta;
-    const double dint1 = (be1 + be2 / f1 + be3 / (f1 * f1 * f1 * f1)) / eta;
+    const double int1 = (be1 * f1 + be2 * -4.017383521085972 /* ln 0.018 */ - be3 / (3.0 * f1 * f1 * f1)) * ieta;
+    const double dint1 = (be1 + be2 / f1 + be3 / (f1 * f1 * f1 * f1)) * ieta;
     const double c2int = dphi_ins - dint1;
     const double c1int = phi_ins - int1 - c2int * f1;
-    const double lnf2 = log(f2), f2m14 = exp(-0.25 * lnf2);                 // f2^(-1/4)
-    const double int2 = (be1 * f2 + be2 * lnf2 - be3 / (3.0 * f2 * f2 * f2)) / eta + c1int + c2int * f2;
-    const double dint2 = (be1 + be2 / f2 + be3 / (f2 * f2 * f2 * f2)) / eta + c2int;
+    const double lnf2 = plog(f2), f2m14 = pexp(-0.25 * lnf2);                 // f2^(-1/4)
+    const double int2 = (be1 * f2 + be2 * lnf2 - be3 / (3.0 * f2 * f2 * f2)) * ieta + c1int + c2int * f2;
+    const double dint2 = (be1 + be2 / f2 + be3 / (f2 * f2 * f2 * f2)) * ieta + c2int;
     const double x2 = (f2 - al5 * f_rd) / f_dm;
-    const double mr2 = (al1 * f2 - al2 / f2 + 4.0 / 3.0 * al3 * (f2 * f2m14) + al4 * atan(x2)) / eta;
-    const double dmr2 = (al1 + al2 / (f2 * f2) + al3 * f2m14 + al4 / (f_dm * (1.0 + x2 * x2))) / eta;
+    const double mr2 = (al1 * f2 - al2 / f2 + 4.0 / 3.0 * al3 * (f2 * f2m14) + al4 * atan(x2)) * ieta;
+    const double dmr2 = (al1 + al2 / (f2 * f2) + al3 * f2m14 + al4 / (f_dm * (1.0 + x2 * x2))) * ieta;
     const double c2mr = dint2 - dmr2;
     const double c1mr = int2 - mr2 - c2mr * f2;
     // amplitude peak and time alignment
@@ -296,33 +306,33 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     const double f_peak = (g2 > 1.0) ? fabs(f_rd - f_dm * g3 / g2)
                                      : fabs(f_rd + f_dm * (sqrt(1.0 - g2 * g2) - 1.0) * g3 / g2);
     const double xp = (f_peak - al5 * f_rd) / f_dm;
-    const double t0 = (al1 + al2 / (f_peak * f_peak) + al3 * rsqrt(sqrt(f_peak)) + al4 / (f_dm * (1.0 + xp * xp))) / eta
+    const double t0 = (al1 + al2 / (f_peak * f_peak) + al3 * rsqrt(sqrt(f_peak)) + al4 / (f_dm * (1.0 + xp * xp))) * ieta
                       + c2mr;
 
-    c.kp1 = f1 / mu;
-    c.kp2 = f2 / mu;
-    const double mu13 = exp(lnmu / 3.0);
-    c.lin1 = tc_turns + (sg1 / eta - t0) * mu / TWO_PI;
+    c.kp1 = f1 * imu;
+    c.kp2 = f2 * imu;
+    const double mu13 = pexp(lnmu / 3.0);
+    c.lin1 = tc_turns + (sg1 * ieta - t0) * mu * I2PI;
     c.c01 = const1;
-    c.s_p4 = 0.75 * sg2 / eta * mu * mu13 / TWO_PI;
-    c.s_p5 = 0.6 * sg3 / eta * mu * mu13 * mu13 / TWO_PI;
-    c.s_p6 = 0.5 * sg4 / eta * mu * mu / TWO_PI;
-    c.lin2 = tc_turns + (be1 / eta + c2int - t0) * mu / TWO_PI;
-    c.c02 = (c1int + be2 / eta * lnmu) / TWO_PI + phic_turns;
-    c.b_ln = be2 / eta / TWO_PI;
-    c.b_m9 = -be3 / (3.0 * eta * mu * mu * mu) / TWO_PI;
-    c.lin3 = tc_turns + (al1 / eta + c2mr - t0) * mu / TWO_PI;
-    c.c03 = c1mr / TWO_PI + phic_turns;
-    c.r_m3 = -al2 / (eta * mu) / TWO_PI;
-    c.r_34 = 4.0 / 3.0 * al3 / eta * exp(0.75 * lnmu) / TWO_PI;
-    c.r_at = (float)(al4 / eta / TWO_PI);
-    c.at_k0 = (float)(al5 * f_rd / mu);
+    c.s_p4 = 0.75 * sg2 * ieta * mu * mu13 * I2PI;
+    c.s_p5 = 0.6 * sg3 * ieta * mu * mu13 * mu13 * I2PI;
+    c.s_p6 = 0.5 * sg4 * ieta * mu * mu * I2PI;
+    c.lin2 = tc_turns + (be1 * ieta + c2int - t0) * mu * I2PI;
+    c.c02 = (c1int + be2 * ieta * lnmu) * I2PI + phic_turns;
+    c.b_ln = be2 * ieta * I2PI;
+    c.b_m9 = -be3 / (3.0 * eta * mu * mu * mu) * I2PI;
+    c.lin3 = tc_turns + (al1 * ieta + c2mr - t0) * mu * I2PI;
+    c.c03 = c1mr * I2PI + phic_turns;
+    c.r_m3 = -al2 / (eta * mu) * I2PI;
+    c.r_34 = 4.0 / 3.0 * al3 * ieta * pexp(0.75 * lnmu) * I2PI;
+    c.r_at = (float)(al4 * ieta * I2PI);
+    c.at_k0 = (float)(al5 * f_rd * imu);
     c.at_invw = (float)(mu / f_dm);
 
     // ---- amplitude ----
     const double amp0 = 2.0 * sqrt(5.0 / (64.0 * PI)) * mtot * mtot * AMPLFI_MTSUN * (AMPLFI_MTSUN * AMPLFI_C_SI)
                         / (dist * AMPLFI_MPC);
-    c.amp_scale = (float)(amp0 * sqrt(2.0 * eta / 3.0) * 0.8263074871107581 * exp(-7.0 / 6.0 * lnmu) * amp_mul);   // pi^(-1/6)
+    c.amp_scale = (float)(amp0 * sqrt(2.0 * eta / 3.0) * 0.8263074871107581 * pexp(-7.0 / 6.0 * lnmu) * amp_mul);   // pi^(-1/6)
     const double c12 = chi1 * chi1, c22 = chi2 * chi2;
     double A[7];
     A[2] = (-969.0 + 1804.0 * eta) / 672.0;
@@ -364,7 +374,7 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     {
         const double d = fc - f_rd;
         const double lor = w * g1 / (d * d + w * w);
-        const double ex = exp(-d * g2 / w);
+        const double ex = pexp(-d * g2 / w);
         vc = ex * lor;
         dc = ex * lor * (-g2 / w - 2.0 * d / (d * d + w * w));
     }
@@ -374,12 +384,12 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     const double Dp = 0.5 * (dc + da) * h, Dm = 0.5 * (dc - da) * h;
     const double q3 = 0.5 * (Dp - Aodd), q1 = Aodd - q3, q4 = 0.5 * (Dm - 2.0 * S), q2 = S - q4;
     c.q[0] = (float)vm; c.q[1] = (float)q1; c.q[2] = (float)q2; c.q[3] = (float)q3; c.q[4] = (float)q4;
-    c.q_mid = (float)(fm / mu);
+    c.q_mid = (float)(fm * imu);
     c.q_invh = (float)(mu / h);
-    c.ka1 = (float)(fa / mu);
-    c.ka2 = (float)(fc / mu);
+    c.ka1 = (float)(fa * imu);
+    c.ka2 = (float)(fc * imu);
     c.g0 = (float)(g1 / w);
-    c.g_krd = (float)(f_rd / mu);
+    c.g_krd = (float)(f_rd * imu);
     c.g_invw = (float)(mu / w);
     c.g2 = (float)g2;
 }
