@@ -209,7 +209,7 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     double pv7 = PI * (77096675.0 / 254016.0 + 378515.0 / 1512.0 * eta - 74045.0 / 756.0 * e2)
                  + (-8980424995.0 / 762048.0 + 6586595.0 * eta / 756.0 - 305.0 * e2 / 36.0) * SL
                  - (170978035.0 / 48384.0 - 2876425.0 * eta / 672.0 - 4735.0 * e2 / 144.0) * dSL;
-    const double pfa = 3.0 / (128.0 * eta) * I2PI;          // everything below is in turns
+    const double pfa = 3.0 / 128.0 * ieta * I2PI;          // everything below is in turns
     const double iv = 1.0 / v1;
     c.a_m5 = pfa * iv * iv * iv * iv * iv;
     c.a_m3 = pfa * pv2 * iv * iv * iv;
@@ -272,7 +272,7 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     // phases in radians as functions of Mf (value, derivative) at the two junctions
     const double pn[8] = {1.0, 0.0, pv2, pv3, pv4, pv5, pv6, pv7};
     const double pl[8] = {0.0, 0.0, 0.0, 0.0, 0.0, pl5, pl6, 0.0};
-    const double pfar = 3.0 / (128.0 * eta);
+    const double pfar = 3.0 / 128.0 * ieta;
     const double f1 = 0.018, f2 = 0.5 * f_rd;
     double phi_ins, dphi_ins;
     {
@@ -289,24 +289,27 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
                   + (sg1 * f1 + 0.75 * sg2 * f1 * c13 + 0.6 * sg3 * f1 * c13 * c13 + 0.5 * sg4 * f1 * f1) * ieta;
         dphi_ins = pfar * ds * v / (3.0 * f1) + (sg1 + sg2 * c13 + sg3 * c13 * c13 + sg4 * f1) * ieta;
     }
-    const double int1 = (be1 * f1 + be2 * -4.017383521085972 /* ln 0.018 */ - be3 / (3.0 * f1 * f1 * f1)) * ieta;
-    const double dint1 = (be1 + be2 / f1 + be3 / (f1 * f1 * f1 * f1)) * ieta;
+    const double if1 = 1.0 / 0.018, if1_3 = if1 * if1 * if1;      // constant: folded at compile time
+    const double int1 = (be1 * f1 + be2 * -4.017383521085972 /* ln 0.018 */ - be3 * if1_3 * (1.0 / 3.0)) * ieta;
+    const double dint1 = (be1 + be2 * if1 + be3 * if1_3 * if1) * ieta;
     const double c2int = dphi_ins - dint1;
     const double c1int = phi_ins - int1 - c2int * f1;
     const double lnf2 = plog(f2), f2m14 = pexp(-0.25 * lnf2);                 // f2^(-1/4)
-    const double int2 = (be1 * f2 + be2 * lnf2 - be3 / (3.0 * f2 * f2 * f2)) * ieta + c1int + c2int * f2;
-    const double dint2 = (be1 + be2 / f2 + be3 / (f2 * f2 * f2 * f2)) * ieta + c2int;
-    const double x2 = (f2 - al5 * f_rd) / f_dm;
-    const double mr2 = (al1 * f2 - al2 / f2 + 4.0 / 3.0 * al3 * (f2 * f2m14) + al4 * atan(x2)) * ieta;
-    const double dmr2 = (al1 + al2 / (f2 * f2) + al3 * f2m14 + al4 / (f_dm * (1.0 + x2 * x2))) * ieta;
+    const double if2 = 1.0 / f2, if2_3 = if2 * if2 * if2;
+    const double int2 = (be1 * f2 + be2 * lnf2 - be3 * if2_3 * (1.0 / 3.0)) * ieta + c1int + c2int * f2;
+    const double dint2 = (be1 + be2 * if2 + be3 * if2_3 * if2) * ieta + c2int;
+    const double ifdm = 1.0 / f_dm;
+    const double x2 = (f2 - al5 * f_rd) * ifdm;
+    const double mr2 = (al1 * f2 - al2 * if2 + 4.0 / 3.0 * al3 * (f2 * f2m14) + al4 * atan(x2)) * ieta;
+    const double dmr2 = (al1 + al2 * if2 * if2 + al3 * f2m14 + al4 * ifdm / (1.0 + x2 * x2)) * ieta;
     const double c2mr = dint2 - dmr2;
     const double c1mr = int2 - mr2 - c2mr * f2;
     // amplitude peak and time alignment
     const double g1 = fit[PD_GAMMA1], g2 = fit[PD_GAMMA2], g3 = fit[PD_GAMMA3];
     const double f_peak = (g2 > 1.0) ? fabs(f_rd - f_dm * g3 / g2)
                                      : fabs(f_rd + f_dm * (sqrt(1.0 - g2 * g2) - 1.0) * g3 / g2);
-    const double xp = (f_peak - al5 * f_rd) / f_dm;
-    const double t0 = (al1 + al2 / (f_peak * f_peak) + al3 * rsqrt(sqrt(f_peak)) + al4 / (f_dm * (1.0 + xp * xp))) * ieta
+    const double xp = (f_peak - al5 * f_rd) * ifdm;
+    const double t0 = (al1 + al2 / (f_peak * f_peak) + al3 * rsqrt(sqrt(f_peak)) + al4 * ifdm / (1.0 + xp * xp)) * ieta
                       + c2mr;
 
     c.kp1 = f1 * imu;
@@ -320,14 +323,14 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     c.lin2 = tc_turns + (be1 * ieta + c2int - t0) * mu * I2PI;
     c.c02 = (c1int + be2 * ieta * lnmu) * I2PI + phic_turns;
     c.b_ln = be2 * ieta * I2PI;
-    c.b_m9 = -be3 / (3.0 * eta * mu * mu * mu) * I2PI;
+    c.b_m9 = -be3 * (1.0 / 3.0) * ieta * imu * imu * imu * I2PI;
     c.lin3 = tc_turns + (al1 * ieta + c2mr - t0) * mu * I2PI;
     c.c03 = c1mr * I2PI + phic_turns;
-    c.r_m3 = -al2 / (eta * mu) * I2PI;
+    c.r_m3 = -al2 * ieta * imu * I2PI;
     c.r_34 = 4.0 / 3.0 * al3 * ieta * pexp(0.75 * lnmu) * I2PI;
     c.r_at = (float)(al4 * ieta * I2PI);
     c.at_k0 = (float)(al5 * f_rd * imu);
-    c.at_invw = (float)(mu / f_dm);
+    c.at_invw = (float)(mu * ifdm);
 
     // ---- amplitude ----
     const double amp0 = 2.0 * sqrt(5.0 / (64.0 * PI)) * mtot * mtot * AMPLFI_MTSUN * (AMPLFI_MTSUN * AMPLFI_C_SI)
@@ -373,10 +376,11 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     double vc, dc;
     {
         const double d = fc - f_rd;
-        const double lor = w * g1 / (d * d + w * w);
-        const double ex = pexp(-d * g2 / w);
+        const double iw = 1.0 / w, ilor = 1.0 / (d * d + w * w);
+        const double lor = w * g1 * ilor;
+        const double ex = pexp(-d * g2 * iw);
         vc = ex * lor;
-        dc = ex * lor * (-g2 / w - 2.0 * d / (d * d + w * w));
+        dc = ex * lor * (-g2 * iw - 2.0 * d * ilor);
     }
     // quartic through (fa: value, slope), (midpoint: v2), (fc: value, slope) in u = (f - fm)/h in [-1, 1]
     const double h = 0.5 * (fc - fa), fm = 0.5 * (fc + fa), vm = fit[PD_V2];
