@@ -54,15 +54,24 @@ __device__ __constant__ DetGeom kDet[3] = {
 #define AMPLFI_GAMMA_E 0.5772156649015329
 #define AMPLFI_PI 3.141592653589793238
 
+// prepare_kernel runs one warp per SM through ~7000 straight-line instructions, so it is bound by instruction fetch
+// (ncu: 45 % of its stall samples are "no instruction").  The fp64 library routines and the division are therefore kept
+// out of line: one copy each, hit in the instruction cache from the second call on.
+static __device__ __noinline__ double pexp(double x) { return exp(x); }
+static __device__ __noinline__ double plog(double x) { return log(x); }
+static __device__ __noinline__ double psqrt(double x) { return sqrt(x); }
+static __device__ __noinline__ double pcos(double x) { return cos(x); }
+static __device__ __noinline__ void psincos(double x, double* s, double* c) { sincos(x, s, c); }
+
 // antenna patterns and geocentric delay of detector `det`
 struct SkyFrame { double X[3], Y[3], n[3]; };
 
 // polarisation axes X, Y and direction n toward the source in the Earth-fixed frame (shared by all detectors)
 __device__ inline SkyFrame sky_frame(double ra, double dec, double psi, double gmst) {
     double sg, cg, sd, cd, sp, cp;
-    sincos(gmst - ra, &sg, &cg);
-    sincos(dec, &sd, &cd);
-    sincos(psi, &sp, &cp);
+    psincos(gmst - ra, &sg, &cg);
+    psincos(dec, &sd, &cd);
+    psincos(psi, &sp, &cp);
     SkyFrame f;
     f.X[0] = -cp * sg - sp * cg * sd; f.X[1] = -cp * cg + sp * sg * sd; f.X[2] = sp * cd;
     f.Y[0] = sp * sg - cp * cg * sd;  f.Y[1] = sp * cg + cp * sg * sd;  f.Y[2] = cp * cd;
@@ -95,13 +104,6 @@ __device__ inline double pd_fit(const double* t, double eta, double xi) {
 
 // p: 11 parameters; t_seg = n/fs; amp_mul multiplies the strain amplitude (1 for the API in strain/Hz).
 // tab: [19][11] fit table in global/constant memory.
-// prepare_kernel runs one warp per SM through ~7000 straight-line instructions, so it is bound by instruction fetch
-// (ncu: 45 % of its stall samples are "no instruction").  The fp64 library routines and the division are therefore kept
-// out of line: one copy each, hit in the instruction cache from the second call on.
-static __device__ __noinline__ double pexp(double x) { return exp(x); }
-static __device__ __noinline__ double plog(double x) { return log(x); }
-static __device__ __noinline__ double pdiv(double a, double b) { return a / b; }
-
 // Sine-Gaussian burst (reading R-W12): row = f0, Q, -, -, A, iota, phi, t0, ra, dec, psi.
 //   h0(f_k) = A tau sqrt(pi)/2 exp(-(pi tau (f_k - f0))^2) exp(-i (2 pi f_k t0 - phi)),  tau = Q / (sqrt2 pi f0)
 // Fields used: lin1 (t0/T, turns per bin), c01 (-phi / 2 pi), amp_scale, g_krd (f0 T), g_invw (pi tau / T), pol_p, pol_c.
@@ -169,7 +171,7 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     const double lnmu = plog(mu);
     const double lnv1 = (lnmu + 1.1447298858494002) / 3.0;     // ln(pi) = 1.14472988584940017...
     const double v1 = pexp(lnv1);                     // (pi mu)^(1/3): v = v1 * k^(1/3)
-    const double cosi = cos(p[5]);
+    const double cosi = pcos(p[5]);
     c.pol_p = (float)(0.5 * (1.0 + cosi * cosi));
     c.pol_c = (float)cosi;
 
@@ -188,7 +190,7 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
 
     // ---- TaylorF2 phasing series (aligned spins for IMRPhenomD, none for TaylorF2) ----
     const double s1 = (approx == 0) ? 0.0 : chi1, s2 = (approx == 0) ? 0.0 : chi2;
-    const double seta = sqrt(fmax(1.0 - 4.0 * eta, 0.0));
+    const double seta = psqrt(fmax(1.0 - 4.0 * eta, 0.0));
     const double m1 = 0.5 * (1.0 + seta), m2 = 0.5 * (1.0 - seta);
     const double SL = m1 * m1 * s1 + m2 * m2 * s2;
     const double dSL = (m1 - m2) * (m2 * s2 - m1 * s1);
@@ -231,7 +233,7 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
         c.lin3 = c.c03 = c.r_m3 = c.r_34 = 0.0;
         c.r_at = 0.f; c.at_k0 = 0.f; c.at_invw = 0.f;
         // A0 f^(-7/6), A0 = sqrt(5/24) pi^(-2/3) (G Mc/c^3)^(5/6) c / D
-        const double a0 = sqrt(5.0 / 24.0) * pow(PI, -2.0 / 3.0) * pow(mc * AMPLFI_MTSUN, 5.0 / 6.0)
+        const double a0 = 0.45643546458763845 /* sqrt(5/24) */ * 0.46619407703541166 /* pi^(-2/3) */ * pow(mc * AMPLFI_MTSUN, 5.0 / 6.0)
                           * AMPLFI_C_SI / (dist * AMPLFI_MPC);
         c.amp_scale = (float)(a0 * pow(t_seg, 7.0 / 6.0) * amp_mul);
         c.ka1 = 3.0e38f; c.ka2 = 3.0e38f;
@@ -307,9 +309,9 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     // amplitude peak and time alignment
     const double g1 = fit[PD_GAMMA1], g2 = fit[PD_GAMMA2], g3 = fit[PD_GAMMA3];
     const double f_peak = (g2 > 1.0) ? fabs(f_rd - f_dm * g3 / g2)
-                                     : fabs(f_rd + f_dm * (sqrt(1.0 - g2 * g2) - 1.0) * g3 / g2);
+                                     : fabs(f_rd + f_dm * (psqrt(1.0 - g2 * g2) - 1.0) * g3 / g2);
     const double xp = (f_peak - al5 * f_rd) * ifdm;
-    const double t0 = (al1 + al2 / (f_peak * f_peak) + al3 * rsqrt(sqrt(f_peak)) + al4 * ifdm / (1.0 + xp * xp)) * ieta
+    const double t0 = (al1 + al2 / (f_peak * f_peak) + al3 * rsqrt(psqrt(f_peak)) + al4 * ifdm / (1.0 + xp * xp)) * ieta
                       + c2mr;
 
     c.kp1 = f1 * imu;
@@ -333,9 +335,9 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     c.at_invw = (float)(mu * ifdm);
 
     // ---- amplitude ----
-    const double amp0 = 2.0 * sqrt(5.0 / (64.0 * PI)) * mtot * mtot * AMPLFI_MTSUN * (AMPLFI_MTSUN * AMPLFI_C_SI)
+    const double amp0 = 2.0 * 0.15769578262626002 /* sqrt(5 / (64 pi)) */ * mtot * mtot * AMPLFI_MTSUN * (AMPLFI_MTSUN * AMPLFI_C_SI)
                         / (dist * AMPLFI_MPC);
-    c.amp_scale = (float)(amp0 * sqrt(2.0 * eta / 3.0) * 0.8263074871107581 * pexp(-7.0 / 6.0 * lnmu) * amp_mul);   // pi^(-1/6)
+    c.amp_scale = (float)(amp0 * psqrt(2.0 * eta / 3.0) * 0.8263074871107581 * pexp(-7.0 / 6.0 * lnmu) * amp_mul);   // pi^(-1/6)
     const double c12 = chi1 * chi1, c22 = chi2 * chi2;
     double A[7];
     A[2] = (-969.0 + 1804.0 * eta) / 672.0;
