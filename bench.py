@@ -488,6 +488,12 @@ def run_extra(args):
         rows.append(("amplfi_psd_welch average=mean (64 s, 63 segments x 3)", ms, nl, 3 * nb, 4.0 * 3 * nb))
         ms, nl = timed(lambda: A.amplfi_psd_welch(plan, bg, average=1, psd=psd, stream=stream))
         rows.append(("amplfi_psd_welch average=median", ms, nl, 3 * nb, 4.0 * 3 * nb))
+        hp = torch.empty((B, N // 2 + 1, 2), dtype=torch.float32, device=dev)
+        hc = torch.empty_like(hp)
+        fl = torch.empty((B,), dtype=torch.int32, device=dev)
+        ms, nl = timed(lambda: A.amplfi_waveform_fd(plan, A.IMRPHENOMD, params, wl.f_lo, wl.f_hi, hp=hp, hc=hc, flags=fl, stream=stream))
+        rows.append(("amplfi_waveform_fd (IMRPhenomD h+, hx materialised; %.3g waveforms/s; the paper: 1000 in ~0.15 s on an A40, "
+                     "PAPER.md:104)" % (B / (ms * 1e-3)), ms, nl, 2 * B * (N // 2 + 1), 16.0 * B * (N // 2 + 1)))
         for name, ms, nl, samples, alg_bytes in rows:
             print(json.dumps({"metric": "8(f) rows on the c2 workload", "call": name, "ms_per_call": ms, "gpu_launches_per_call": int(nl),
                               "samples_per_s": samples / (ms * 1e-3), "algorithmic_gbs": alg_bytes / (ms * 1e-3) / 1e9,

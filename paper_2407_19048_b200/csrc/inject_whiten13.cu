@@ -280,9 +280,16 @@ __global__ void __launch_bounds__(Geo<LOGM>::T / VT, LOGM == 13 ? 2 : (LOGM == 1
     };
 
     PwOps ops[VT];
-    pw_load(tt, ops[0]);                                     // in flight during the barrier and P3
-    if (fwd) tw_load8(&g_tw13.p3[0][tt & 7], 8, gtw);
+    constexpr bool HOIST = (VIEWS == 1);                     // the two-view variant is short of registers: it requests after the barrier
+    if (HOIST) {
+        pw_load(tt, ops[0]);                                 // in flight during the barrier and P3
+        if (fwd) tw_load8(&g_tw13.p3[0][tt & 7], 8, gtw);
+    }
     __syncthreads();
+    if (!HOIST) {
+        pw_load(tt, ops[0]);
+        if (fwd) tw_load8(&g_tw13.p3[0][tt & 7], 8, gtw);
+    }
     if (fwd) {
 #pragma unroll
         for (int vt = 0; vt < VT; ++vt) p3_fwd(tt + vt * TT, re, im, gtw);
@@ -317,16 +324,17 @@ __global__ void __launch_bounds__(Geo<LOGM>::T / VT, LOGM == 13 ? 2 : (LOGM == 1
                 if (vt + 1 < VT) pw_load(t + TT, ops[vt + 1]);
                 p4_inv<LOGM>(klow_a, klow_b, v, re, im);
             }
-            tw_load8(&g_tw13.p3i[0][tt & 63], 64, gtw);
             __syncthreads();
+            tw_load8(&g_tw13.p3i[0][tt & 63], 64, gtw);
 #pragma unroll
             for (int vt = 0; vt < VT; ++vt) p3_inv(tt + vt * TT, re, im, gtw);
-            C2 tw2[VT][8];
-#pragma unroll
-            for (int vt = 0; vt < VT; ++vt) p2_inv_twiddles<LOGM>(tt + vt * TT, tw2[vt]);
             __syncthreads();
 #pragma unroll
-            for (int vt = 0; vt < VT; ++vt) p2_inv(tt + vt * TT, re, im, tw2[vt]);
+            for (int vt = 0; vt < VT; ++vt) {                // (no hoisting here: this variant is short of registers)
+                C2 tw2[8];
+                p2_inv_twiddles<LOGM>(tt + vt * TT, tw2);
+                p2_inv(tt + vt * TT, re, im, tw2);
+            }
             __syncthreads();
 #pragma unroll
             for (int vt = 0; vt < VT; ++vt) {
