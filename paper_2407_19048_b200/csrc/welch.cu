@@ -90,16 +90,29 @@ __global__ void __launch_bounds__(Fft<LOGM>::T) welch_segment_kernel(const float
 }
 
 // psd[d][k] = c_k * (sum_seg part) / (nseg * fs * sum w^2), c_k = 2 except DC/Nyquist; sum w^2 = 3 NPS / 8.
-__global__ void welch_mean_kernel(const float* __restrict__ part, int nseg, int n_w, float scale,
-                                  float* __restrict__ psd) {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+// Fixed summation order (deterministic): warp j of a CTA sums the segments s = j, j + 8, ... of 32 bins (coalesced 128-byte
+// rows, at most ceil(nseg / 8) dependent loads instead of nseg), then the eight partial sums are added in the order j = 0..7.
+constexpr int MEAN_PARTS = 8;
+__global__ void __launch_bounds__(32 * MEAN_PARTS) welch_mean_kernel(const float* __restrict__ part, int nseg, int n_w,
+                                                                     float scale, float* __restrict__ psd) {
+    __shared__ float partial[MEAN_PARTS][32];
+    const int lane = threadIdx.x & 31, j = threadIdx.x >> 5;
+    const int k = blockIdx.x * 32 + lane;
     const int d = blockIdx.y;
-    if (k >= n_w) return;
-    const float* p = part + (size_t)d * nseg * n_w + k;
     float acc = 0.f;
-    for (int s = 0; s < nseg; ++s) acc += p[(size_t)s * n_w];
-    const float ck = (k == 0 || k == n_w - 1) ? 1.0f : 2.0f;
-    psd[(size_t)d * n_w + k] = acc * scale * ck;
+    if (k < n_w) {
+        const float* p = part + (size_t)d * nseg * n_w + k;
+        for (int s = j; s < nseg; s += MEAN_PARTS) acc += p[(size_t)s * n_w];
+    }
+    partial[j][lane] = acc;
+    __syncthreads();
+    if (j == 0 && k < n_w) {
+        float tot = partial[0][lane];
+#pragma unroll
+        for (int q = 1; q < MEAN_PARTS; ++q) tot += partial[q][lane];
+        const float ck = (k == 0 || k == n_w - 1) ? 1.0f : 2.0f;
+        psd[(size_t)d * n_w + k] = tot * scale * ck;
+    }
 }
 
 // Median over segments: per bin, the middle order statistic of the nseg periodogram values (the
@@ -194,8 +207,8 @@ int launch_welch(const amplfi_plan* p, const float* bg, long n_bg, long row_stri
         return check_launch("welch_median_kernel");
     }
     const float scale = (float)(1.0 / ((double)nseg * p->fs * 0.375 * (double)nps));
-    dim3 grid((n_w + 255) / 256, p->n_det);
-    welch_mean_kernel<<<grid, 256, 0, st>>>(p->welch_part, nseg, n_w, scale, psd);
+    dim3 grid((n_w + 31) / 32, p->n_det);
+    welch_mean_kernel<<<grid, 32 * MEAN_PARTS, 0, st>>>(p->welch_part, nseg, n_w, scale, psd);
     count_launch();
     return check_launch("welch_mean_kernel");
 }
