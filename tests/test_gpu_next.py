@@ -297,3 +297,33 @@ def test_two_plans_side_by_side_and_plan_reuse():
     a3 = run(pa, par16, noise16, s16, 4, A.IMRPHENOMD)          # and back
     torch.cuda.synchronize()
     assert torch.equal(a1, fresh16) and torch.equal(b1, fresh8) and torch.equal(a2, fresh16b) and torch.equal(a3, fresh16)
+
+
+# ------------------------------------------------------------------------------------------ bench.py's own call at full size
+def test_full_size_assemble_batch_and_views_sampled_rows():
+    """BASELINE configs[2] at full size through the call bench.py times (amplfi_assemble_batch: strided background window of
+    the strip, PSD chain on the plan's side stream), plus the two-view call on the same inputs; sampled rows against the
+    oracle, every row finite."""
+    wl = WL.make_c2(batch=2048, strip_len=1 << 24)
+    B = wl.batch
+    plan = A.Plan(wl.n, wl.fs, wl.det_ids, B, nperseg=wl.nperseg)
+    strip = dev(wl.strip)
+    o, nb = wl.extra["bg_offset"], wl.extra["n_bg"]
+    params, offsets = dev(wl.params), dev(wl.offsets)
+    out, psd = A.amplfi_assemble_batch(plan, B, strip[:, o:o + nb], strip, params, wl.f_lo, wl.f_hi, offsets=offsets,
+                                       approximant=wl.approximant, gmst=wl.gmst)
+    t_shift = np.random.Generator(np.random.Philox(3)).uniform(0.0, 1.0, B)
+    v1, v2 = A.amplfi_inject_whiten_views(plan, B, strip, psd, wl.f_lo, wl.f_hi, params, dev(t_shift), offsets=offsets,
+                                          approximant=wl.approximant, gmst=wl.gmst)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(out).all()) and bool(torch.isfinite(v1).all()) and bool(torch.isfinite(v2).all())
+    rows = np.random.default_rng(1).choice(B, size=4, replace=False)
+    psd_ref = OWE.welch(wl.strip[:, o:o + nb].astype(np.float64), wl.fs, wl.nperseg)
+    assert np.abs(psd.cpu().numpy().astype(np.float64) / PSD_SCALE / psd_ref - 1)[:, 41:2001].max() <= TOL
+    noise = OWH.gather(wl.strip, wl.offsets[rows], wl.n)
+    d, d2 = OV.two_views(wl.approximant, wl.params[rows], t_shift[rows], noise, psd_ref, wl.gmst, wl.det_ids, wl.fs,
+                         wl.f_lo, wl.f_hi)
+    idx = torch.from_numpy(rows).to(out.device)
+    assert row_err(out[idx].cpu().numpy().astype(np.float64), d).max() <= TOL
+    assert row_err(v1[idx].cpu().numpy().astype(np.float64), d).max() <= TOL
+    assert row_err(v2[idx].cpu().numpy().astype(np.float64), d2).max() <= TOL
