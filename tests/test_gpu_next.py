@@ -21,7 +21,7 @@ from oracle import whiten as OWH           # noqa: E402
 from test_gpu_parity import TOL, PSD_SCALE, dev, row_err, edge_params      # noqa: E402
 
 
-def _workload(n, fs, batch, dets, seed):
+def _make_inputs(n, fs, batch, dets, seed):
     rng = np.random.Generator(np.random.Philox(seed))
     t_seg = n / fs
     par = WL.draw_params(rng, batch, t_c=(t_seg - 2.5, t_seg - 1.5) if t_seg >= 4 else (0.5 * t_seg, 0.6 * t_seg))
@@ -36,7 +36,7 @@ def _workload(n, fs, batch, dets, seed):
 def test_two_views_parity(n, fs, approx):
     dets = [0, 1, 2]
     batch = 6
-    par, noise, psd = _workload(n, fs, batch, dets, 1000 + n)
+    par, noise, psd = _make_inputs(n, fs, batch, dets, 1000 + n)
     par[0, 4] = 100.0                                         # one very loud signal: phase errors would show
     t_shift = np.array([1.0, 0.0, 0.37, 1.0 / fs, 0.999, 0.5])[:batch]
     plan = A.Plan(n, fs, dets, batch)
@@ -121,7 +121,7 @@ def test_inject_whiten_fir_parity(n, fs, fdur, crop):
         pytest.skip("nothing left after cropping")
     dets = [0, 1]
     batch = 3
-    par, noise, psd = _workload(n, fs, batch, dets, 2000 + n)
+    par, noise, psd = _make_inputs(n, fs, batch, dets, 2000 + n)
     psd = psd * (1.0 + 0.5 * np.sin(np.arange(n // 2 + 1) / 7.0) ** 2)      # a structured PSD: truncation matters
     psd_s = (psd * PSD_SCALE).astype(np.float32)
     plan = A.Plan(n, fs, dets, batch)
@@ -158,7 +158,7 @@ def test_fused_invalid_and_empty_band_rows_inject_nothing(n, fs):
     whitened noise, even when the plan's h0 workspace still holds a previous, loud batch."""
     dets = [0, 1, 2]
     batch = 4
-    par, noise, psd = _workload(n, fs, batch, dets, 3000 + n)
+    par, noise, psd = _make_inputs(n, fs, batch, dets, 3000 + n)
     par[:, 4] = 50.0                                           # loud batch that fills the workspace
     psd_s = dev((psd * PSD_SCALE).astype(np.float32))
     plan = A.Plan(n, fs, dets, batch)
@@ -280,8 +280,8 @@ def test_sine_gaussian_parity(n, fs):
 def test_two_plans_side_by_side_and_plan_reuse():
     """Two plans of different lengths alive at once (they share the packed kernel's twiddle tables), one of them reused for
     another batch size, approximant and mode: results equal those of fresh plans bit for bit."""
-    par16, noise16, psd16 = _workload(16384, 2048.0, 4, [0, 1], 4242)
-    par8, noise8, psd8 = _workload(8192, 2048.0, 3, [0, 1], 4243)
+    par16, noise16, psd16 = _make_inputs(16384, 2048.0, 4, [0, 1], 4242)
+    par8, noise8, psd8 = _make_inputs(8192, 2048.0, 3, [0, 1], 4243)
     s16, s8 = dev((psd16 * PSD_SCALE).astype(np.float32)), dev((psd8 * PSD_SCALE).astype(np.float32))
 
     def run(plan, par, noise, psd_s, batch, approx):
