@@ -40,7 +40,7 @@ def parse():
     ap.add_argument("--cpu-sample", type=int, default=1024, help="samples of the batch the CPU oracle is timed on")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--config", default="c2", choices=["c2", "c3", "c4", "sweep", "next"],
+    ap.add_argument("--config", default="c2", choices=["c0", "c1", "c2", "c3", "c4", "sweep", "next"],
                     help="c2 (default): the contract line.  c3: online latency p50/p99 over --runs seeded runs.  "
                          "c4: bandwidth stress (batch 8192 x 3 x 65536).  sweep: segment length 1-16 s at 4096 Hz.")
     ap.add_argument("--runs", type=int, default=1000)
@@ -438,6 +438,53 @@ def run_extra(args):
                                                      "preceding background (4 s Hann, 50% overlap), IMRPhenomD injection; run r "
                                                      "uses seed 0xA3D30003 + r; CUDA events around one amplfi_assemble_batch "
                                                      "call, inputs resident"}}))
+        return
+
+    if args.config in ("c0", "c1"):
+        # the two small BASELINE configs: device time of one step (c0: fused inject+whiten with the analytic PSD, dense noise;
+        # c1: amplfi_assemble_batch with its own 64 s background), stream launches and a replayed CUDA graph
+        wl = WL.make_c0() if args.config == "c0" else WL.make_c1()
+        B, D, N = wl.batch, wl.n_det, wl.n
+        plan = A.Plan(N, wl.fs, wl.det_ids, B, nperseg=wl.nperseg)
+        noise = torch.from_numpy(wl.noise).to(dev)
+        params = torch.from_numpy(wl.params).to(dev)
+        out = torch.empty((B, D, N), dtype=torch.float32, device=dev)
+        if args.config == "c0":
+            psd = torch.from_numpy(wl.psd_scaled).to(dev)
+
+            def call(st):
+                A.amplfi_inject_whiten(plan, B, noise, psd, wl.f_lo, wl.f_hi, approximant=wl.approximant, params=params,
+                                       gmst=wl.gmst, out=out, stream=st)
+        else:
+            bg = torch.from_numpy(wl.bg).to(dev)
+            psd = torch.empty((D, wl.nperseg // 2 + 1), dtype=torch.float32, device=dev)
+
+            def call(st):
+                A.amplfi_assemble_batch(plan, B, bg, noise, params, wl.f_lo, wl.f_hi, approximant=wl.approximant, gmst=wl.gmst,
+                                        psd=psd, out=out, stream=st)
+        for _ in range(3):
+            call(stream)
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        cs = torch.cuda.Stream()
+        cs.wait_stream(stream)
+        with torch.cuda.graph(graph, stream=cs):
+            call(torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        res = {}
+        for name, fn in (("stream launches", lambda: call(stream)), ("CUDA graph replay", graph.replay)):
+            lat = []
+            for _ in range(args.runs):
+                e0.record(stream); fn(); e1.record(stream)
+                torch.cuda.synchronize()
+                lat.append(e0.elapsed_time(e1) * 1e3)
+            res[name] = np.array(lat)
+        for name, v in res.items():
+            print(json.dumps({"metric": "device time of one step", "unit": "us", "higher_is_better": False, "launch": name,
+                              "p50": float(np.percentile(v, 50)), "p99": float(np.percentile(v, 99)), "runs": len(v),
+                              "samples_per_s_at_p50": B * D * N / (float(np.percentile(v, 50)) * 1e-6), "dtype": "f32",
+                              "data": "synthetic", "config": {"workload": args.config, "batch": B, "n_det": D, "n": N}}))
         return
 
     if args.config == "next":
