@@ -36,6 +36,7 @@ struct amplfi_plan {
                            //                  amplfi_waveform_td ((F+, Fx, dt) = (1,0,0), (0,1,0) per sample)
     float2* h0;            // [max_batch * n_bins]   fused path: 2 fs h0
     float* filt;           // [n_det * filt_stride]  whitening filter incl. 1/(2n); rows padded to 16 B
+    float* filt_slots;     // n = 16384: the same filter in the slot layout of the fused kernel [n_det * 8192] (spec_layout.cuh)
     int filt_stride;       // n_bins rounded up to a multiple of 4
     float* filt_flat;      // [filt_stride] constant 1/(2n): the "no filter" row of the inverse-only launches
     float2* fir_spec;      // [n_det * n_bins]  truncated-filter construction: spectrum-side workspace
@@ -79,7 +80,7 @@ inline int ensure_dynamic_smem(Kernel kernel, int bytes, std::atomic<unsigned>& 
 int launch_prepare(const amplfi_plan* p, int approximant, int batch, const double* params, double gmst,
                    double f_lo, double f_hi, double amp_mul, int* flags, cudaStream_t st);
 int launch_waveform_pol(const amplfi_plan* p, int batch, float* hp, float* hc, cudaStream_t st);
-int launch_waveform_h0(const amplfi_plan* p, int batch, cudaStream_t st);
+int launch_waveform_h0(const amplfi_plan* p, int batch, cudaStream_t st, int slots);   // slots: spec_layout.cuh (n = 16384)
 int launch_project(const amplfi_plan* p, int batch, const float* hp, const float* hc, float* h_det,
                    double* resp_out, cudaStream_t st);
 int launch_tables(amplfi_plan* p, cudaStream_t st);
@@ -101,6 +102,7 @@ struct IwArgs {
     const DetResp* resp;
     const float* filt;        // [D, filt_stride]
     int filt_stride;
+    const float* filt_slots;  // n = 16384: [D, 8192] slot layout (stride 0 when filt_stride is 0); h0 is then in slot layout too
     float* out;               // [B, D, N - 2 crop]
     float* out2;              // packed kernel, two-view launch: second view [B, D, N] (16-byte aligned); else nullptr
     const double* t_shift;    // two-view launch: [B] seconds added to the arrival time in the second view
@@ -116,7 +118,7 @@ struct IwArgs {
 struct IwOpts {
     int n_det;                // units per sample (2 for the polarisations of amplfi_waveform_td, 1 for filter design)
     const DetResp* resp;      // nullptr: plan->resp
-    const float* filt;        // nullptr: plan->filt
+    const float* filt;        // nullptr: plan->filt (a given row must be constant: it is also used as its own slot layout)
     int filt_stride;
     int crop;
     int phase64;
@@ -127,6 +129,10 @@ struct IwOpts {
 // inject_whiten13.cu (packed 4-pass kernel for n = 16384)
 int launch_iw13(const IwArgs& a, int logm /*11, 12 or 13*/, int mode, int units, cudaStream_t st);
 int init_iw13_tables(cudaStream_t st);      // fills the packed kernel's twiddle tables (idempotent; called by plan_create)
+
+// inject_whiten_v3.cu (three-pass cosine-tangent kernel for n = 16384)
+int launch_iw3(const IwArgs& a, int mode, int units, cudaStream_t st);
+int init_iw3_tables(cudaStream_t st);
 
 // inject_whiten.cu
 int launch_filter(const amplfi_plan* p, const float* psd, int n_psd, double f_lo, double f_hi, cudaStream_t st);

@@ -170,6 +170,7 @@ int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_
     if (!rc) rc = dev_alloc(&p->h0, (size_t)max_batch * p->n_bins);
     p->filt_stride = (p->n_bins + 3) & ~3;
     if (!rc) rc = dev_alloc(&p->filt, (size_t)n_det * p->filt_stride);
+    if (!rc && p->logm == 13) rc = dev_alloc(&p->filt_slots, (size_t)n_det * 8192);
     if (!rc) rc = dev_alloc(&p->filt_flat, (size_t)p->filt_stride);
     if (!rc) rc = dev_alloc(&p->fir_spec, (size_t)n_det * p->n_bins);
     if (!rc) rc = dev_alloc(&p->fir_time, (size_t)n_det * n);
@@ -195,6 +196,7 @@ int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_
     }
     if (!rc) rc = launch_tables(p, nullptr);
     if (!rc && p->logm >= 11 && p->logm <= 13) rc = init_iw13_tables(nullptr);
+    if (!rc && p->logm == 13) rc = init_iw3_tables(nullptr);
     if (!rc) {
         fill_kernel<<<(p->filt_stride + 255) / 256, 256>>>(p->filt_flat, p->filt_stride, (float)(1.0 / (2.0 * (double)n)));
         count_launch();
@@ -243,7 +245,7 @@ void amplfi_plan_destroy(amplfi_plan* p) {
     if (p->ev_fork) cudaEventDestroy(p->ev_fork);
     if (p->ev_join) cudaEventDestroy(p->ev_join);
     cudaFree(p->tab_ci); cudaFree(p->tab_lnk); cudaFree(p->pd_table); cudaFree(p->coef); cudaFree(p->resp);
-    cudaFree(p->resp2); cudaFree(p->filt_flat); cudaFree(p->fir_spec); cudaFree(p->fir_time);
+    cudaFree(p->resp2); cudaFree(p->filt_slots); cudaFree(p->filt_flat); cudaFree(p->fir_spec); cudaFree(p->fir_time);
     cudaFree(p->h0); cudaFree(p->filt); cudaFree(p->welch_part); cudaFree(p->d_det_ids); cudaFree(p->long_spec);
     delete p;
 }
@@ -307,7 +309,7 @@ int amplfi_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
     if (fused) {
         rc = launch_prepare(p, approximant, batch, params, gmst, f_lo, f_hi, 2.0 * p->fs, nullptr, st);
         if (rc) return rc;
-        rc = launch_waveform_h0(p, batch, st);
+        rc = launch_waveform_h0(p, batch, st, p->logm == 13);
         if (rc) return rc;
     }
     const bool timed = p->timing && p->ev_count < AMPLFI_TIMING_RING;
@@ -347,7 +349,7 @@ int amplfi_assemble_batch(const amplfi_plan* p, int batch, const float* bg, long
     if (!rc) rc = launch_filter(p, psd, n_psd, f_lo, f_hi, mp->side);
     e = cudaEventRecord(mp->ev_join, mp->side);
     if (!rc) rc = launch_prepare(p, approximant, batch, params, gmst, f_lo, f_hi, 2.0 * p->fs, nullptr, st);
-    if (!rc) rc = launch_waveform_h0(p, batch, st);
+    if (!rc) rc = launch_waveform_h0(p, batch, st, p->logm == 13);
     // join (always, so the side stream never runs past the call unobserved)
     if (e == cudaSuccess) e = cudaStreamWaitEvent(st, mp->ev_join, 0);
     if (e != cudaSuccess) { set_error("amplfi_assemble_batch: join: %s", cudaGetErrorString(e)); return AMPLFI_ERR_CUDA; }
@@ -384,12 +386,14 @@ int amplfi_inject_whiten_views(const amplfi_plan* p, int batch, const float* noi
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     rc = launch_filter(p, psd, n_psd, f_lo, f_hi, st);
     if (!rc) rc = launch_prepare(p, approximant, batch, params, gmst, f_lo, f_hi, 2.0 * p->fs, nullptr, st);
-    if (!rc) rc = launch_waveform_h0(p, batch, st);
+    // n = 4096, 8192, 16384: one launch, one forward transform for both views (inject_whiten13.cu, VIEWS = 2; linear h0)
+    const bool one_launch = p->logm >= 11 && p->logm <= 13 && (reinterpret_cast<size_t>(out2) & 15) == 0;
+    if (!rc) rc = launch_waveform_h0(p, batch, st, p->logm == 13 && !one_launch);
     // both views with the fp64-reduced phase, so that a zero shift reproduces the first view bit for bit
     IwOpts o;
     o.n_det = p->n_det; o.resp = nullptr; o.filt = nullptr; o.filt_stride = 0; o.crop = 0; o.phase64 = 1;
     o.out2 = nullptr; o.t_shift = nullptr;
-    if (!rc && p->logm >= 11 && p->logm <= 13 && (reinterpret_cast<size_t>(out2) & 15) == 0) {
+    if (!rc && one_launch) {
         // n = 16384: one launch, one forward transform for both views (inject_whiten13.cu, VIEWS = 2)
         o.out2 = out2; o.t_shift = t_shift;
         return launch_inject_whiten(p, batch, noise, offsets, strip_len, nullptr, 1, out, st, &o);
@@ -411,7 +415,7 @@ int amplfi_waveform_td(const amplfi_plan* p, int approximant, int batch, const d
     if (reinterpret_cast<size_t>(h_t) & 7) { set_error("amplfi_waveform_td: h_t must be 8-byte aligned"); return AMPLFI_ERR_ALIGNMENT; }
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     rc = launch_prepare(p, approximant, batch, params, 0.0, f_lo, f_hi, 2.0 * p->fs, flags, st);
-    if (!rc) rc = launch_waveform_h0(p, batch, st);
+    if (!rc) rc = launch_waveform_h0(p, batch, st, p->logm == 13);
     if (!rc) rc = launch_td_resp(p, batch, st);
     if (rc) return rc;
     IwOpts o;
@@ -440,7 +444,7 @@ int amplfi_inject_whiten_fir(const amplfi_plan* p, int batch, const float* noise
     if (!rc) rc = launch_fir_truncate(p, fduration, st);
     if (!rc && fused) {
         rc = launch_prepare(p, approximant, batch, params, gmst, f_lo, f_hi, 2.0 * p->fs, nullptr, st);
-        if (!rc) rc = launch_waveform_h0(p, batch, st);
+        if (!rc) rc = launch_waveform_h0(p, batch, st, p->logm == 13);
     }
     if (rc) return rc;
     IwOpts o;

@@ -7,6 +7,7 @@
 // filter and, on the fused path, the per-sample h0 spectrum shared by the detectors of a sample).
 #include "amplfi_internal.h"
 #include "fft_core.cuh"
+#include "spec_layout.cuh"
 #include "waveform.cuh"
 
 namespace amplfi {
@@ -14,7 +15,7 @@ namespace amplfi {
 // ---- whitening filter on the segment grid: w[k] = sqrt(2/(fs S)) / (2N) inside the band, else 0 ----
 // psd holds S * 2^140, so sqrt(2/(fs S)) = 2^70 * rsqrt(fs * psd / 2).
 __global__ void filter_kernel(const float* __restrict__ psd, int n_psd, int n_bins, int ratio, float fs, float norm,
-                              int k_lo, int k_hi, float* __restrict__ filt, int filt_stride) {
+                              int k_lo, int k_hi, float* __restrict__ filt, int filt_stride, float* __restrict__ filt_slots) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     const int d = blockIdx.y;
     if (k >= filt_stride) return;
@@ -33,6 +34,7 @@ __global__ void filter_kernel(const float* __restrict__ psd, int n_psd, int n_bi
         w = rsqrtf(0.5f * fs * sv) * norm;
     }
     filt[(size_t)d * filt_stride + k] = w;
+    if (filt_slots != nullptr && k < slot::M) filt_slots[(size_t)d * slot::FILT_ROW + slot::filt_index(k)] = w;      // n = 16384
 }
 
 int launch_filter(const amplfi_plan* p, const float* psd, int n_psd, double f_lo, double f_hi, cudaStream_t st) {
@@ -48,7 +50,7 @@ int launch_filter(const amplfi_plan* p, const float* psd, int n_psd, double f_lo
     const float norm = (float)(1180591620717411303424.0 / (2.0 * (double)p->n));      // 2^70 / (2N)
     dim3 grid((p->filt_stride + 255) / 256, p->n_det);
     filter_kernel<<<grid, 256, 0, st>>>(psd, n_psd, p->n_bins, ratio, (float)p->fs, norm, (int)k_lo, (int)k_hi, p->filt,
-                                        p->filt_stride);
+                                        p->filt_stride, p->filt_slots);
     count_launch();
     return check_launch("filter_kernel");
 }
@@ -72,11 +74,13 @@ __global__ void fir_real_to_spec_kernel(const float* __restrict__ src, int src_s
 }
 
 __global__ void fir_time_to_filt_kernel(const float* __restrict__ time, int n, int n_bins, float mul, float* __restrict__ filt,
-                                        int filt_stride) {
+                                        int filt_stride, float* __restrict__ filt_slots) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     const int d = blockIdx.y;
     if (k >= filt_stride) return;
-    filt[(size_t)d * filt_stride + k] = k < n_bins ? time[(size_t)d * n + k] * mul : 0.f;
+    const float w = k < n_bins ? time[(size_t)d * n + k] * mul : 0.f;
+    filt[(size_t)d * filt_stride + k] = w;
+    if (filt_slots != nullptr && k < slot::M) filt_slots[(size_t)d * slot::FILT_ROW + slot::filt_index(k)] = w;
 }
 
 // plan->filt (already holding the band-limited filter of launch_filter) is replaced by its time-truncated version.
@@ -99,7 +103,7 @@ int launch_fir_truncate(const amplfi_plan* p, double fduration, cudaStream_t st)
     rc = launch_inject_whiten(p, p->n_det, nullptr, nullptr, 0, reinterpret_cast<const float*>(p->fir_spec), 0, p->fir_time,
                               st, &o);
     if (rc) return rc;
-    fir_time_to_filt_kernel<<<gf, 256, 0, st>>>(p->fir_time, p->n, nb, (float)((double)p->n / p->fs), p->filt, p->filt_stride);
+    fir_time_to_filt_kernel<<<gf, 256, 0, st>>>(p->fir_time, p->n, nb, (float)((double)p->n / p->fs), p->filt, p->filt_stride, p->filt_slots);
     count_launch();
     return check_launch("fir_truncate");
 }
@@ -285,13 +289,14 @@ int launch_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
     a.noise = noise; a.offsets = offsets; a.strip_len = strip_len;
     a.h_det = reinterpret_cast<const float2*>(h_det);
     a.h0 = p->h0; a.coef = p->coef; a.resp = p->resp; a.filt = p->filt; a.filt_stride = p->filt_stride; a.out = out;
+    a.filt_slots = p->filt_slots;
     a.crop = 0; a.phase64 = 0; a.out2 = nullptr; a.t_shift = nullptr;
     a.n_det = p->n_det; a.two_fs = (float)(2.0 * p->fs); a.inv_tseg = (float)(1.0 / p->t_seg);
     a.prefetch_ahead = 2 * p->sm_count;
     if (opts != nullptr) {
         a.n_det = opts->n_det;
         if (opts->resp != nullptr) a.resp = opts->resp;
-        if (opts->filt != nullptr) { a.filt = opts->filt; a.filt_stride = opts->filt_stride; }
+        if (opts->filt != nullptr) { a.filt = opts->filt; a.filt_stride = opts->filt_stride; a.filt_slots = opts->filt; }
         a.crop = opts->crop; a.phase64 = opts->phase64;
         if (p->logm >= 11 && p->logm <= 13) { a.out2 = opts->out2; a.t_shift = opts->t_shift; }
     }
@@ -302,7 +307,7 @@ int launch_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
         case 10: return launch_iw_mode<10>(a, mode, units, st);
         case 11: return launch_iw13(a, 11, mode, units, st);
         case 12: return launch_iw13(a, 12, mode, units, st);
-        case 13: return launch_iw13(a, 13, mode, units, st);
+        case 13: return a.out2 != nullptr ? launch_iw13(a, 13, mode, units, st) : launch_iw3(a, mode, units, st);
         case 14: return launch_iw_mode<14>(a, mode, units, st);
         case 15: case 16: case 17: case 18: case 19: return launch_inject_whiten_long(p, a, mode, units, st);
         default:

@@ -1,0 +1,619 @@
+// inject_whiten_v3.cu -- fused gather -> FFT -> inject -> whiten -> iFFT, third generation (n = 16384; configs c1, c2, c3).
+// PAPER.md:103 (background chunks sliced from the GPU-resident strip), PAPER.md:105 (inject, whiten with the estimated PSD).
+//
+// M = 8192 complex points = 32 * 16 * 16: THREE passes per direction (two shared-memory exchanges instead of three),
+// 256 threads x 32 points, two CTAs per SM.  Every pass is a radix-2 decimation-in-time network whose butterflies carry
+// the inter-pass twiddle in cosine-tangent form (fft_tan.cuh: 6 FMA per butterfly, no separate twiddle multiplication).
+//
+// Index algebra.  n = 256 n1 + 16 n2 + n3,  k = k1 + 32 k2 + 512 k3  (n1, k1 < 32; n2, n3, k2, k3 < 16);
+//   n k / M = n1 k1/32 + n2 k1/512 + n2 k2/16 + n3 (k1 + 32 k2)/8192 + n3 k3/16   (mod 1)
+//   FA  thread j = 16 n2 + n3:     A[k1; j]      = sum_n1 z[256 n1 + j] w32^(n1 k1)            operands from global memory;
+//                                  scalar radix-2 stage (n1, n1 + 16), then lanes (even k1 | odd k1) run one packed DFT16
+//   FB  thread (kap, n3):          B[k1, k2; n3] = sum_n2 A[k1; n2, n3] w512^(n2 k1) w16^(n2 k2)   lanes k1 = 2 kap | 2 kap + 1
+//   FC  thread t: klow = k1 + 32 k2 = t (lane A) and 512 - t (lane B; t = 0: 256):
+//                                  Z[klow + 512 k3] = sum_n3 B[klow; n3] w8192^(n3 klow) w16^(n3 k3)
+//       bins k and M - k meet in one thread (A[k3] <-> B[15 - k3]): split / inject / whiten / merge in registers
+//   I1  same threads:              C[klow; n3]   = sum_k3 Y[klow + 512 k3] w16^(-n3 k3)
+//   I2  thread (kap, n3):          D[k1; n2, n3] = sum_k2 C[k1, k2; n3] w256^(-n3 k2) w16^(-n2 k2)
+//   I3  thread j:                  y[256 n1 + j] = sum_k1 D[k1; j] w8192^(-k1 j) w32^(-n1 k1)   packed DFT16 on the lanes
+//                                  (even k1 | odd k1), scalar last radix-2 stage, natural-order float2 stores
+// Twiddles: FA / I1 exact constants; FB / I2 from two 2 KB tables (fp64-computed); FC / I3 depend on the whole thread index
+// and are evaluated on the fly (fast sincos + reciprocal; every angle lies in [-pi, 0], no range reduction).
+//
+// Shared memory: two float planes, element (d2, n3, k1) at d2*544 + n3*34 + k1 (d2 = n2 or k2).  The row padding 32 -> 34
+// makes the 64-bit (lane A, lane B) accesses of FA/FB/I2/I3 and the 32-bit accesses of FC/I1 bank-conflict free with
+// immediate offsets only (no swizzle arithmetic).  Every pass works in place: 4 barriers per segment.
+#include "amplfi_internal.h"
+#include "fft_tan.cuh"
+#include "spec_layout.cuh"
+#include "waveform.cuh"
+
+namespace amplfi {
+namespace v3 {
+
+using namespace tn;
+
+constexpr int LOGM = 13, M = 8192, N = 16384, K = M + 1, T = 256, KL = 512;
+constexpr int ROW = 34, BLK = 16 * ROW, PLANE = 16 * BLK;        // 544, 8704 floats
+constexpr int SMEM_BYTES = 2 * PLANE * (int)sizeof(float);       // 69632
+
+// FB: per-lane twiddles of W = w512^k1, k1 = 2 kap (lane A), 2 kap + 1 (lane B): (cA, cB, tauA, tauB)
+// I2: shared twiddles of W = w256^n3 (used conjugated): (c, tau)
+struct Tables {
+    float4 fb[16][8];
+    float2 i2[16][8];
+};
+static __device__ Tables g_tab;
+
+__device__ __forceinline__ C2 lds2(const float* re, const float* im, int o) {
+    return C2{*reinterpret_cast<const u64*>(re + o), *reinterpret_cast<const u64*>(im + o)};
+}
+__device__ __forceinline__ void sts2(float* re, float* im, int o, C2 v) {
+    *reinterpret_cast<u64*>(re + o) = v.r;
+    *reinterpret_cast<u64*>(im + o) = v.i;
+}
+
+// theta = -(2 pi / 8192) * (mul * x + off): the eight twiddles of a radix-16 pass with W = w8192^x
+// (fft_tan.cuh: W^8, W^4, W^2, W^2 w8, W w16^q); every exponent stays below 4096 for the callers' x, so theta in [-pi, 0]
+__device__ __forceinline__ void pass_twiddles(float x, Tw1 (&tw)[8]) {
+    constexpr float u = -6.283185307179586f / 8192.0f;
+    tw[0] = tan_twiddle(x * (8.0f * u));
+    tw[1] = tan_twiddle(x * (4.0f * u));
+    tw[2] = tan_twiddle(x * (2.0f * u));
+    tw[3] = tan_twiddle(fmaf(x, 2.0f * u, 1024.0f * u));
+#pragma unroll
+    for (int q = 0; q < 4; ++q) tw[4 + q] = tan_twiddle(fmaf(x, u, 512.0f * q * u));
+}
+
+template <int MODE, bool FWD>
+__global__ void __launch_bounds__(T, 2) inject_whiten3_kernel(const IwArgs a, int units) {
+    extern __shared__ float smem3[];
+    float* re = smem3;
+    float* im = smem3 + PLANE;
+    __shared__ float4 sp[8];          // (S[2w].re, S[2w+1].re, S[2w].im, S[2w+1].im), S[u] = exp(-2 pi i 512 u dt/T)
+    __shared__ float2 s_em;           // exp(-2 pi i M dt/T)
+    __shared__ float2 sc[32];         // the two self-paired butterflies of thread 0
+    const int unit = blockIdx.x, tid = threadIdx.x;
+    const int b = unit / a.n_det, d = unit - b * a.n_det;
+
+    // ---- a-5 gather ----
+    const float* x = nullptr;
+    const int n_out = N - 2 * a.crop;
+    float* out = a.out + (size_t)unit * n_out;
+    if (!FWD) {
+    } else if (a.offsets != nullptr) {
+        const long off = a.offsets[unit];
+        if (off < 0 || off + N > a.strip_len) {            // never read out of bounds: poison the row instead
+            const float qnan = __int_as_float(0x7fc00000);
+            for (int i = tid; i < n_out; i += T) out[i] = qnan;
+            return;
+        }
+        x = a.noise + (size_t)d * a.strip_len + off;
+    } else {
+        x = a.noise + (size_t)unit * N;
+    }
+    // L2 prefetch of the segment a CTA two waves later will gather (one bulk instruction for the whole 64 KB)
+    if (tid == 0 && FWD) {
+        const int nu = unit + a.prefetch_ahead;
+        if (nu < units) {
+            const float* nx;
+            bool ok = true;
+            if (a.offsets != nullptr) {
+                const long noff = a.offsets[nu];
+                ok = noff >= 0 && noff + N <= a.strip_len;
+                nx = a.noise + (size_t)(nu % a.n_det) * a.strip_len + noff;
+            } else {
+                nx = a.noise + (size_t)nu * N;
+            }
+            const size_t p0 = (reinterpret_cast<size_t>(nx) + 15) & ~(size_t)15;      // inside the segment
+            if (ok) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p0), "r"(N * 4 - 16) : "memory");
+        }
+    }
+
+    const int n2 = tid >> 4, n3 = tid & 15;                // FA / I3: j = tid = 16 n2 + n3;  FB / I2: kap = n2
+    const int oj = n2 * BLK + n3 * ROW;                    // FA / I3: element (n2, n3, k1 = 0)
+    const int ob = n3 * ROW + 2 * n2;                      // FB / I2: element (d2 = 0, n3, k1 = 2 kap)
+
+    // ---- FA: radix 32 over n1, operands from global memory ----
+    if (FWD) {
+        float2 z[32];
+        if ((reinterpret_cast<size_t>(x) & 7) == 0) {
+            const float2* x2 = reinterpret_cast<const float2*>(x) + tid;
+#pragma unroll
+            for (int n1 = 0; n1 < 32; ++n1) z[n1] = __ldcs(x2 + n1 * 256);
+        } else {
+#pragma unroll
+            for (int n1 = 0; n1 < 32; ++n1) {
+                const int m = n1 * 256 + tid;
+                z[n1] = make_float2(__ldg(x + 2 * m), __ldg(x + 2 * m + 1));
+            }
+        }
+        C2 v[16];
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            const float2 s = amplfi::cadd(z[r], z[r + 16]);
+            float2 df = amplfi::csub(z[r], z[r + 16]);
+            switch (r) {      // df *= w32^r
+                case 0: break;
+                case 1: df = mul_w32<1, false>(df); break;
+                case 2: df = mul_w32<2, false>(df); break;
+                case 3: df = mul_w32<3, false>(df); break;
+                case 4: df = mul_w32<4, false>(df); break;
+                case 5: df = mul_w32<5, false>(df); break;
+                case 6: df = mul_w32<6, false>(df); break;
+                case 7: df = mul_w32<7, false>(df); break;
+                case 8: df = mul_w32<8, false>(df); break;
+                case 9: df = mul_w32<9, false>(df); break;
+                case 10: df = mul_w32<10, false>(df); break;
+                case 11: df = mul_w32<11, false>(df); break;
+                case 12: df = mul_w32<12, false>(df); break;
+                case 13: df = mul_w32<13, false>(df); break;
+                case 14: df = mul_w32<14, false>(df); break;
+                default: df = mul_w32<15, false>(df); break;
+            }
+            v[brev<16>(r)] = C2{pack(s.x, df.x), pack(s.y, df.y)};
+        }
+        dit16_const<false>(v);
+#pragma unroll
+        for (int kap = 0; kap < 16; ++kap) sts2(re, im, oj + 2 * kap, v[kap]);
+    }
+    // ---- FB: radix 16 over n2 ----
+    if (FWD) {
+        Tw2 tw[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const float4 f = __ldg(&g_tab.fb[n2][i]);
+            tw[i] = Tw2{pack(f.x, f.y), pack(f.z, f.w)};
+        }
+        __syncthreads();
+        C2 v[16];
+#pragma unroll
+        for (int r = 0; r < 16; ++r) v[brev<16>(r)] = lds2(re, im, ob + r * BLK);
+        dit16<false, Tw2, true>(v, tw);                      // k2 >= 8 (the klow >= 256 read by lane B of FC) stored conjugated
+#pragma unroll
+        for (int k2 = 0; k2 < 16; ++k2) sts2(re, im, ob + k2 * BLK, v[k2]);
+    }
+
+    // ---- per-unit constants of the pointwise stage ----
+    const float* hsrc = nullptr;                             // HDET: complex spectrum as floats, re at 2k, im at 2k + 1
+    int w_lo = 0x40000000, w_hi = -1;                        // empty band
+    float cre = 0.f, cim = 0.f;
+    double delta = 0.0;
+    if (MODE == MODE_HDET) hsrc = reinterpret_cast<const float*>(a.h_det + (size_t)unit * K);
+    if (MODE == MODE_FUSED) {
+        const WfCoef* c = a.coef + b;
+        hsrc = reinterpret_cast<const float*>(a.h0) + (size_t)b * slot::H0_ROW;        // slot layout
+        if (c->valid) { w_lo = c->k_lo; w_hi = c->k_hi; }       // an empty band is stored as (2^30, -1) by prepare_kernel
+        const DetResp r = a.resp[unit];
+        cre = (float)r.fp * c->pol_p;                       // C = F+ (1+cos^2 i)/2 - i Fx cos i
+        cim = -(float)r.fc * c->pol_c;
+        delta = r.dt * (double)a.inv_tseg;                   // turns per bin
+    }
+    auto unit_phase = [&](int k) {                           // exp(-2 pi i k delta)
+        float turns;
+        if (a.phase64) { const double xx = (double)k * delta; turns = (float)(xx - rint(xx)); }
+        else { turns = (float)k * (float)delta; turns -= rintf(turns); }
+        float s, co;
+        __sincosf(turns * -6.283185307179586f, &s, &co);
+        return make_float2(co, s);
+    };
+    if (MODE == MODE_FUSED && tid <= 16) {
+        if (tid < 16) {
+            const float2 e = unit_phase(KL * tid);
+            float* spf = reinterpret_cast<float*>(sp);
+            spf[(tid >> 1) * 4 + (tid & 1)] = e.x;
+            spf[(tid >> 1) * 4 + 2 + (tid & 1)] = e.y;
+        } else {
+            s_em = unit_phase(M);
+        }
+    }
+
+    // Operands of the pointwise stage in the slot layout (spec_layout.cuh): pulled into L1 now, a whole pass ahead of
+    // their use, so that the 16-byte requests of the pointwise stage find them there instead of waiting on L2.
+    const int t = tid;
+    unsigned need = 0;                                       // bit w: first h0 slots of unit w needed, bit 8 + w: second
+    if (MODE == MODE_FUSED) {
+        const int l = t & 31;
+        need = __ballot_sync(0xffffffffu, l < 16 && slot::window_needed(l >> 3, l & 7, t >> 5, w_lo, w_hi));
+    }
+    const float4* fsl = reinterpret_cast<const float4*>(a.filt_slots) + (a.filt_stride ? d * (slot::FILT_ROW / 4) : 0) + t;
+    const float4* hsl = reinterpret_cast<const float4*>(a.h0) + (size_t)b * (slot::H0_ROW / 4) + t;
+    if ((t & 7) == 0) {                                      // one request per 128-byte line
+#pragma unroll
+        for (int w = 0; w < 8; ++w) {
+            asm volatile("prefetch.global.L1 [%0];" ::"l"(fsl + w * 256));
+            if (MODE == MODE_FUSED) {
+                if (need & (1u << w)) asm volatile("prefetch.global.L1 [%0];" ::"l"(hsl + w * 256));
+                if (need & (256u << w)) asm volatile("prefetch.global.L1 [%0];" ::"l"(hsl + (8 + w) * 256));
+            }
+        }
+    }
+
+    // ---- FC: radix 16 over n3; lane A klow = t, lane B klow = 512 - t ----
+    const int ka = t, kb = (t == 0) ? KL / 2 : KL - t;
+    const int oa = (ka >> 5) * BLK + (ka & 31), obb = (kb >> 5) * BLK + (kb & 31);
+    // Lane B works on the CONJUGATED column 512 - t (FB stored it so): conj Z[512 - t + 512 q] = sum_n3 conj(B[n3]) W^n3
+    // w16^(-n3 (q + 1)) with lane A's own W = w8192^t, i.e. the same twiddles serve both lanes and lane B's outputs appear
+    // conjugated and reversed: v[q] = (Z[t + 512 q] | conj Z[512 - t + 512 (15 - q)]) -- exactly the partner bin of lane A.
+    // Thread 0's lane B holds the self-paired column 256: its inputs take the factor conj(w32^n3) and its outputs sit at
+    // v[q] = conj Z[256 + 512 ((16 - q) & 15)].
+    C2 v[16];
+    if (FWD) {
+        Tw1 tw[8];
+        pass_twiddles((float)ka, tw);
+        __syncthreads();
+        float xr[16], xi[16];
+#pragma unroll
+        for (int r = 0; r < 16; ++r) { xr[r] = re[obb + r * ROW]; xi[r] = im[obb + r * ROW]; }
+        if (t == 0) {
+#pragma unroll
+            for (int r = 1; r < 16; ++r) {
+                float2 q = make_float2(xr[r], xi[r]);
+                switch (r) {      // q *= conj(w32^r)
+                    case 1: q = mul_w32<1, true>(q); break;
+                    case 2: q = mul_w32<2, true>(q); break;
+                    case 3: q = mul_w32<3, true>(q); break;
+                    case 4: q = mul_w32<4, true>(q); break;
+                    case 5: q = mul_w32<5, true>(q); break;
+                    case 6: q = mul_w32<6, true>(q); break;
+                    case 7: q = mul_w32<7, true>(q); break;
+                    case 8: q = mul_w32<8, true>(q); break;
+                    case 9: q = mul_w32<9, true>(q); break;
+                    case 10: q = mul_w32<10, true>(q); break;
+                    case 11: q = mul_w32<11, true>(q); break;
+                    case 12: q = mul_w32<12, true>(q); break;
+                    case 13: q = mul_w32<13, true>(q); break;
+                    case 14: q = mul_w32<14, true>(q); break;
+                    default: q = mul_w32<15, true>(q); break;
+                }
+                xr[r] = q.x; xi[r] = q.y;
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < 16; ++r) v[brev<16>(r)] = C2{pack(re[oa + r * ROW], xr[r]), pack(im[oa + r * ROW], xi[r])};
+        dit16<false>(v, tw);
+    } else {
+#pragma unroll
+        for (int r = 0; r < 16; ++r) v[r] = C2{0ull, 0ull};
+        __syncthreads();
+    }
+
+    // ---- a-7 inject, a-8 whiten + band-limit ----
+    // v[k3] = (Z[t + 512 k3] | Z[512 - t + 512 k3]) = (A[k3] | B[k3]).  Unit w < 8 (u = 2w) works on the two bin pairs
+    //   lane 0: k0 = t + 512 u <-> M - k0 : (A[u], B[15-u]),      lane 1: k1 = k0 + 512 <-> M - k1 : (A[u+1], B[14-u])
+    // as the two lanes of packed arithmetic; the first and last steps of split/merge are scalar so that operands meet in
+    // the right lanes without moves.  Operands come in the slot layout (spec_layout.cuh): one 16-byte request each for
+    // the four filter values, the two first h0 values and the two second ones, one unit ahead of their use.
+    {
+        // cr/ci[q]: conj B[15 - q] on entry (lane B of FC), B[q] on exit (lane B of I1)
+        float ar[16], ai[16], cr[16], ci[16], br[16], bi[16];
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            unpack(v[q].r, ar[q], cr[q]);
+            unpack(v[q].i, ai[q], ci[q]);
+        }
+        if (t == 0) {
+#pragma unroll
+            for (int q = 0; q < 16; ++q) {
+                sc[q] = make_float2(ar[q], ai[q]);
+                sc[16 + q] = make_float2(cr[(16 - q) & 15], -ci[(16 - q) & 15]);
+            }
+        }
+        const float2 wt = twiddle<N>(t);                     // w_N^t
+        float2 cf = make_float2(0.f, 0.f), cs = make_float2(0.f, 0.f);
+        if (MODE == MODE_FUSED) {
+            const float2 et = unit_phase(t);
+            const float2 cc = make_float2(cre, cim);
+            cf = amplfi::cmul(cc, et);                                        // C e(t)
+            cs = amplfi::cmul_conj(amplfi::cmul(cc, s_em), et);               // C e(M) conj(e(t))
+        }
+        struct PwOps { float4 f, hf, hs; };
+        auto pw_load = [&](int w, PwOps& L) {
+            L.f = __ldg(fsl + w * 256);
+            L.hf = L.hs = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (MODE == MODE_HDET) {
+                const int k0 = t + KL * 2 * w, k1 = k0 + KL;
+                L.hf = make_float4(__ldg(hsrc + 2 * k0), __ldg(hsrc + 2 * k1), __ldg(hsrc + 2 * k0 + 1), __ldg(hsrc + 2 * k1 + 1));
+                L.hs = make_float4(__ldg(hsrc + 2 * (M - k0)), __ldg(hsrc + 2 * (M - k1)), __ldg(hsrc + 2 * (M - k0) + 1),
+                                   __ldg(hsrc + 2 * (M - k1) + 1));
+            } else if (MODE == MODE_FUSED) {
+                if (need & (1u << w)) L.hf = __ldg(hsl + w * 256);
+                if (need & (256u << w)) L.hs = __ldg(hsl + (8 + w) * 256);
+            }
+        };
+        // operands of the self-paired butterflies (processed by lanes 0..16 of warp 0 after the unit loop) into L1
+        const float* sfilt = a.filt + (size_t)d * a.filt_stride;
+        const int sk = t <= 8 ? KL * t : KL / 2 + KL * (t - 9);                // bin of lane t (1 <= t <= 16)
+        if (t >= 1 && t <= 16) {
+            asm volatile("prefetch.global.L1 [%0];" ::"l"(sfilt + sk));
+            asm volatile("prefetch.global.L1 [%0];" ::"l"(sfilt + M - sk));
+            if (MODE == MODE_FUSED) {
+                asm volatile("prefetch.global.L1 [%0];" ::"l"(hsrc + slot::h0_index(sk)));
+                asm volatile("prefetch.global.L1 [%0];" ::"l"(hsrc + slot::h0_index(M - sk)));
+            }
+        }
+        PwOps ops[8];
+        pw_load(0, ops[0]);
+#pragma unroll
+        for (int w8 = 0; w8 < 8; ++w8) {
+            if (w8 + 1 < 8) pw_load(w8 + 1, ops[w8 + 1]);
+            const PwOps& L = ops[w8];
+            const int u = 2 * w8;
+            const u64 ff = pack(L.f.x, L.f.y), fs = pack(L.f.z, L.f.w);
+            // split twiddles (w_N^k0 | w_N^k1) = w_N^t (w32^u | w32^(u+1))
+            const u64 kr = pack(kCos32[u], kCos32[u + 1]), ki = pack(-kSin32[u], -kSin32[u + 1]);
+            C2 w;
+            w.r = fma2(bc(wt.x), kr, neg2(mul2(bc(wt.y), ki)));
+            w.i = fma2(bc(wt.x), ki, mul2(bc(wt.y), kr));
+            // split: e = za + conj(zb), dd = za - conj(zb), wo = (-i dd) w, xa = e + wo, xb = conj(e - wo)
+            const C2 e = C2{pack(ar[u] + cr[u], ar[u + 1] + cr[u + 1]), pack(ai[u] + ci[u], ai[u + 1] + ci[u + 1])};
+            const C2 dd = C2{pack(ar[u] - cr[u], ar[u + 1] - cr[u + 1]), pack(ai[u] - ci[u], ai[u + 1] - ci[u + 1])};
+            const C2 wo = C2{fma2(dd.i, w.r, mul2(dd.r, w.i)), fma2(dd.i, w.i, neg2(mul2(dd.r, w.r)))};
+            C2 xa = C2{add2(e.r, wo.r), add2(e.i, wo.i)};
+            C2 xb = C2{sub2(e.r, wo.r), sub2(wo.i, e.i)};
+            if (MODE == MODE_HDET) {
+                const u64 tf = bc(a.two_fs);
+                xa.r = fma2(tf, pack(L.hf.x, L.hf.y), xa.r);
+                xa.i = fma2(tf, pack(L.hf.z, L.hf.w), xa.i);
+                xb.r = fma2(tf, pack(L.hs.x, L.hs.y), xb.r);
+                xb.i = fma2(tf, pack(L.hs.z, L.hs.w), xb.i);
+            } else if (MODE == MODE_FUSED) {
+                if (need & (0x101u << w8)) {                 // warp-uniform
+                    const float4 s4 = sp[w8];
+                    const C2 spk = C2{pack(s4.x, s4.y), pack(s4.z, s4.w)};
+                    if (need & (1u << w8)) {
+                        const C2 h = C2{pack(L.hf.x, L.hf.y), pack(L.hf.z, L.hf.w)};
+                        // PF = C e(t) (S[u] | S[u+1])
+                        const C2 p = C2{fma2(bc(cf.x), spk.r, neg2(mul2(bc(cf.y), spk.i))), fma2(bc(cf.x), spk.i, mul2(bc(cf.y), spk.r))};
+                        xa.r = fma2(h.r, p.r, fma2(neg2(h.i), p.i, xa.r));
+                        xa.i = fma2(h.r, p.i, fma2(h.i, p.r, xa.i));
+                    }
+                    if (need & (256u << w8)) {
+                        const C2 h = C2{pack(L.hs.x, L.hs.y), pack(L.hs.z, L.hs.w)};
+                        // PS = C e(M) conj(e(t)) conj(S[u] | S[u+1])
+                        const C2 p = C2{fma2(bc(cs.x), spk.r, mul2(bc(cs.y), spk.i)), fma2(bc(cs.y), spk.r, neg2(mul2(bc(cs.x), spk.i)))};
+                        xb.r = fma2(h.r, p.r, fma2(neg2(h.i), p.i, xb.r));
+                        xb.i = fma2(h.r, p.i, fma2(h.i, p.r, xb.i));
+                    }
+                }
+            }
+            xa.r = mul2(xa.r, ff); xa.i = mul2(xa.i, ff);
+            xb.r = mul2(xb.r, fs); xb.i = mul2(xb.i, fs);
+            // merge: e' = ya + conj(yb), d' = ya - conj(yb), o = d' conj(w), za' = e' + i o, zb' = conj(e') + i conj(o)
+            const C2 e2 = C2{add2(xa.r, xb.r), sub2(xa.i, xb.i)};
+            const C2 d2 = C2{sub2(xa.r, xb.r), add2(xa.i, xb.i)};
+            const C2 o = C2{fma2(d2.r, w.r, mul2(d2.i, w.i)), fma2(d2.i, w.r, neg2(mul2(d2.r, w.i)))};
+            float e0r, e1r, e0i, e1i, o0r, o1r, o0i, o1i;
+            unpack(e2.r, e0r, e1r);
+            unpack(e2.i, e0i, e1i);
+            unpack(o.r, o0r, o1r);
+            unpack(o.i, o0i, o1i);
+            // lane 0: za' -> A[u], zb' -> B[15-u];  lane 1: za' -> A[u+1], zb' -> B[14-u]
+            ar[u] = e0r - o0i;      ai[u] = e0i + o0r;      br[15 - u] = e0r + o0i; bi[15 - u] = o0r - e0i;
+            ar[u + 1] = e1r - o1i;  ai[u + 1] = e1i + o1r;  br[14 - u] = e1r + o1i; bi[14 - u] = o1r - e1i;
+        }
+#pragma unroll
+        for (int q = 0; q < 16; ++q) v[q] = C2{pack(ar[q], br[q]), pack(ai[q], bi[q])};
+        // ---- the self-paired butterflies klow = 0 (lane A) and 256 (lane B) of thread 0, on 17 lanes of warp 0 ----
+        // lane 0: Z[0] (DC and Nyquist);  lanes 1..7: (A[l], A[16-l]), k = 512 l;  lane 8: A[8] with itself, k = M/2;
+        // lanes 9..16: (B[q], B[15-q]), q = l - 9, k = 256 + 512 q.  Their operands were pulled into L1 before the unit loop.
+        if (t < 32) {
+            __syncwarp();
+            if (t == 0) {
+                const float2 z0 = sc[0];
+                float x0 = 2.0f * (z0.x + z0.y), xm = 2.0f * (z0.x - z0.y);
+                if (MODE == MODE_HDET) {
+                    x0 = fmaf(a.two_fs, __ldg(hsrc), x0);
+                    xm = fmaf(a.two_fs, __ldg(hsrc + 2 * M), xm);
+                }
+                const float y0 = x0 * __ldg(sfilt), ym = xm * __ldg(sfilt + M);
+                sc[0] = make_float2(y0 + ym, y0 - ym);
+            } else if (t <= 16) {
+                const int ia = t <= 8 ? t : 7 + t, ib = t <= 8 ? 16 - t : 40 - t;
+                const int k = sk;
+                // every operand is requested before the first is used (one L1 round trip)
+                const float fa = __ldg(sfilt + k), fb = __ldg(sfilt + M - k);
+                float2 ha = make_float2(0.f, 0.f), hb = make_float2(0.f, 0.f);
+                bool in_a = false, in_b = false;
+                float cre = 0.f, cim = 0.f;
+                double delta = 0.0;
+                if (MODE == MODE_HDET) {
+                    ha = make_float2(__ldg(hsrc + 2 * k), __ldg(hsrc + 2 * k + 1));
+                    hb = make_float2(__ldg(hsrc + 2 * (M - k)), __ldg(hsrc + 2 * (M - k) + 1));
+                } else if (MODE == MODE_FUSED) {
+                    // (the per-unit constants are fetched again here instead of being kept in registers by every warp)
+                    const WfCoef* c = a.coef + b;
+                    const DetResp r = a.resp[unit];
+                    const int valid = c->valid, k_lo = c->k_lo, k_hi = c->k_hi;
+                    const float pp = c->pol_p, pc = c->pol_c;
+                    const float* hpa = hsrc + slot::h0_index(k);
+                    const float* hpb = hsrc + slot::h0_index(M - k);
+                    ha = make_float2(__ldg(hpa), __ldg(hpa + 2));              // (unwritten slots are read but not used)
+                    hb = make_float2(__ldg(hpb), __ldg(hpb + 2));
+                    in_a = valid && k >= k_lo && k <= k_hi;
+                    in_b = valid && M - k >= k_lo && M - k <= k_hi;
+                    cre = (float)r.fp * pp;
+                    cim = -(float)r.fc * pc;
+                    delta = r.dt * (double)a.inv_tseg;
+                }
+                auto inject = [&](int kk, bool in, float2 h, float2& x2) {
+                    if (MODE == MODE_HDET) {
+                        x2.x = fmaf(a.two_fs, h.x, x2.x);
+                        x2.y = fmaf(a.two_fs, h.y, x2.y);
+                    } else if (MODE == MODE_FUSED) {
+                        if (in) {
+                            double td = (double)kk * delta;
+                            td -= rint(td);
+                            float s, co;
+                            __sincosf((float)td * -6.283185307179586f, &s, &co);      // exp(-2 pi i k dt / T)
+                            const float2 cp = make_float2(cre * co - cim * s, cre * s + cim * co);
+                            x2.x += h.x * cp.x - h.y * cp.y;
+                            x2.y += h.x * cp.y + h.y * cp.x;
+                        }
+                    }
+                };
+                float2 pa = sc[ia], pb = sc[ib];
+                const float2 w = twiddle<N>(k);
+                float2 xa, xb;
+                split_pair(pa, pb, w, xa, xb);
+                inject(k, in_a, ha, xa);
+                inject(M - k, in_b, hb, xb);
+                // (explicitly rounded products: the result must not depend on how a MODE's surrounding code was contracted)
+                xa.x = __fmul_rn(xa.x, fa); xa.y = __fmul_rn(xa.y, fa); xb.x = __fmul_rn(xb.x, fb); xb.y = __fmul_rn(xb.y, fb);
+                merge_pair(xa, xb, w, pa, pb);
+                sc[ia] = pa;
+                if (ib != ia) sc[ib] = pb;
+            }
+            __syncwarp();
+            if (t == 0) {
+#pragma unroll
+                for (int q = 0; q < 16; ++q) {
+                    const float2 pa = sc[q], pb = sc[16 + q];
+                    v[q] = C2{pack(pa.x, pb.x), pack(pa.y, pb.y)};
+                }
+            }
+        }
+    }
+
+    // ---- I1: inverse radix 16 over k3 ----
+    {
+        C2 w[16];
+#pragma unroll
+        for (int r = 0; r < 16; ++r) w[brev<16>(r)] = v[r];
+        dit16_const<true>(w);
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            float ar, br, ai, bi;
+            unpack(w[q].r, ar, br);
+            unpack(w[q].i, ai, bi);
+            re[oa + q * ROW] = ar; im[oa + q * ROW] = ai;
+            re[obb + q * ROW] = br; im[obb + q * ROW] = bi;
+        }
+    }
+    // ---- I2: inverse radix 16 over k2 ----
+    {
+        Tw1 tw[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const float2 f = __ldg(&g_tab.i2[n3][i]);
+            tw[i] = Tw1{f.x, f.y};
+        }
+        __syncthreads();
+        C2 w[16];
+#pragma unroll
+        for (int r = 0; r < 16; ++r) w[brev<16>(r)] = lds2(re, im, ob + r * BLK);
+        dit16<true>(w, tw);
+#pragma unroll
+        for (int q = 0; q < 16; ++q) sts2(re, im, ob + q * BLK, w[q]);
+    }
+    // ---- I3: inverse radix 32 over k1, natural-order stores ----
+    {
+        const float jf = (float)tid;
+        Tw1 tw[8];
+        pass_twiddles(2.0f * jf, tw);                        // base W^2, W = w8192^j
+        __syncthreads();
+        C2 w[16];
+#pragma unroll
+        for (int r = 0; r < 16; ++r) w[brev<16>(r)] = lds2(re, im, oj + 2 * r);
+        dit16<true>(w, tw);
+        float2* out2 = reinterpret_cast<float2*>(out) + tid;
+        constexpr float uu = -6.283185307179586f / 8192.0f;
+        auto last_stage = [&](auto store) {
+#pragma unroll
+            for (int q = 0; q < 16; ++q) {
+                float er, orr, ei, oi;
+                unpack(w[q].r, er, orr);
+                unpack(w[q].i, ei, oi);
+                const Tw1 tq = tan_twiddle(fmaf(jf, uu, 256.0f * (q & 7) * uu));      // W w32^q (the +i of q >= 8 as ROT)
+                float2 lo, hi;
+                if (q < 8) bf_s<true, false>(make_float2(er, ei), make_float2(orr, oi), tq, lo, hi);
+                else bf_s<true, true>(make_float2(er, ei), make_float2(orr, oi), tq, lo, hi);
+                store(q, lo);
+                store(q + 16, hi);
+            }
+        };
+        if (a.crop == 0) {
+            last_stage([&](int n1, float2 val) { __stcs(out2 + n1 * 256, val); });
+        } else {
+            const int c2 = a.crop >> 1;                      // crop is even: whole float2 pairs
+            last_stage([&](int n1, float2 val) {
+                const int m = n1 * 256 + tid;
+                if (m >= c2 && m < M - c2) __stcs(out2 + n1 * 256 - c2, val);
+            });
+        }
+    }
+}
+
+__global__ void init_tables3_kernel() {
+    const int i = threadIdx.x;                                 // 0 .. 127: row = i >> 3, entry = i & 7
+    const int row = i >> 3, ent = i & 7;
+    auto ct = [](int e, float& c, float& tau) {                // (c, tau) of w8192^e, fp64 -> fp32
+        double s, co;
+        sincospi(-2.0 * (double)(e & 8191) / 8192.0, &s, &co);
+        if (fabs(co) < 1e-12) co = 1e-12;
+        c = (float)co;
+        tau = (float)(s / co);
+    };
+    auto expo = [](int x, int ent) {                           // exponent of entry `ent` for W = w8192^x
+        switch (ent) {
+            case 0: return 8 * x;
+            case 1: return 4 * x;
+            case 2: return 2 * x;
+            case 3: return 2 * x + 1024;
+            default: return x + 512 * (ent - 4);
+        }
+    };
+    if (i < 128) {
+        float4 f;
+        ct(expo(16 * (2 * row), ent), f.x, f.z);               // FB lane A: W = w512^(2 kap) = w8192^(32 kap)
+        ct(expo(16 * (2 * row + 1), ent), f.y, f.w);           // lane B: k1 = 2 kap + 1
+        g_tab.fb[row][ent] = f;
+        float2 g;
+        ct(expo(32 * row, ent), g.x, g.y);                     // I2: W = w256^n3 = w8192^(32 n3)
+        g_tab.i2[row][ent] = g;
+    }
+}
+
+}  // namespace v3
+
+// Once per device (amplfi_plan_create synchronises before it returns).
+int init_iw3_tables(cudaStream_t st) {
+    static std::atomic<unsigned> done{0};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    const unsigned bit = 1u << (dev & 31);
+    if (done.load(std::memory_order_acquire) & bit) return AMPLFI_OK;
+    v3::init_tables3_kernel<<<1, 128, 0, st>>>();
+    count_launch();
+    const int rc = check_launch("init_tables3_kernel");
+    if (rc) return rc;
+    if (cudaStreamSynchronize(st) != cudaSuccess) { set_error("init_tables3_kernel: synchronise failed"); return AMPLFI_ERR_CUDA; }
+    done.fetch_or(bit, std::memory_order_release);
+    return AMPLFI_OK;
+}
+
+template <int MODE, bool FWD>
+static int launch_iw3_t(const IwArgs& a, int units, cudaStream_t st) {
+    static std::atomic<unsigned> attr_done{0};
+    const int rc = ensure_dynamic_smem(v3::inject_whiten3_kernel<MODE, FWD>, v3::SMEM_BYTES, attr_done);
+    if (rc) return rc;
+    v3::inject_whiten3_kernel<MODE, FWD><<<units, v3::T, v3::SMEM_BYTES, st>>>(a, units);
+    count_launch();
+    return check_launch("inject_whiten3_kernel");
+}
+
+int launch_iw3(const IwArgs& a, int mode, int units, cudaStream_t st) {
+    if (a.noise == nullptr) {       // inverse-only launches (time-domain waveform, filter design)
+        if (mode == MODE_HDET) return launch_iw3_t<MODE_HDET, false>(a, units, st);
+        if (mode == MODE_FUSED) return launch_iw3_t<MODE_FUSED, false>(a, units, st);
+        set_error("inject_whiten3: no data and nothing to inject");
+        return AMPLFI_ERR_INVALID_ARG;
+    }
+    switch (mode) {
+        case MODE_NONE: return launch_iw3_t<MODE_NONE, true>(a, units, st);
+        case MODE_HDET: return launch_iw3_t<MODE_HDET, true>(a, units, st);
+        default: return launch_iw3_t<MODE_FUSED, true>(a, units, st);
+    }
+}
+
+}  // namespace amplfi

@@ -1,6 +1,7 @@
 // waveform.cu -- per-sample preparation, materialised waveform and projection kernels.
 // PAPER.md:87, :104 (waveform on the GPU), PAPER.md:190 (antenna response on the fly).
 #include "amplfi_internal.h"
+#include "spec_layout.cuh"
 #include "waveform.cuh"
 
 namespace amplfi {
@@ -126,6 +127,63 @@ __global__ void __launch_bounds__(256) sine_gaussian_kernel(const WfCoef* __rest
     }
 }
 
+
+// ---- h0 in the slot layout of the n = 16384 fused kernel (spec_layout.cuh) ----
+// One CTA of 256 threads per (slice, sample); thread t produces whole 16-byte slots, i.e. TWO bins per store, for the
+// groups (second, w) of its warp that slot::window_needed() marks (the consumer skips exactly the others).  The table
+// values of a thread's next slot are requested before the current one is evaluated.
+template <int FAMILY>       // 0: TaylorF2 / IMRPhenomD (power tables), 1: sine-Gaussian (closed form)
+__global__ void __launch_bounds__(256, 2) waveform_slots_kernel(const WfCoef* __restrict__ coef, const double* __restrict__ tab_ci,
+                                                                const double* __restrict__ tab_lnk, float* __restrict__ h0) {
+    const int b = blockIdx.y, t = threadIdx.x, wi = t >> 5;
+    __shared__ WfCoef c;
+    {
+        const int* src = reinterpret_cast<const int*>(coef + b);
+        int* dst = reinterpret_cast<int*>(&c);
+        if (threadIdx.x < (int)(sizeof(WfCoef) / sizeof(int))) dst[threadIdx.x] = src[threadIdx.x];
+    }
+    __syncthreads();
+    if (!c.valid || c.k_lo > c.k_hi) return;
+    const int k_lo = c.k_lo, k_hi = c.k_hi;
+    float4* row = reinterpret_cast<float4*>(h0 + (size_t)b * slot::H0_ROW);
+    // groups g = second * 8 + w, taken round-robin by the slices of a sample
+    auto fetch = [&](int g, int& kA, int& kB, bool& inA, bool& inB, double& ciA, double& lnA, double& ciB, double& lnB) {
+        slot::slot_bins(g >> 3, g & 7, t, kA, kB);
+        inA = kA >= k_lo && kA <= k_hi;
+        inB = kB >= k_lo && kB <= k_hi;
+        ciA = 1.0; lnA = 0.0; ciB = 1.0; lnB = 0.0;
+        if (FAMILY == 0) {
+            if (inA) { ciA = tab_ci[kA]; lnA = tab_lnk[kA]; }
+            if (inB) { ciB = tab_ci[kB]; lnB = tab_lnk[kB]; }
+        }
+    };
+    int g = blockIdx.x;
+    while (g < 16 && !slot::window_needed(g >> 3, g & 7, wi, k_lo, k_hi)) g += gridDim.x;
+    if (g >= 16) return;
+    int kA, kB;
+    bool inA, inB;
+    double ciA, lnA, ciB, lnB;
+    fetch(g, kA, kB, inA, inB, ciA, lnA, ciB, lnB);
+    while (g < 16) {
+        int gn = g + gridDim.x;
+        while (gn < 16 && !slot::window_needed(gn >> 3, gn & 7, wi, k_lo, k_hi)) gn += gridDim.x;
+        int kAn = 0, kBn = 0;
+        bool inAn = false, inBn = false;
+        double ciAn = 1.0, lnAn = 0.0, ciBn = 1.0, lnBn = 0.0;
+        if (gn < 16) fetch(gn, kAn, kBn, inAn, inBn, ciAn, lnAn, ciBn, lnBn);
+        float2 hA = make_float2(0.f, 0.f), hB = make_float2(0.f, 0.f);
+        if (FAMILY == 0) {
+            if (inA) hA = eval_h0(c, kA, ciA, lnA);
+            if (inB) hB = eval_h0(c, kB, ciB, lnB);
+        } else {
+            if (inA) hA = eval_sine_gaussian(c, kA);
+            if (inB) hB = eval_sine_gaussian(c, kB);
+        }
+        row[g * 256 + t] = make_float4(hA.x, hB.x, hA.y, hB.y);
+        g = gn; kA = kAn; kB = kBn; inA = inAn; inB = inBn; ciA = ciAn; lnA = lnAn; ciB = ciBn; lnB = lnBn;
+    }
+}
+
 int launch_waveform_pol(const amplfi_plan* p, int batch, float* hp, float* hc, cudaStream_t st) {
     if (p->last_approx == 2) {
         dim3 g((p->n_bins + 255) / 256, batch);
@@ -141,7 +199,14 @@ int launch_waveform_pol(const amplfi_plan* p, int batch, float* hp, float* hc, c
     return check_launch("waveform_kernel<pol>");
 }
 
-int launch_waveform_h0(const amplfi_plan* p, int batch, cudaStream_t st) {
+int launch_waveform_h0(const amplfi_plan* p, int batch, cudaStream_t st, int slots) {
+    if (slots) {            // slot layout of the n = 16384 fused kernel
+        dim3 grid(WF_SLICES, batch);
+        if (p->last_approx == 2) waveform_slots_kernel<1><<<grid, 256, 0, st>>>(p->coef, p->tab_ci, p->tab_lnk, reinterpret_cast<float*>(p->h0));
+        else waveform_slots_kernel<0><<<grid, 256, 0, st>>>(p->coef, p->tab_ci, p->tab_lnk, reinterpret_cast<float*>(p->h0));
+        count_launch();
+        return check_launch("waveform_slots_kernel");
+    }
     if (p->last_approx == 2) {
         dim3 g((p->n_bins + 255) / 256, batch);
         sine_gaussian_kernel<false><<<g, 256, 0, st>>>(p->coef, p->n_bins, p->h0, nullptr);
