@@ -8,7 +8,7 @@
 // so the inter-pass twiddle costs nothing extra: 32 butterflies x 6 FMA = 12 lane-operations per point and pass against
 // 14.25 for butterflies with exact constants followed by a twiddle multiplication.  Multiplication of T by -i (forward) /
 // +i (inverse) is a relabelling of (u, v).  |c| is kept away from zero by the producers of (c, tau) (tables: fp64, clamped;
-// on the fly: c + 1e-30), the rounding error of c * (tau * x) is that of Im T * x.
+// on the fly: c + 1e-8), the rounding error of c * (tau * x) is that of Im T * x.
 //
 // Lanes: C2{r, i} holds two complex numbers (A.re, B.re), (A.im, B.im) (fft_packed.cuh); a twiddle is either per lane
 // (Tw2: packed c, packed tau) or shared (Tw1: scalars, broadcast by the FFMA2 operand modifier R.F32).

@@ -292,7 +292,7 @@ int launch_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
     a.filt_slots = p->filt_slots;
     a.crop = 0; a.phase64 = 0; a.out2 = nullptr; a.t_shift = nullptr;
     a.n_det = p->n_det; a.two_fs = (float)(2.0 * p->fs); a.inv_tseg = (float)(1.0 / p->t_seg);
-    a.prefetch_ahead = 2 * p->sm_count;
+    a.prefetch_ahead = (p->logm == 13 ? 1 : 2) * p->sm_count;      // measured optimum of each kernel generation
     if (opts != nullptr) {
         a.n_det = opts->n_det;
         if (opts->resp != nullptr) a.resp = opts->resp;

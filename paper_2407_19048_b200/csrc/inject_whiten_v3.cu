@@ -157,23 +157,6 @@ __global__ void __launch_bounds__(T, 2) inject_whiten3_kernel(const IwArgs a, in
 #pragma unroll
         for (int kap = 0; kap < 16; ++kap) sts2(re, im, oj + 2 * kap, v[kap]);
     }
-    // ---- FB: radix 16 over n2 ----
-    if (FWD) {
-        Tw2 tw[8];
-#pragma unroll
-        for (int i = 0; i < 8; ++i) {
-            const float4 f = __ldg(&g_tab.fb[n2][i]);
-            tw[i] = Tw2{pack(f.x, f.y), pack(f.z, f.w)};
-        }
-        __syncthreads();
-        C2 v[16];
-#pragma unroll
-        for (int r = 0; r < 16; ++r) v[brev<16>(r)] = lds2(re, im, ob + r * BLK);
-        dit16<false, Tw2, true>(v, tw);                      // k2 >= 8 (the klow >= 256 read by lane B of FC) stored conjugated
-#pragma unroll
-        for (int k2 = 0; k2 < 16; ++k2) sts2(re, im, ob + k2 * BLK, v[k2]);
-    }
-
     // ---- per-unit constants of the pointwise stage ----
     const float* hsrc = nullptr;                             // HDET: complex spectrum as floats, re at 2k, im at 2k + 1
     int w_lo = 0x40000000, w_hi = -1;                        // empty band
@@ -227,6 +210,23 @@ __global__ void __launch_bounds__(T, 2) inject_whiten3_kernel(const IwArgs a, in
                 if (need & (256u << w)) asm volatile("prefetch.global.L1 [%0];" ::"l"(hsl + (8 + w) * 256));
             }
         }
+    }
+
+    // ---- FB: radix 16 over n2 ----
+    if (FWD) {
+        Tw2 tw[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const float4 f = __ldg(&g_tab.fb[n2][i]);
+            tw[i] = Tw2{pack(f.x, f.y), pack(f.z, f.w)};
+        }
+        __syncthreads();
+        C2 v[16];
+#pragma unroll
+        for (int r = 0; r < 16; ++r) v[brev<16>(r)] = lds2(re, im, ob + r * BLK);
+        dit16<false, Tw2, true>(v, tw);                      // k2 >= 8 (the klow >= 256 read by lane B of FC) stored conjugated
+#pragma unroll
+        for (int k2 = 0; k2 < 16; ++k2) sts2(re, im, ob + k2 * BLK, v[k2]);
     }
 
     // ---- FC: radix 16 over n3; lane A klow = t, lane B klow = 512 - t ----
@@ -321,17 +321,6 @@ __global__ void __launch_bounds__(T, 2) inject_whiten3_kernel(const IwArgs a, in
                 if (need & (256u << w)) L.hs = __ldg(hsl + (8 + w) * 256);
             }
         };
-        // operands of the self-paired butterflies (processed by lanes 0..16 of warp 0 after the unit loop) into L1
-        const float* sfilt = a.filt + (size_t)d * a.filt_stride;
-        const int sk = t <= 8 ? KL * t : KL / 2 + KL * (t - 9);                // bin of lane t (1 <= t <= 16)
-        if (t >= 1 && t <= 16) {
-            asm volatile("prefetch.global.L1 [%0];" ::"l"(sfilt + sk));
-            asm volatile("prefetch.global.L1 [%0];" ::"l"(sfilt + M - sk));
-            if (MODE == MODE_FUSED) {
-                asm volatile("prefetch.global.L1 [%0];" ::"l"(hsrc + slot::h0_index(sk)));
-                asm volatile("prefetch.global.L1 [%0];" ::"l"(hsrc + slot::h0_index(M - sk)));
-            }
-        }
         PwOps ops[8];
         pw_load(0, ops[0]);
 #pragma unroll
@@ -396,9 +385,40 @@ __global__ void __launch_bounds__(T, 2) inject_whiten3_kernel(const IwArgs a, in
         for (int q = 0; q < 16; ++q) v[q] = C2{pack(ar[q], br[q]), pack(ai[q], bi[q])};
         // ---- the self-paired butterflies klow = 0 (lane A) and 256 (lane B) of thread 0, on 17 lanes of warp 0 ----
         // lane 0: Z[0] (DC and Nyquist);  lanes 1..7: (A[l], A[16-l]), k = 512 l;  lane 8: A[8] with itself, k = M/2;
-        // lanes 9..16: (B[q], B[15-q]), q = l - 9, k = 256 + 512 q.  Their operands were pulled into L1 before the unit loop.
+        // lanes 9..16: (B[q], B[15-q]), q = l - 9, k = 256 + 512 q
         if (t < 32) {
             __syncwarp();
+            // (the per-unit constants are fetched again here instead of being kept in registers by every warp)
+            int w_lo = 0x40000000, w_hi = -1;
+            float cre = 0.f, cim = 0.f;
+            double delta = 0.0;
+            if (MODE == MODE_FUSED) {
+                const WfCoef* c = a.coef + b;
+                if (c->valid) { w_lo = c->k_lo; w_hi = c->k_hi; }
+                const DetResp r = a.resp[unit];
+                cre = (float)r.fp * c->pol_p;
+                cim = -(float)r.fc * c->pol_c;
+                delta = r.dt * (double)a.inv_tseg;
+            }
+            const float* filt = a.filt + (size_t)d * a.filt_stride;
+            auto inject = [&](int k, float2& x2) {
+                if (MODE == MODE_HDET) {
+                    x2.x = fmaf(a.two_fs, __ldg(hsrc + 2 * k), x2.x);
+                    x2.y = fmaf(a.two_fs, __ldg(hsrc + 2 * k + 1), x2.y);
+                } else if (MODE == MODE_FUSED) {
+                    if (k >= w_lo && k <= w_hi) {
+                        const float* hp = hsrc + slot::h0_index(k);
+                        const float2 h = make_float2(__ldg(hp), __ldg(hp + 2));
+                        double td = (double)k * delta;
+                        td -= rint(td);
+                        float s, co;
+                        __sincosf((float)td * -6.283185307179586f, &s, &co);      // exp(-2 pi i k dt / T)
+                        const float2 cp = make_float2(cre * co - cim * s, cre * s + cim * co);
+                        x2.x += h.x * cp.x - h.y * cp.y;
+                        x2.y += h.x * cp.y + h.y * cp.x;
+                    }
+                }
+            };
             if (t == 0) {
                 const float2 z0 = sc[0];
                 float x0 = 2.0f * (z0.x + z0.y), xm = 2.0f * (z0.x - z0.y);
@@ -406,58 +426,18 @@ __global__ void __launch_bounds__(T, 2) inject_whiten3_kernel(const IwArgs a, in
                     x0 = fmaf(a.two_fs, __ldg(hsrc), x0);
                     xm = fmaf(a.two_fs, __ldg(hsrc + 2 * M), xm);
                 }
-                const float y0 = x0 * __ldg(sfilt), ym = xm * __ldg(sfilt + M);
+                const float y0 = x0 * __ldg(filt), ym = xm * __ldg(filt + M);
                 sc[0] = make_float2(y0 + ym, y0 - ym);
             } else if (t <= 16) {
                 const int ia = t <= 8 ? t : 7 + t, ib = t <= 8 ? 16 - t : 40 - t;
-                const int k = sk;
-                // every operand is requested before the first is used (one L1 round trip)
-                const float fa = __ldg(sfilt + k), fb = __ldg(sfilt + M - k);
-                float2 ha = make_float2(0.f, 0.f), hb = make_float2(0.f, 0.f);
-                bool in_a = false, in_b = false;
-                float cre = 0.f, cim = 0.f;
-                double delta = 0.0;
-                if (MODE == MODE_HDET) {
-                    ha = make_float2(__ldg(hsrc + 2 * k), __ldg(hsrc + 2 * k + 1));
-                    hb = make_float2(__ldg(hsrc + 2 * (M - k)), __ldg(hsrc + 2 * (M - k) + 1));
-                } else if (MODE == MODE_FUSED) {
-                    // (the per-unit constants are fetched again here instead of being kept in registers by every warp)
-                    const WfCoef* c = a.coef + b;
-                    const DetResp r = a.resp[unit];
-                    const int valid = c->valid, k_lo = c->k_lo, k_hi = c->k_hi;
-                    const float pp = c->pol_p, pc = c->pol_c;
-                    const float* hpa = hsrc + slot::h0_index(k);
-                    const float* hpb = hsrc + slot::h0_index(M - k);
-                    ha = make_float2(__ldg(hpa), __ldg(hpa + 2));              // (unwritten slots are read but not used)
-                    hb = make_float2(__ldg(hpb), __ldg(hpb + 2));
-                    in_a = valid && k >= k_lo && k <= k_hi;
-                    in_b = valid && M - k >= k_lo && M - k <= k_hi;
-                    cre = (float)r.fp * pp;
-                    cim = -(float)r.fc * pc;
-                    delta = r.dt * (double)a.inv_tseg;
-                }
-                auto inject = [&](int kk, bool in, float2 h, float2& x2) {
-                    if (MODE == MODE_HDET) {
-                        x2.x = fmaf(a.two_fs, h.x, x2.x);
-                        x2.y = fmaf(a.two_fs, h.y, x2.y);
-                    } else if (MODE == MODE_FUSED) {
-                        if (in) {
-                            double td = (double)kk * delta;
-                            td -= rint(td);
-                            float s, co;
-                            __sincosf((float)td * -6.283185307179586f, &s, &co);      // exp(-2 pi i k dt / T)
-                            const float2 cp = make_float2(cre * co - cim * s, cre * s + cim * co);
-                            x2.x += h.x * cp.x - h.y * cp.y;
-                            x2.y += h.x * cp.y + h.y * cp.x;
-                        }
-                    }
-                };
+                const int k = t <= 8 ? KL * t : KL / 2 + KL * (t - 9);
                 float2 pa = sc[ia], pb = sc[ib];
                 const float2 w = twiddle<N>(k);
                 float2 xa, xb;
                 split_pair(pa, pb, w, xa, xb);
-                inject(k, in_a, ha, xa);
-                inject(M - k, in_b, hb, xb);
+                inject(k, xa);
+                inject(M - k, xb);
+                const float fa = __ldg(filt + k), fb = __ldg(filt + M - k);
                 // (explicitly rounded products: the result must not depend on how a MODE's surrounding code was contracted)
                 xa.x = __fmul_rn(xa.x, fa); xa.y = __fmul_rn(xa.y, fa); xb.x = __fmul_rn(xb.x, fb); xb.y = __fmul_rn(xb.y, fb);
                 merge_pair(xa, xb, w, pa, pb);
@@ -516,30 +496,26 @@ __global__ void __launch_bounds__(T, 2) inject_whiten3_kernel(const IwArgs a, in
 #pragma unroll
         for (int r = 0; r < 16; ++r) w[brev<16>(r)] = lds2(re, im, oj + 2 * r);
         dit16<true>(w, tw);
-        float2* out2 = reinterpret_cast<float2*>(out) + tid;
+        float2* out2 = reinterpret_cast<float2*>(out);
         constexpr float uu = -6.283185307179586f / 8192.0f;
-        auto last_stage = [&](auto store) {
+        const int c2 = a.crop >> 1;                          // crop is even: whole float2 pairs
 #pragma unroll
-            for (int q = 0; q < 16; ++q) {
-                float er, orr, ei, oi;
-                unpack(w[q].r, er, orr);
-                unpack(w[q].i, ei, oi);
-                const Tw1 tq = tan_twiddle(fmaf(jf, uu, 256.0f * (q & 7) * uu));      // W w32^q (the +i of q >= 8 as ROT)
-                float2 lo, hi;
-                if (q < 8) bf_s<true, false>(make_float2(er, ei), make_float2(orr, oi), tq, lo, hi);
-                else bf_s<true, true>(make_float2(er, ei), make_float2(orr, oi), tq, lo, hi);
-                store(q, lo);
-                store(q + 16, hi);
+        for (int q = 0; q < 16; ++q) {
+            float er, orr, ei, oi;
+            unpack(w[q].r, er, orr);
+            unpack(w[q].i, ei, oi);
+            const Tw1 tq = tan_twiddle(fmaf(jf, uu, 256.0f * (q & 7) * uu));      // W w32^q (the +i of q >= 8 as ROT)
+            float2 lo, hi;
+            if (q < 8) bf_s<true, false>(make_float2(er, ei), make_float2(orr, oi), tq, lo, hi);
+            else bf_s<true, true>(make_float2(er, ei), make_float2(orr, oi), tq, lo, hi);
+            const int m0 = q * 256 + tid, m1 = (q + 16) * 256 + tid;
+            if (a.crop == 0) {
+                __stcs(out2 + m0, lo);
+                __stcs(out2 + m1, hi);
+            } else {
+                if (m0 >= c2 && m0 < M - c2) __stcs(out2 + m0 - c2, lo);
+                if (m1 >= c2 && m1 < M - c2) __stcs(out2 + m1 - c2, hi);
             }
-        };
-        if (a.crop == 0) {
-            last_stage([&](int n1, float2 val) { __stcs(out2 + n1 * 256, val); });
-        } else {
-            const int c2 = a.crop >> 1;                      // crop is even: whole float2 pairs
-            last_stage([&](int n1, float2 val) {
-                const int m = n1 * 256 + tid;
-                if (m >= c2 && m < M - c2) __stcs(out2 + n1 * 256 - c2, val);
-            });
         }
     }
 }
