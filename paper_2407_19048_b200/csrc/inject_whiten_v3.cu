@@ -73,6 +73,7 @@ __global__ void __launch_bounds__(T, 2) inject_whiten3_kernel(const IwArgs a, in
     __shared__ float4 sp[8];          // (S[2w].re, S[2w+1].re, S[2w].im, S[2w+1].im), S[u] = exp(-2 pi i 512 u dt/T)
     __shared__ float2 s_em;           // exp(-2 pi i M dt/T)
     __shared__ float2 sc[32];         // the two self-paired butterflies of thread 0
+    __shared__ float4 sx[17][2];      // their operands, prepared by lanes 0..16 of warp 0 long before they are needed
     const int unit = blockIdx.x, tid = threadIdx.x;
     const int b = unit / a.n_det, d = unit - b * a.n_det;
 
@@ -212,6 +213,31 @@ __global__ void __launch_bounds__(T, 2) inject_whiten3_kernel(const IwArgs a, in
         }
     }
 
+    // Operands of the self-paired butterflies klow = 0 and 256 (thread 0 holds them; lanes 0..16 of warp 0 process their
+    // 17 bin pairs after the unit loop): lane 0: Z[0] (DC and Nyquist); lanes 1..7: k = 512 l; lane 8: k = M/2;
+    // lanes 9..16: k = 256 + 512 (l - 9).  Requested here, turned into (filter values, injected terms, split twiddle)
+    // after pass FB and parked in shared memory, so that nothing in that late section waits on memory.
+    // (prepared by lanes 0..16 of the LAST warp, so that warp 0 does not carry all the extra work of these butterflies)
+    const int sl = t - (T - 32);                             // task index of this thread, valid if 0 <= sl <= 16
+    const int sk = sl <= 0 ? 0 : (sl <= 8 ? KL * sl : KL / 2 + KL * (sl - 9));
+    float sfa = 0.f, sfb = 0.f;
+    float2 sha = make_float2(0.f, 0.f), shb = make_float2(0.f, 0.f);
+    bool sin_a = false, sin_b = false;
+    if (sl >= 0 && sl <= 16) {
+        const float* filt = a.filt + (size_t)d * a.filt_stride;
+        sfa = __ldg(filt + sk);
+        sfb = __ldg(filt + M - sk);
+        if (MODE == MODE_HDET) {
+            sha = make_float2(__ldg(hsrc + 2 * sk), __ldg(hsrc + 2 * sk + 1));
+            shb = make_float2(__ldg(hsrc + 2 * (M - sk)), __ldg(hsrc + 2 * (M - sk) + 1));
+        } else if (MODE == MODE_FUSED && sl != 0) {
+            sin_a = sk >= w_lo && sk <= w_hi;
+            sin_b = M - sk >= w_lo && M - sk <= w_hi;
+            if (sin_a) { const float* hp = hsrc + slot::h0_index(sk); sha = make_float2(__ldg(hp), __ldg(hp + 2)); }
+            if (sin_b) { const float* hp = hsrc + slot::h0_index(M - sk); shb = make_float2(__ldg(hp), __ldg(hp + 2)); }
+        }
+    }
+
     // ---- FB: radix 16 over n2 ----
     if (FWD) {
         Tw2 tw[8];
@@ -225,8 +251,31 @@ __global__ void __launch_bounds__(T, 2) inject_whiten3_kernel(const IwArgs a, in
 #pragma unroll
         for (int r = 0; r < 16; ++r) v[brev<16>(r)] = lds2(re, im, ob + r * BLK);
         dit16<false, Tw2, true>(v, tw);                      // k2 >= 8 (the klow >= 256 read by lane B of FC) stored conjugated
+        if (n2 == 0) {
+            // the self-paired column klow = 256 (k1 = 0, k2 = 8; lane B of thread 0 in FC, whose twiddles are those of
+            // klow = 0, i.e. 1) takes its factor conj(w32^n3) here: one complex product in 16 threads
+            float ar_, br_, ai_, bi_;
+            unpack(v[8].r, ar_, br_);
+            unpack(v[8].i, ai_, bi_);
+            const float co = kCos32[n3], si = kSin32[n3];
+            v[8] = C2{pack(ar_ * co - ai_ * si, br_), pack(ar_ * si + ai_ * co, bi_)};
+        }
 #pragma unroll
         for (int k2 = 0; k2 < 16; ++k2) sts2(re, im, ob + k2 * BLK, v[k2]);
+    }
+    if (sl >= 0 && sl <= 16) {
+        float2 ia = make_float2(0.f, 0.f), ib = make_float2(0.f, 0.f);            // what the injection adds to 2 X[k], 2 X[M-k]
+        if (MODE == MODE_HDET) {
+            ia = make_float2(a.two_fs * sha.x, sl == 0 ? 0.f : a.two_fs * sha.y);
+            ib = make_float2(a.two_fs * shb.x, sl == 0 ? 0.f : a.two_fs * shb.y);
+        } else if (MODE == MODE_FUSED) {
+            const float2 cc = make_float2(cre, cim);
+            if (sin_a) ia = amplfi::cmul(sha, amplfi::cmul(cc, unit_phase(sk)));
+            if (sin_b) ib = amplfi::cmul(shb, amplfi::cmul(cc, unit_phase(M - sk)));
+        }
+        const float2 w = twiddle<N>(sk);
+        sx[sl][0] = make_float4(sfa, sfb, ia.x, ia.y);
+        sx[sl][1] = make_float4(ib.x, ib.y, w.x, w.y);
     }
 
     // ---- FC: radix 16 over n3; lane A klow = t, lane B klow = 512 - t ----
@@ -235,42 +284,16 @@ __global__ void __launch_bounds__(T, 2) inject_whiten3_kernel(const IwArgs a, in
     // Lane B works on the CONJUGATED column 512 - t (FB stored it so): conj Z[512 - t + 512 q] = sum_n3 conj(B[n3]) W^n3
     // w16^(-n3 (q + 1)) with lane A's own W = w8192^t, i.e. the same twiddles serve both lanes and lane B's outputs appear
     // conjugated and reversed: v[q] = (Z[t + 512 q] | conj Z[512 - t + 512 (15 - q)]) -- exactly the partner bin of lane A.
-    // Thread 0's lane B holds the self-paired column 256: its inputs take the factor conj(w32^n3) and its outputs sit at
+    // Thread 0's lane B holds the self-paired column 256: its inputs took the factor conj(w32^n3) in FB and its outputs sit at
     // v[q] = conj Z[256 + 512 ((16 - q) & 15)].
     C2 v[16];
     if (FWD) {
         Tw1 tw[8];
         pass_twiddles((float)ka, tw);
         __syncthreads();
-        float xr[16], xi[16];
 #pragma unroll
-        for (int r = 0; r < 16; ++r) { xr[r] = re[obb + r * ROW]; xi[r] = im[obb + r * ROW]; }
-        if (t == 0) {
-#pragma unroll
-            for (int r = 1; r < 16; ++r) {
-                float2 q = make_float2(xr[r], xi[r]);
-                switch (r) {      // q *= conj(w32^r)
-                    case 1: q = mul_w32<1, true>(q); break;
-                    case 2: q = mul_w32<2, true>(q); break;
-                    case 3: q = mul_w32<3, true>(q); break;
-                    case 4: q = mul_w32<4, true>(q); break;
-                    case 5: q = mul_w32<5, true>(q); break;
-                    case 6: q = mul_w32<6, true>(q); break;
-                    case 7: q = mul_w32<7, true>(q); break;
-                    case 8: q = mul_w32<8, true>(q); break;
-                    case 9: q = mul_w32<9, true>(q); break;
-                    case 10: q = mul_w32<10, true>(q); break;
-                    case 11: q = mul_w32<11, true>(q); break;
-                    case 12: q = mul_w32<12, true>(q); break;
-                    case 13: q = mul_w32<13, true>(q); break;
-                    case 14: q = mul_w32<14, true>(q); break;
-                    default: q = mul_w32<15, true>(q); break;
-                }
-                xr[r] = q.x; xi[r] = q.y;
-            }
-        }
-#pragma unroll
-        for (int r = 0; r < 16; ++r) v[brev<16>(r)] = C2{pack(re[oa + r * ROW], xr[r]), pack(im[oa + r * ROW], xi[r])};
+        for (int r = 0; r < 16; ++r)
+            v[brev<16>(r)] = C2{pack(re[oa + r * ROW], re[obb + r * ROW]), pack(im[oa + r * ROW], im[obb + r * ROW])};
         dit16<false>(v, tw);
     } else {
 #pragma unroll
@@ -384,65 +407,30 @@ __global__ void __launch_bounds__(T, 2) inject_whiten3_kernel(const IwArgs a, in
 #pragma unroll
         for (int q = 0; q < 16; ++q) v[q] = C2{pack(ar[q], br[q]), pack(ai[q], bi[q])};
         // ---- the self-paired butterflies klow = 0 (lane A) and 256 (lane B) of thread 0, on 17 lanes of warp 0 ----
-        // lane 0: Z[0] (DC and Nyquist);  lanes 1..7: (A[l], A[16-l]), k = 512 l;  lane 8: A[8] with itself, k = M/2;
-        // lanes 9..16: (B[q], B[15-q]), q = l - 9, k = 256 + 512 q
+        // lane 0: Z[0];  lanes 1..7: (A[l], A[16-l]);  lane 8: A[8] with itself;  lanes 9..16: (B[q], B[15-q]), q = l - 9;
+        // operands from sx (prepared after pass FB)
         if (t < 32) {
             __syncwarp();
-            // (the per-unit constants are fetched again here instead of being kept in registers by every warp)
-            int w_lo = 0x40000000, w_hi = -1;
-            float cre = 0.f, cim = 0.f;
-            double delta = 0.0;
-            if (MODE == MODE_FUSED) {
-                const WfCoef* c = a.coef + b;
-                if (c->valid) { w_lo = c->k_lo; w_hi = c->k_hi; }
-                const DetResp r = a.resp[unit];
-                cre = (float)r.fp * c->pol_p;
-                cim = -(float)r.fc * c->pol_c;
-                delta = r.dt * (double)a.inv_tseg;
-            }
-            const float* filt = a.filt + (size_t)d * a.filt_stride;
-            auto inject = [&](int k, float2& x2) {
-                if (MODE == MODE_HDET) {
-                    x2.x = fmaf(a.two_fs, __ldg(hsrc + 2 * k), x2.x);
-                    x2.y = fmaf(a.two_fs, __ldg(hsrc + 2 * k + 1), x2.y);
-                } else if (MODE == MODE_FUSED) {
-                    if (k >= w_lo && k <= w_hi) {
-                        const float* hp = hsrc + slot::h0_index(k);
-                        const float2 h = make_float2(__ldg(hp), __ldg(hp + 2));
-                        double td = (double)k * delta;
-                        td -= rint(td);
-                        float s, co;
-                        __sincosf((float)td * -6.283185307179586f, &s, &co);      // exp(-2 pi i k dt / T)
-                        const float2 cp = make_float2(cre * co - cim * s, cre * s + cim * co);
-                        x2.x += h.x * cp.x - h.y * cp.y;
-                        x2.y += h.x * cp.y + h.y * cp.x;
-                    }
+            if (t <= 16) {
+                const float4 s0 = sx[t][0], s1 = sx[t][1];
+                if (t == 0) {       // Z[0] carries the DC and Nyquist bins of the real transform
+                    const float2 z0 = sc[0];
+                    const float x0 = 2.0f * (z0.x + z0.y) + s0.z, xm = 2.0f * (z0.x - z0.y) + s1.x;
+                    const float y0 = x0 * s0.x, ym = xm * s0.y;
+                    sc[0] = make_float2(y0 + ym, y0 - ym);
+                } else {
+                    const int ia = t <= 8 ? t : 7 + t, ib = t <= 8 ? 16 - t : 40 - t;
+                    float2 pa = sc[ia], pb = sc[ib];
+                    const float2 w = make_float2(s1.z, s1.w);
+                    float2 xa, xb;
+                    split_pair(pa, pb, w, xa, xb);
+                    if (MODE != MODE_NONE) { xa.x += s0.z; xa.y += s0.w; xb.x += s1.x; xb.y += s1.y; }
+                    // (explicitly rounded products: the result must not depend on how a MODE's surrounding code was contracted)
+                    xa.x = __fmul_rn(xa.x, s0.x); xa.y = __fmul_rn(xa.y, s0.x); xb.x = __fmul_rn(xb.x, s0.y); xb.y = __fmul_rn(xb.y, s0.y);
+                    merge_pair(xa, xb, w, pa, pb);
+                    sc[ia] = pa;
+                    if (ib != ia) sc[ib] = pb;
                 }
-            };
-            if (t == 0) {
-                const float2 z0 = sc[0];
-                float x0 = 2.0f * (z0.x + z0.y), xm = 2.0f * (z0.x - z0.y);
-                if (MODE == MODE_HDET) {
-                    x0 = fmaf(a.two_fs, __ldg(hsrc), x0);
-                    xm = fmaf(a.two_fs, __ldg(hsrc + 2 * M), xm);
-                }
-                const float y0 = x0 * __ldg(filt), ym = xm * __ldg(filt + M);
-                sc[0] = make_float2(y0 + ym, y0 - ym);
-            } else if (t <= 16) {
-                const int ia = t <= 8 ? t : 7 + t, ib = t <= 8 ? 16 - t : 40 - t;
-                const int k = t <= 8 ? KL * t : KL / 2 + KL * (t - 9);
-                float2 pa = sc[ia], pb = sc[ib];
-                const float2 w = twiddle<N>(k);
-                float2 xa, xb;
-                split_pair(pa, pb, w, xa, xb);
-                inject(k, xa);
-                inject(M - k, xb);
-                const float fa = __ldg(filt + k), fb = __ldg(filt + M - k);
-                // (explicitly rounded products: the result must not depend on how a MODE's surrounding code was contracted)
-                xa.x = __fmul_rn(xa.x, fa); xa.y = __fmul_rn(xa.y, fa); xb.x = __fmul_rn(xb.x, fb); xb.y = __fmul_rn(xb.y, fb);
-                merge_pair(xa, xb, w, pa, pb);
-                sc[ia] = pa;
-                if (ib != ia) sc[ib] = pb;
             }
             __syncwarp();
             if (t == 0) {
