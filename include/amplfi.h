@@ -119,7 +119,9 @@ int amplfi_project(const amplfi_plan* plan, int batch, const double* params, dou
  *   median-to-mean ratio of nseg exponentially distributed values (the middle order statistic of n unit
  *   exponentials has expectation sum_{j=n-k+1}^{n} 1/j; two middle ones averaged for even nseg), which is
  *   robust against loud transients in the background;  psd [n_det, nperseg/2+1] fp32 receives S * 2^140.
- * Deterministic (fixed summation order; ties in the median broken by segment index). */
+ * Deterministic (fixed summation order; ties in the median broken by segment index).  Backgrounds of more than 256
+ * segments (the paper fits the PSD to a quarter-day chunk) are processed in groups of 256 whose sums are
+ * added in order (mean only; the median of more than 256 segments returns AMPLFI_ERR_UNSUPPORTED_SIZE). */
 int amplfi_psd_welch(const amplfi_plan* plan, const float* bg, long n_bg, long row_stride, int noverlap,
                      int detrend, int average, float* psd, void* stream);
 

@@ -102,6 +102,27 @@ def _ptr(t, dtype=None, name="tensor"):
     return ctypes.c_void_p(t.data_ptr())
 
 
+def _need(t, count, name):
+    """The C ABI takes plain pointers: an undersized tensor would be an out-of-bounds device access, so sizes are checked here."""
+    if t is not None and t.numel() < count:
+        raise ValueError("%s holds %d elements, the call needs %d" % (name, t.numel(), count))
+
+
+def _need_iw(plan, batch, noise, offsets, psd, h_det, params, out, n_out=None):
+    nd, n, k = plan.n_det, plan.n, plan.n_bins
+    if offsets is None:
+        _need(noise, batch * nd * n, "noise")
+    else:
+        if noise.dim() != 2 or noise.shape[0] != nd:
+            raise ValueError("with offsets, noise must be the strip [n_det, L]")
+        _need(offsets, batch * nd, "offsets")
+    if psd.dim() != 2 or psd.shape[0] != nd:
+        raise ValueError("psd must be [n_det, n_psd]")
+    _need(h_det, batch * nd * k * 2, "h_det")
+    _need(params, batch * N_PARAMS, "params")
+    _need(out, batch * nd * (n if n_out is None else n_out), "out")
+
+
 def _stream(stream):
     if stream is None:
         stream = torch.cuda.current_stream()
@@ -177,6 +198,8 @@ def amplfi_waveform_fd(plan, approximant, params, f_lo, f_hi, hp=None, hc=None, 
         hc = torch.empty((batch, plan.n_bins, 2), dtype=torch.float32, device=dev)
     if flags is None:
         flags = torch.empty((batch,), dtype=torch.int32, device=dev)
+    _need(params, batch * N_PARAMS, "params"); _need(hp, batch * plan.n_bins * 2, "hp"); _need(hc, batch * plan.n_bins * 2, "hc")
+    _need(flags, batch, "flags")
     _check(_lib.amplfi_waveform_fd(plan._h, int(approximant), int(batch), _ptr(params, torch.float64, "params"),
                                    float(f_lo), float(f_hi), _ptr(hp, torch.float32, "hp"),
                                    _ptr(hc, torch.float32, "hc"), _ptr(flags, torch.int32, "flags"), _stream(stream)))
@@ -191,6 +214,8 @@ def amplfi_project(plan, params, gmst, hp=None, hc=None, h_det=None, resp=None, 
         h_det = torch.empty((batch, plan.n_det, plan.n_bins, 2), dtype=torch.float32, device=dev)
     if want_resp and resp is None:
         resp = torch.empty((batch, plan.n_det, 3), dtype=torch.float64, device=dev)
+    _need(params, batch * N_PARAMS, "params"); _need(hp, batch * plan.n_bins * 2, "hp"); _need(hc, batch * plan.n_bins * 2, "hc")
+    _need(h_det, batch * plan.n_det * plan.n_bins * 2, "h_det"); _need(resp, batch * plan.n_det * 3, "resp")
     _check(_lib.amplfi_project(plan._h, int(batch), _ptr(params, torch.float64, "params"), float(gmst),
                                _ptr(hp, torch.float32, "hp"), _ptr(hc, torch.float32, "hc"),
                                _ptr(h_det, torch.float32, "h_det"), _ptr(resp, torch.float64, "resp"),
@@ -209,6 +234,7 @@ def amplfi_psd_welch(plan, bg, noverlap=None, detrend=1, average=0, psd=None, st
     if not bg.is_cuda or bg.dtype != torch.float32:
         raise TypeError("bg must be a CUDA float32 tensor (no CPU fallback)")
     row_stride = int(bg.stride(0)) if plan.n_det > 1 else int(bg.shape[1])
+    _need(psd, plan.n_det * (plan.nperseg // 2 + 1), "psd")
     _check(_lib.amplfi_psd_welch(plan._h, ctypes.c_void_p(bg.data_ptr()), int(bg.shape[1]), row_stride, int(noverlap), int(detrend),
                                  int(average), _ptr(psd, torch.float32, "psd"), _stream(stream)))
     return psd
@@ -220,6 +246,7 @@ def amplfi_inject_whiten(plan, batch, noise, psd, f_lo, f_hi, offsets=None, h_de
     if out is None:
         out = torch.empty((batch, plan.n_det, plan.n), dtype=torch.float32, device=noise.device)
     strip_len = int(noise.shape[-1]) if offsets is not None else 0
+    _need_iw(plan, batch, noise, offsets, psd, h_det, params, out)
     _check(_lib.amplfi_inject_whiten(plan._h, int(batch), _ptr(noise, torch.float32, "noise"),
                                      _ptr(offsets, torch.int64, "offsets"), strip_len,
                                      _ptr(h_det, torch.float32, "h_det"), int(approximant),
@@ -237,6 +264,8 @@ def amplfi_inject_whiten_views(plan, batch, noise, psd, f_lo, f_hi, params, t_sh
     if out2 is None:
         out2 = torch.empty((batch, plan.n_det, plan.n), dtype=torch.float32, device=noise.device)
     strip_len = int(noise.shape[-1]) if offsets is not None else 0
+    _need_iw(plan, batch, noise, offsets, psd, None, params, out)
+    _need(out2, batch * plan.n_det * plan.n, "out2"); _need(t_shift, batch, "t_shift")
     _check(_lib.amplfi_inject_whiten_views(plan._h, int(batch), _ptr(noise, torch.float32, "noise"),
                                            _ptr(offsets, torch.int64, "offsets"), strip_len, int(approximant),
                                            _ptr(params, torch.float64, "params"), _ptr(t_shift, torch.float64, "t_shift"),
@@ -253,6 +282,7 @@ def amplfi_waveform_td(plan, approximant, params, f_lo, f_hi, h_t=None, flags=No
         h_t = torch.empty((batch, 2, plan.n), dtype=torch.float32, device=params.device)
     if flags is None:
         flags = torch.empty((batch,), dtype=torch.int32, device=params.device)
+    _need(params, batch * N_PARAMS, "params"); _need(h_t, batch * 2 * plan.n, "h_t"); _need(flags, batch, "flags")
     _check(_lib.amplfi_waveform_td(plan._h, int(approximant), int(batch), _ptr(params, torch.float64, "params"), float(f_lo),
                                    float(f_hi), _ptr(h_t, torch.float32, "h_t"), _ptr(flags, torch.int32, "flags"),
                                    _stream(stream)))
@@ -268,6 +298,7 @@ def amplfi_inject_whiten_fir(plan, batch, noise, psd, f_lo, f_hi, fduration, cro
     if out is None:
         out = torch.empty((batch, plan.n_det, n_out), dtype=torch.float32, device=noise.device)
     strip_len = int(noise.shape[-1]) if offsets is not None else 0
+    _need_iw(plan, batch, noise, offsets, psd, h_det, params, out, n_out)
     _check(_lib.amplfi_inject_whiten_fir(plan._h, int(batch), _ptr(noise, torch.float32, "noise"),
                                          _ptr(offsets, torch.int64, "offsets"), strip_len,
                                          _ptr(h_det, torch.float32, "h_det"), int(approximant),
@@ -294,6 +325,7 @@ def amplfi_assemble_batch(plan, batch, bg, noise, params, f_lo, f_hi, offsets=No
         raise TypeError("bg must be a CUDA float32 tensor (no CPU fallback)")
     row_stride = int(bg.stride(0)) if plan.n_det > 1 else int(bg.shape[1])
     strip_len = int(noise.shape[-1]) if offsets is not None else 0
+    _need_iw(plan, batch, noise, offsets, psd, None, params, out)
     _check(_lib.amplfi_assemble_batch(plan._h, int(batch), ctypes.c_void_p(bg.data_ptr()), int(bg.shape[1]), row_stride,
                                       int(noverlap), int(detrend), _ptr(psd, torch.float32, "psd"),
                                       _ptr(noise, torch.float32, "noise"), _ptr(offsets, torch.int64, "offsets"),

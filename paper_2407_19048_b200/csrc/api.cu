@@ -49,7 +49,19 @@ static int dev_alloc(T** ptr, size_t count) {
 
 static bool known_approximant(int a) { return a == AMPLFI_TAYLORF2 || a == AMPLFI_IMRPHENOMD || a == AMPLFI_SINE_GAUSSIAN; }
 
+// a plan's tables and workspaces live on the device it was created on
+static int check_device(const amplfi_plan* p, const char* who) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != p->device) {
+        set_error("%s: the plan belongs to device %d, the current device is %d", who, p->device, dev);
+        return AMPLFI_ERR_INVALID_ARG;
+    }
+    return AMPLFI_OK;
+}
+
 static int validate_band(const amplfi_plan* p, double f_lo, double f_hi, const char* who) {
+    const int rcd = check_device(p, who);
+    if (rcd) return rcd;
     if (!(f_lo >= 0.0) || !(f_hi > f_lo) || !(f_hi <= 0.5 * p->fs)) {
         set_error("%s: need 0 <= f_lo < f_hi <= fs/2 (got %g, %g, fs %g)", who, f_lo, f_hi, p->fs);
         return AMPLFI_ERR_INVALID_ARG;
@@ -268,6 +280,7 @@ int amplfi_project(const amplfi_plan* p, int batch, const double* params, double
                    const float* hc, float* h_det, double* resp, void* stream) {
     if (p == nullptr || params == nullptr) { set_error("amplfi_project: null pointer"); return AMPLFI_ERR_INVALID_ARG; }
     if (batch < 1 || batch > p->max_batch) { set_error("amplfi_project: batch %d outside [1, %d]", batch, p->max_batch); return AMPLFI_ERR_INVALID_ARG; }
+    if (check_device(p, "amplfi_project")) return AMPLFI_ERR_INVALID_ARG;
     const bool any = hp != nullptr || hc != nullptr || h_det != nullptr;
     if (any && (hp == nullptr || hc == nullptr || h_det == nullptr)) { set_error("amplfi_project: hp, hc, h_det must be all given or all NULL"); return AMPLFI_ERR_INVALID_ARG; }
     if (!any && resp == nullptr) { set_error("amplfi_project: nothing to compute"); return AMPLFI_ERR_INVALID_ARG; }
@@ -282,6 +295,7 @@ int amplfi_psd_welch(const amplfi_plan* p, const float* bg, long n_bg, long row_
                      int average, float* psd, void* stream) {
     if (p == nullptr || bg == nullptr || psd == nullptr) { set_error("amplfi_psd_welch: null pointer"); return AMPLFI_ERR_INVALID_ARG; }
     if (p->nperseg == 0) { set_error("amplfi_psd_welch: plan was created with nperseg = 0"); return AMPLFI_ERR_INVALID_ARG; }
+    if (check_device(p, "amplfi_psd_welch")) return AMPLFI_ERR_INVALID_ARG;
     if (n_bg < p->nperseg) { set_error("amplfi_psd_welch: nperseg %d > n_bg %ld", p->nperseg, n_bg); return AMPLFI_ERR_UNSUPPORTED_SIZE; }
     if (noverlap < 0 || noverlap >= p->nperseg || (detrend != 0 && detrend != 1) || (average != 0 && average != 1)) {
         set_error("amplfi_psd_welch: need 0 <= noverlap < nperseg, detrend in {0,1}, average in {0 mean, 1 median}");

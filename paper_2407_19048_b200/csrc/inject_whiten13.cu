@@ -36,6 +36,10 @@ __global__ void __launch_bounds__(Geo<LOGM>::T / VT, LOGM == 13 ? 2 : (LOGM == 1
         if (off < 0 || off + N > a.strip_len) {            // never read out of bounds: poison the row instead
             const float qnan = __int_as_float(0x7fc00000);
             for (int i = tt; i < n_out; i += TT) out[i] = qnan;
+            if constexpr (VIEWS == 2) {                      // the second view's row as well
+                float* o2 = a.out2 + (size_t)unit * N;
+                for (int i = tt; i < N; i += TT) o2[i] = qnan;
+            }
             return;
         }
         x = a.noise + (size_t)d * a.strip_len + off;
@@ -58,8 +62,8 @@ __global__ void __launch_bounds__(Geo<LOGM>::T / VT, LOGM == 13 ? 2 : (LOGM == 1
                 nx = a.noise + (size_t)nu * N;
             }
             if (ok) {
-                const size_t p0 = reinterpret_cast<size_t>(nx) & ~(size_t)15;
-                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p0), "r"(N * 4) : "memory");
+                const size_t p0 = (reinterpret_cast<size_t>(nx) + 15) & ~(size_t)15;      // inside the segment
+                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p0), "r"(N * 4 - 16) : "memory");
             }
         }
     }

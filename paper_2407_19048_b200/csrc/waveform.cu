@@ -129,11 +129,13 @@ __global__ void __launch_bounds__(256) sine_gaussian_kernel(const WfCoef* __rest
 
 
 // ---- h0 in the slot layout of the n = 16384 fused kernel (spec_layout.cuh) ----
-// One CTA of 256 threads per (slice, sample); thread t produces whole 16-byte slots, i.e. TWO bins per store, for the
-// groups (second, w) of its warp that slot::window_needed() marks (the consumer skips exactly the others).  The table
-// values of a thread's next slot are requested before the current one is evaluated.
+// gridDim.x CTAs share one sample and take its 16 slot groups (second, w) round-robin; a warp skips the groups that
+// slot::window_needed() does not mark (the consumer skips exactly those).  Thread t produces whole 16-byte slots: the
+// two bins of a slot are evaluated one after the other by ONE copy of the evaluation code (64 registers, four CTAs per
+// SM: the kernel is bound by the latency of the fp64 phase chain, so resident warps count), the table values of the next
+// bin requested before the current one is evaluated; bins outside the band are written as exact zeros.
 template <int FAMILY>       // 0: TaylorF2 / IMRPhenomD (power tables), 1: sine-Gaussian (closed form)
-__global__ void __launch_bounds__(256, 2) waveform_slots_kernel(const WfCoef* __restrict__ coef, const double* __restrict__ tab_ci,
+__global__ void __launch_bounds__(256, 4) waveform_slots_kernel(const WfCoef* __restrict__ coef, const double* __restrict__ tab_ci,
                                                                 const double* __restrict__ tab_lnk, float* __restrict__ h0) {
     const int b = blockIdx.y, t = threadIdx.x, wi = t >> 5;
     __shared__ WfCoef c;
@@ -146,41 +148,23 @@ __global__ void __launch_bounds__(256, 2) waveform_slots_kernel(const WfCoef* __
     if (!c.valid || c.k_lo > c.k_hi) return;
     const int k_lo = c.k_lo, k_hi = c.k_hi;
     float4* row = reinterpret_cast<float4*>(h0 + (size_t)b * slot::H0_ROW);
-    // groups g = second * 8 + w, taken round-robin by the slices of a sample
-    auto fetch = [&](int g, int& kA, int& kB, bool& inA, bool& inB, double& ciA, double& lnA, double& ciB, double& lnB) {
+#pragma unroll 1
+    for (int g = blockIdx.x; g < 16; g += gridDim.x) {
+        if (!slot::window_needed(g >> 3, g & 7, wi, k_lo, k_hi)) continue;
+        int kA, kB;
         slot::slot_bins(g >> 3, g & 7, t, kA, kB);
-        inA = kA >= k_lo && kA <= k_hi;
-        inB = kB >= k_lo && kB <= k_hi;
-        ciA = 1.0; lnA = 0.0; ciB = 1.0; lnB = 0.0;
-        if (FAMILY == 0) {
-            if (inA) { ciA = tab_ci[kA]; lnA = tab_lnk[kA]; }
-            if (inB) { ciB = tab_ci[kB]; lnB = tab_lnk[kB]; }
-        }
-    };
-    int g = blockIdx.x;
-    while (g < 16 && !slot::window_needed(g >> 3, g & 7, wi, k_lo, k_hi)) g += gridDim.x;
-    if (g >= 16) return;
-    int kA, kB;
-    bool inA, inB;
-    double ciA, lnA, ciB, lnB;
-    fetch(g, kA, kB, inA, inB, ciA, lnA, ciB, lnB);
-    while (g < 16) {
-        int gn = g + gridDim.x;
-        while (gn < 16 && !slot::window_needed(gn >> 3, gn & 7, wi, k_lo, k_hi)) gn += gridDim.x;
-        int kAn = 0, kBn = 0;
-        bool inAn = false, inBn = false;
-        double ciAn = 1.0, lnAn = 0.0, ciBn = 1.0, lnBn = 0.0;
-        if (gn < 16) fetch(gn, kAn, kBn, inAn, inBn, ciAn, lnAn, ciBn, lnBn);
         float2 hA = make_float2(0.f, 0.f), hB = make_float2(0.f, 0.f);
-        if (FAMILY == 0) {
-            if (inA) hA = eval_h0(c, kA, ciA, lnA);
-            if (inB) hB = eval_h0(c, kB, ciB, lnB);
-        } else {
-            if (inA) hA = eval_sine_gaussian(c, kA);
-            if (inB) hB = eval_sine_gaussian(c, kB);
+#pragma unroll 1
+        for (int lane = 0; lane < 2; ++lane) {
+            const int k = lane ? kB : kA;
+            float2 h = make_float2(0.f, 0.f);
+            if (k >= k_lo && k <= k_hi) {
+                if (FAMILY == 0) h = eval_h0(c, k, tab_ci[k], tab_lnk[k]);
+                else h = eval_sine_gaussian(c, k);
+            }
+            if (lane) hB = h; else hA = h;
         }
         row[g * 256 + t] = make_float4(hA.x, hB.x, hA.y, hB.y);
-        g = gn; kA = kAn; kB = kBn; inA = inAn; inB = inBn; ciA = ciAn; lnA = lnAn; ciB = ciBn; lnB = lnBn;
     }
 }
 
@@ -201,7 +185,7 @@ int launch_waveform_pol(const amplfi_plan* p, int batch, float* hp, float* hc, c
 
 int launch_waveform_h0(const amplfi_plan* p, int batch, cudaStream_t st, int slots) {
     if (slots) {            // slot layout of the n = 16384 fused kernel
-        dim3 grid(WF_SLICES, batch);
+        dim3 grid(batch >= 1024 ? 2 : (batch >= 64 ? 4 : 8), batch);
         if (p->last_approx == 2) waveform_slots_kernel<1><<<grid, 256, 0, st>>>(p->coef, p->tab_ci, p->tab_lnk, reinterpret_cast<float*>(p->h0));
         else waveform_slots_kernel<0><<<grid, 256, 0, st>>>(p->coef, p->tab_ci, p->tab_lnk, reinterpret_cast<float*>(p->h0));
         count_launch();

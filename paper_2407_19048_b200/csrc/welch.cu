@@ -94,7 +94,7 @@ __global__ void __launch_bounds__(Fft<LOGM>::T) welch_segment_kernel(const float
 // rows, at most ceil(nseg / 8) dependent loads instead of nseg), then the eight partial sums are added in the order j = 0..7.
 constexpr int MEAN_PARTS = 8;
 __global__ void __launch_bounds__(32 * MEAN_PARTS) welch_mean_kernel(const float* __restrict__ part, int nseg, int n_w,
-                                                                     float scale, float* __restrict__ psd) {
+                                                                     float scale, float* __restrict__ psd, int accumulate) {
     __shared__ float partial[MEAN_PARTS][32];
     const int lane = threadIdx.x & 31, j = threadIdx.x >> 5;
     const int k = blockIdx.x * 32 + lane;
@@ -111,7 +111,8 @@ __global__ void __launch_bounds__(32 * MEAN_PARTS) welch_mean_kernel(const float
 #pragma unroll
         for (int q = 1; q < MEAN_PARTS; ++q) tot += partial[q][lane];
         const float ck = (k == 0 || k == n_w - 1) ? 1.0f : 2.0f;
-        psd[(size_t)d * n_w + k] = tot * scale * ck;
+        // (accumulate: a later group of segments of a long background, added in launch order)
+        psd[(size_t)d * n_w + k] = accumulate ? psd[(size_t)d * n_w + k] + tot * scale * ck : tot * scale * ck;
     }
 }
 
@@ -179,23 +180,40 @@ int launch_welch(const amplfi_plan* p, const float* bg, long n_bg, long row_stri
     const int nps = p->nperseg;
     const int step = nps - noverlap;
     const long nseg_l = (n_bg - nps) / step + 1;
+    const int n_w = nps / 2 + 1;
+    auto segments = [&](const float* base, int nseg) {
+        switch (ilog2(nps) - 1) {
+            case 9: return launch_welch_t<9>(p, base, row_stride, step, nseg, detrend, st);
+            case 10: return launch_welch_t<10>(p, base, row_stride, step, nseg, detrend, st);
+            case 11: return launch_welch_t<11>(p, base, row_stride, step, nseg, detrend, st);
+            case 12: return launch_welch_t<12>(p, base, row_stride, step, nseg, detrend, st);
+            case 13: return launch_welch_t<13>(p, base, row_stride, step, nseg, detrend, st);
+            case 14: return launch_welch_t<14>(p, base, row_stride, step, nseg, detrend, st);
+            default: set_error("amplfi_psd_welch: unsupported nperseg %d", nps); return (int)AMPLFI_ERR_UNSUPPORTED_SIZE;
+        }
+    };
     if (nseg_l > p->welch_max_seg) {
-        set_error("amplfi_psd_welch: %ld segments exceed the plan's workspace (%d)", nseg_l, p->welch_max_seg);
-        return AMPLFI_ERR_UNSUPPORTED_SIZE;
+        // A long background (the PSD is fit to the whole resident chunk, ~20 000 two-second segments for a
+        // quarter day): groups of welch_max_seg segments, their sums added to psd in launch order (still deterministic).
+        if (average == 1) {
+            set_error("amplfi_psd_welch: the median needs all %ld segments at once, the plan's workspace holds %d", nseg_l,
+                      p->welch_max_seg);
+            return AMPLFI_ERR_UNSUPPORTED_SIZE;
+        }
+        const float gscale = (float)(1.0 / ((double)nseg_l * p->fs * 0.375 * (double)nps));
+        dim3 ggrid((n_w + 31) / 32, p->n_det);
+        for (long s0 = 0; s0 < nseg_l; s0 += p->welch_max_seg) {
+            const int ng = (int)(nseg_l - s0 < p->welch_max_seg ? nseg_l - s0 : p->welch_max_seg);
+            const int grc = segments(bg + s0 * step, ng);
+            if (grc) return grc;
+            welch_mean_kernel<<<ggrid, 32 * MEAN_PARTS, 0, st>>>(p->welch_part, ng, n_w, gscale, psd, s0 != 0);
+            count_launch();
+        }
+        return check_launch("welch_mean_kernel");
     }
     const int nseg = (int)nseg_l;
-    int rc;
-    switch (ilog2(nps) - 1) {
-        case 9: rc = launch_welch_t<9>(p, bg, row_stride, step, nseg, detrend, st); break;
-        case 10: rc = launch_welch_t<10>(p, bg, row_stride, step, nseg, detrend, st); break;
-        case 11: rc = launch_welch_t<11>(p, bg, row_stride, step, nseg, detrend, st); break;
-        case 12: rc = launch_welch_t<12>(p, bg, row_stride, step, nseg, detrend, st); break;
-        case 13: rc = launch_welch_t<13>(p, bg, row_stride, step, nseg, detrend, st); break;
-        case 14: rc = launch_welch_t<14>(p, bg, row_stride, step, nseg, detrend, st); break;
-        default: set_error("amplfi_psd_welch: unsupported nperseg %d", nps); return AMPLFI_ERR_UNSUPPORTED_SIZE;
-    }
+    const int rc = segments(bg, nseg);
     if (rc) return rc;
-    const int n_w = nps / 2 + 1;
     if (average == 1) {
         static std::atomic<unsigned> attr_done{0};
         const int arc = ensure_dynamic_smem(welch_median_kernel, (256 + 2) * 64 * (int)sizeof(float), attr_done);
@@ -208,7 +226,7 @@ int launch_welch(const amplfi_plan* p, const float* bg, long n_bg, long row_stri
     }
     const float scale = (float)(1.0 / ((double)nseg * p->fs * 0.375 * (double)nps));
     dim3 grid((n_w + 31) / 32, p->n_det);
-    welch_mean_kernel<<<grid, 32 * MEAN_PARTS, 0, st>>>(p->welch_part, nseg, n_w, scale, psd);
+    welch_mean_kernel<<<grid, 32 * MEAN_PARTS, 0, st>>>(p->welch_part, nseg, n_w, scale, psd, 0);
     count_launch();
     return check_launch("welch_mean_kernel");
 }

@@ -73,6 +73,30 @@ def test_two_views_from_strip_with_offsets():
     assert row_err(out2.cpu().numpy().astype(np.float64), d2).max() <= TOL
 
 
+@pytest.mark.parametrize("n", [4096, 8192, 16384, 2048])
+def test_two_views_out_of_range_offset_poisons_both_views(n):
+    """include/amplfi.h: an out-of-range gather offset gives an all-NaN row -- in BOTH views (the one-launch two-view
+    kernel of n = 4096 .. 16384 and the two-launch path of the other lengths), every other row finite."""
+    fs = 2048.0
+    dets = [0, 1, 2]
+    batch = 4
+    par, _, psd = _make_inputs(n, fs, batch, dets, 7000 + n)
+    rng = np.random.Generator(np.random.Philox(n + 11))
+    strip = WL.coloured_noise(rng, (3,), 1 << 18, fs)
+    offsets = rng.integers(0, strip.shape[1] - n, size=(batch, 3)).astype(np.int64)
+    offsets[1, 0] = strip.shape[1] - n + 1
+    offsets[2, 2] = -1
+    plan = A.Plan(n, fs, dets, batch)
+    out, out2 = A.amplfi_inject_whiten_views(plan, batch, dev(strip), dev((psd * PSD_SCALE).astype(np.float32)), 20.0, 1000.0,
+                                             dev(par), dev(np.full(batch, 0.25)), offsets=dev(offsets))
+    torch.cuda.synchronize()
+    bad = np.zeros((batch, 3), bool)
+    bad[1, 0] = bad[2, 2] = True
+    for o in (out, out2):
+        g = o.cpu().numpy()
+        assert np.all(np.isnan(g[bad])) and np.all(np.isfinite(g[~bad]))
+
+
 # ------------------------------------------------------------------------------------------ time-domain waveform
 @pytest.mark.parametrize("approx", [A.TAYLORF2, A.IMRPHENOMD])
 @pytest.mark.parametrize("n,fs", [(8192, 2048.0), (16384, 2048.0), (65536, 4096.0), (1024, 2048.0), (4096, 2048.0)])

@@ -172,6 +172,25 @@ def test_welch_parity(nperseg, n_bg, fs, detrend):
         assert np.abs(got / ref - 1).max() <= 5e-4
 
 
+def test_welch_long_background_in_groups():
+    """the PSD is fit to the whole resident chunk.  More than 256 segments (the plan's workspace) are
+    processed in groups whose sums are added in order: 700 segments of 1024 samples here, same bar, deterministic."""
+    nperseg, fs = 1024, 2048.0
+    n_bg = nperseg + 699 * (nperseg // 2)
+    rng = np.random.Generator(np.random.Philox(77))
+    bg = WL.coloured_noise(rng, (2,), 1 << 19, fs)[:, :n_bg].copy()
+    plan = A.Plan(1024, fs, [0, 1], 1, nperseg=nperseg)
+    psd = A.amplfi_psd_welch(plan, dev(bg))
+    assert torch.equal(psd, A.amplfi_psd_welch(plan, dev(bg)))
+    ref = OWE.welch(bg.astype(np.float64), fs, nperseg) * PSD_SCALE
+    got = psd.cpu().numpy().astype(np.float64)
+    f = np.arange(nperseg // 2 + 1) * fs / nperseg
+    band = (f >= 20.0) & (f <= 1000.0)
+    assert np.abs(got[:, band] / ref[:, band] - 1).max() <= TOL
+    with pytest.raises(A.AmplfiError):
+        A.amplfi_psd_welch(plan, dev(bg), average=1)          # the median needs every segment at once
+
+
 # ------------------------------------------------------------------------------------------
 # a-5 .. a-9 inject + whiten
 # ------------------------------------------------------------------------------------------
