@@ -40,11 +40,40 @@ def parse():
     ap.add_argument("--cpu-sample", type=int, default=1024, help="samples of the batch the CPU oracle is timed on")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true",
+                    help="skip the other BASELINE configs (c0, c1, c3 over 1000 seeded runs, c4) measured after the timed region")
     ap.add_argument("--config", default="c2", choices=["c0", "c1", "c2", "c3", "c4", "sweep", "next"],
                     help="c2 (default): the contract line.  c3: online latency p50/p99 over --runs seeded runs.  "
                          "c4: bandwidth stress (batch 8192 x 3 x 65536).  sweep: segment length 1-16 s at 4096 Hz.")
     ap.add_argument("--runs", type=int, default=1000)
     return ap.parse_args()
+
+
+KERNEL_SOURCES = ("inject_whiten_v3.cu", "fft_tan.cuh", "fft_packed.cuh", "fft_core.cuh", "spec_layout.cuh")
+
+
+def kernel_source_hash():
+    """sha256 over the sources of the dominant kernel: profiles/kernel_counters.txt records the hash of the build its ncu
+    numbers were captured from, and they are reported only while the sources still match."""
+    import hashlib
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, "paper_2407_19048_b200", "csrc", name), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def kernel_counters():
+    """(dram bytes per launch, fp32 lane-operations per sample, note) from one ncu capture, or (None, None, why)."""
+    path = os.path.join(ROOT, "profiles", "kernel_counters.txt")
+    try:
+        with open(path) as fh:
+            rec = json.load(fh)
+    except Exception:
+        return None, None, "profiles/kernel_counters.txt missing"
+    if rec.get("source_hash") != kernel_source_hash():
+        return None, None, "kernel sources changed since the capture (%s)" % rec.get("capture", "?")
+    return rec.get("dram_bytes_per_launch"), rec.get("fp32_lane_ops_per_sample"), rec.get("capture")
 
 
 def peaks():
@@ -71,24 +100,17 @@ def oracle_step(wl, rows):
     return OWH.inject_whiten(noise, h_det, psd, wl.fs, wl.f_lo, wl.f_hi)
 
 
-def threads_used():
-    try:
-        from threadpoolctl import threadpool_info
-        n = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
-        return int(n)
-    except Exception:
-        return 1
-
-
 def time_oracle(wl, n_rows, steps=1, warmup=0):
+    """-> (samples/s, seconds per step, cores actually used = process CPU time / wall time)."""
     rows = np.arange(n_rows) % wl.batch
     for _ in range(warmup):
         oracle_step(wl, rows)
-    t0 = time.perf_counter()
+    t0, c0 = time.perf_counter(), time.process_time()
     for _ in range(steps):
         oracle_step(wl, rows)
-    dt = (time.perf_counter() - t0) / steps
-    return n_rows * wl.n_det * wl.n / dt, dt
+    wall, cpu = time.perf_counter() - t0, time.process_time() - c0
+    dt = wall / steps
+    return n_rows * wl.n_det * wl.n / dt, dt, round(cpu / wall, 2)
 
 
 def run_reference(args):
@@ -100,16 +122,16 @@ def run_reference(args):
     n_rows = args.cpu_sample
     steps = max(1, min(args.steps, 3))
     warm = min(args.warmup, 1)
-    value, dt = time_oracle(wl, n_rows, steps=steps, warmup=warm)
+    value, dt, cores = time_oracle(wl, n_rows, steps=steps, warmup=warm)
     sample = "%d of 2048 samples (x3 detectors x 16384) + the full 64 s Welch per step; strip shortened to %d" % (
         n_rows, wl.strip.shape[1])
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
             "warmup": warm, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic", "config": {"workload": WORKLOAD, "sample": sample},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads_used(), "kind": "oracle", "sample": sample,
-                             "host_cores": os.cpu_count()},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                             "cores_note": "process CPU time / wall time of the numpy oracle", "host_cores": os.cpu_count()},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-            "gpu_launches": 0}
+            "gpu_launches": 0, "world_size": int(os.environ.get("WORLD_SIZE", "1"))}
     print(json.dumps(line))
 
 
@@ -290,38 +312,42 @@ def run_b200(args):
     peak, peak_src = peaks()
     k_ms = float(np.mean(kernel_ms)) if kernel_ms else None
     alg_bytes = 8.0 * B * D * N
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "ncu_traffic.txt")
-    if os.path.exists(tpath):
-        try:
-            with open(tpath) as fh:
-                traffic = json.load(fh).get("inject_whiten_kernel_dram_bytes_per_launch")
-        except Exception:
-            traffic = None
+    traffic, lane_ops, counters_note = kernel_counters()
     roofline = None
     if k_ms:
         ach = alg_bytes / (k_ms * 1e-3) / 1e9
-        # secondary ceiling: fp32 lane-operations on the FMA pipe, 128 lanes/clk/SM (measured with
-        # FADD2/FFMA2 microbenchmarks); executed fp32 instructions of the kernel from the ncu source page
-        # (profiles/r01_ncu_inject_whiten_v4.md): 69.2 M packed (2 lanes each) + 43.3 M scalar warp-instructions per launch
-        # = 57.8 lane-operations per output sample
+        # secondary ceiling: fp32 lane-operations on the FMA pipe (128 lanes/clk/SM), executed fp32
+        # instructions per output sample from the ncu source page of the captured build (profiles/kernel_counters.txt)
         sm_clk = (clocks or {}).get("sm_mhz") or 1965.0
         try:
             alu_peak, alu_src = A.probe_fp32_pipe() / 1e12, "measured in this run (amplfi_probe_fp32_pipe: packed FMA loop)"
         except Exception:
             alu_peak, alu_src = 148 * 128 * sm_clk * 1e6 / 1e12, "nominal 148 SMs x 128 lanes x SM clock"
-        alu_ach = 57.8 * B * D * N / (k_ms * 1e-3) / 1e12
-        roofline = {"bound": "hbm", "kernel": "inject_whiten13_kernel<fused, VT=2>", "achieved": ach, "peak": peak,
+        alu = None
+        if lane_ops:
+            alu_ach = lane_ops * B * D * N / (k_ms * 1e-3) / 1e12
+            alu = {"bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "T fp32 lane-op/s",
+                   "frac": alu_ach / alu_peak, "lane_ops_per_sample": lane_ops, "sm_mhz": sm_clk, "peak_source": alu_src}
+        roofline = {"bound": "hbm", "kernel": "v3::inject_whiten3_kernel<fused>", "achieved": ach, "peak": peak,
                     "unit": "GB/s", "frac": ach / peak, "frac_of_nominal_8TBps": ach / 8000.0, "peak_source": peak_src,
-                    "traffic": traffic, "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": k_ms,
-                    "kernel_share_of_step": k_ms / ms_per_step, "launches_timed": len(kernel_ms),
-                    "alu": {"bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "T fp32 lane-op/s",
-                            "frac": alu_ach / alu_peak, "lane_ops_per_sample": 57.8, "sm_mhz": sm_clk, "peak_source": alu_src}}
+                    "traffic": traffic, "counters": counters_note, "algorithmic_bytes_per_launch": alg_bytes, "kernel_ms": k_ms,
+                    "kernel_share_of_step": k_ms / ms_per_step, "launches_timed": len(kernel_ms), "alu": alu}
+
+    # ---- the other BASELINE.json configs (configs[0], [1], [3], [4]) in the same run, after the timed region ----
+    other = None
+    if world == 1 and not args.no_other_configs:
+        del out
+        torch.cuda.empty_cache()
+        other = {"c0": measure_small(A, WL, torch, dev, stream, "c0", 200),
+                 "c1": measure_small(A, WL, torch, dev, stream, "c1", 200),
+                 "c3": measure_c3(A, WL, torch, dev, stream, 1000),
+                 "c4": measure_c4(A, WL, torch, dev, stream, 5)}
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        v, dt = time_oracle(wl, args.cpu_sample)
-        cpu = {"value": v, "unit": UNIT, "cores": threads_used(), "host_cores": os.cpu_count(), "kind": "oracle",
+        v, dt, cores = time_oracle(wl, args.cpu_sample)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "cores_note": "process CPU time / wall time of the numpy oracle",
+               "host_cores": os.cpu_count(), "kind": "oracle",
                "seconds": dt, "sample": "%d of %d samples (x%d detectors x %d) + the full 64 s Welch, one pass"
                % (args.cpu_sample, B, D, N)}
 
@@ -330,14 +356,182 @@ def run_b200(args):
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": WORKLOAD, "batch_per_gpu": B, "n_det": D, "n": N, "strip_len": int(wl.strip.shape[1]),
                        "l2_policy": "inputs larger than L2 (random 64 KB gathers from a %.0f MB strip + %.0f MB output per step)"
-                       % (wl.strip.nbytes / 1e6, out.numel() * 4 / 1e6),
+                       % (wl.strip.nbytes / 1e6, B * D * N * 4 / 1e6),
                        "parallelism": "batch sharded, no collective" if world > 1 else "single GPU"},
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu,
-            "hbm_gbs_step": 8.0 * B * D * N / (ms_per_step * 1e-3) / 1e9}
+            "hbm_gbs_step": 8.0 * B * D * N / (ms_per_step * 1e-3) / 1e9, "other_configs": other}
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
 
+
+
+# ------------------------------------------------------------------------------------------------
+# The other BASELINE.json configs as functions (used by --config c0 | c1 | c3 | c4 and by the "other_configs" key of the
+# contract line)
+# ------------------------------------------------------------------------------------------------
+
+C3_WORKLOAD = ("c3 online-latency: batch 1 x H1+L1+V1, 8 s at 2048 Hz, Welch from the 128 s preceding background (4 s Hann, "
+               "50% overlap), IMRPhenomD injection; run r uses seed 0xA3D30003 + r; CUDA events around one "
+               "amplfi_assemble_batch call, inputs resident")
+
+
+def measure_c3(A, WL, torch, dev, stream, runs):
+    """One amplfi_assemble_batch call per candidate, inputs resident; measured both as plain stream launches and as a
+    replayed CUDA graph of the same call (the online service keeps its buffers in place)."""
+    plan = A.Plan(16384, 2048.0, (0, 1, 2), 1, nperseg=8192)
+    bg = torch.empty((3, 262144), dtype=torch.float32, device=dev)
+    noise = torch.empty((1, 3, 16384), dtype=torch.float32, device=dev)
+    params = torch.empty((1, 11), dtype=torch.float64, device=dev)
+    psd = torch.empty((3, 4097), dtype=torch.float32, device=dev)
+    out = torch.empty((1, 3, 16384), dtype=torch.float32, device=dev)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def call(st):
+        A.amplfi_assemble_batch(plan, 1, bg, noise, params, 20.0, 1000.0, approximant=A.IMRPHENOMD, gmst=0.0,
+                                psd=psd, out=out, stream=st)
+
+    # the seeded inputs are synthesised on host threads in blocks of 125 runs BEFORE the block is timed (no host thread runs
+    # beside the timed launches)
+    from concurrent.futures import ThreadPoolExecutor
+    pool = ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1))
+    ready = {}
+
+    def load(r):
+        if r not in ready:
+            ready.clear()
+            block = range(r, min(r + 125, runs))
+            for q, wl in zip(block, pool.map(lambda q: WL.make_c3(run=q), block)):
+                ready[q] = wl
+        wl = ready[r]
+        bg.copy_(torch.from_numpy(wl.bg)); noise.copy_(torch.from_numpy(wl.noise)); params.copy_(torch.from_numpy(wl.params))
+
+    load(0)
+    for _ in range(3):
+        call(stream)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    cs = torch.cuda.Stream()
+    cs.wait_stream(stream)
+    with torch.cuda.graph(graph, stream=cs):
+        call(torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    lat, lat_g = [], []
+    for r in range(runs):
+        load(r)
+        torch.cuda.synchronize()
+        e0.record(stream); call(stream); e1.record(stream)
+        torch.cuda.synchronize()
+        lat.append(e0.elapsed_time(e1) * 1e3)
+        ref = out.clone()
+        e0.record(stream); graph.replay(); e1.record(stream)
+        torch.cuda.synchronize()
+        lat_g.append(e0.elapsed_time(e1) * 1e3)
+        assert torch.equal(ref, out)
+    pool.shutdown(wait=True)
+    res = []
+    for name, v in (("stream launches", np.array(lat)), ("CUDA graph replay", np.array(lat_g))):
+        res.append({"metric": "online PSD+whiten device latency", "unit": "us", "higher_is_better": False,
+                    "launch": name, "p50": float(np.percentile(v, 50)), "p99": float(np.percentile(v, 99)),
+                    "mean": float(v.mean()), "min": float(v.min()), "max": float(v.max()), "runs": len(v),
+                    "dtype": "f32", "data": "synthetic", "config": {"workload": C3_WORKLOAD}})
+    return res
+
+
+def measure_small(A, WL, torch, dev, stream, config, runs):
+    """The two small BASELINE configs: device time of one step (c0: fused inject+whiten with the analytic PSD, dense noise;
+    c1: amplfi_assemble_batch with its own 64 s background), stream launches and a replayed CUDA graph."""
+    wl = WL.make_c0() if config == "c0" else WL.make_c1()
+    B, D, N = wl.batch, wl.n_det, wl.n
+    plan = A.Plan(N, wl.fs, wl.det_ids, B, nperseg=wl.nperseg)
+    noise = torch.from_numpy(wl.noise).to(dev)
+    params = torch.from_numpy(wl.params).to(dev)
+    out = torch.empty((B, D, N), dtype=torch.float32, device=dev)
+    if config == "c0":
+        psd = torch.from_numpy(wl.psd_scaled).to(dev)
+
+        def call(st):
+            A.amplfi_inject_whiten(plan, B, noise, psd, wl.f_lo, wl.f_hi, approximant=wl.approximant, params=params,
+                                   gmst=wl.gmst, out=out, stream=st)
+    else:
+        bg = torch.from_numpy(wl.bg).to(dev)
+        psd = torch.empty((D, wl.nperseg // 2 + 1), dtype=torch.float32, device=dev)
+
+        def call(st):
+            A.amplfi_assemble_batch(plan, B, bg, noise, params, wl.f_lo, wl.f_hi, approximant=wl.approximant, gmst=wl.gmst,
+                                    psd=psd, out=out, stream=st)
+    for _ in range(3):
+        call(stream)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    cs = torch.cuda.Stream()
+    cs.wait_stream(stream)
+    with torch.cuda.graph(graph, stream=cs):
+        call(torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    res = []
+    for name, fn in (("stream launches", lambda: call(stream)), ("CUDA graph replay", graph.replay)):
+        lat = []
+        for _ in range(runs):
+            e0.record(stream); fn(); e1.record(stream)
+            torch.cuda.synchronize()
+            lat.append(e0.elapsed_time(e1) * 1e3)
+        v = np.array(lat)
+        res.append({"metric": "device time of one step", "unit": "us", "higher_is_better": False, "launch": name,
+                    "p50": float(np.percentile(v, 50)), "p99": float(np.percentile(v, 99)), "runs": len(v),
+                    "samples_per_s_at_p50": B * D * N / (float(np.percentile(v, 50)) * 1e-6), "dtype": "f32",
+                    "data": "synthetic", "config": {"workload": config, "batch": B, "n_det": D, "n": N}})
+    return res
+
+
+def measure_throughput(A, torch, dev, stream, wl, steps, warmup):
+    """ms per step, samples/s and launches per step of amplfi_psd_welch + fused amplfi_inject_whiten on a strip workload."""
+    B, D, N = wl.batch, wl.n_det, wl.n
+    plan = A.Plan(N, wl.fs, wl.det_ids, B, nperseg=wl.nperseg)
+    strip = torch.from_numpy(wl.strip).to(dev)
+    params = torch.from_numpy(wl.params).to(dev)
+    offsets = torch.from_numpy(wl.offsets).to(dev)
+    o, nb = wl.extra["bg_offset"], wl.extra["n_bg"]
+    bg = strip[:, o:o + nb]
+    psd = torch.empty((D, wl.nperseg // 2 + 1), dtype=torch.float32, device=dev)
+    out = torch.empty((B, D, N), dtype=torch.float32, device=dev)
+
+    def step():
+        A.amplfi_psd_welch(plan, bg, psd=psd, stream=stream)
+        A.amplfi_inject_whiten(plan, B, strip, psd, wl.f_lo, wl.f_hi, offsets=offsets, approximant=wl.approximant,
+                               params=params, gmst=wl.gmst, out=out, stream=stream)
+    for _ in range(warmup):
+        step()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = A.launch_count()
+    e0.record(stream)
+    for _ in range(steps):
+        step()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    assert bool(torch.isfinite(out[:: max(1, B // 16)]).all())
+    sps = B * D * N / (ms * 1e-3)
+    n_l = (A.launch_count() - l0) // steps
+    del plan, strip, out
+    torch.cuda.empty_cache()
+    return ms, sps, n_l
+
+
+C4_WORKLOAD = ("c4 bandwidth stress: batch 8192 x H1+L1+V1, fs 4096 Hz, 16 s segments (65536), gathered from a [3, 2^26] strip, "
+               "Welch from 128 s (4 s Hann), IMRPhenomD")
+
+
+def measure_c4(A, WL, torch, dev, stream, steps, batch=8192):
+    peak, peak_src = peaks()
+    wl = WL.make_c4(batch=batch)
+    ms, sps, n_l = measure_throughput(A, torch, dev, stream, wl, steps, 3)
+    return {"metric": METRIC.replace("2048 Hz", "4096 Hz"), "value": sps, "unit": UNIT, "ms_per_step": ms,
+            "higher_is_better": True, "dtype": "f32", "data": "synthetic", "gpu_launches_per_step": int(n_l),
+            "hbm_gbs_step": 8.0 * sps / 1e9, "frac_of_measured_hbm": 8.0 * sps / 1e9 / peak, "peak_source": peak_src,
+            "config": {"workload": C4_WORKLOAD, "batch": batch}}
 
 # ------------------------------------------------------------------------------------------------
 # Other BASELINE.json configs (SURVEY.md 8(d)): not the contract line; one JSON line per measurement
@@ -355,136 +549,16 @@ def run_extra(args):
     peak, peak_src = peaks()
 
     def throughput(wl, steps, warmup):
-        B, D, N = wl.batch, wl.n_det, wl.n
-        plan = A.Plan(N, wl.fs, wl.det_ids, B, nperseg=wl.nperseg)
-        strip = torch.from_numpy(wl.strip).to(dev)
-        params = torch.from_numpy(wl.params).to(dev)
-        offsets = torch.from_numpy(wl.offsets).to(dev)
-        o, nb = wl.extra["bg_offset"], wl.extra["n_bg"]
-        bg = strip[:, o:o + nb]
-        psd = torch.empty((D, wl.nperseg // 2 + 1), dtype=torch.float32, device=dev)
-        out = torch.empty((B, D, N), dtype=torch.float32, device=dev)
-
-        def step():
-            A.amplfi_psd_welch(plan, bg, psd=psd, stream=stream)
-            A.amplfi_inject_whiten(plan, B, strip, psd, wl.f_lo, wl.f_hi, offsets=offsets, approximant=wl.approximant,
-                                   params=params, gmst=wl.gmst, out=out, stream=stream)
-        for _ in range(warmup):
-            step()
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        l0 = A.launch_count()
-        e0.record(stream)
-        for _ in range(steps):
-            step()
-        e1.record(stream)
-        torch.cuda.synchronize()
-        ms = e0.elapsed_time(e1) / steps
-        assert bool(torch.isfinite(out[:: max(1, B // 16)]).all())
-        sps = B * D * N / (ms * 1e-3)
-        n_l = (A.launch_count() - l0) // steps
-        del plan, strip, out
-        torch.cuda.empty_cache()
-        return ms, sps, n_l
+        return measure_throughput(A, torch, dev, stream, wl, steps, warmup)
 
     if args.config == "c3":
-        # one amplfi_assemble_batch call per candidate, inputs resident; measured both as plain stream launches and as a
-        # replayed CUDA graph of the same call (the online service keeps its buffers in place)
-        plan = A.Plan(16384, 2048.0, (0, 1, 2), 1, nperseg=8192)
-        bg = torch.empty((3, 262144), dtype=torch.float32, device=dev)
-        noise = torch.empty((1, 3, 16384), dtype=torch.float32, device=dev)
-        params = torch.empty((1, 11), dtype=torch.float64, device=dev)
-        psd = torch.empty((3, 4097), dtype=torch.float32, device=dev)
-        out = torch.empty((1, 3, 16384), dtype=torch.float32, device=dev)
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-
-        def call(st):
-            A.amplfi_assemble_batch(plan, 1, bg, noise, params, 20.0, 1000.0, approximant=A.IMRPHENOMD, gmst=0.0,
-                                    psd=psd, out=out, stream=st)
-
-        def load(r):
-            wl = WL.make_c3(run=r)
-            bg.copy_(torch.from_numpy(wl.bg)); noise.copy_(torch.from_numpy(wl.noise)); params.copy_(torch.from_numpy(wl.params))
-
-        load(0)
-        for _ in range(3):
-            call(stream)
-        torch.cuda.synchronize()
-        graph = torch.cuda.CUDAGraph()
-        cs = torch.cuda.Stream()
-        cs.wait_stream(stream)
-        with torch.cuda.graph(graph, stream=cs):
-            call(torch.cuda.current_stream())
-        torch.cuda.synchronize()
-        lat, lat_g = [], []
-        ref = None
-        for r in range(args.runs):
-            load(r)
-            torch.cuda.synchronize()
-            e0.record(stream); call(stream); e1.record(stream)
-            torch.cuda.synchronize()
-            lat.append(e0.elapsed_time(e1) * 1e3)
-            ref = out.clone()
-            e0.record(stream); graph.replay(); e1.record(stream)
-            torch.cuda.synchronize()
-            lat_g.append(e0.elapsed_time(e1) * 1e3)
-            assert torch.equal(ref, out)
-        for name, v in (("stream launches", np.array(lat)), ("CUDA graph replay", np.array(lat_g))):
-            print(json.dumps({"metric": "online PSD+whiten device latency", "unit": "us", "higher_is_better": False,
-                              "launch": name, "p50": float(np.percentile(v, 50)), "p99": float(np.percentile(v, 99)),
-                              "mean": float(v.mean()), "min": float(v.min()), "max": float(v.max()), "runs": len(v),
-                              "dtype": "f32", "data": "synthetic",
-                              "config": {"workload": "c3 online-latency: batch 1 x H1+L1+V1, 8 s at 2048 Hz, Welch from the 128 s "
-                                                     "preceding background (4 s Hann, 50% overlap), IMRPhenomD injection; run r "
-                                                     "uses seed 0xA3D30003 + r; CUDA events around one amplfi_assemble_batch "
-                                                     "call, inputs resident"}}))
+        for d in measure_c3(A, WL, torch, dev, stream, args.runs):
+            print(json.dumps(d))
         return
 
     if args.config in ("c0", "c1"):
-        # the two small BASELINE configs: device time of one step (c0: fused inject+whiten with the analytic PSD, dense noise;
-        # c1: amplfi_assemble_batch with its own 64 s background), stream launches and a replayed CUDA graph
-        wl = WL.make_c0() if args.config == "c0" else WL.make_c1()
-        B, D, N = wl.batch, wl.n_det, wl.n
-        plan = A.Plan(N, wl.fs, wl.det_ids, B, nperseg=wl.nperseg)
-        noise = torch.from_numpy(wl.noise).to(dev)
-        params = torch.from_numpy(wl.params).to(dev)
-        out = torch.empty((B, D, N), dtype=torch.float32, device=dev)
-        if args.config == "c0":
-            psd = torch.from_numpy(wl.psd_scaled).to(dev)
-
-            def call(st):
-                A.amplfi_inject_whiten(plan, B, noise, psd, wl.f_lo, wl.f_hi, approximant=wl.approximant, params=params,
-                                       gmst=wl.gmst, out=out, stream=st)
-        else:
-            bg = torch.from_numpy(wl.bg).to(dev)
-            psd = torch.empty((D, wl.nperseg // 2 + 1), dtype=torch.float32, device=dev)
-
-            def call(st):
-                A.amplfi_assemble_batch(plan, B, bg, noise, params, wl.f_lo, wl.f_hi, approximant=wl.approximant, gmst=wl.gmst,
-                                        psd=psd, out=out, stream=st)
-        for _ in range(3):
-            call(stream)
-        torch.cuda.synchronize()
-        graph = torch.cuda.CUDAGraph()
-        cs = torch.cuda.Stream()
-        cs.wait_stream(stream)
-        with torch.cuda.graph(graph, stream=cs):
-            call(torch.cuda.current_stream())
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        res = {}
-        for name, fn in (("stream launches", lambda: call(stream)), ("CUDA graph replay", graph.replay)):
-            lat = []
-            for _ in range(args.runs):
-                e0.record(stream); fn(); e1.record(stream)
-                torch.cuda.synchronize()
-                lat.append(e0.elapsed_time(e1) * 1e3)
-            res[name] = np.array(lat)
-        for name, v in res.items():
-            print(json.dumps({"metric": "device time of one step", "unit": "us", "higher_is_better": False, "launch": name,
-                              "p50": float(np.percentile(v, 50)), "p99": float(np.percentile(v, 99)), "runs": len(v),
-                              "samples_per_s_at_p50": B * D * N / (float(np.percentile(v, 50)) * 1e-6), "dtype": "f32",
-                              "data": "synthetic", "config": {"workload": args.config, "batch": B, "n_det": D, "n": N}}))
+        for d in measure_small(A, WL, torch, dev, stream, args.config, args.runs):
+            print(json.dumps(d))
         return
 
     if args.config == "next":
@@ -549,14 +623,7 @@ def run_extra(args):
         return
 
     if args.config == "c4":
-        wl = WL.make_c4(batch=8192)
-        ms, sps, n_l = throughput(wl, max(3, min(args.steps, 10)), 3)
-        print(json.dumps({"metric": METRIC.replace("2048 Hz", "4096 Hz"), "value": sps, "unit": UNIT, "ms_per_step": ms,
-                          "higher_is_better": True, "dtype": "f32", "data": "synthetic", "gpu_launches_per_step": int(n_l),
-                          "hbm_gbs_step": 8.0 * sps / 1e9, "frac_of_measured_hbm": 8.0 * sps / 1e9 / peak,
-                          "peak_source": peak_src,
-                          "config": {"workload": "c4 bandwidth stress: batch 8192 x H1+L1+V1, fs 4096 Hz, 16 s segments (65536), "
-                                                 "gathered from a [3, 2^26] strip, Welch from 128 s (4 s Hann), IMRPhenomD"}}))
+        print(json.dumps(measure_c4(A, WL, torch, dev, stream, max(3, min(args.steps, 10)))))
         return
 
     # sweep: fixed total samples (2^27 per detector), segment length 1..256 s at 4096 Hz (n = 2^12 .. 2^20)
@@ -573,8 +640,24 @@ def run_extra(args):
                           "data": "synthetic"}))
 
 
+def respawn_under_torchrun(args):
+    """`python bench.py --gpus N` with N > 1 and no launcher: start N ranks (one per GPU) under torch.distributed.run on
+    this node and let them run this same command line.  Returns the launcher's exit code."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")                  # the communicator line shows the ranks and the transport
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd, env=env)
+
+
 if __name__ == "__main__":
     a = parse()
+    if a.gpus > 1 and "WORLD_SIZE" not in os.environ and a.config == "c2":
+        sys.exit(respawn_under_torchrun(a))
     if a.impl == "reference":
         run_reference(a)
     elif a.config != "c2":

@@ -26,7 +26,7 @@ def test_reference_arm_prints_the_contract_line():
                 "vs_baseline", "dtype", "data", "config", "cpu_baseline", "e2e"):
         assert key in d, key
     assert d["impl"] == "reference" and d["unit"] == "samples/s" and d["value"] > 0 and d["vs_baseline"] is None
-    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1 and "sample" in d["cpu_baseline"]
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] > 0 and "sample" in d["cpu_baseline"]
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["e2e"]["d2h_bytes_per_step"] == 0 and d["e2e"]["value"] == d["value"]
     assert "workload" in d["config"] and "model" not in d["config"]
 
@@ -34,6 +34,30 @@ def test_reference_arm_prints_the_contract_line():
 def test_reference_arm_other_ranks_do_nothing():
     r = _run("--impl", "reference", "--gpus", "2", env={"RANK": "1", "WORLD_SIZE": "2", "LOCAL_RANK": "1"})
     assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+def test_gpus_flag_spawns_the_ranks_itself():
+    """`--gpus N` without a launcher starts N ranks under torch.distributed.run (WORLD_SIZE set for them); the reference
+    arm needs no GPU, so the spawn path is exercised here: rank 0 prints the one line, with the world size it saw."""
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--cpu-sample", "4",
+                        "--steps", "1", "--warmup", "0", "--strip-len", "1048576"], capture_output=True, text=True, cwd=ROOT,
+                       env=env, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["world_size"] == 2
+
+
+def test_kernel_counters_file_matches_the_contract():
+    """profiles/kernel_counters.txt (if present) is JSON with the keys bench.py reads; a stale hash only nulls the fields."""
+    sys.path.insert(0, ROOT)
+    import bench
+    traffic, lane_ops, note = bench.kernel_counters()
+    assert note
+    if traffic is not None:
+        assert traffic > 0 and lane_ops > 0
 
 
 def test_b200_arm_has_no_cpu_fallback():

@@ -405,3 +405,73 @@ def test_full_size_c2_sampled_rows():
                       params=wl.params[rows], strip=wl.strip, offsets=wl.offsets[rows], extra=wl.extra)
     ref = oracle_inject_whiten(sub, "fused")
     assert row_err(got[rows], ref).max() <= TOL
+
+
+# ------------------------------------------------------------------------------------------
+# the claimed sizes themselves: sampled rows against the oracle
+# ------------------------------------------------------------------------------------------
+
+def _sampled_rows(wl, got, rows, mode="fused"):
+    kw = dict(nperseg=wl.nperseg, params=wl.params[rows], extra=wl.extra)
+    if wl.strip is not None:
+        kw.update(strip=wl.strip, offsets=wl.offsets[rows])
+    else:
+        kw.update(noise=wl.noise[rows], bg=wl.bg)
+    sub = WL.Workload(wl.name + "s", len(rows), wl.det_ids, wl.fs, wl.n, wl.approximant, **kw)
+    return row_err(got[rows], oracle_inject_whiten(sub, mode)).max()
+
+
+def test_full_size_c1_sampled_rows():
+    # BASELINE configs[1] at its full batch of 256 (768 units = 2.6 waves of the fused kernel)
+    wl = WL.make_c1()
+    got, _ = run_inject_whiten(wl, "fused")
+    assert got.shape == (256, 3, 16384) and np.all(np.isfinite(got))
+    rows = np.array([0, 1, 97, 98, 147, 148, 200, 255])
+    assert _sampled_rows(wl, got, rows) <= TOL
+
+
+@pytest.mark.parametrize("run", range(8))
+def test_c3_parity_over_seeds_with_snr12_rescale(run):
+    # BASELINE configs[3]: run r of the latency measurement uses seed 0xA3D30003 + r; the distance is rescaled so that
+    # the network optimal SNR (computed by the oracle) is 12
+    wl = WL.make_c3(run=run)
+    psd = OWE.welch(wl.bg.astype(np.float64), wl.fs, wl.nperseg)
+    hp, hc, _ = OW.waveform_fd(wl.approximant, wl.params, wl.n, wl.fs, wl.f_lo, wl.f_hi)
+    h_det, _ = OP.project(hp, hc, wl.params, wl.gmst, wl.det_ids, wl.n, wl.fs)
+    rho = OWH.optimal_snr(h_det, psd, wl.n, wl.fs, wl.f_lo, wl.f_hi)[0]
+    if rho > 0:
+        wl.params[0, 4] *= rho / 12.0
+    got, _ = run_inject_whiten(wl, "fused")
+    assert row_err(got, oracle_inject_whiten(wl, "fused")).max() <= TOL
+
+
+@pytest.mark.parametrize("batch", [99, 101, 149])
+def test_batch_not_a_multiple_of_the_wave(batch):
+    # 3 * batch units against waves of 296 CTAs: the last wave is ragged, the L2 prefetch runs past the end of the batch
+    wl = WL.make_c2(batch=batch, strip_len=1 << 22)
+    got, _ = run_inject_whiten(wl, "fused")
+    assert np.all(np.isfinite(got))
+    rows = np.array([0, batch // 3, batch - 2, batch - 1])
+    assert _sampled_rows(wl, got, rows) <= TOL
+
+
+def test_full_size_c4_sampled_rows():
+    # BASELINE configs[4] at its full size (batch 8192 x 3 x 65536 = 6.4 GB out, 166 chunks of the long-segment path),
+    # in the launch configuration bench.py --config c4 times
+    wl = WL.make_c4()
+    plan = A.Plan(wl.n, wl.fs, wl.det_ids, wl.batch, nperseg=wl.nperseg)
+    o, nb = wl.extra["bg_offset"], wl.extra["n_bg"]
+    strip = dev(wl.strip)
+    psd = A.amplfi_psd_welch(plan, strip[:, o:o + nb])
+    out = A.amplfi_inject_whiten(plan, wl.batch, strip, psd, wl.f_lo, wl.f_hi, offsets=dev(wl.offsets),
+                                 approximant=wl.approximant, params=dev(wl.params), gmst=wl.gmst)
+    torch.cuda.synchronize()
+    rows = np.array([0, 49, 50, 4095, 8191])
+    got_rows = out[torch.from_numpy(rows).to(out.device)].cpu().numpy().astype(np.float64)
+    assert bool(torch.isfinite(out[::64]).all())
+    var = out[::64].var(dim=-1).cpu().numpy()
+    assert abs(np.median(var) / (980.0 / 2048.0) - 1.017) < 0.05            # kept band 20-1000 Hz of 0-2048 Hz
+    del out
+    sub = WL.Workload("c4s", len(rows), wl.det_ids, wl.fs, wl.n, wl.approximant, nperseg=wl.nperseg,
+                      params=wl.params[rows], strip=wl.strip, offsets=wl.offsets[rows], extra=wl.extra)
+    assert row_err(got_rows, oracle_inject_whiten(sub, "fused")).max() <= TOL
