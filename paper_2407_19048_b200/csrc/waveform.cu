@@ -154,12 +154,19 @@ __global__ void __launch_bounds__(256, 4) waveform_slots_kernel(const WfCoef* __
         int kA, kB;
         slot::slot_bins(g >> 3, g & 7, t, kA, kB);
         float2 hA = make_float2(0.f, 0.f), hB = make_float2(0.f, 0.f);
+        const bool inA = kA >= k_lo && kA <= k_hi, inB = kB >= k_lo && kB <= k_hi;
+        // the table values of both bins are requested together (one L2 round trip per slot)
+        double ciA = 1.0, lnA = 0.0, ciB = 1.0, lnB = 0.0;
+        if (FAMILY == 0) {
+            if (inA) { ciA = tab_ci[kA]; lnA = tab_lnk[kA]; }
+            if (inB) { ciB = tab_ci[kB]; lnB = tab_lnk[kB]; }
+        }
 #pragma unroll 1
         for (int lane = 0; lane < 2; ++lane) {
             const int k = lane ? kB : kA;
             float2 h = make_float2(0.f, 0.f);
-            if (k >= k_lo && k <= k_hi) {
-                if (FAMILY == 0) h = eval_h0(c, k, tab_ci[k], tab_lnk[k]);
+            if (lane ? inB : inA) {
+                if (FAMILY == 0) h = eval_h0(c, k, lane ? ciB : ciA, lane ? lnB : lnA);
                 else h = eval_sine_gaussian(c, k);
             }
             if (lane) hB = h; else hA = h;
