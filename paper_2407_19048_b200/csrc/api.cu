@@ -47,6 +47,9 @@ static int dev_alloc(T** ptr, size_t count) {
     return AMPLFI_OK;
 }
 
+// segment lengths of the three-pass fused kernel (inject_whiten_v3.cu), whose h0 workspace is in the slot layout
+static bool v3_family(const amplfi_plan* p) { return p->logm >= 11 && p->logm <= 13; }
+
 static bool known_approximant(int a) { return a == AMPLFI_TAYLORF2 || a == AMPLFI_IMRPHENOMD || a == AMPLFI_SINE_GAUSSIAN; }
 
 // a plan's tables and workspaces live on the device it was created on
@@ -182,7 +185,7 @@ int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_
     if (!rc) rc = dev_alloc(&p->h0, (size_t)max_batch * p->n_bins);
     p->filt_stride = (p->n_bins + 3) & ~3;
     if (!rc) rc = dev_alloc(&p->filt, (size_t)n_det * p->filt_stride);
-    if (!rc && p->logm == 13) rc = dev_alloc(&p->filt_slots, (size_t)n_det * 8192);
+    if (!rc && p->logm >= 11 && p->logm <= 13) rc = dev_alloc(&p->filt_slots, (size_t)n_det * (n / 2));
     if (!rc) rc = dev_alloc(&p->filt_flat, (size_t)p->filt_stride);
     if (!rc) rc = dev_alloc(&p->fir_spec, (size_t)n_det * p->n_bins);
     if (!rc) rc = dev_alloc(&p->fir_time, (size_t)n_det * n);
@@ -208,7 +211,7 @@ int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_
     }
     if (!rc) rc = launch_tables(p, nullptr);
     if (!rc && p->logm >= 11 && p->logm <= 13) rc = init_iw13_tables(nullptr);
-    if (!rc && p->logm == 13) rc = init_iw3_tables(nullptr);
+    if (!rc && p->logm >= 11 && p->logm <= 13) rc = init_iw3_tables(nullptr);
     if (!rc) {
         fill_kernel<<<(p->filt_stride + 255) / 256, 256>>>(p->filt_flat, p->filt_stride, (float)(1.0 / (2.0 * (double)n)));
         count_launch();
@@ -323,7 +326,7 @@ int amplfi_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
     if (fused) {
         rc = launch_prepare(p, approximant, batch, params, gmst, f_lo, f_hi, 2.0 * p->fs, nullptr, st);
         if (rc) return rc;
-        rc = launch_waveform_h0(p, batch, st, p->logm == 13);
+        rc = launch_waveform_h0(p, batch, st, v3_family(p));
         if (rc) return rc;
     }
     const bool timed = p->timing && p->ev_count < AMPLFI_TIMING_RING;
@@ -363,7 +366,7 @@ int amplfi_assemble_batch(const amplfi_plan* p, int batch, const float* bg, long
     if (!rc) rc = launch_filter(p, psd, n_psd, f_lo, f_hi, mp->side);
     e = cudaEventRecord(mp->ev_join, mp->side);
     if (!rc) rc = launch_prepare(p, approximant, batch, params, gmst, f_lo, f_hi, 2.0 * p->fs, nullptr, st);
-    if (!rc) rc = launch_waveform_h0(p, batch, st, p->logm == 13);
+    if (!rc) rc = launch_waveform_h0(p, batch, st, v3_family(p));
     // join (always, so the side stream never runs past the call unobserved)
     if (e == cudaSuccess) e = cudaStreamWaitEvent(st, mp->ev_join, 0);
     if (e != cudaSuccess) { set_error("amplfi_assemble_batch: join: %s", cudaGetErrorString(e)); return AMPLFI_ERR_CUDA; }
@@ -402,7 +405,7 @@ int amplfi_inject_whiten_views(const amplfi_plan* p, int batch, const float* noi
     if (!rc) rc = launch_prepare(p, approximant, batch, params, gmst, f_lo, f_hi, 2.0 * p->fs, nullptr, st);
     // n = 4096, 8192, 16384: one launch, one forward transform for both views (inject_whiten13.cu, VIEWS = 2; linear h0)
     const bool one_launch = p->logm >= 11 && p->logm <= 13 && (reinterpret_cast<size_t>(out2) & 15) == 0;
-    if (!rc) rc = launch_waveform_h0(p, batch, st, p->logm == 13 && !one_launch);
+    if (!rc) rc = launch_waveform_h0(p, batch, st, v3_family(p) && !one_launch);
     // both views with the fp64-reduced phase, so that a zero shift reproduces the first view bit for bit
     IwOpts o;
     o.n_det = p->n_det; o.resp = nullptr; o.filt = nullptr; o.filt_stride = 0; o.crop = 0; o.phase64 = 1;
@@ -429,7 +432,7 @@ int amplfi_waveform_td(const amplfi_plan* p, int approximant, int batch, const d
     if (reinterpret_cast<size_t>(h_t) & 7) { set_error("amplfi_waveform_td: h_t must be 8-byte aligned"); return AMPLFI_ERR_ALIGNMENT; }
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     rc = launch_prepare(p, approximant, batch, params, 0.0, f_lo, f_hi, 2.0 * p->fs, flags, st);
-    if (!rc) rc = launch_waveform_h0(p, batch, st, p->logm == 13);
+    if (!rc) rc = launch_waveform_h0(p, batch, st, v3_family(p));
     if (!rc) rc = launch_td_resp(p, batch, st);
     if (rc) return rc;
     IwOpts o;
@@ -458,7 +461,7 @@ int amplfi_inject_whiten_fir(const amplfi_plan* p, int batch, const float* noise
     if (!rc) rc = launch_fir_truncate(p, fduration, st);
     if (!rc && fused) {
         rc = launch_prepare(p, approximant, batch, params, gmst, f_lo, f_hi, 2.0 * p->fs, nullptr, st);
-        if (!rc) rc = launch_waveform_h0(p, batch, st, p->logm == 13);
+        if (!rc) rc = launch_waveform_h0(p, batch, st, v3_family(p));
     }
     if (rc) return rc;
     IwOpts o;

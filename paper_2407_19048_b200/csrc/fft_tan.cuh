@@ -137,9 +137,10 @@ __device__ __forceinline__ void dit16_const(C2 (&v)[16]) {
     bf<INV, true>(v[7], v[15], Tw1{kC16_3, kT16_3});
 }
 
-// radix 8 (W general): tw[0] = W^4, tw[1] = W^2, tw[2 + q] = W w8^q (q < 2); y[r] from v[brev8(r)]
-template <bool INV, class TW>
-__device__ __forceinline__ void dit8(C2 (&v)[8], const TW (&tw)[4]) {
+// radix 8 (W general): tw[0] = W^4, tw[1] = W^2, tw[2 + q] = W w8^q (q < 2); y[r] from v[brev8(r)];
+// CONJ_HI: outputs X[4..7] are left conjugated
+template <bool INV, class TW, bool CONJ_HI = false>
+__device__ __forceinline__ void dit8(C2 (&v)[8], const TW (&tw)[8]) {
 #pragma unroll
     for (int i = 0; i < 4; ++i) bf<INV, false>(v[2 * i], v[2 * i + 1], tw[0]);
 #pragma unroll
@@ -149,9 +150,24 @@ __device__ __forceinline__ void dit8(C2 (&v)[8], const TW (&tw)[4]) {
     }
 #pragma unroll
     for (int q = 0; q < 2; ++q) {
-        bf<INV, false>(v[q], v[q + 4], tw[2 + q]);
-        bf<INV, true>(v[q + 2], v[q + 6], tw[2 + q]);
+        bf<INV, false, CONJ_HI>(v[q], v[q + 4], tw[2 + q]);
+        bf<INV, true, CONJ_HI>(v[q + 2], v[q + 6], tw[2 + q]);
     }
+}
+// radix 4: tw[0] = W^2, tw[1] = W; y[r] from v[brev4(r)];  CONJ_HI: outputs X[2], X[3] are left conjugated
+template <bool INV, class TW, bool CONJ_HI = false>
+__device__ __forceinline__ void dit4(C2 (&v)[4], const TW (&tw)[8]) {
+    bf<INV, false>(v[0], v[1], tw[0]);
+    bf<INV, false>(v[2], v[3], tw[0]);
+    bf<INV, false, CONJ_HI>(v[0], v[2], tw[1]);
+    bf<INV, true, CONJ_HI>(v[1], v[3], tw[1]);
+}
+// radix R in {4, 8, 16} with the twiddle row layout of each (entries beyond the radix's need are unused)
+template <int R, bool INV, class TW, bool CONJ_HI = false>
+__device__ __forceinline__ void dit_r(C2 (&v)[R], const TW (&tw)[8]) {
+    if constexpr (R == 16) dit16<INV, TW, CONJ_HI>(v, tw);
+    else if constexpr (R == 8) dit8<INV, TW, CONJ_HI>(v, tw);
+    else dit4<INV, TW, CONJ_HI>(v, tw);
 }
 
 // (c, tau) of exp(i theta) computed on the fly: theta in [-pi, pi]; c is nudged off an exact zero by 1e-8 (below half an ulp

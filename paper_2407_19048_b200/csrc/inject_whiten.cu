@@ -15,7 +15,8 @@ namespace amplfi {
 // ---- whitening filter on the segment grid: w[k] = sqrt(2/(fs S)) / (2N) inside the band, else 0 ----
 // psd holds S * 2^140, so sqrt(2/(fs S)) = 2^70 * rsqrt(fs * psd / 2).
 __global__ void filter_kernel(const float* __restrict__ psd, int n_psd, int n_bins, int ratio, float fs, float norm,
-                              int k_lo, int k_hi, float* __restrict__ filt, int filt_stride, float* __restrict__ filt_slots) {
+                              int k_lo, int k_hi, float* __restrict__ filt, int filt_stride, float* __restrict__ filt_slots,
+                              int kl) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     const int d = blockIdx.y;
     if (k >= filt_stride) return;
@@ -34,7 +35,7 @@ __global__ void filter_kernel(const float* __restrict__ psd, int n_psd, int n_bi
         w = rsqrtf(0.5f * fs * sv) * norm;
     }
     filt[(size_t)d * filt_stride + k] = w;
-    if (filt_slots != nullptr && k < slot::M) filt_slots[(size_t)d * slot::FILT_ROW + slot::filt_index(k)] = w;      // n = 16384
+    if (filt_slots != nullptr && k < 16 * kl) filt_slots[(size_t)d * slot::filt_row(kl) + slot::filt_index(kl, k)] = w;
 }
 
 int launch_filter(const amplfi_plan* p, const float* psd, int n_psd, double f_lo, double f_hi, cudaStream_t st) {
@@ -50,7 +51,7 @@ int launch_filter(const amplfi_plan* p, const float* psd, int n_psd, double f_lo
     const float norm = (float)(1180591620717411303424.0 / (2.0 * (double)p->n));      // 2^70 / (2N)
     dim3 grid((p->filt_stride + 255) / 256, p->n_det);
     filter_kernel<<<grid, 256, 0, st>>>(psd, n_psd, p->n_bins, ratio, (float)p->fs, norm, (int)k_lo, (int)k_hi, p->filt,
-                                        p->filt_stride, p->filt_slots);
+                                        p->filt_stride, p->filt_slots, p->n / 32);
     count_launch();
     return check_launch("filter_kernel");
 }
@@ -74,13 +75,13 @@ __global__ void fir_real_to_spec_kernel(const float* __restrict__ src, int src_s
 }
 
 __global__ void fir_time_to_filt_kernel(const float* __restrict__ time, int n, int n_bins, float mul, float* __restrict__ filt,
-                                        int filt_stride, float* __restrict__ filt_slots) {
+                                        int filt_stride, float* __restrict__ filt_slots, int kl) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     const int d = blockIdx.y;
     if (k >= filt_stride) return;
     const float w = k < n_bins ? time[(size_t)d * n + k] * mul : 0.f;
     filt[(size_t)d * filt_stride + k] = w;
-    if (filt_slots != nullptr && k < slot::M) filt_slots[(size_t)d * slot::FILT_ROW + slot::filt_index(k)] = w;
+    if (filt_slots != nullptr && k < 16 * kl) filt_slots[(size_t)d * slot::filt_row(kl) + slot::filt_index(kl, k)] = w;
 }
 
 // plan->filt (already holding the band-limited filter of launch_filter) is replaced by its time-truncated version.
@@ -103,7 +104,7 @@ int launch_fir_truncate(const amplfi_plan* p, double fduration, cudaStream_t st)
     rc = launch_inject_whiten(p, p->n_det, nullptr, nullptr, 0, reinterpret_cast<const float*>(p->fir_spec), 0, p->fir_time,
                               st, &o);
     if (rc) return rc;
-    fir_time_to_filt_kernel<<<gf, 256, 0, st>>>(p->fir_time, p->n, nb, (float)((double)p->n / p->fs), p->filt, p->filt_stride, p->filt_slots);
+    fir_time_to_filt_kernel<<<gf, 256, 0, st>>>(p->fir_time, p->n, nb, (float)((double)p->n / p->fs), p->filt, p->filt_stride, p->filt_slots, p->n / 32);
     count_launch();
     return check_launch("fir_truncate");
 }
@@ -292,7 +293,7 @@ int launch_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
     a.filt_slots = p->filt_slots;
     a.crop = 0; a.phase64 = 0; a.out2 = nullptr; a.t_shift = nullptr;
     a.n_det = p->n_det; a.two_fs = (float)(2.0 * p->fs); a.inv_tseg = (float)(1.0 / p->t_seg);
-    a.prefetch_ahead = (p->logm == 13 ? 1 : 2) * p->sm_count;      // measured optimum of each kernel generation
+    a.prefetch_ahead = (p->logm >= 11 && p->logm <= 13 ? 1 : 2) * p->sm_count * (8192 / (p->n / 2 < 8192 ? p->n / 2 : 8192));   // one wave ahead
     if (opts != nullptr) {
         a.n_det = opts->n_det;
         if (opts->resp != nullptr) a.resp = opts->resp;
@@ -305,9 +306,8 @@ int launch_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
     switch (p->logm) {
         case 9: return launch_iw_mode<9>(a, mode, units, st);
         case 10: return launch_iw_mode<10>(a, mode, units, st);
-        case 11: return launch_iw13(a, 11, mode, units, st);
-        case 12: return launch_iw13(a, 12, mode, units, st);
-        case 13: return a.out2 != nullptr ? launch_iw13(a, 13, mode, units, st) : launch_iw3(a, mode, units, st);
+        case 11: case 12: case 13:      // three-pass kernel; the one-launch two-view variant still runs the packed four-pass one
+            return a.out2 != nullptr ? launch_iw13(a, p->logm, mode, units, st) : launch_iw3(a, p->logm, mode, units, st);
         case 14: return launch_iw_mode<14>(a, mode, units, st);
         case 15: case 16: case 17: case 18: case 19: return launch_inject_whiten_long(p, a, mode, units, st);
         default:

@@ -33,15 +33,28 @@ namespace v3 {
 
 using namespace tn;
 
-constexpr int LOGM = 13, M = 8192, N = 16384, K = M + 1, T = 256, KL = 512;
-constexpr int ROW = 34, BLK = 16 * ROW, PLANE = 16 * BLK;        // 544, 8704 floats
-constexpr int SMEM_BYTES = 2 * PLANE * (int)sizeof(float);       // 69632
+// Geometry of a segment length: M = 2^LOGM = 32 * RB * 16 complex points, RB = 16 / 8 / 4 for n = 16384 / 8192 / 4096
+// (the paper's own 4 s at 2048 Hz is n = 8192); T = M/32 threads (256 / 128 / 64), 2 / 4 / 8 CTAs per SM.
+// Pass FB / I2 is then a radix RB, of which every thread takes 16/RB.
+template <int LOGM>
+struct Geo {
+    static constexpr int M = 1 << LOGM, N = 2 * M, K = M + 1;
+    static constexpr int T = M / 32;                  // threads
+    static constexpr int KL = M / 16;                 // span of klow = k1 + 32 k2
+    static constexpr int RB = M / 512;                // radix of the middle pass
+    static constexpr int NB = 16 / RB;                // middle-pass butterflies per thread
+    static constexpr int PLANE = RB * 544;            // floats per plane
+    static constexpr int SMEM_BYTES = 2 * PLANE * (int)sizeof(float);
+    static constexpr int CTAS = 512 / T;              // per SM (registers: 128 per thread)
+};
+constexpr int ROW = 34, BLK = 16 * ROW;               // 34, 544 floats
 
-// FB: per-lane twiddles of W = w512^k1, k1 = 2 kap (lane A), 2 kap + 1 (lane B): (cA, cB, tauA, tauB)
-// I2: shared twiddles of W = w256^n3 (used conjugated): (c, tau)
+// FB: per-lane twiddles of W = w_(32 RB)^k1, k1 = 2 kap (lane A), 2 kap + 1 (lane B): (cA, cB, tauA, tauB)
+// I2: shared twiddles of W = w_(16 RB)^n3 (used conjugated): (c, tau)
+// rows in the layout fft_tan.cuh gives each radix; one set per segment length [LOGM - 11]
 struct Tables {
-    float4 fb[16][8];
-    float2 i2[16][8];
+    float4 fb[3][16][8];
+    float2 i2[3][16][8];
 };
 static __device__ Tables g_tab;
 
@@ -53,20 +66,23 @@ __device__ __forceinline__ void sts2(float* re, float* im, int o, C2 v) {
     *reinterpret_cast<u64*>(im + o) = v.i;
 }
 
-// theta = -(2 pi / 8192) * (mul * x + off): the eight twiddles of a radix-16 pass with W = w8192^x
-// (fft_tan.cuh: W^8, W^4, W^2, W^2 w8, W w16^q); every exponent stays below 4096 for the callers' x, so theta in [-pi, 0]
+// the eight twiddles of a radix-16 pass with W = w_M^x (fft_tan.cuh: W^8, W^4, W^2, W^2 w8, W w16^q), theta = -(2 pi / M) e;
+// every exponent e stays at or below M/2 for the callers' x, so theta lies in [-pi, 0] (no range reduction)
+template <int M>
 __device__ __forceinline__ void pass_twiddles(float x, Tw1 (&tw)[8]) {
-    constexpr float u = -6.283185307179586f / 8192.0f;
+    constexpr float u = -6.283185307179586f / (float)M;
     tw[0] = tan_twiddle(x * (8.0f * u));
     tw[1] = tan_twiddle(x * (4.0f * u));
     tw[2] = tan_twiddle(x * (2.0f * u));
-    tw[3] = tan_twiddle(fmaf(x, 2.0f * u, 1024.0f * u));
+    tw[3] = tan_twiddle(fmaf(x, 2.0f * u, (float)(M / 8) * u));
 #pragma unroll
-    for (int q = 0; q < 4; ++q) tw[4 + q] = tan_twiddle(fmaf(x, u, 512.0f * q * u));
+    for (int q = 0; q < 4; ++q) tw[4 + q] = tan_twiddle(fmaf(x, u, (float)(M / 16 * q) * u));
 }
 
-template <int MODE, bool FWD>
-__global__ void __launch_bounds__(T, 2) inject_whiten3_kernel(const IwArgs a, int units) {
+template <int LOGM, int MODE, bool FWD>
+__global__ void __launch_bounds__(Geo<LOGM>::T, Geo<LOGM>::CTAS) inject_whiten3_kernel(const IwArgs a, int units) {
+    using G = Geo<LOGM>;
+    constexpr int M = G::M, N = G::N, K = G::K, T = G::T, KL = G::KL, RB = G::RB, NB = G::NB, PLANE = G::PLANE;
     extern __shared__ float smem3[];
     float* re = smem3;
     float* im = smem3 + PLANE;
@@ -111,9 +127,10 @@ __global__ void __launch_bounds__(T, 2) inject_whiten3_kernel(const IwArgs a, in
         }
     }
 
-    const int n2 = tid >> 4, n3 = tid & 15;                // FA / I3: j = tid = 16 n2 + n3;  FB / I2: kap = n2
+    const int n2 = tid >> 4, n3 = tid & 15;                // FA / I3: j = tid = 16 n2 + n3 (n2 < RB)
     const int oj = n2 * BLK + n3 * ROW;                    // FA / I3: element (n2, n3, k1 = 0)
-    const int ob = n3 * ROW + 2 * n2;                      // FB / I2: element (d2 = 0, n3, k1 = 2 kap)
+    // FB / I2: butterfly i of this thread is (kap, n3) = ((tid + T i) >> 4, tid & 15): element (d2 = 0, n3, k1 = 2 kap)
+    auto ob_of = [&](int i) { return n3 * ROW + 2 * ((tid + T * i) >> 4); };
 
     // ---- FA: radix 32 over n1, operands from global memory ----
     if (FWD) {
@@ -121,11 +138,11 @@ __global__ void __launch_bounds__(T, 2) inject_whiten3_kernel(const IwArgs a, in
         if ((reinterpret_cast<size_t>(x) & 7) == 0) {
             const float2* x2 = reinterpret_cast<const float2*>(x) + tid;
 #pragma unroll
-            for (int n1 = 0; n1 < 32; ++n1) z[n1] = __ldcs(x2 + n1 * 256);
+            for (int n1 = 0; n1 < 32; ++n1) z[n1] = __ldcs(x2 + n1 * T);
         } else {
 #pragma unroll
             for (int n1 = 0; n1 < 32; ++n1) {
-                const int m = n1 * 256 + tid;
+                const int m = n1 * T + tid;
                 z[n1] = make_float2(__ldg(x + 2 * m), __ldg(x + 2 * m + 1));
             }
         }
@@ -166,7 +183,7 @@ __global__ void __launch_bounds__(T, 2) inject_whiten3_kernel(const IwArgs a, in
     if (MODE == MODE_HDET) hsrc = reinterpret_cast<const float*>(a.h_det + (size_t)unit * K);
     if (MODE == MODE_FUSED) {
         const WfCoef* c = a.coef + b;
-        hsrc = reinterpret_cast<const float*>(a.h0) + (size_t)b * slot::H0_ROW;        // slot layout
+        hsrc = reinterpret_cast<const float*>(a.h0) + (size_t)b * (2 * M);              // slot layout
         if (c->valid) { w_lo = c->k_lo; w_hi = c->k_hi; }       // an empty band is stored as (2^30, -1) by prepare_kernel
         const DetResp r = a.resp[unit];
         cre = (float)r.fp * c->pol_p;                       // C = F+ (1+cos^2 i)/2 - i Fx cos i
@@ -198,17 +215,17 @@ __global__ void __launch_bounds__(T, 2) inject_whiten3_kernel(const IwArgs a, in
     unsigned need = 0;                                       // bit w: first h0 slots of unit w needed, bit 8 + w: second
     if (MODE == MODE_FUSED) {
         const int l = t & 31;
-        need = __ballot_sync(0xffffffffu, l < 16 && slot::window_needed(l >> 3, l & 7, t >> 5, w_lo, w_hi));
+        need = __ballot_sync(0xffffffffu, l < 16 && slot::window_needed(KL, l >> 3, l & 7, t >> 5, w_lo, w_hi));
     }
-    const float4* fsl = reinterpret_cast<const float4*>(a.filt_slots) + (a.filt_stride ? d * (slot::FILT_ROW / 4) : 0) + t;
-    const float4* hsl = reinterpret_cast<const float4*>(a.h0) + (size_t)b * (slot::H0_ROW / 4) + t;
+    const float4* fsl = reinterpret_cast<const float4*>(a.filt_slots) + (a.filt_stride ? d * (M / 4) : 0) + t;
+    const float4* hsl = reinterpret_cast<const float4*>(a.h0) + (size_t)b * (M / 2) + t;
     if ((t & 7) == 0) {                                      // one request per 128-byte line
 #pragma unroll
         for (int w = 0; w < 8; ++w) {
-            asm volatile("prefetch.global.L1 [%0];" ::"l"(fsl + w * 256));
+            asm volatile("prefetch.global.L1 [%0];" ::"l"(fsl + w * T));
             if (MODE == MODE_FUSED) {
-                if (need & (1u << w)) asm volatile("prefetch.global.L1 [%0];" ::"l"(hsl + w * 256));
-                if (need & (256u << w)) asm volatile("prefetch.global.L1 [%0];" ::"l"(hsl + (8 + w) * 256));
+                if (need & (1u << w)) asm volatile("prefetch.global.L1 [%0];" ::"l"(hsl + w * T));
+                if (need & (256u << w)) asm volatile("prefetch.global.L1 [%0];" ::"l"(hsl + (8 + w) * T));
             }
         }
     }
@@ -233,35 +250,41 @@ __global__ void __launch_bounds__(T, 2) inject_whiten3_kernel(const IwArgs a, in
         } else if (MODE == MODE_FUSED && sl != 0) {
             sin_a = sk >= w_lo && sk <= w_hi;
             sin_b = M - sk >= w_lo && M - sk <= w_hi;
-            if (sin_a) { const float* hp = hsrc + slot::h0_index(sk); sha = make_float2(__ldg(hp), __ldg(hp + 2)); }
-            if (sin_b) { const float* hp = hsrc + slot::h0_index(M - sk); shb = make_float2(__ldg(hp), __ldg(hp + 2)); }
+            if (sin_a) { const float* hp = hsrc + slot::h0_index(KL, sk); sha = make_float2(__ldg(hp), __ldg(hp + 2)); }
+            if (sin_b) { const float* hp = hsrc + slot::h0_index(KL, M - sk); shb = make_float2(__ldg(hp), __ldg(hp + 2)); }
         }
     }
 
-    // ---- FB: radix 16 over n2 ----
+    // ---- FB: radix RB over n2 (NB butterflies per thread) ----
     if (FWD) {
-        Tw2 tw[8];
+        Tw2 tw[NB][8];
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
-            const float4 f = __ldg(&g_tab.fb[n2][i]);
-            tw[i] = Tw2{pack(f.x, f.y), pack(f.z, f.w)};
-        }
+        for (int i = 0; i < NB; ++i)
+#pragma unroll
+            for (int e = 0; e < (RB == 16 ? 8 : (RB == 8 ? 4 : 2)); ++e) {
+                const float4 f = __ldg(&g_tab.fb[LOGM - 11][(tid + T * i) >> 4][e]);
+                tw[i][e] = Tw2{pack(f.x, f.y), pack(f.z, f.w)};
+            }
         __syncthreads();
-        C2 v[16];
 #pragma unroll
-        for (int r = 0; r < 16; ++r) v[brev<16>(r)] = lds2(re, im, ob + r * BLK);
-        dit16<false, Tw2, true>(v, tw);                      // k2 >= 8 (the klow >= 256 read by lane B of FC) stored conjugated
-        if (n2 == 0) {
-            // the self-paired column klow = 256 (k1 = 0, k2 = 8; lane B of thread 0 in FC, whose twiddles are those of
-            // klow = 0, i.e. 1) takes its factor conj(w32^n3) here: one complex product in 16 threads
-            float ar_, br_, ai_, bi_;
-            unpack(v[8].r, ar_, br_);
-            unpack(v[8].i, ai_, bi_);
-            const float co = kCos32[n3], si = kSin32[n3];
-            v[8] = C2{pack(ar_ * co - ai_ * si, br_), pack(ar_ * si + ai_ * co, bi_)};
+        for (int i = 0; i < NB; ++i) {
+            const int ob = ob_of(i);
+            C2 v[RB];
+#pragma unroll
+            for (int r = 0; r < RB; ++r) v[brev<RB>(r)] = lds2(re, im, ob + r * BLK);
+            dit_r<RB, false, Tw2, true>(v, tw[i]);           // k2 >= RB/2 (the klow >= KL/2 read by lane B of FC) stored conjugated
+            if (((tid + T * i) >> 4) == 0) {
+                // the self-paired column klow = KL/2 (k1 = 0, k2 = RB/2; lane B of thread 0 in FC, whose twiddles are those
+                // of klow = 0, i.e. 1) takes its factor conj(w32^n3) here: one complex product in 16 threads
+                float ar_, br_, ai_, bi_;
+                unpack(v[RB / 2].r, ar_, br_);
+                unpack(v[RB / 2].i, ai_, bi_);
+                const float co = kCos32[n3], si = kSin32[n3];
+                v[RB / 2] = C2{pack(ar_ * co - ai_ * si, br_), pack(ar_ * si + ai_ * co, bi_)};
+            }
+#pragma unroll
+            for (int k2 = 0; k2 < RB; ++k2) sts2(re, im, ob + k2 * BLK, v[k2]);
         }
-#pragma unroll
-        for (int k2 = 0; k2 < 16; ++k2) sts2(re, im, ob + k2 * BLK, v[k2]);
     }
     if (sl >= 0 && sl <= 16) {
         float2 ia = make_float2(0.f, 0.f), ib = make_float2(0.f, 0.f);            // what the injection adds to 2 X[k], 2 X[M-k]
@@ -289,7 +312,7 @@ __global__ void __launch_bounds__(T, 2) inject_whiten3_kernel(const IwArgs a, in
     C2 v[16];
     if (FWD) {
         Tw1 tw[8];
-        pass_twiddles((float)ka, tw);
+        pass_twiddles<M>((float)ka, tw);
         __syncthreads();
 #pragma unroll
         for (int r = 0; r < 16; ++r)
@@ -332,7 +355,7 @@ __global__ void __launch_bounds__(T, 2) inject_whiten3_kernel(const IwArgs a, in
         }
         struct PwOps { float4 f, hf, hs; };
         auto pw_load = [&](int w, PwOps& L) {
-            L.f = __ldg(fsl + w * 256);
+            L.f = __ldg(fsl + w * T);
             L.hf = L.hs = make_float4(0.f, 0.f, 0.f, 0.f);
             if (MODE == MODE_HDET) {
                 const int k0 = t + KL * 2 * w, k1 = k0 + KL;
@@ -340,8 +363,8 @@ __global__ void __launch_bounds__(T, 2) inject_whiten3_kernel(const IwArgs a, in
                 L.hs = make_float4(__ldg(hsrc + 2 * (M - k0)), __ldg(hsrc + 2 * (M - k1)), __ldg(hsrc + 2 * (M - k0) + 1),
                                    __ldg(hsrc + 2 * (M - k1) + 1));
             } else if (MODE == MODE_FUSED) {
-                if (need & (1u << w)) L.hf = __ldg(hsl + w * 256);
-                if (need & (256u << w)) L.hs = __ldg(hsl + (8 + w) * 256);
+                if (need & (1u << w)) L.hf = __ldg(hsl + w * T);
+                if (need & (256u << w)) L.hs = __ldg(hsl + (8 + w) * T);
             }
         };
         PwOps ops[8];
@@ -458,45 +481,49 @@ __global__ void __launch_bounds__(T, 2) inject_whiten3_kernel(const IwArgs a, in
             re[obb + q * ROW] = br; im[obb + q * ROW] = bi;
         }
     }
-    // ---- I2: inverse radix 16 over k2 ----
+    // ---- I2: inverse radix RB over k2 (NB butterflies per thread; the twiddles depend on n3 only) ----
     {
         Tw1 tw[8];
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
-            const float2 f = __ldg(&g_tab.i2[n3][i]);
-            tw[i] = Tw1{f.x, f.y};
+        for (int e = 0; e < (RB == 16 ? 8 : (RB == 8 ? 4 : 2)); ++e) {
+            const float2 f = __ldg(&g_tab.i2[LOGM - 11][n3][e]);
+            tw[e] = Tw1{f.x, f.y};
         }
         __syncthreads();
-        C2 w[16];
 #pragma unroll
-        for (int r = 0; r < 16; ++r) w[brev<16>(r)] = lds2(re, im, ob + r * BLK);
-        dit16<true>(w, tw);
+        for (int i = 0; i < NB; ++i) {
+            const int ob = ob_of(i);
+            C2 w[RB];
 #pragma unroll
-        for (int q = 0; q < 16; ++q) sts2(re, im, ob + q * BLK, w[q]);
+            for (int r = 0; r < RB; ++r) w[brev<RB>(r)] = lds2(re, im, ob + r * BLK);
+            dit_r<RB, true>(w, tw);
+#pragma unroll
+            for (int q = 0; q < RB; ++q) sts2(re, im, ob + q * BLK, w[q]);
+        }
     }
     // ---- I3: inverse radix 32 over k1, natural-order stores ----
     {
         const float jf = (float)tid;
         Tw1 tw[8];
-        pass_twiddles(2.0f * jf, tw);                        // base W^2, W = w8192^j
+        pass_twiddles<M>(2.0f * jf, tw);                     // base W^2, W = w_M^j
         __syncthreads();
         C2 w[16];
 #pragma unroll
         for (int r = 0; r < 16; ++r) w[brev<16>(r)] = lds2(re, im, oj + 2 * r);
         dit16<true>(w, tw);
         float2* out2 = reinterpret_cast<float2*>(out);
-        constexpr float uu = -6.283185307179586f / 8192.0f;
+        constexpr float uu = -6.283185307179586f / (float)M;
         const int c2 = a.crop >> 1;                          // crop is even: whole float2 pairs
 #pragma unroll
         for (int q = 0; q < 16; ++q) {
             float er, orr, ei, oi;
             unpack(w[q].r, er, orr);
             unpack(w[q].i, ei, oi);
-            const Tw1 tq = tan_twiddle(fmaf(jf, uu, 256.0f * (q & 7) * uu));      // W w32^q (the +i of q >= 8 as ROT)
+            const Tw1 tq = tan_twiddle(fmaf(jf, uu, (float)(M / 32 * (q & 7)) * uu));      // W w32^q (the +i of q >= 8 as ROT)
             float2 lo, hi;
             if (q < 8) bf_s<true, false>(make_float2(er, ei), make_float2(orr, oi), tq, lo, hi);
             else bf_s<true, true>(make_float2(er, ei), make_float2(orr, oi), tq, lo, hi);
-            const int m0 = q * 256 + tid, m1 = (q + 16) * 256 + tid;
+            const int m0 = q * T + tid, m1 = (q + 16) * T + tid;
             if (a.crop == 0) {
                 __stcs(out2 + m0, lo);
                 __stcs(out2 + m1, hi);
@@ -509,33 +536,45 @@ __global__ void __launch_bounds__(T, 2) inject_whiten3_kernel(const IwArgs a, in
 }
 
 __global__ void init_tables3_kernel() {
-    const int i = threadIdx.x;                                 // 0 .. 127: row = i >> 3, entry = i & 7
-    const int row = i >> 3, ent = i & 7;
-    auto ct = [](int e, float& c, float& tau) {                // (c, tau) of w8192^e, fp64 -> fp32
+    // one thread per (segment length lg, row, entry): rows in the layout fft_tan.cuh gives each radix
+    //   RB = 16: W^8, W^4, W^2, W^2 w8, W w16^q (q < 4);   RB = 8: W^4, W^2, W w8^q (q < 2);   RB = 4: W^2, W
+    const int i = threadIdx.x;                                 // 0 .. 383
+    if (i >= 384) return;
+    const int lg = i >> 7, row = (i >> 3) & 15, ent = i & 7;
+    const int m = 2048 << lg, rb = m / 512;
+    auto ct = [m](int e, float& c, float& tau) {               // (c, tau) of w_M^e, fp64 -> fp32
         double s, co;
-        sincospi(-2.0 * (double)(e & 8191) / 8192.0, &s, &co);
+        sincospi(-2.0 * (double)(e & (m - 1)) / (double)m, &s, &co);
         if (fabs(co) < 1e-12) co = 1e-12;
         c = (float)co;
         tau = (float)(s / co);
     };
-    auto expo = [](int x, int ent) {                           // exponent of entry `ent` for W = w8192^x
-        switch (ent) {
-            case 0: return 8 * x;
-            case 1: return 4 * x;
-            case 2: return 2 * x;
-            case 3: return 2 * x + 1024;
-            default: return x + 512 * (ent - 4);
+    auto expo = [m, rb](int x, int ent) {                      // exponent of entry `ent` for W = w_M^x
+        if (rb == 16) {
+            switch (ent) {
+                case 0: return 8 * x;
+                case 1: return 4 * x;
+                case 2: return 2 * x;
+                case 3: return 2 * x + m / 8;
+                default: return x + m / 16 * (ent - 4);
+            }
         }
+        if (rb == 8) {
+            switch (ent) {
+                case 0: return 4 * x;
+                case 1: return 2 * x;
+                default: return x + m / 8 * ((ent - 2) & 1);
+            }
+        }
+        return ent == 0 ? 2 * x : x;
     };
-    if (i < 128) {
-        float4 f;
-        ct(expo(16 * (2 * row), ent), f.x, f.z);               // FB lane A: W = w512^(2 kap) = w8192^(32 kap)
-        ct(expo(16 * (2 * row + 1), ent), f.y, f.w);           // lane B: k1 = 2 kap + 1
-        g_tab.fb[row][ent] = f;
-        float2 g;
-        ct(expo(32 * row, ent), g.x, g.y);                     // I2: W = w256^n3 = w8192^(32 n3)
-        g_tab.i2[row][ent] = g;
-    }
+    float4 f;
+    ct(expo(16 * (2 * row), ent), f.x, f.z);                   // FB lane A: W = w_(32 RB)^(2 kap) = w_M^(32 kap)
+    ct(expo(16 * (2 * row + 1), ent), f.y, f.w);               // lane B: k1 = 2 kap + 1
+    g_tab.fb[lg][row][ent] = f;
+    float2 g;
+    ct(expo(32 * row, ent), g.x, g.y);                         // I2: W = w_(16 RB)^n3 = w_M^(32 n3)
+    g_tab.i2[lg][row][ent] = g;
 }
 
 }  // namespace v3
@@ -547,7 +586,7 @@ int init_iw3_tables(cudaStream_t st) {
     cudaGetDevice(&dev);
     const unsigned bit = 1u << (dev & 31);
     if (done.load(std::memory_order_acquire) & bit) return AMPLFI_OK;
-    v3::init_tables3_kernel<<<1, 128, 0, st>>>();
+    v3::init_tables3_kernel<<<1, 384, 0, st>>>();
     count_launch();
     const int rc = check_launch("init_tables3_kernel");
     if (rc) return rc;
@@ -556,28 +595,36 @@ int init_iw3_tables(cudaStream_t st) {
     return AMPLFI_OK;
 }
 
-template <int MODE, bool FWD>
+template <int LOGM, int MODE, bool FWD>
 static int launch_iw3_t(const IwArgs& a, int units, cudaStream_t st) {
+    using G = v3::Geo<LOGM>;
     static std::atomic<unsigned> attr_done{0};
-    const int rc = ensure_dynamic_smem(v3::inject_whiten3_kernel<MODE, FWD>, v3::SMEM_BYTES, attr_done);
+    const int rc = ensure_dynamic_smem(v3::inject_whiten3_kernel<LOGM, MODE, FWD>, G::SMEM_BYTES, attr_done);
     if (rc) return rc;
-    v3::inject_whiten3_kernel<MODE, FWD><<<units, v3::T, v3::SMEM_BYTES, st>>>(a, units);
+    v3::inject_whiten3_kernel<LOGM, MODE, FWD><<<units, G::T, G::SMEM_BYTES, st>>>(a, units);
     count_launch();
     return check_launch("inject_whiten3_kernel");
 }
 
-int launch_iw3(const IwArgs& a, int mode, int units, cudaStream_t st) {
+template <int LOGM>
+static int launch_iw3_l(const IwArgs& a, int mode, int units, cudaStream_t st) {
     if (a.noise == nullptr) {       // inverse-only launches (time-domain waveform, filter design)
-        if (mode == MODE_HDET) return launch_iw3_t<MODE_HDET, false>(a, units, st);
-        if (mode == MODE_FUSED) return launch_iw3_t<MODE_FUSED, false>(a, units, st);
+        if (mode == MODE_HDET) return launch_iw3_t<LOGM, MODE_HDET, false>(a, units, st);
+        if (mode == MODE_FUSED) return launch_iw3_t<LOGM, MODE_FUSED, false>(a, units, st);
         set_error("inject_whiten3: no data and nothing to inject");
         return AMPLFI_ERR_INVALID_ARG;
     }
     switch (mode) {
-        case MODE_NONE: return launch_iw3_t<MODE_NONE, true>(a, units, st);
-        case MODE_HDET: return launch_iw3_t<MODE_HDET, true>(a, units, st);
-        default: return launch_iw3_t<MODE_FUSED, true>(a, units, st);
+        case MODE_NONE: return launch_iw3_t<LOGM, MODE_NONE, true>(a, units, st);
+        case MODE_HDET: return launch_iw3_t<LOGM, MODE_HDET, true>(a, units, st);
+        default: return launch_iw3_t<LOGM, MODE_FUSED, true>(a, units, st);
     }
+}
+
+int launch_iw3(const IwArgs& a, int logm, int mode, int units, cudaStream_t st) {
+    if (logm == 13) return launch_iw3_l<13>(a, mode, units, st);
+    if (logm == 12) return launch_iw3_l<12>(a, mode, units, st);
+    return launch_iw3_l<11>(a, mode, units, st);
 }
 
 }  // namespace amplfi

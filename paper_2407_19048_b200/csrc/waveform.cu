@@ -136,23 +136,24 @@ __global__ void __launch_bounds__(256) sine_gaussian_kernel(const WfCoef* __rest
 // bin requested before the current one is evaluated; bins outside the band are written as exact zeros.
 template <int FAMILY>       // 0: TaylorF2 / IMRPhenomD (power tables), 1: sine-Gaussian (closed form)
 __global__ void __launch_bounds__(256, 4) waveform_slots_kernel(const WfCoef* __restrict__ coef, const double* __restrict__ tab_ci,
-                                                                const double* __restrict__ tab_lnk, float* __restrict__ h0) {
-    const int b = blockIdx.y, t = threadIdx.x, wi = t >> 5;
+                                                                const double* __restrict__ tab_lnk, float* __restrict__ h0, int kl) {
+    // blockDim.x = kl / 2 threads (the consumer's thread count)
+    const int b = blockIdx.y, t = threadIdx.x, wi = t >> 5, nt = kl >> 1;
     __shared__ WfCoef c;
     {
         const int* src = reinterpret_cast<const int*>(coef + b);
         int* dst = reinterpret_cast<int*>(&c);
-        if (threadIdx.x < (int)(sizeof(WfCoef) / sizeof(int))) dst[threadIdx.x] = src[threadIdx.x];
+        for (int q = threadIdx.x; q < (int)(sizeof(WfCoef) / sizeof(int)); q += blockDim.x) dst[q] = src[q];      // (64 .. 256 threads)
     }
     __syncthreads();
     if (!c.valid || c.k_lo > c.k_hi) return;
     const int k_lo = c.k_lo, k_hi = c.k_hi;
-    float4* row = reinterpret_cast<float4*>(h0 + (size_t)b * slot::H0_ROW);
+    float4* row = reinterpret_cast<float4*>(h0 + (size_t)b * slot::h0_row(kl));
 #pragma unroll 1
     for (int g = blockIdx.x; g < 16; g += gridDim.x) {
-        if (!slot::window_needed(g >> 3, g & 7, wi, k_lo, k_hi)) continue;
+        if (!slot::window_needed(kl, g >> 3, g & 7, wi, k_lo, k_hi)) continue;
         int kA, kB;
-        slot::slot_bins(g >> 3, g & 7, t, kA, kB);
+        slot::slot_bins(kl, g >> 3, g & 7, t, kA, kB);
         float2 hA = make_float2(0.f, 0.f), hB = make_float2(0.f, 0.f);
         const bool inA = kA >= k_lo && kA <= k_hi, inB = kB >= k_lo && kB <= k_hi;
         // the table values of both bins are requested together (one L2 round trip per slot)
@@ -171,7 +172,7 @@ __global__ void __launch_bounds__(256, 4) waveform_slots_kernel(const WfCoef* __
             }
             if (lane) hB = h; else hA = h;
         }
-        row[g * 256 + t] = make_float4(hA.x, hB.x, hA.y, hB.y);
+        row[g * nt + t] = make_float4(hA.x, hB.x, hA.y, hB.y);
     }
 }
 
@@ -191,10 +192,12 @@ int launch_waveform_pol(const amplfi_plan* p, int batch, float* hp, float* hc, c
 }
 
 int launch_waveform_h0(const amplfi_plan* p, int batch, cudaStream_t st, int slots) {
-    if (slots) {            // slot layout of the n = 16384 fused kernel
+    if (slots) {            // slot layout of the three-pass fused kernel (n = 4096 .. 16384)
+        const int kl = p->n / 32;
         dim3 grid(batch >= 1024 ? 2 : (batch >= 64 ? 4 : 8), batch);
-        if (p->last_approx == 2) waveform_slots_kernel<1><<<grid, 256, 0, st>>>(p->coef, p->tab_ci, p->tab_lnk, reinterpret_cast<float*>(p->h0));
-        else waveform_slots_kernel<0><<<grid, 256, 0, st>>>(p->coef, p->tab_ci, p->tab_lnk, reinterpret_cast<float*>(p->h0));
+        float* h0f = reinterpret_cast<float*>(p->h0);
+        if (p->last_approx == 2) waveform_slots_kernel<1><<<grid, kl / 2, 0, st>>>(p->coef, p->tab_ci, p->tab_lnk, h0f, kl);
+        else waveform_slots_kernel<0><<<grid, kl / 2, 0, st>>>(p->coef, p->tab_ci, p->tab_lnk, h0f, kl);
         count_launch();
         return check_launch("waveform_slots_kernel");
     }
