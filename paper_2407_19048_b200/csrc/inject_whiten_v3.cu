@@ -36,25 +36,31 @@ using namespace tn;
 // Geometry of a segment length: M = 2^LOGM = 32 * RB * 16 complex points, RB = 16 / 8 / 4 for n = 16384 / 8192 / 4096
 // (the paper's own 4 s at 2048 Hz is n = 8192); T = M/32 threads (256 / 128 / 64), 2 / 4 / 8 CTAs per SM.
 // Pass FB / I2 is then a radix RB, of which every thread takes 16/RB.
+// n = 32768 (LOGM = 14): M = 32 * (4 * 8) * 16, the middle pass split in two (FB1 radix 4 over n2a, FB2 radix 8 over
+// n2b; a third exchange), 512 threads, one CTA per SM.
 template <int LOGM>
 struct Geo {
     static constexpr int M = 1 << LOGM, N = 2 * M, K = M + 1;
     static constexpr int T = M / 32;                  // threads
     static constexpr int KL = M / 16;                 // span of klow = k1 + 32 k2
-    static constexpr int RB = M / 512;                // radix of the middle pass
+    static constexpr int RB = LOGM <= 13 ? M / 512 : 4;   // radix of the middle pass (LOGM = 14: of its first half)
     static constexpr int NB = 16 / RB;                // middle-pass butterflies per thread
-    static constexpr int PLANE = RB * 544;            // floats per plane
+    static constexpr int PLANE = (M / 512) * 544;     // floats per plane
     static constexpr int SMEM_BYTES = 2 * PLANE * (int)sizeof(float);
-    static constexpr int CTAS = 512 / T;              // per SM (registers: 128 per thread)
+    static constexpr int CTAS = T >= 512 ? 1 : 512 / T;   // per SM (registers: 128 per thread)
 };
 constexpr int ROW = 34, BLK = 16 * ROW;               // 34, 544 floats
 
 // FB: per-lane twiddles of W = w_(32 RB)^k1, k1 = 2 kap (lane A), 2 kap + 1 (lane B): (cA, cB, tauA, tauB)
 // I2: shared twiddles of W = w_(16 RB)^n3 (used conjugated): (c, tau)
-// rows in the layout fft_tan.cuh gives each radix; one set per segment length [LOGM - 11]
+// rows in the layout fft_tan.cuh gives each radix; one set per segment length [LOGM - 11].
+// LOGM = 14: fb1 W = w_128^k1 [kap], fb2 W = w_1024^(k1 + 32 k2a) [4 kap + k2a], i2b W = w_128^n3 [n3],
+//            i2a W = w_512^(n3 + 16 n2b) [16 n2b + n3].
 struct Tables {
     float4 fb[3][16][8];
     float2 i2[3][16][8];
+    float4 fb1_14[16][2], fb2_14[64][4];
+    float2 i2b_14[16][4], i2a_14[128][2];
 };
 static __device__ Tables g_tab;
 
@@ -255,6 +261,16 @@ __global__ void __launch_bounds__(Geo<LOGM>::T, Geo<LOGM>::CTAS) inject_whiten3_
         }
     }
 
+    // the factor conj(w32^n3) of the self-paired column klow = KL/2 (lane B of thread 0 in FC, whose twiddles are those of
+    // klow = 0, i.e. 1): one complex product in the 16 threads that produce that column
+    auto column_factor = [&](C2& v) {
+        float ar_, br_, ai_, bi_;
+        unpack(v.r, ar_, br_);
+        unpack(v.i, ai_, bi_);
+        const float co = kCos32[n3], si = kSin32[n3];
+        v = C2{pack(ar_ * co - ai_ * si, br_), pack(ar_ * si + ai_ * co, bi_)};
+    };
+    if constexpr (LOGM <= 13) {
     // ---- FB: radix RB over n2 (NB butterflies per thread) ----
     if (FWD) {
         Tw2 tw[NB][8];
@@ -273,18 +289,53 @@ __global__ void __launch_bounds__(Geo<LOGM>::T, Geo<LOGM>::CTAS) inject_whiten3_
 #pragma unroll
             for (int r = 0; r < RB; ++r) v[brev<RB>(r)] = lds2(re, im, ob + r * BLK);
             dit_r<RB, false, Tw2, true>(v, tw[i]);           // k2 >= RB/2 (the klow >= KL/2 read by lane B of FC) stored conjugated
-            if (((tid + T * i) >> 4) == 0) {
-                // the self-paired column klow = KL/2 (k1 = 0, k2 = RB/2; lane B of thread 0 in FC, whose twiddles are those
-                // of klow = 0, i.e. 1) takes its factor conj(w32^n3) here: one complex product in 16 threads
-                float ar_, br_, ai_, bi_;
-                unpack(v[RB / 2].r, ar_, br_);
-                unpack(v[RB / 2].i, ai_, bi_);
-                const float co = kCos32[n3], si = kSin32[n3];
-                v[RB / 2] = C2{pack(ar_ * co - ai_ * si, br_), pack(ar_ * si + ai_ * co, bi_)};
-            }
+            if (((tid + T * i) >> 4) == 0) column_factor(v[RB / 2]);        // column KL/2: k1 = 0, k2 = RB/2
 #pragma unroll
             for (int k2 = 0; k2 < RB; ++k2) sts2(re, im, ob + k2 * BLK, v[k2]);
         }
+    }
+    } else {
+    // ---- n = 32768: FB1 radix 4 over n2a (4 butterflies per thread), FB2 radix 8 over n2b (2 per thread) ----
+    // element (d2a, d2b, n3, k1) at (8 d2a + d2b) * BLK + n3 * ROW + k1
+    if (FWD) {
+        __syncthreads();
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int c = tid + T * i, n2b = (c >> 4) & 7, kap = c >> 7;
+            Tw2 tw[8];
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const float4 f = __ldg(&g_tab.fb1_14[kap][e]);
+                tw[e] = Tw2{pack(f.x, f.y), pack(f.z, f.w)};
+            }
+            const int o = n2b * BLK + n3 * ROW + 2 * kap;
+            C2 v[4];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) v[brev<4>(r)] = lds2(re, im, o + r * 8 * BLK);
+            dit4<false>(v, tw);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) sts2(re, im, o + q * 8 * BLK, v[q]);
+        }
+        __syncthreads();
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            const int c = tid + T * i, k2a = (c >> 4) & 3, kap = c >> 6;
+            Tw2 tw[8];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const float4 f = __ldg(&g_tab.fb2_14[4 * kap + k2a][e]);
+                tw[e] = Tw2{pack(f.x, f.y), pack(f.z, f.w)};
+            }
+            const int o = k2a * 8 * BLK + n3 * ROW + 2 * kap;
+            C2 v[8];
+#pragma unroll
+            for (int r = 0; r < 8; ++r) v[brev<8>(r)] = lds2(re, im, o + r * BLK);
+            dit8<false, Tw2, true>(v, tw);                   // k2b >= 4 (klow >= KL/2) stored conjugated
+            if (kap == 0 && k2a == 0) column_factor(v[4]);   // column KL/2 = 512: k1 = 0, k2a = 0, k2b = 4
+#pragma unroll
+            for (int q = 0; q < 8; ++q) sts2(re, im, o + q * BLK, v[q]);
+        }
+    }
     }
     if (sl >= 0 && sl <= 16) {
         float2 ia = make_float2(0.f, 0.f), ib = make_float2(0.f, 0.f);            // what the injection adds to 2 X[k], 2 X[M-k]
@@ -303,7 +354,9 @@ __global__ void __launch_bounds__(Geo<LOGM>::T, Geo<LOGM>::CTAS) inject_whiten3_
 
     // ---- FC: radix 16 over n3; lane A klow = t, lane B klow = 512 - t ----
     const int ka = t, kb = (t == 0) ? KL / 2 : KL - t;
-    const int oa = (ka >> 5) * BLK + (ka & 31), obb = (kb >> 5) * BLK + (kb & 31);
+    // column klow = k1 + 32 k2 lives at d2 = k2 (n = 32768: klow = k1 + 32 k2a + 128 k2b at d2 = 8 k2a + k2b)
+    auto column = [](int klow) { return (LOGM <= 13 ? (klow >> 5) : 8 * ((klow >> 5) & 3) + (klow >> 7)) * BLK + (klow & 31); };
+    const int oa = column(ka), obb = column(kb);
     // Lane B works on the CONJUGATED column 512 - t (FB stored it so): conj Z[512 - t + 512 q] = sum_n3 conj(B[n3]) W^n3
     // w16^(-n3 (q + 1)) with lane A's own W = w8192^t, i.e. the same twiddles serve both lanes and lane B's outputs appear
     // conjugated and reversed: v[q] = (Z[t + 512 q] | conj Z[512 - t + 512 (15 - q)]) -- exactly the partner bin of lane A.
@@ -481,6 +534,7 @@ __global__ void __launch_bounds__(Geo<LOGM>::T, Geo<LOGM>::CTAS) inject_whiten3_
             re[obb + q * ROW] = br; im[obb + q * ROW] = bi;
         }
     }
+    if constexpr (LOGM <= 13) {
     // ---- I2: inverse radix RB over k2 (NB butterflies per thread; the twiddles depend on n3 only) ----
     {
         Tw1 tw[8];
@@ -500,6 +554,47 @@ __global__ void __launch_bounds__(Geo<LOGM>::T, Geo<LOGM>::CTAS) inject_whiten3_
 #pragma unroll
             for (int q = 0; q < RB; ++q) sts2(re, im, ob + q * BLK, w[q]);
         }
+    }
+    } else {
+    // ---- n = 32768: I2b inverse radix 8 over k2b (twiddles by n3), I2a inverse radix 4 over k2a (twiddles by n3, n2b) ----
+    {
+        Tw1 tw[8];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const float2 f = __ldg(&g_tab.i2b_14[n3][e]);
+            tw[e] = Tw1{f.x, f.y};
+        }
+        __syncthreads();
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            const int c = tid + T * i, k2a = (c >> 4) & 3, kap = c >> 6;
+            const int o = k2a * 8 * BLK + n3 * ROW + 2 * kap;
+            C2 w[8];
+#pragma unroll
+            for (int r = 0; r < 8; ++r) w[brev<8>(r)] = lds2(re, im, o + r * BLK);
+            dit8<true>(w, tw);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) sts2(re, im, o + q * BLK, w[q]);
+        }
+        __syncthreads();
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            const int c = tid + T * i, n2b = (c >> 4) & 7, kap = c >> 7;
+            Tw1 ta[8];
+#pragma unroll
+            for (int e = 0; e < 2; ++e) {
+                const float2 f = __ldg(&g_tab.i2a_14[16 * n2b + n3][e]);
+                ta[e] = Tw1{f.x, f.y};
+            }
+            const int o = n2b * BLK + n3 * ROW + 2 * kap;
+            C2 w[4];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) w[brev<4>(r)] = lds2(re, im, o + r * 8 * BLK);
+            dit4<true>(w, ta);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) sts2(re, im, o + q * 8 * BLK, w[q]);
+        }
+    }
     }
     // ---- I3: inverse radix 32 over k1, natural-order stores ----
     {
@@ -577,6 +672,45 @@ __global__ void init_tables3_kernel() {
     g_tab.i2[lg][row][ent] = g;
 }
 
+// n = 32768 (M = 16384): radix-4 rows (W^2, W) and radix-8 rows (W^4, W^2, W, W w8)
+__global__ void init_tables3_14_kernel() {
+    constexpr int m = 16384;
+    auto ct = [](int e, float& c, float& tau) {
+        double s, co;
+        sincospi(-2.0 * (double)(e & (m - 1)) / (double)m, &s, &co);
+        if (fabs(co) < 1e-12) co = 1e-12;
+        c = (float)co;
+        tau = (float)(s / co);
+    };
+    auto e4 = [](int x, int ent) { return ent == 0 ? 2 * x : x; };
+    auto e8 = [](int x, int ent) { return ent == 0 ? 4 * x : (ent == 1 ? 2 * x : x + m / 8 * (ent - 2)); };
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;       // 0 .. 511
+    if (i < 32) {                                              // fb1: W = w_128^k1 = w_M^(128 k1), lanes k1 = 2 kap, 2 kap + 1
+        const int kap = i >> 1, ent = i & 1;
+        float4 f;
+        ct(e4(128 * (2 * kap), ent), f.x, f.z);
+        ct(e4(128 * (2 * kap + 1), ent), f.y, f.w);
+        g_tab.fb1_14[kap][ent] = f;
+    }
+    if (i < 256) {                                             // fb2: W = w_1024^(k1 + 32 k2a) = w_M^(16 (k1 + 32 k2a))
+        const int row = i >> 2, ent = i & 3, kap = row >> 2, k2a = row & 3;
+        float4 f;
+        ct(e8(16 * (2 * kap + 32 * k2a), ent), f.x, f.z);
+        ct(e8(16 * (2 * kap + 1 + 32 * k2a), ent), f.y, f.w);
+        g_tab.fb2_14[row][ent] = f;
+        const int row2 = i >> 1, ent2 = i & 1;                  // i2a: W = w_512^(n3 + 16 n2b) = w_M^(32 row), row = 16 n2b + n3
+        float2 g;
+        ct(e4(32 * row2, ent2), g.x, g.y);
+        g_tab.i2a_14[row2][ent2] = g;
+    }
+    if (i < 64) {                                              // i2b: W = w_128^n3 = w_M^(128 n3)
+        const int n3 = i >> 2, ent = i & 3;
+        float2 g;
+        ct(e8(128 * n3, ent), g.x, g.y);
+        g_tab.i2b_14[n3][ent] = g;
+    }
+}
+
 }  // namespace v3
 
 // Once per device (amplfi_plan_create synchronises before it returns).
@@ -587,7 +721,8 @@ int init_iw3_tables(cudaStream_t st) {
     const unsigned bit = 1u << (dev & 31);
     if (done.load(std::memory_order_acquire) & bit) return AMPLFI_OK;
     v3::init_tables3_kernel<<<1, 384, 0, st>>>();
-    count_launch();
+    v3::init_tables3_14_kernel<<<1, 256, 0, st>>>();
+    count_launch(2);
     const int rc = check_launch("init_tables3_kernel");
     if (rc) return rc;
     if (cudaStreamSynchronize(st) != cudaSuccess) { set_error("init_tables3_kernel: synchronise failed"); return AMPLFI_ERR_CUDA; }
@@ -622,6 +757,7 @@ static int launch_iw3_l(const IwArgs& a, int mode, int units, cudaStream_t st) {
 }
 
 int launch_iw3(const IwArgs& a, int logm, int mode, int units, cudaStream_t st) {
+    if (logm == 14) return launch_iw3_l<14>(a, mode, units, st);
     if (logm == 13) return launch_iw3_l<13>(a, mode, units, st);
     if (logm == 12) return launch_iw3_l<12>(a, mode, units, st);
     return launch_iw3_l<11>(a, mode, units, st);

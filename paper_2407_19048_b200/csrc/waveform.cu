@@ -135,7 +135,7 @@ __global__ void __launch_bounds__(256) sine_gaussian_kernel(const WfCoef* __rest
 // SM: the kernel is bound by the latency of the fp64 phase chain, so resident warps count), the table values of the next
 // bin requested before the current one is evaluated; bins outside the band are written as exact zeros.
 template <int FAMILY>       // 0: TaylorF2 / IMRPhenomD (power tables), 1: sine-Gaussian (closed form)
-__global__ void __launch_bounds__(256, 4) waveform_slots_kernel(const WfCoef* __restrict__ coef, const double* __restrict__ tab_ci,
+__global__ void __launch_bounds__(512, 2) waveform_slots_kernel(const WfCoef* __restrict__ coef, const double* __restrict__ tab_ci,
                                                                 const double* __restrict__ tab_lnk, float* __restrict__ h0, int kl) {
     // blockDim.x = kl / 2 threads (the consumer's thread count)
     const int b = blockIdx.y, t = threadIdx.x, wi = t >> 5, nt = kl >> 1;
