@@ -75,6 +75,17 @@ const char* amplfi_version(void);
  * 209 doubles.  (Used by the tests to check the library's copy against the oracle's.) */
 int amplfi_phenomd_table(double* out);
 
+/* The Kerr l = m = 2, n = 0 quasi-normal mode the IMRPhenomD ringdown uses (ref. [32]), as
+ * the library tabulates it at first use (Leaver's continued fractions, csrc/kerr_qnm.cu): 512 nodes uniform in
+ * y = sqrt(1 - a/M) from a/M = +0.998 (node 0) down to -0.998; `out` is a HOST buffer of 1024 doubles receiving
+ * (Re M omega, -Im M omega) per node.  Returns the node count, or a negative status.  M f_RD = Re/(2 pi),
+ * M f_damp = -Im/(2 pi) per remnant mass, interpolated with a four-point Lagrange cubic in y.
+ * Conventions of the approximant (reading R-W1 of DESIGN.md): Psi(f) = 2 pi f t_c - 2 phi_c + phi_IMR(Mf) - t0 Mf with
+ * t0 = d phi_IMR / d(Mf) at the amplitude peak f_peak INCLUDING the C1-junction constant of the merger-ringdown
+ * region (the true phase derivative there), so that the time-domain amplitude peak sits at t_c; there is no
+ * reference-frequency term. */
+int amplfi_qnm_table(double* out);
+
 /* Create a plan for segments of n samples at fs Hz seen by n_det detectors.
  *   n        power of two, 2^10 .. 2^20 (4 s at 2048 Hz = 8192; minutes-long
  *            binary-neutron-star segments are "larger by an order of magnitude": 256 s at 4096 Hz = 2^20)

@@ -129,10 +129,20 @@ def e_rad(eta, chi1, chi2):
 
 
 def ringdown_freqs(eta, chi1, chi2):
-    """(M f_RD, M f_damp) of the l=m=2, n=0 Kerr mode of the remnant, in units of the INITIAL total
-    mass.  R-W1b: the Berti-Cardoso-Will closed-form fit (f = [1.5251 - 1.1568 (1-a)^0.1292]/(2 pi),
-    Q = 0.7 + 1.4187 (1-a)^(-0.4990), f_damp = f/(2Q)) replaces the tabulated QNM data that [32]
-    interpolates; both are divided by the remnant mass 1 - E_rad."""
+    """(M f_RD, M f_damp) of the l = m = 2, n = 0 Kerr mode of the remnant, in units of the INITIAL total mass:
+    f_RD = Re(omega)/(2 pi), f_damp = -Im(omega)/(2 pi) with M_f omega of the mode at the final spin (oracle/qnm.py:
+    Leaver's continued fractions, tabulated and spline-interpolated, i.e. the function whose Berti-Cardoso-Will
+    tabulation [32] interpolates), both divided by the remnant mass 1 - E_rad.  Reading R-W1b."""
+    from .qnm import qnm_220
+    a = final_spin(eta, chi1, chi2)
+    w_re, w_im = qnm_220(a)
+    m_f = 1.0 - e_rad(eta, chi1, chi2)
+    return w_re / (2.0 * np.pi) / m_f, w_im / (2.0 * np.pi) / m_f
+
+
+def ringdown_freqs_fit(eta, chi1, chi2):
+    """The same from the Berti-Cardoso-Will closed-form fit (f = [1.5251 - 1.1568 (1-a)^0.1292]/(2 pi),
+    Q = 0.7 + 1.4187 (1-a)^(-0.4990), f_damp = f/(2Q); accurate to a few per cent): kept as a cross-check of the table."""
     a = final_spin(eta, chi1, chi2)
     a = min(max(a, -0.999999), 0.999999)
     f_ring = (1.5251 - 1.1568 * (1.0 - a) ** 0.1292) / (2.0 * np.pi)

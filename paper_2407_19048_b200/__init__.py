@@ -24,7 +24,7 @@ EXPORTS = ("amplfi_last_error", "amplfi_psd_scale", "amplfi_version", "amplfi_ph
            "amplfi_plan_create", "amplfi_plan_destroy", "amplfi_waveform_fd", "amplfi_project",
            "amplfi_psd_welch", "amplfi_inject_whiten", "amplfi_launch_count", "amplfi_plan_set_timing",
            "amplfi_plan_kernel_times", "amplfi_assemble_batch", "amplfi_probe_fp32_pipe",
-           "amplfi_inject_whiten_views", "amplfi_waveform_td", "amplfi_inject_whiten_fir")
+           "amplfi_inject_whiten_views", "amplfi_waveform_td", "amplfi_inject_whiten_fir", "amplfi_qnm_table")
 
 
 class AmplfiError(RuntimeError):
@@ -50,6 +50,8 @@ def _load():
     lib.amplfi_launch_count.argtypes = []
     lib.amplfi_phenomd_table.restype = i32
     lib.amplfi_phenomd_table.argtypes = [vp]
+    lib.amplfi_qnm_table.restype = i32
+    lib.amplfi_qnm_table.argtypes = [vp]
     lib.amplfi_plan_create.restype = i32
     lib.amplfi_plan_create.argtypes = [i32, dbl, i32, c.POINTER(i32), i32, i32, c.POINTER(vp)]
     lib.amplfi_plan_destroy.restype = None
@@ -149,6 +151,17 @@ def phenomd_table():
     buf = (ctypes.c_double * 209)()
     _check(_lib.amplfi_phenomd_table(ctypes.cast(buf, ctypes.c_void_p)))
     return [list(buf[r * 11:(r + 1) * 11]) for r in range(19)]
+
+
+def qnm_table():
+    """(spins, Re M omega, -Im M omega) of the Kerr (2,2,0) mode as the library tabulates it (host computation, no GPU)."""
+    buf = (ctypes.c_double * 1024)()
+    n = _lib.amplfi_qnm_table(ctypes.cast(buf, ctypes.c_void_p))
+    if n < 0:
+        _check(n)
+    y_lo, y_hi = (1.0 - 0.998) ** 0.5, (1.0 + 0.998) ** 0.5
+    spins = [1.0 - (y_lo + (y_hi - y_lo) * i / (n - 1)) ** 2 for i in range(n)]
+    return spins, [buf[2 * i] for i in range(n)], [buf[2 * i + 1] for i in range(n)]
 
 
 class Plan:

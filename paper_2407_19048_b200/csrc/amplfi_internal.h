@@ -8,6 +8,8 @@
 #include "phenomd_table.h"
 
 #define AMPLFI_TIMING_RING 512
+#define AMPLFI_QNM_NODES 512         /* Kerr (2,2,0) mode on a grid uniform in sqrt(1 - a/M), a/M from +0.998 down to -0.998 */
+#define AMPLFI_QNM_OFFSET 216        /* doubles: the mode table follows the 19 x 11 fit table in plan->pd_table */
 
 namespace amplfi {
 struct WfCoef;
@@ -29,7 +31,7 @@ struct amplfi_plan {
     // device tables / workspace (owned)
     double* tab_ci;        // [n_bins] k^(-1/3)   (tab_ci[0] = 0)
     double* tab_lnk;       // [n_bins] ln k       (tab_lnk[0] = 0)
-    double* pd_table;      // [19*11]
+    double* pd_table;      // [19*11] fit table, then at AMPLFI_QNM_OFFSET the Kerr mode table [AMPLFI_QNM_NODES][2]
     amplfi::WfCoef* coef;  // [max_batch]
     amplfi::DetResp* resp; // [max_batch * n_det]
     amplfi::DetResp* resp2; // [max_batch * 3]  second view: resp with dt + t_shift[b]; also the two "polarisation detectors" of
@@ -75,6 +77,9 @@ inline int ensure_dynamic_smem(Kernel kernel, int bytes, std::atomic<unsigned>& 
     done.fetch_or(bit, std::memory_order_release);
     return AMPLFI_OK;
 }
+
+// kerr_qnm.cu (host): (Re M omega, -Im M omega) of the Kerr (2,2,0) mode per node, computed once per process; nullptr on failure
+const double* kerr_qnm_table();
 
 // waveform.cu
 int launch_prepare(const amplfi_plan* p, int approximant, int batch, const double* params, double gmst,

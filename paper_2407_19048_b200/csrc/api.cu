@@ -146,6 +146,14 @@ int amplfi_phenomd_table(double* out) {
     return AMPLFI_OK;
 }
 
+int amplfi_qnm_table(double* out) {
+    if (out == nullptr) { set_error("amplfi_qnm_table: null output"); return AMPLFI_ERR_INVALID_ARG; }
+    const double* qnm = kerr_qnm_table();
+    if (qnm == nullptr) { set_error("amplfi_qnm_table: the continued-fraction iteration did not converge"); return AMPLFI_ERR_CUDA; }
+    std::memcpy(out, qnm, sizeof(double) * 2 * AMPLFI_QNM_NODES);
+    return AMPLFI_QNM_NODES;
+}
+
 int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_batch, int nperseg,
                        amplfi_plan** out) {
     if (out == nullptr || det_ids == nullptr) { set_error("amplfi_plan_create: null pointer"); return AMPLFI_ERR_INVALID_ARG; }
@@ -178,7 +186,7 @@ int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_
     int rc = AMPLFI_OK;
     if (!rc) rc = dev_alloc(&p->tab_ci, (size_t)p->n_bins);
     if (!rc) rc = dev_alloc(&p->tab_lnk, (size_t)p->n_bins);
-    if (!rc) rc = dev_alloc(&p->pd_table, (size_t)AMPLFI_PD_ROWS * AMPLFI_PD_COLS);
+    if (!rc) rc = dev_alloc(&p->pd_table, (size_t)AMPLFI_QNM_OFFSET + 2 * AMPLFI_QNM_NODES);
     if (!rc) rc = dev_alloc(&p->coef, (size_t)max_batch);
     if (!rc) rc = dev_alloc(&p->resp, (size_t)max_batch * n_det);
     if (!rc) rc = dev_alloc(&p->resp2, (size_t)max_batch * 3);
@@ -200,6 +208,9 @@ int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_
     if (!rc && nperseg) rc = dev_alloc(&p->welch_part, (size_t)n_det * p->welch_max_seg * (nperseg / 2 + 1));
     if (!rc) {
         e = cudaMemcpy(p->pd_table, kPdTable, sizeof(kPdTable), cudaMemcpyHostToDevice);
+        const double* qnm = kerr_qnm_table();
+        if (qnm == nullptr) { set_error("amplfi_plan_create: the Kerr quasi-normal-mode table did not converge"); rc = AMPLFI_ERR_CUDA; }
+        else if (e == cudaSuccess) e = cudaMemcpy(p->pd_table + AMPLFI_QNM_OFFSET, qnm, sizeof(double) * 2 * AMPLFI_QNM_NODES, cudaMemcpyHostToDevice);
         if (e == cudaSuccess) e = cudaMemcpy(p->d_det_ids, p->det_ids, sizeof(int) * 3, cudaMemcpyHostToDevice);
         if (e != cudaSuccess) { set_error("amplfi_plan_create: cudaMemcpy: %s", cudaGetErrorString(e)); rc = AMPLFI_ERR_CUDA; }
     }

@@ -255,17 +255,31 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
                 + (0.1014665242971878 * eta - 2.0967746996832157 * e2) * stot * stot
                 + (-1.3546806617824356 * eta + 4.108962025369336 * e2) * stot * stot * stot
                 + (-0.8676969352555539 * eta + 2.064046835273906 * e2) * stot * stot * stot * stot;
-    af = fmin(fmax(af, -0.999999), 0.999999);
+    af = fmin(fmax(af, -0.998), 0.998);                    // the mode table's range
     const double sn = stot / (m1 * m1 + m2 * m2);
     const double erad = (eta * (0.055974469826360077 + 0.5809510763115132 * eta - 0.9606726679372312 * e2
                                 + 3.352411249771192 * e3)
                          * (1.0 + (-0.0030302335878845507 - 2.0066110851351073 * eta + 7.7050567802399215 * e2) * sn))
                         / (1.0 + (-0.6714403054720589 - 1.4756929437702908 * eta + 7.304676214885011 * e2) * sn);
-    const double ln1maf = plog(1.0 - af);
-    const double fring0 = (1.5251 - 1.1568 * pexp(0.1292 * ln1maf)) * I2PI;
-    const double qual = 0.7 + 1.4187 * pexp(-0.4990 * ln1maf);
-    const double f_rd = fring0 / (1.0 - erad);
-    const double f_dm = fring0 / (2.0 * qual) / (1.0 - erad);
+    // Kerr (2,2,0) mode at the final spin: four-point Lagrange cubic on the plan's table (kerr_qnm.cu; nodes uniform in
+    // y = sqrt(1 - a), from a = +0.998 down to -0.998), f_RD = Re(omega)/2 pi, f_damp = -Im(omega)/2 pi per remnant mass
+    double w_re, w_im;
+    {
+        const double* qnm = tab + AMPLFI_QNM_OFFSET;
+        const double y_lo = 0.044721359549995794 /* sqrt(0.002) */, y_hi = 1.4135062787267694 /* sqrt(1.998) */;
+        const double inv_h = (double)(AMPLFI_QNM_NODES - 1) / (y_hi - y_lo);
+        const double u = (psqrt(1.0 - af) - y_lo) * inv_h;
+        int i = (int)floor(u);
+        i = i < 1 ? 1 : (i > AMPLFI_QNM_NODES - 3 ? AMPLFI_QNM_NODES - 3 : i);
+        const double t = u - (double)i;
+        const double l0 = -t * (t - 1.0) * (t - 2.0) * (1.0 / 6.0), l1 = (t + 1.0) * (t - 1.0) * (t - 2.0) * 0.5;
+        const double l2 = -(t + 1.0) * t * (t - 2.0) * 0.5, l3 = (t + 1.0) * t * (t - 1.0) * (1.0 / 6.0);
+        const double* q = qnm + 2 * (i - 1);
+        w_re = l0 * q[0] + l1 * q[2] + l2 * q[4] + l3 * q[6];
+        w_im = l0 * q[1] + l1 * q[3] + l2 * q[5] + l3 * q[7];
+    }
+    const double f_rd = w_re * I2PI / (1.0 - erad);
+    const double f_dm = w_im * I2PI / (1.0 - erad);
 
     const double sg1 = fit[PD_SIGMA1], sg2 = fit[PD_SIGMA2], sg3 = fit[PD_SIGMA3], sg4 = fit[PD_SIGMA4];
     const double be1 = fit[PD_BETA1], be2 = fit[PD_BETA2], be3 = fit[PD_BETA3];

@@ -63,6 +63,21 @@ def test_phenomd_table_matches_oracle_copy(lib):
     assert np.array_equal(got, want)
 
 
+def test_kerr_mode_table_of_the_library_against_the_oracle_solver(lib):
+    """The library tabulates the Kerr (2,2,0) mode with its own C++ continued-fraction solver (csrc/kerr_qnm.cu, host code:
+    no GPU needed); the oracle's Python solver / table (oracle/qnm.py) is an independent implementation of Leaver's method."""
+    from oracle import qnm
+    spins, w_re, w_im = lib.qnm_table()
+    assert len(spins) == 512 and abs(spins[0] - 0.998) < 1e-12 and abs(spins[-1] + 0.998) < 1e-12
+    for i in range(0, 512, 7):
+        r, im = qnm.qnm_220(spins[i])
+        tol = 1e-8 if abs(spins[i]) <= 0.98 else 1e-6           # (the oracle's spline is coarser next to the extremal hole)
+        assert abs(w_re[i] / r - 1.0) < tol and abs(w_im[i] / im - 1.0) < tol
+    i0 = min(range(512), key=lambda i: abs(spins[i]))
+    w, _ = qnm.kerr_qnm_220(spins[i0])                      # a direct solve, not the oracle's table
+    assert abs(w_re[i0] - w.real) < 1e-10 and abs(w_im[i0] + w.imag) < 1e-10
+
+
 def test_argument_validation_without_device(lib):
     L = lib._lib
     h = ctypes.c_void_p()
