@@ -149,12 +149,17 @@ __global__ void __launch_bounds__(512, 2) waveform_slots_kernel(const WfCoef* __
     if (!c.valid || c.k_lo > c.k_hi) return;
     const int k_lo = c.k_lo, k_hi = c.k_hi;
     float4* row = reinterpret_cast<float4*>(h0 + (size_t)b * slot::h0_row(kl));
+    // groups of this warp: bit g = second * 8 + w set iff the consumer reads it (one ballot instead of a test per group);
+    // the CTAs of a sample share them round-robin
+    const int lane_id = t & 31;
+    unsigned todo = __ballot_sync(0xffffffffu, lane_id < 16 && (lane_id % gridDim.x) == blockIdx.x &&
+                                                   slot::window_needed(kl, lane_id >> 3, lane_id & 7, wi, k_lo, k_hi));
 #pragma unroll 1
-    for (int g = blockIdx.x; g < 16; g += gridDim.x) {
-        if (!slot::window_needed(kl, g >> 3, g & 7, wi, k_lo, k_hi)) continue;
+    while (todo) {
+        const int g = __ffs(todo) - 1;
+        todo &= todo - 1;
         int kA, kB;
         slot::slot_bins(kl, g >> 3, g & 7, t, kA, kB);
-        float2 hA = make_float2(0.f, 0.f), hB = make_float2(0.f, 0.f);
         const bool inA = kA >= k_lo && kA <= k_hi, inB = kB >= k_lo && kB <= k_hi;
         // the table values of both bins are requested together (one L2 round trip per slot)
         double ciA = 1.0, lnA = 0.0, ciB = 1.0, lnB = 0.0;
@@ -162,6 +167,7 @@ __global__ void __launch_bounds__(512, 2) waveform_slots_kernel(const WfCoef* __
             if (inA) { ciA = tab_ci[kA]; lnA = tab_lnk[kA]; }
             if (inB) { ciB = tab_ci[kB]; lnB = tab_lnk[kB]; }
         }
+        float2 hA = make_float2(0.f, 0.f), hB = make_float2(0.f, 0.f);
 #pragma unroll 1
         for (int lane = 0; lane < 2; ++lane) {
             const int k = lane ? kB : kA;
