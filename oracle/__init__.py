@@ -23,8 +23,11 @@ Parity status of the oracle itself:
   * oracle.fft, oracle.welch, oracle.whiten, oracle.project, TaylorF2 in oracle.waveform:
     pinned (numpy.fft / scipy.signal.welch / numpy.interp agreement, closed forms,
     brute force, worked-example values under tests/golden/).
-  * oracle.waveform.imrphenomd: **parity unpinned** against a true IMRPhenomD
-    implementation (lalsimulation is not available and PAPER.md prints neither the ansatz
-    nor the fit table).  Only structural pins hold (reduction to TaylorF2, C1 junctions,
-    low-frequency amplitude limit, symmetries, remnant textbook values).
+  * oracle.waveform.imrphenomd: every closed-form ingredient is pinned (aligned-spin PN phase and
+    amplitude coefficients against the (chi_s, chi_a, delta) form of [32] App. B, test-mass limits of
+    the remnant fits, exchange symmetry, C1 junctions, the time-domain peak at t_c:
+    tests/test_oracle_phenomd_pins.py; the Kerr (2,2,0) mode against published values and the
+    defining continued fractions: tests/test_oracle_qnm.py).  What stays **parity unpinned** is
+    oracle.phenomd_coeffs.TABLE, the 19 x 11 fitted numbers of [32] Table V, typed as recalled:
+    lalsimulation is not available and PAPER.md prints none of them (DESIGN.md R-W1).
 """

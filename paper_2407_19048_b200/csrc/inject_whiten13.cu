@@ -466,24 +466,13 @@ static int launch_iw13_t(const IwArgs& a, int units, cudaStream_t st) {
 
 template <int LOGM>
 static int launch_iw13_l(const IwArgs& a, int mode, int units, cudaStream_t st) {
-    if (a.out2 != nullptr) {        // two data views from one forward transform
-        if (mode != MODE_FUSED || a.noise == nullptr || a.t_shift == nullptr || a.crop != 0) {
-            set_error("inject_whiten13: the two-view launch needs the fused mode");
-            return AMPLFI_ERR_INVALID_ARG;
-        }
-        return launch_iw13_t<LOGM, MODE_FUSED, true, 2>(a, units, st);
-    }
-    if (a.noise == nullptr) {       // inverse-only launches (time-domain waveform, filter design)
-        if (mode == MODE_HDET) return launch_iw13_t<LOGM, MODE_HDET, false>(a, units, st);
-        if (mode == MODE_FUSED) return launch_iw13_t<LOGM, MODE_FUSED, false>(a, units, st);
-        set_error("inject_whiten13: no data and nothing to inject");
+    // only the one-launch two-view call still runs this kernel (every single-view launch of n = 4096, 8192, 16384 goes to
+    // inject_whiten_v3.cu)
+    if (a.out2 == nullptr || mode != MODE_FUSED || a.noise == nullptr || a.t_shift == nullptr || a.crop != 0) {
+        set_error("inject_whiten13: the two-view launch needs the fused mode");
         return AMPLFI_ERR_INVALID_ARG;
     }
-    switch (mode) {
-        case MODE_NONE: return launch_iw13_t<LOGM, MODE_NONE, true>(a, units, st);
-        case MODE_HDET: return launch_iw13_t<LOGM, MODE_HDET, true>(a, units, st);
-        default: return launch_iw13_t<LOGM, MODE_FUSED, true>(a, units, st);
-    }
+    return launch_iw13_t<LOGM, MODE_FUSED, true, 2>(a, units, st);
 }
 
 int launch_iw13(const IwArgs& a, int logm, int mode, int units, cudaStream_t st) {
