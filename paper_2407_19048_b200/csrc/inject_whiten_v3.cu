@@ -23,6 +23,8 @@
 // Shared memory: two float planes, element (d2, n3, k1) at d2*544 + n3*34 + k1 (d2 = n2 or k2).  The row padding 32 -> 34
 // makes the 64-bit (lane A, lane B) accesses of FA/FB/I2/I3 and the 32-bit accesses of FC/I1 bank-conflict free with
 // immediate offsets only (no swizzle arithmetic).  Every pass works in place: 4 barriers per segment.
+#include <cooperative_groups.h>
+
 #include "amplfi_internal.h"
 #include "fft_tan.cuh"
 #include "spec_layout.cuh"
@@ -38,18 +40,26 @@ using namespace tn;
 // Pass FB / I2 is then a radix RB, of which every thread takes 16/RB.
 // n = 32768 (LOGM = 14): M = 32 * (4 * 8) * 16, the middle pass split in two (FB1 radix 4 over n2a, FB2 radix 8 over
 // n2b; a third exchange), 512 threads, one CTA per SM.
+// n = 65536 (LOGM = 15): M = 32 * (8 * 8) * 16 does not fit one SM's shared memory (256 KB + padding), so a CLUSTER OF TWO
+// CTAs of 512 threads holds it: CTA r owns the elements with n3 in [8r, 8r + 8), i.e. element (d2, n3, k1) sits in CTA
+// n3 >> 3 at d2 * 272 + (n3 & 7) * 34 + k1.  FA, FB1, FB2 and I2b, I2a, I3 then touch their own CTA only; FC reads half
+// of its operands from the peer through distributed shared memory and I1 writes half of its results there: one remote
+// exchange per direction, bracketed by the two cluster barriers.
 template <int LOGM>
 struct Geo {
     static constexpr int M = 1 << LOGM, N = 2 * M, K = M + 1;
-    static constexpr int T = M / 32;                  // threads
+    static constexpr int T = M / 32;                  // threads per segment
+    static constexpr int CL = LOGM == 15 ? 2 : 1;     // CTAs per segment (cluster size)
+    static constexpr int TC = T / CL;                 // threads per CTA
     static constexpr int KL = M / 16;                 // span of klow = k1 + 32 k2
-    static constexpr int RB = LOGM <= 13 ? M / 512 : 4;   // radix of the middle pass (LOGM = 14: of its first half)
+    static constexpr int RB = LOGM <= 13 ? M / 512 : (LOGM == 14 ? 4 : 8);   // radix of the middle pass (LOGM >= 14: of its first half)
     static constexpr int NB = 16 / RB;                // middle-pass butterflies per thread
-    static constexpr int PLANE = (M / 512) * 544;     // floats per plane
+    static constexpr int PLANE = (M / 512) * 544 / CL;    // floats per plane and CTA
     static constexpr int SMEM_BYTES = 2 * PLANE * (int)sizeof(float);
-    static constexpr int CTAS = T >= 512 ? 1 : 512 / T;   // per SM (registers: 128 per thread)
+    static constexpr int CTAS = TC >= 512 ? 1 : 512 / TC; // per SM (registers: 128 per thread)
 };
 constexpr int ROW = 34, BLK = 16 * ROW;               // 34, 544 floats
+constexpr int BLKH = 8 * ROW;                         // 272: one d2 block of a CTA of the LOGM = 15 cluster (8 rows)
 
 // FB: per-lane twiddles of W = w_(32 RB)^k1, k1 = 2 kap (lane A), 2 kap + 1 (lane B): (cA, cB, tauA, tauB)
 // I2: shared twiddles of W = w_(16 RB)^n3 (used conjugated): (c, tau)
@@ -61,6 +71,10 @@ struct Tables {
     float2 i2[3][16][8];
     float4 fb1_14[16][2], fb2_14[64][4];
     float2 i2b_14[16][4], i2a_14[128][2];
+    // LOGM = 15: fb1 W = w_256^k1 [kap], fb2 W = w_2048^(k1 + 32 k2a) [8 kap + k2a], i2b W = w_128^n3 [n3],
+    //            i2a W = w_1024^(n3 + 16 n2b) [16 n2b + n3]; radix-8 rows (W^4, W^2, W, W w8)
+    float4 fb1_15[16][4], fb2_15[128][4];
+    float2 i2b_15[16][4], i2a_15[128][4];
 };
 static __device__ Tables g_tab;
 
@@ -86,9 +100,10 @@ __device__ __forceinline__ void pass_twiddles(float x, Tw1 (&tw)[8]) {
 }
 
 template <int LOGM, int MODE, bool FWD>
-__global__ void __launch_bounds__(Geo<LOGM>::T, Geo<LOGM>::CTAS) inject_whiten3_kernel(const IwArgs a, int units) {
+__global__ void __launch_bounds__(Geo<LOGM>::TC, Geo<LOGM>::CTAS) inject_whiten3_kernel(const IwArgs a, int units) {
     using G = Geo<LOGM>;
-    constexpr int M = G::M, N = G::N, K = G::K, T = G::T, KL = G::KL, RB = G::RB, NB = G::NB, PLANE = G::PLANE;
+    constexpr int M = G::M, N = G::N, K = G::K, T = G::T, TC = G::TC, KL = G::KL, RB = G::RB, NB = G::NB, PLANE = G::PLANE;
+    namespace cg = cooperative_groups;
     extern __shared__ float smem3[];
     float* re = smem3;
     float* im = smem3 + PLANE;
@@ -96,8 +111,17 @@ __global__ void __launch_bounds__(Geo<LOGM>::T, Geo<LOGM>::CTAS) inject_whiten3_
     __shared__ float2 s_em;           // exp(-2 pi i M dt/T)
     __shared__ float2 sc[32];         // the two self-paired butterflies of thread 0
     __shared__ float4 sx[17][2];      // their operands, prepared by lanes 0..16 of warp 0 long before they are needed
-    const int unit = blockIdx.x, tid = threadIdx.x;
+    // LOGM = 15: blocks 2u and 2u + 1 form the cluster of unit u; t is the thread's index within the segment
+    const int rank = LOGM == 15 ? (int)(blockIdx.x & 1) : 0;
+    const int unit = LOGM == 15 ? (int)(blockIdx.x >> 1) : (int)blockIdx.x, tid = threadIdx.x;
+    const int t = rank * TC + tid;
     const int b = unit / a.n_det, d = unit - b * a.n_det;
+    float* rre = nullptr;                                    // the peer CTA's planes (LOGM = 15)
+    float* rim = nullptr;
+    if constexpr (LOGM == 15) {
+        rre = cg::this_cluster().map_shared_rank(re, rank ^ 1);
+        rim = cg::this_cluster().map_shared_rank(im, rank ^ 1);
+    }
 
     // ---- a-5 gather ----
     const float* x = nullptr;
@@ -108,7 +132,7 @@ __global__ void __launch_bounds__(Geo<LOGM>::T, Geo<LOGM>::CTAS) inject_whiten3_
         const long off = a.offsets[unit];
         if (off < 0 || off + N > a.strip_len) {            // never read out of bounds: poison the row instead
             const float qnan = __int_as_float(0x7fc00000);
-            for (int i = tid; i < n_out; i += T) out[i] = qnan;
+            for (int i = t; i < n_out; i += T) out[i] = qnan;
             return;
         }
         x = a.noise + (size_t)d * a.strip_len + off;
@@ -116,7 +140,7 @@ __global__ void __launch_bounds__(Geo<LOGM>::T, Geo<LOGM>::CTAS) inject_whiten3_
         x = a.noise + (size_t)unit * N;
     }
     // L2 prefetch of the segment a CTA two waves later will gather (one bulk instruction for the whole 64 KB)
-    if (tid == 0 && FWD) {
+    if (t == 0 && FWD) {
         const int nu = unit + a.prefetch_ahead;
         if (nu < units) {
             const float* nx;
@@ -133,8 +157,10 @@ __global__ void __launch_bounds__(Geo<LOGM>::T, Geo<LOGM>::CTAS) inject_whiten3_
         }
     }
 
-    const int n2 = tid >> 4, n3 = tid & 15;                // FA / I3: j = tid = 16 n2 + n3 (n2 < RB)
-    const int oj = n2 * BLK + n3 * ROW;                    // FA / I3: element (n2, n3, k1 = 0)
+    // FA / I3: point j = 16 n2 + n3 of the 16 RB.. columns (LOGM <= 14: j = tid; LOGM = 15: the CTA's 8 values of n3)
+    const int n2 = LOGM == 15 ? tid >> 3 : tid >> 4, n3 = LOGM == 15 ? 8 * rank + (tid & 7) : tid & 15;
+    const int j = 16 * n2 + n3;
+    const int oj = LOGM == 15 ? n2 * BLKH + (tid & 7) * ROW : n2 * BLK + n3 * ROW;     // element (n2, n3, k1 = 0)
     // FB / I2: butterfly i of this thread is (kap, n3) = ((tid + T i) >> 4, tid & 15): element (d2 = 0, n3, k1 = 2 kap)
     auto ob_of = [&](int i) { return n3 * ROW + 2 * ((tid + T * i) >> 4); };
 
@@ -142,13 +168,13 @@ __global__ void __launch_bounds__(Geo<LOGM>::T, Geo<LOGM>::CTAS) inject_whiten3_
     if (FWD) {
         float2 z[32];
         if ((reinterpret_cast<size_t>(x) & 7) == 0) {
-            const float2* x2 = reinterpret_cast<const float2*>(x) + tid;
+            const float2* x2 = reinterpret_cast<const float2*>(x) + j;
 #pragma unroll
             for (int n1 = 0; n1 < 32; ++n1) z[n1] = __ldcs(x2 + n1 * T);
         } else {
 #pragma unroll
             for (int n1 = 0; n1 < 32; ++n1) {
-                const int m = n1 * T + tid;
+                const int m = n1 * T + j;
                 z[n1] = make_float2(__ldg(x + 2 * m), __ldg(x + 2 * m + 1));
             }
         }
@@ -217,7 +243,6 @@ __global__ void __launch_bounds__(Geo<LOGM>::T, Geo<LOGM>::CTAS) inject_whiten3_
 
     // Operands of the pointwise stage in the slot layout (spec_layout.cuh): pulled into L1 now, a whole pass ahead of
     // their use, so that the 16-byte requests of the pointwise stage find them there instead of waiting on L2.
-    const int t = tid;
     unsigned need = 0;                                       // bit w: first h0 slots of unit w needed, bit 8 + w: second
     if (MODE == MODE_FUSED) {
         const int l = t & 31;
@@ -241,7 +266,7 @@ __global__ void __launch_bounds__(Geo<LOGM>::T, Geo<LOGM>::CTAS) inject_whiten3_
     // lanes 9..16: k = 256 + 512 (l - 9).  Requested here, turned into (filter values, injected terms, split twiddle)
     // after pass FB and parked in shared memory, so that nothing in that late section waits on memory.
     // (prepared by lanes 0..16 of the LAST warp, so that warp 0 does not carry all the extra work of these butterflies)
-    const int sl = t - (T - 32);                             // task index of this thread, valid if 0 <= sl <= 16
+    const int sl = rank == 0 ? tid - (TC - 32) : -1;         // task index of this thread, valid if 0 <= sl <= 16 (CTA 0 holds thread 0)
     const int sk = sl <= 0 ? 0 : (sl <= 8 ? KL * sl : KL / 2 + KL * (sl - 9));
     float sfa = 0.f, sfb = 0.f;
     float2 sha = make_float2(0.f, 0.f), shb = make_float2(0.f, 0.f);
@@ -292,6 +317,50 @@ __global__ void __launch_bounds__(Geo<LOGM>::T, Geo<LOGM>::CTAS) inject_whiten3_
             if (((tid + T * i) >> 4) == 0) column_factor(v[RB / 2]);        // column KL/2: k1 = 0, k2 = RB/2
 #pragma unroll
             for (int k2 = 0; k2 < RB; ++k2) sts2(re, im, ob + k2 * BLK, v[k2]);
+        }
+    }
+    } else if constexpr (LOGM == 15) {
+    // ---- n = 65536: FB1 radix 8 over n2a, FB2 radix 8 over n2b (2 butterflies per thread each), both inside the CTA ----
+    // element (d2a, d2b, n3l, k1) at (8 d2a + d2b) * BLKH + n3l * ROW + k1; bit 3 of the lane index is given to an index
+    // that moves the address by 16 banks (n2b & 1 in FB1: 272 = 16 mod 32; bit 3 of kap in FB2), so that the 64-bit
+    // accesses of a half-warp (8 values of n3l x 2) stay conflict-free
+    if (FWD) {
+        __syncthreads();
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            const int c = tid + TC * i, n2b = (c >> 3) & 7, kap = c >> 6;
+            Tw2 tw[8];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const float4 f = __ldg(&g_tab.fb1_15[kap][e]);
+                tw[e] = Tw2{pack(f.x, f.y), pack(f.z, f.w)};
+            }
+            const int o = n2b * BLKH + (tid & 7) * ROW + 2 * kap;
+            C2 v[8];
+#pragma unroll
+            for (int r = 0; r < 8; ++r) v[brev<8>(r)] = lds2(re, im, o + r * 8 * BLKH);
+            dit8<false>(v, tw);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) sts2(re, im, o + q * 8 * BLKH, v[q]);
+        }
+        __syncthreads();
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            const int c = tid + TC * i, k2a = (c >> 4) & 7, kap = 8 * ((c >> 3) & 1) + ((c >> 7) & 7);
+            Tw2 tw[8];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const float4 f = __ldg(&g_tab.fb2_15[8 * kap + k2a][e]);
+                tw[e] = Tw2{pack(f.x, f.y), pack(f.z, f.w)};
+            }
+            const int o = k2a * 8 * BLKH + (tid & 7) * ROW + 2 * kap;
+            C2 v[8];
+#pragma unroll
+            for (int r = 0; r < 8; ++r) v[brev<8>(r)] = lds2(re, im, o + r * BLKH);
+            dit8<false, Tw2, true>(v, tw);                   // k2b >= 4 (klow >= KL/2) stored conjugated
+            if (kap == 0 && k2a == 0) column_factor(v[4]);   // column KL/2 = 1024: k1 = 0, k2a = 0, k2b = 4
+#pragma unroll
+            for (int q = 0; q < 8; ++q) sts2(re, im, o + q * BLKH, v[q]);
         }
     }
     } else {
@@ -355,7 +424,11 @@ __global__ void __launch_bounds__(Geo<LOGM>::T, Geo<LOGM>::CTAS) inject_whiten3_
     // ---- FC: radix 16 over n3; lane A klow = t, lane B klow = 512 - t ----
     const int ka = t, kb = (t == 0) ? KL / 2 : KL - t;
     // column klow = k1 + 32 k2 lives at d2 = k2 (n = 32768: klow = k1 + 32 k2a + 128 k2b at d2 = 8 k2a + k2b)
-    auto column = [](int klow) { return (LOGM <= 13 ? (klow >> 5) : 8 * ((klow >> 5) & 3) + (klow >> 7)) * BLK + (klow & 31); };
+    // (n = 65536: klow = k1 + 32 k2a + 256 k2b at d2 = 8 k2a + k2b, blocks of BLKH in each CTA)
+    auto column = [](int klow) {
+        if (LOGM == 15) return (8 * ((klow >> 5) & 7) + (klow >> 8)) * BLKH + (klow & 31);
+        return (LOGM <= 13 ? (klow >> 5) : 8 * ((klow >> 5) & 3) + (klow >> 7)) * BLK + (klow & 31);
+    };
     const int oa = column(ka), obb = column(kb);
     // Lane B works on the CONJUGATED column 512 - t (FB stored it so): conj Z[512 - t + 512 q] = sum_n3 conj(B[n3]) W^n3
     // w16^(-n3 (q + 1)) with lane A's own W = w8192^t, i.e. the same twiddles serve both lanes and lane B's outputs appear
@@ -366,15 +439,32 @@ __global__ void __launch_bounds__(Geo<LOGM>::T, Geo<LOGM>::CTAS) inject_whiten3_
     if (FWD) {
         Tw1 tw[8];
         pass_twiddles<M>((float)ka, tw);
-        __syncthreads();
+        if constexpr (LOGM == 15) {
+            cg::this_cluster().sync();                       // both CTAs have stored their columns (and have started)
+            // rows n3 = 8 h + l of a column sit in CTA h: eight from this CTA's planes, eight from the peer's
+            auto load = [&](auto own_first) {
+                constexpr bool OWN_FIRST = decltype(own_first)::value;
 #pragma unroll
-        for (int r = 0; r < 16; ++r)
-            v[brev<16>(r)] = C2{pack(re[oa + r * ROW], re[obb + r * ROW]), pack(im[oa + r * ROW], im[obb + r * ROW])};
+                for (int r = 0; r < 16; ++r) {
+                    const int o = (r & 7) * ROW;
+                    if ((r < 8) == OWN_FIRST)
+                        v[brev<16>(r)] = C2{pack(re[oa + o], re[obb + o]), pack(im[oa + o], im[obb + o])};
+                    else
+                        v[brev<16>(r)] = C2{pack(rre[oa + o], rre[obb + o]), pack(rim[oa + o], rim[obb + o])};
+                }
+            };
+            if (rank == 0) load(std::true_type{}); else load(std::false_type{});
+        } else {
+            __syncthreads();
+#pragma unroll
+            for (int r = 0; r < 16; ++r)
+                v[brev<16>(r)] = C2{pack(re[oa + r * ROW], re[obb + r * ROW]), pack(im[oa + r * ROW], im[obb + r * ROW])};
+        }
         dit16<false>(v, tw);
     } else {
 #pragma unroll
         for (int r = 0; r < 16; ++r) v[r] = C2{0ull, 0ull};
-        __syncthreads();
+        if constexpr (LOGM == 15) cg::this_cluster().sync(); else __syncthreads();
     }
 
     // ---- a-7 inject, a-8 whiten + band-limit ----
@@ -525,6 +615,26 @@ __global__ void __launch_bounds__(Geo<LOGM>::T, Geo<LOGM>::CTAS) inject_whiten3_
 #pragma unroll
         for (int r = 0; r < 16; ++r) w[brev<16>(r)] = v[r];
         dit16_const<true>(w);
+        if constexpr (LOGM == 15) {
+            auto store = [&](auto own_first) {
+                constexpr bool OWN_FIRST = decltype(own_first)::value;
+#pragma unroll
+                for (int q = 0; q < 16; ++q) {
+                    float ar, br, ai, bi;
+                    unpack(w[q].r, ar, br);
+                    unpack(w[q].i, ai, bi);
+                    const int o = (q & 7) * ROW;
+                    if ((q < 8) == OWN_FIRST) {
+                        re[oa + o] = ar; im[oa + o] = ai;
+                        re[obb + o] = br; im[obb + o] = bi;
+                    } else {
+                        rre[oa + o] = ar; rim[oa + o] = ai;
+                        rre[obb + o] = br; rim[obb + o] = bi;
+                    }
+                }
+            };
+            if (rank == 0) store(std::true_type{}); else store(std::false_type{});
+        } else {
 #pragma unroll
         for (int q = 0; q < 16; ++q) {
             float ar, br, ai, bi;
@@ -532,6 +642,7 @@ __global__ void __launch_bounds__(Geo<LOGM>::T, Geo<LOGM>::CTAS) inject_whiten3_
             unpack(w[q].i, ai, bi);
             re[oa + q * ROW] = ar; im[oa + q * ROW] = ai;
             re[obb + q * ROW] = br; im[obb + q * ROW] = bi;
+        }
         }
     }
     if constexpr (LOGM <= 13) {
@@ -553,6 +664,46 @@ __global__ void __launch_bounds__(Geo<LOGM>::T, Geo<LOGM>::CTAS) inject_whiten3_
             dit_r<RB, true>(w, tw);
 #pragma unroll
             for (int q = 0; q < RB; ++q) sts2(re, im, ob + q * BLK, w[q]);
+        }
+    }
+    } else if constexpr (LOGM == 15) {
+    // ---- n = 65536: I2b inverse radix 8 over k2b (twiddles by n3), I2a inverse radix 8 over k2a (twiddles by n3, n2b) ----
+    {
+        Tw1 tw[8];
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const float2 f = __ldg(&g_tab.i2b_15[n3][e]);
+            tw[e] = Tw1{f.x, f.y};
+        }
+        cg::this_cluster().sync();                           // the peer's I1 results have arrived
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            const int c = tid + TC * i, k2a = (c >> 4) & 7, kap = 8 * ((c >> 3) & 1) + ((c >> 7) & 7);
+            const int o = k2a * 8 * BLKH + (tid & 7) * ROW + 2 * kap;
+            C2 w[8];
+#pragma unroll
+            for (int r = 0; r < 8; ++r) w[brev<8>(r)] = lds2(re, im, o + r * BLKH);
+            dit8<true>(w, tw);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) sts2(re, im, o + q * BLKH, w[q]);
+        }
+        __syncthreads();
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            const int c = tid + TC * i, n2b = (c >> 3) & 7, kap = c >> 6;
+            Tw1 ta[8];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const float2 f = __ldg(&g_tab.i2a_15[16 * n2b + n3][e]);
+                ta[e] = Tw1{f.x, f.y};
+            }
+            const int o = n2b * BLKH + (tid & 7) * ROW + 2 * kap;
+            C2 w[8];
+#pragma unroll
+            for (int r = 0; r < 8; ++r) w[brev<8>(r)] = lds2(re, im, o + r * 8 * BLKH);
+            dit8<true>(w, ta);
+#pragma unroll
+            for (int q = 0; q < 8; ++q) sts2(re, im, o + q * 8 * BLKH, w[q]);
         }
     }
     } else {
@@ -598,7 +749,7 @@ __global__ void __launch_bounds__(Geo<LOGM>::T, Geo<LOGM>::CTAS) inject_whiten3_
     }
     // ---- I3: inverse radix 32 over k1, natural-order stores ----
     {
-        const float jf = (float)tid;
+        const float jf = (float)j;
         Tw1 tw[8];
         pass_twiddles<M>(2.0f * jf, tw);                     // base W^2, W = w_M^j
         __syncthreads();
@@ -618,7 +769,7 @@ __global__ void __launch_bounds__(Geo<LOGM>::T, Geo<LOGM>::CTAS) inject_whiten3_
             float2 lo, hi;
             if (q < 8) bf_s<true, false>(make_float2(er, ei), make_float2(orr, oi), tq, lo, hi);
             else bf_s<true, true>(make_float2(er, ei), make_float2(orr, oi), tq, lo, hi);
-            const int m0 = q * T + tid, m1 = (q + 16) * T + tid;
+            const int m0 = q * T + j, m1 = (q + 16) * T + j;
             if (a.crop == 0) {
                 __stcs(out2 + m0, lo);
                 __stcs(out2 + m1, hi);
@@ -711,6 +862,40 @@ __global__ void init_tables3_14_kernel() {
     }
 }
 
+// n = 65536 (M = 32768): radix-8 rows (W^4, W^2, W, W w8) of the four middle-pass tables
+__global__ void init_tables3_15_kernel() {
+    constexpr int m = 32768;
+    auto ct = [](int e, float& c, float& tau) {
+        double s, co;
+        sincospi(-2.0 * (double)(e & (m - 1)) / (double)m, &s, &co);
+        if (fabs(co) < 1e-12) co = 1e-12;
+        c = (float)co;
+        tau = (float)(s / co);
+    };
+    auto e8 = [](int x, int ent) { return ent == 0 ? 4 * x : (ent == 1 ? 2 * x : x + m / 8 * (ent - 2)); };
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;       // 0 .. 511
+    const int row = i >> 2, ent = i & 3;                       // row 0 .. 127
+    if (row < 16) {                                            // fb1: W = w_256^k1 = w_M^(128 k1), lanes k1 = 2 kap, 2 kap + 1
+        float4 f;
+        ct(e8(128 * (2 * row), ent), f.x, f.z);
+        ct(e8(128 * (2 * row + 1), ent), f.y, f.w);
+        g_tab.fb1_15[row][ent] = f;
+        float2 g;                                              // i2b: W = w_128^n3 = w_M^(256 n3)
+        ct(e8(256 * row, ent), g.x, g.y);
+        g_tab.i2b_15[row][ent] = g;
+    }
+    if (row < 128) {                                           // fb2: W = w_2048^(k1 + 32 k2a) = w_M^(16 (k1 + 32 k2a)), row = 8 kap + k2a
+        const int kap = row >> 3, k2a = row & 7;
+        float4 f;
+        ct(e8(16 * (2 * kap + 32 * k2a), ent), f.x, f.z);
+        ct(e8(16 * (2 * kap + 1 + 32 * k2a), ent), f.y, f.w);
+        g_tab.fb2_15[row][ent] = f;
+        float2 g;                                              // i2a: W = w_1024^(n3 + 16 n2b) = w_M^(32 row), row = 16 n2b + n3
+        ct(e8(32 * row, ent), g.x, g.y);
+        g_tab.i2a_15[row][ent] = g;
+    }
+}
+
 }  // namespace v3
 
 // Once per device (amplfi_plan_create synchronises before it returns).
@@ -722,7 +907,8 @@ int init_iw3_tables(cudaStream_t st) {
     if (done.load(std::memory_order_acquire) & bit) return AMPLFI_OK;
     v3::init_tables3_kernel<<<1, 384, 0, st>>>();
     v3::init_tables3_14_kernel<<<1, 256, 0, st>>>();
-    count_launch(2);
+    v3::init_tables3_15_kernel<<<1, 512, 0, st>>>();
+    count_launch(3);
     const int rc = check_launch("init_tables3_kernel");
     if (rc) return rc;
     if (cudaStreamSynchronize(st) != cudaSuccess) { set_error("init_tables3_kernel: synchronise failed"); return AMPLFI_ERR_CUDA; }
@@ -736,7 +922,24 @@ static int launch_iw3_t(const IwArgs& a, int units, cudaStream_t st) {
     static std::atomic<unsigned> attr_done{0};
     const int rc = ensure_dynamic_smem(v3::inject_whiten3_kernel<LOGM, MODE, FWD>, G::SMEM_BYTES, attr_done);
     if (rc) return rc;
-    v3::inject_whiten3_kernel<LOGM, MODE, FWD><<<units, G::T, G::SMEM_BYTES, st>>>(a, units);
+    if constexpr (G::CL == 1) {
+        v3::inject_whiten3_kernel<LOGM, MODE, FWD><<<units, G::TC, G::SMEM_BYTES, st>>>(a, units);
+    } else {                        // one cluster of G::CL CTAs per unit
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)units * G::CL);
+        cfg.blockDim = dim3(G::TC);
+        cfg.dynamicSmemBytes = G::SMEM_BYTES;
+        cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = G::CL;
+        at[0].val.clusterDim.y = 1;
+        at[0].val.clusterDim.z = 1;
+        cfg.attrs = at;
+        cfg.numAttrs = 1;
+        const cudaError_t e = cudaLaunchKernelEx(&cfg, v3::inject_whiten3_kernel<LOGM, MODE, FWD>, a, units);
+        if (e != cudaSuccess) { set_error("inject_whiten3_kernel: cluster launch: %s", cudaGetErrorString(e)); return AMPLFI_ERR_CUDA; }
+    }
     count_launch();
     return check_launch("inject_whiten3_kernel");
 }
@@ -757,6 +960,7 @@ static int launch_iw3_l(const IwArgs& a, int mode, int units, cudaStream_t st) {
 }
 
 int launch_iw3(const IwArgs& a, int logm, int mode, int units, cudaStream_t st) {
+    if (logm == 15) return launch_iw3_l<15>(a, mode, units, st);
     if (logm == 14) return launch_iw3_l<14>(a, mode, units, st);
     if (logm == 13) return launch_iw3_l<13>(a, mode, units, st);
     if (logm == 12) return launch_iw3_l<12>(a, mode, units, st);

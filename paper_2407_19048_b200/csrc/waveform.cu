@@ -137,8 +137,8 @@ __global__ void __launch_bounds__(256) sine_gaussian_kernel(const WfCoef* __rest
 template <int FAMILY>       // 0: TaylorF2 / IMRPhenomD (power tables), 1: sine-Gaussian (closed form)
 __global__ void __launch_bounds__(512, 2) waveform_slots_kernel(const WfCoef* __restrict__ coef, const double* __restrict__ tab_ci,
                                                                 const double* __restrict__ tab_lnk, float* __restrict__ h0, int kl) {
-    // blockDim.x = kl / 2 threads (the consumer's thread count)
-    const int b = blockIdx.y, t = threadIdx.x, wi = t >> 5, nt = kl >> 1;
+    // kl / 2 threads per sample (the consumer's thread count), in gridDim.z blocks of at most 512
+    const int b = blockIdx.y, t = blockIdx.z * blockDim.x + threadIdx.x, wi = t >> 5, nt = kl >> 1;
     __shared__ WfCoef c;
     {
         const int* src = reinterpret_cast<const int*>(coef + b);
@@ -200,10 +200,11 @@ int launch_waveform_pol(const amplfi_plan* p, int batch, float* hp, float* hc, c
 int launch_waveform_h0(const amplfi_plan* p, int batch, cudaStream_t st, int slots) {
     if (slots) {            // slot layout of the three-pass fused kernel (n = 4096 .. 16384)
         const int kl = p->n / 32;
-        dim3 grid(batch >= 1024 ? 2 : (batch >= 64 ? 4 : 8), batch);
+        const int nthr = kl / 2 > 512 ? 512 : kl / 2;
+        dim3 grid(batch >= 1024 ? 2 : (batch >= 64 ? 4 : 8), batch, (kl / 2) / nthr);
         float* h0f = reinterpret_cast<float*>(p->h0);
-        if (p->last_approx == 2) waveform_slots_kernel<1><<<grid, kl / 2, 0, st>>>(p->coef, p->tab_ci, p->tab_lnk, h0f, kl);
-        else waveform_slots_kernel<0><<<grid, kl / 2, 0, st>>>(p->coef, p->tab_ci, p->tab_lnk, h0f, kl);
+        if (p->last_approx == 2) waveform_slots_kernel<1><<<grid, nthr, 0, st>>>(p->coef, p->tab_ci, p->tab_lnk, h0f, kl);
+        else waveform_slots_kernel<0><<<grid, nthr, 0, st>>>(p->coef, p->tab_ci, p->tab_lnk, h0f, kl);
         count_launch();
         return check_launch("waveform_slots_kernel");
     }
