@@ -1,4 +1,4 @@
-// inject_whiten_v3.cu -- fused gather -> FFT -> inject -> whiten -> iFFT, third generation (n = 16384; configs c1, c2, c3).
+// inject_whiten_v3.cu -- fused gather -> FFT -> inject -> whiten -> iFFT, third generation (n = 4096 ... 65536; all five configs).
 // PAPER.md:103 (background chunks sliced from the GPU-resident strip), PAPER.md:105 (inject, whiten with the estimated PSD).
 //
 // M = 8192 complex points = 32 * 16 * 16: THREE passes per direction (two shared-memory exchanges instead of three),
