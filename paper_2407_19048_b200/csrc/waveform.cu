@@ -22,10 +22,31 @@ int launch_tables(amplfi_plan* p, cudaStream_t st) {
     return check_launch("tables_kernel");
 }
 
-// ---- per sample: waveform coefficients (one warp role) and detector responses (the other), fp64 ----
-// Both are long dependent chains of fp64 library calls; a CTA of 64 threads serves 32 samples, warp 0 computing the
-// coefficients and warp 1 the responses, so the two chains run side by side on different schedulers.
-__global__ void __launch_bounds__(64) prepare_kernel(const double* __restrict__ params, int batch, int approx, double t_seg,
+// ---- per sample: waveform coefficients and detector responses, fp64 ----
+// All three are long dependent chains of fp64 arithmetic and library calls; a CTA of 96 threads serves 32 samples, warp 0
+// computing the phase coefficients, warp 1 the amplitude coefficients (waveform.cuh: the two roles of prepare_sample, each
+// writing its own fields of WfCoef) and warp 2 the responses, so the three chains run side by side on different schedulers.
+__device__ __forceinline__ void store_phase_fields(WfCoef* __restrict__ o, const WfCoef& c) {
+    o->valid = c.valid; o->approx = c.approx; o->k_lo = c.k_lo; o->k_hi = c.k_hi;
+    o->kp1 = c.kp1; o->kp2 = c.kp2;
+    o->lin1 = c.lin1; o->c01 = c.c01; o->a_m5 = c.a_m5; o->a_m3 = c.a_m3; o->a_m2 = c.a_m2; o->a_m1 = c.a_m1; o->a_ln = c.a_ln;
+    o->a_p1 = c.a_p1; o->a_p1ln = c.a_p1ln; o->a_p2 = c.a_p2; o->s_p4 = c.s_p4; o->s_p5 = c.s_p5; o->s_p6 = c.s_p6;
+    o->lin2 = c.lin2; o->c02 = c.c02; o->b_ln = c.b_ln; o->b_m9 = c.b_m9;
+    o->lin3 = c.lin3; o->c03 = c.c03; o->r_m3 = c.r_m3; o->r_34 = c.r_34;
+    o->r_at = c.r_at; o->at_k0 = c.at_k0; o->at_invw = c.at_invw;
+    o->pol_p = c.pol_p; o->pol_c = c.pol_c;
+}
+__device__ __forceinline__ void store_amp_fields(WfCoef* __restrict__ o, const WfCoef& c) {
+    o->amp_scale = c.amp_scale; o->ka1 = c.ka1; o->ka2 = c.ka2;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) o->e[i] = c.e[i];
+#pragma unroll
+    for (int i = 0; i < 5; ++i) o->q[i] = c.q[i];
+    o->q_mid = c.q_mid; o->q_invh = c.q_invh;
+    o->g0 = c.g0; o->g_krd = c.g_krd; o->g_invw = c.g_invw; o->g2 = c.g2;
+}
+
+__global__ void __launch_bounds__(96) prepare_kernel(const double* __restrict__ params, int batch, int approx, double t_seg,
                                                      int n_bins, double f_lo, double f_hi, double amp_mul, double gmst,
                                                      const double* __restrict__ pd_table, const int* __restrict__ det_ids,
                                                      int n_det, WfCoef* __restrict__ coef, DetResp* __restrict__ resp,
@@ -33,14 +54,21 @@ __global__ void __launch_bounds__(64) prepare_kernel(const double* __restrict__ 
     const int b = blockIdx.x * 32 + (threadIdx.x & 31);
     if (b >= batch) return;
     const double* p = params + (size_t)b * AMPLFI_N_PARAMS;
-    if (threadIdx.x < 32) {
+    const int role = threadIdx.x >> 5;
+    if (role == 0) {
         if (coef != nullptr) {
             WfCoef c;
-            prepare_sample(p, approx, t_seg, n_bins, f_lo, f_hi, amp_mul, pd_table, c);
+            prepare_sample<WF_PHASE>(p, approx, t_seg, n_bins, f_lo, f_hi, amp_mul, pd_table, c);
             // canonical empty band: no 32-bin window of the fused kernel's operand loads may overlap it
             if (c.k_lo > c.k_hi) { c.k_lo = 0x40000000; c.k_hi = -1; }
-            coef[b] = c;
+            store_phase_fields(coef + b, c);
             if (flags != nullptr) flags[b] = c.valid ? 0 : 1;
+        }
+    } else if (role == 1) {
+        if (coef != nullptr) {
+            WfCoef c;
+            prepare_sample<WF_AMP>(p, approx, t_seg, n_bins, f_lo, f_hi, amp_mul, pd_table, c);
+            store_amp_fields(coef + b, c);
         }
     } else {
         const SkyFrame f = sky_frame(p[8], p[9], p[10], gmst);
@@ -51,7 +79,7 @@ __global__ void __launch_bounds__(64) prepare_kernel(const double* __restrict__ 
 int launch_prepare(const amplfi_plan* p, int approximant, int batch, const double* params, double gmst,
                    double f_lo, double f_hi, double amp_mul, int* flags, cudaStream_t st) {
     if (approximant >= 0) p->last_approx = approximant;     // selects the evaluation kernel that follows
-    prepare_kernel<<<(batch + 31) / 32, 64, 0, st>>>(
+    prepare_kernel<<<(batch + 31) / 32, 96, 0, st>>>(
         params, batch, approximant, p->t_seg, p->n_bins, f_lo, f_hi, amp_mul, gmst, p->pd_table, p->d_det_ids,
         p->n_det, approximant < 0 ? nullptr : p->coef, p->resp, flags);
     count_launch();

@@ -149,8 +149,15 @@ __device__ __forceinline__ float2 eval_sine_gaussian(const WfCoef& c, int k) {
     return make_float2(amp * co, -amp * s);
 }
 
-__device__ inline void prepare_sample(const double* p, int approx, double t_seg, int n_bins, double f_lo,
-                                      double f_hi, double amp_mul, const double* tab, WfCoef& c) {
+// ROLE: bit 0 = the phase fields of WfCoef (and validity, band, polarisation factors), bit 1 = the amplitude fields.
+// prepare_kernel runs the two halves in different warps (each recomputes the few quantities both need), which halves the
+// dependent fp64 chain a sample waits for; whatever feeds only the other role's fields is removed by the compiler, the
+// out-of-line library calls are guarded explicitly.
+#define WF_PHASE 1
+#define WF_AMP 2
+template <int ROLE>
+__device__ __forceinline__ void prepare_sample(const double* p, int approx, double t_seg, int n_bins, double f_lo,
+                                               double f_hi, double amp_mul, const double* tab, WfCoef& c) {
     if (approx == 2) { prepare_sine_gaussian(p, t_seg, n_bins, f_lo, f_hi, amp_mul, c); return; }
     const double PI = AMPLFI_PI, TWO_PI = 2.0 * AMPLFI_PI, I2PI = 0.15915494309189535;   // 1 / (2 pi)
     const double mc = p[0], q = p[1], chi1 = p[2], chi2 = p[3], dist = p[4];
@@ -169,7 +176,7 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     const double mu = ms / t_seg;                    // Mf = mu * k
     const double imu = 1.0 / mu;
     const double lnmu = plog(mu);
-    const double lnv1 = (lnmu + 1.1447298858494002) / 3.0;     // ln(pi) = 1.14472988584940017...
+    const double lnv1 = (lnmu + 1.1447298858494002) * (1.0 / 3.0);     // ln(pi) = 1.14472988584940017...
     const double v1 = pexp(lnv1);                     // (pi mu)^(1/3): v = v1 * k^(1/3)
     const double cosi = pcos(p[5]);
     c.pol_p = (float)(0.5 * (1.0 + cosi * cosi));
@@ -195,31 +202,32 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     const double SL = m1 * m1 * s1 + m2 * m2 * s2;
     const double dSL = (m1 - m2) * (m2 * s2 - m1 * s1);
     const double e2 = eta * eta, e3 = e2 * eta;
-    double pv2 = 5.0 * (743.0 / 84.0 + 11.0 * eta) / 9.0;
-    double pv3 = -16.0 * PI + 188.0 * SL / 3.0 + 25.0 * dSL;
+    // (divisions by constants are written as multiplications by the reciprocal: an fp64 division is ~25 dependent instructions)
+    double pv2 = (5.0 / 9.0) * (743.0 / 84.0 + 11.0 * eta);
+    double pv3 = -16.0 * PI + (188.0 / 3.0) * SL + 25.0 * dSL;
     const double sig = eta * (721.0 / 48.0 - 247.0 / 48.0) * s1 * s2
                        + (719.0 / 96.0 - 233.0 / 96.0) * (m1 * m1 * s1 * s1 + m2 * m2 * s2 * s2);
-    double pv4 = 5.0 * (3058.673 / 7.056 + 5429.0 / 7.0 * eta + 617.0 * e2) / 72.0 - 10.0 * sig;
-    const double gam = (554345.0 / 1134.0 + 110.0 * eta / 9.0) * SL + (13915.0 / 84.0 - 10.0 * eta / 3.0) * dSL;
+    double pv4 = (5.0 / 72.0) * (3058.673 / 7.056 + 5429.0 / 7.0 * eta + 617.0 * e2) - 10.0 * sig;
+    const double gam = (554345.0 / 1134.0 + (110.0 / 9.0) * eta) * SL + (13915.0 / 84.0 - (10.0 / 3.0) * eta) * dSL;
     double pv5 = 5.0 / 9.0 * (7729.0 / 84.0 - 13.0 * eta) * PI - gam;
     double pl5 = 5.0 / 3.0 * (7729.0 / 84.0 - 13.0 * eta) * PI - 3.0 * gam;
     double pv6 = 11583.231236531 / 4.694215680 - 640.0 / 3.0 * PI * PI - 6848.0 / 21.0 * AMPLFI_GAMMA_E
-                 + eta * (-15737.765635 / 3.048192 + 2255.0 / 12.0 * PI * PI) + e2 * 76055.0 / 1728.0
-                 - e3 * 127825.0 / 1296.0 - 6848.0 / 21.0 * 1.3862943611198906        /* ln 4 */
-                 + PI * (3760.0 * SL + 1490.0 * dSL) / 3.0;
+                 + eta * (-15737.765635 / 3.048192 + 2255.0 / 12.0 * PI * PI) + e2 * (76055.0 / 1728.0)
+                 - e3 * (127825.0 / 1296.0) - 6848.0 / 21.0 * 1.3862943611198906        /* ln 4 */
+                 + (PI / 3.0) * (3760.0 * SL + 1490.0 * dSL);
     double pl6 = -6848.0 / 21.0;
     double pv7 = PI * (77096675.0 / 254016.0 + 378515.0 / 1512.0 * eta - 74045.0 / 756.0 * e2)
-                 + (-8980424995.0 / 762048.0 + 6586595.0 * eta / 756.0 - 305.0 * e2 / 36.0) * SL
-                 - (170978035.0 / 48384.0 - 2876425.0 * eta / 672.0 - 4735.0 * e2 / 144.0) * dSL;
+                 + (-8980424995.0 / 762048.0 + (6586595.0 / 756.0) * eta - (305.0 / 36.0) * e2) * SL
+                 - (170978035.0 / 48384.0 - (2876425.0 / 672.0) * eta - (4735.0 / 144.0) * e2) * dSL;
     const double pfa = 3.0 / 128.0 * ieta * I2PI;          // everything below is in turns
     const double iv = 1.0 / v1;
     c.a_m5 = pfa * iv * iv * iv * iv * iv;
     c.a_m3 = pfa * pv2 * iv * iv * iv;
     c.a_m2 = pfa * pv3 * iv * iv;
     c.a_m1 = pfa * pv4 * iv;
-    c.a_ln = pfa * pl5 / 3.0;
+    c.a_ln = pfa * pl5 * (1.0 / 3.0);
     c.a_p1 = pfa * (pv6 + pl6 * lnv1) * v1;
-    c.a_p1ln = pfa * pl6 / 3.0 * v1;
+    c.a_p1ln = pfa * pl6 * (1.0 / 3.0) * v1;
     c.a_p2 = pfa * pv7 * v1 * v1;
     const double tc_turns = p[7] / t_seg;                     // 2 pi f t_c / 2 pi = k t_c / T
     const double phic_turns = -2.0 * p[6] * I2PI;
@@ -233,9 +241,11 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
         c.lin3 = c.c03 = c.r_m3 = c.r_34 = 0.0;
         c.r_at = 0.f; c.at_k0 = 0.f; c.at_invw = 0.f;
         // A0 f^(-7/6), A0 = sqrt(5/24) pi^(-2/3) (G Mc/c^3)^(5/6) c / D
-        const double a0 = 0.45643546458763845 /* sqrt(5/24) */ * 0.46619407703541166 /* pi^(-2/3) */ * pow(mc * AMPLFI_MTSUN, 5.0 / 6.0)
-                          * AMPLFI_C_SI / (dist * AMPLFI_MPC);
-        c.amp_scale = (float)(a0 * pow(t_seg, 7.0 / 6.0) * amp_mul);
+        if (ROLE & WF_AMP) {
+            const double a0 = 0.45643546458763845 /* sqrt(5/24) */ * 0.46619407703541166 /* pi^(-2/3) */ * pow(mc * AMPLFI_MTSUN, 5.0 / 6.0)
+                              * AMPLFI_C_SI / (dist * AMPLFI_MPC);
+            c.amp_scale = (float)(a0 * pow(t_seg, 7.0 / 6.0) * amp_mul);
+        }
         c.ka1 = 3.0e38f; c.ka2 = 3.0e38f;
         for (int i = 0; i < 8; ++i) c.e[i] = 0.f;
         for (int i = 0; i < 5; ++i) c.q[i] = 0.f;
@@ -244,8 +254,9 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     }
 
     // ---- IMRPhenomD ----
-    const double xi = (m1 * chi1 + m2 * chi2 - 38.0 * eta / 113.0 * (chi1 + chi2)) - 1.0;
+    const double xi = (m1 * chi1 + m2 * chi2 - (38.0 / 113.0) * eta * (chi1 + chi2)) - 1.0;
     double fit[AMPLFI_PD_ROWS];
+#pragma unroll
     for (int r = 0; r < AMPLFI_PD_ROWS; ++r) fit[r] = pd_fit(tab + r * AMPLFI_PD_COLS, eta, xi);
     // remnant: final spin, radiated energy, ringdown / damping frequency (Kerr 220 closed-form fit)
     const double stot = m1 * m1 * chi1 + m2 * m2 * chi2;
@@ -278,8 +289,16 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
         w_re = l0 * q[0] + l1 * q[2] + l2 * q[4] + l3 * q[6];
         w_im = l0 * q[1] + l1 * q[3] + l2 * q[5] + l3 * q[7];
     }
-    const double f_rd = w_re * I2PI / (1.0 - erad);
-    const double f_dm = w_im * I2PI / (1.0 - erad);
+    const double imf = 1.0 / (1.0 - erad);           // remnant mass
+    const double f_rd = w_re * I2PI * imf;
+    const double f_dm = w_im * I2PI * imf;
+    // amplitude peak (both roles: the phase is aligned in time there)
+    const double g1 = fit[PD_GAMMA1], g2 = fit[PD_GAMMA2], g3 = fit[PD_GAMMA3];
+    const double f_peak = (g2 > 1.0) ? fabs(f_rd - f_dm * g3 / g2)
+                                     : fabs(f_rd + f_dm * (psqrt(1.0 - g2 * g2) - 1.0) * g3 / g2);
+    const double mu13 = v1 * 0.6827840632552957;      // mu^(1/3) = (pi mu)^(1/3) pi^(-1/3)
+
+    if (ROLE & WF_PHASE) {
 
     const double sg1 = fit[PD_SIGMA1], sg2 = fit[PD_SIGMA2], sg3 = fit[PD_SIGMA3], sg4 = fit[PD_SIGMA4];
     const double be1 = fit[PD_BETA1], be2 = fit[PD_BETA2], be3 = fit[PD_BETA3];
@@ -303,14 +322,14 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
         const double c13 = 0.26207413942088964;   // cbrt(0.018)
         phi_ins = pfar * s - PI / 4.0
                   + (sg1 * f1 + 0.75 * sg2 * f1 * c13 + 0.6 * sg3 * f1 * c13 * c13 + 0.5 * sg4 * f1 * f1) * ieta;
-        dphi_ins = pfar * ds * v / (3.0 * f1) + (sg1 + sg2 * c13 + sg3 * c13 * c13 + sg4 * f1) * ieta;
+        dphi_ins = pfar * ds * (v / (3.0 * f1)) + (sg1 + sg2 * c13 + sg3 * c13 * c13 + sg4 * f1) * ieta;
     }
     const double if1 = 1.0 / 0.018, if1_3 = if1 * if1 * if1;      // constant: folded at compile time
     const double int1 = (be1 * f1 + be2 * -4.017383521085972 /* ln 0.018 */ - be3 * if1_3 * (1.0 / 3.0)) * ieta;
     const double dint1 = (be1 + be2 * if1 + be3 * if1_3 * if1) * ieta;
     const double c2int = dphi_ins - dint1;
     const double c1int = phi_ins - int1 - c2int * f1;
-    const double lnf2 = plog(f2), f2m14 = pexp(-0.25 * lnf2);                 // f2^(-1/4)
+    const double lnf2 = plog(f2), f2m14 = rsqrt(psqrt(f2));                   // f2^(-1/4)
     const double if2 = 1.0 / f2, if2_3 = if2 * if2 * if2;
     const double int2 = (be1 * f2 + be2 * lnf2 - be3 * if2_3 * (1.0 / 3.0)) * ieta + c1int + c2int * f2;
     const double dint2 = (be1 + be2 * if2 + be3 * if2_3 * if2) * ieta + c2int;
@@ -320,17 +339,13 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     const double dmr2 = (al1 + al2 * if2 * if2 + al3 * f2m14 + al4 * ifdm / (1.0 + x2 * x2)) * ieta;
     const double c2mr = dint2 - dmr2;
     const double c1mr = int2 - mr2 - c2mr * f2;
-    // amplitude peak and time alignment
-    const double g1 = fit[PD_GAMMA1], g2 = fit[PD_GAMMA2], g3 = fit[PD_GAMMA3];
-    const double f_peak = (g2 > 1.0) ? fabs(f_rd - f_dm * g3 / g2)
-                                     : fabs(f_rd + f_dm * (psqrt(1.0 - g2 * g2) - 1.0) * g3 / g2);
+    // time alignment at the amplitude peak
     const double xp = (f_peak - al5 * f_rd) * ifdm;
     const double t0 = (al1 + al2 / (f_peak * f_peak) + al3 * rsqrt(psqrt(f_peak)) + al4 * ifdm / (1.0 + xp * xp)) * ieta
                       + c2mr;
 
     c.kp1 = f1 * imu;
     c.kp2 = f2 * imu;
-    const double mu13 = pexp(lnmu / 3.0);
     c.lin1 = tc_turns + (sg1 * ieta - t0) * mu * I2PI;
     c.c01 = const1;
     c.s_p4 = 0.75 * sg2 * ieta * mu * mu13 * I2PI;
@@ -347,28 +362,30 @@ __device__ inline void prepare_sample(const double* p, int approx, double t_seg,
     c.r_at = (float)(al4 * ieta * I2PI);
     c.at_k0 = (float)(al5 * f_rd * imu);
     c.at_invw = (float)(mu * ifdm);
+    }
+    if (!(ROLE & WF_AMP)) return;
 
     // ---- amplitude ----
     const double amp0 = 2.0 * 0.15769578262626002 /* sqrt(5 / (64 pi)) */ * mtot * mtot * AMPLFI_MTSUN * (AMPLFI_MTSUN * AMPLFI_C_SI)
                         / (dist * AMPLFI_MPC);
-    c.amp_scale = (float)(amp0 * psqrt(2.0 * eta / 3.0) * 0.8263074871107581 * pexp(-7.0 / 6.0 * lnmu) * amp_mul);   // pi^(-1/6)
+    c.amp_scale = (float)(amp0 * psqrt(eta * (2.0 / 3.0)) * 0.8263074871107581 * pexp(-7.0 / 6.0 * lnmu) * amp_mul);   // pi^(-1/6)
     const double c12 = chi1 * chi1, c22 = chi2 * chi2;
     double A[7];
-    A[2] = (-969.0 + 1804.0 * eta) / 672.0;
-    A[3] = (chi1 * (81.0 * (1.0 + seta) - 44.0 * eta) + chi2 * (81.0 - 81.0 * seta - 44.0 * eta)) / 48.0;
+    A[2] = (-969.0 + 1804.0 * eta) * (1.0 / 672.0);
+    A[3] = (chi1 * (81.0 * (1.0 + seta) - 44.0 * eta) + chi2 * (81.0 - 81.0 * seta - 44.0 * eta)) * (1.0 / 48.0);
     A[4] = (-27312085.0 - 10287648.0 * c22 - 10287648.0 * c12 * (1.0 + seta) + 10287648.0 * c22 * seta
             + 24.0 * (-1975055.0 + 857304.0 * c12 - 994896.0 * chi1 * chi2 + 857304.0 * c22) * eta
-            + 35371056.0 * e2) / 8128512.0;
+            + 35371056.0 * e2) * (1.0 / 8128512.0);
     A[5] = (chi2 * (-285197.0 * (-1.0 + seta) + 4.0 * (-91902.0 + 1579.0 * seta) * eta - 35632.0 * e2)
             + chi1 * (285197.0 * (1.0 + seta) - 4.0 * (91902.0 + 1579.0 * seta) * eta - 35632.0 * e2)
-            + 42840.0 * (-1.0 + 4.0 * eta) * PI) / 32256.0;
+            + 42840.0 * (-1.0 + 4.0 * eta) * PI) * (1.0 / 32256.0);
     A[6] = -(-336.0 * (-3248849057.0 + 2943675504.0 * c12 - 3339284256.0 * chi1 * chi2 + 2943675504.0 * c22) * e2
              - 324322727232.0 * e3
              - 7.0 * (-177520268561.0 + 107414046432.0 * c22 + 107414046432.0 * c12 * (1.0 + seta)
                       - 107414046432.0 * c22 * seta + 11087290368.0 * (chi1 + chi2 + chi1 * seta - chi2 * seta) * PI)
              + 12.0 * eta * (-545384828789.0 - 176491177632.0 * chi1 * chi2 + 202603761360.0 * c22
                              + 77616.0 * c12 * (2610335.0 + 995766.0 * seta) - 77287373856.0 * c22 * seta
-                             + 5841690624.0 * (chi1 + chi2) * PI + 21384760320.0 * PI * PI)) / 60085960704.0;
+                             + 5841690624.0 * (chi1 + chi2) * PI + 21384760320.0 * PI * PI)) * (1.0 / 60085960704.0);
     const double rho1 = fit[PD_RHO1], rho2 = fit[PD_RHO2], rho3 = fit[PD_RHO3];
     {
         double vp = v1 * v1;
