@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libamplfi.so")
-SOURCES = ["api.cu", "kerr_qnm.cu", "waveform.cu", "welch.cu", "inject_whiten.cu", "inject_whiten13.cu", "inject_whiten_v3.cu", "inject_whiten_long.cu"]
+SOURCES = ["api.cu", "kerr_qnm.cu", "waveform.cu", "welch.cu", "inject_whiten.cu", "inject_whiten_v3.cu", "inject_whiten_long.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
               "--expt-relaxed-constexpr", "--extended-lambda", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

@@ -131,9 +131,6 @@ struct IwOpts {
     const double* t_shift;
 };
 
-// inject_whiten13.cu (packed 4-pass kernel for n = 16384)
-int launch_iw13(const IwArgs& a, int logm /*11, 12 or 13*/, int mode, int units, cudaStream_t st);
-int init_iw13_tables(cudaStream_t st);      // fills the packed kernel's twiddle tables (idempotent; called by plan_create)
 
 // inject_whiten_v3.cu (three-pass cosine-tangent kernel for n = 4096, 8192, 16384)
 int launch_iw3(const IwArgs& a, int logm /*11 .. 14*/, int mode, int units, cudaStream_t st);

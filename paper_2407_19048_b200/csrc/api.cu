@@ -221,7 +221,6 @@ int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_
         if (e != cudaSuccess) { set_error("amplfi_plan_create: stream/event: %s", cudaGetErrorString(e)); rc = AMPLFI_ERR_CUDA; }
     }
     if (!rc) rc = launch_tables(p, nullptr);
-    if (!rc && p->logm >= 11 && p->logm <= 13) rc = init_iw13_tables(nullptr);
     if (!rc && p->logm >= 11 && p->logm <= 15) rc = init_iw3_tables(nullptr);
     if (!rc) {
         fill_kernel<<<(p->filt_stride + 255) / 256, 256>>>(p->filt_flat, p->filt_stride, (float)(1.0 / (2.0 * (double)n)));
@@ -414,15 +413,14 @@ int amplfi_inject_whiten_views(const amplfi_plan* p, int batch, const float* noi
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     rc = launch_filter(p, psd, n_psd, f_lo, f_hi, st);
     if (!rc) rc = launch_prepare(p, approximant, batch, params, gmst, f_lo, f_hi, 2.0 * p->fs, nullptr, st);
-    // n = 4096, 8192, 16384: one launch, one forward transform for both views (inject_whiten13.cu, VIEWS = 2; linear h0)
+    // n = 4096, 8192, 16384: one launch, one forward transform for both views (inject_whiten_v3.cu, VIEWS = 2)
     const bool one_launch = p->logm >= 11 && p->logm <= 13 && (reinterpret_cast<size_t>(out2) & 15) == 0;
-    if (!rc) rc = launch_waveform_h0(p, batch, st, v3_family(p) && !one_launch);
+    if (!rc) rc = launch_waveform_h0(p, batch, st, v3_family(p));
     // both views with the fp64-reduced phase, so that a zero shift reproduces the first view bit for bit
     IwOpts o;
     o.n_det = p->n_det; o.resp = nullptr; o.filt = nullptr; o.filt_stride = 0; o.crop = 0; o.phase64 = 1;
     o.out2 = nullptr; o.t_shift = nullptr;
     if (!rc && one_launch) {
-        // n = 16384: one launch, one forward transform for both views (inject_whiten13.cu, VIEWS = 2)
         o.out2 = out2; o.t_shift = t_shift;
         return launch_inject_whiten(p, batch, noise, offsets, strip_len, nullptr, 1, out, st, &o);
     }

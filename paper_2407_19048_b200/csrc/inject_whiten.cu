@@ -307,9 +307,7 @@ int launch_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
     switch (p->logm) {
         case 9: return launch_iw_mode<9>(a, mode, units, st);
         case 10: return launch_iw_mode<10>(a, mode, units, st);
-        case 11: case 12: case 13:      // three-pass kernel; the one-launch two-view variant still runs the packed four-pass one
-            return a.out2 != nullptr ? launch_iw13(a, p->logm, mode, units, st) : launch_iw3(a, p->logm, mode, units, st);
-        case 14: case 15: return launch_iw3(a, p->logm, mode, units, st);
+        case 11: case 12: case 13: case 14: case 15: return launch_iw3(a, p->logm, mode, units, st);
         case 16: case 17: case 18: case 19: return launch_inject_whiten_long(p, a, mode, units, st);
         default:
             set_error("amplfi_inject_whiten: segment length %d not supported by this build", p->n);

@@ -99,7 +99,11 @@ __device__ __forceinline__ void pass_twiddles(float x, Tw1 (&tw)[8]) {
     for (int q = 0; q < 4; ++q) tw[4 + q] = tan_twiddle(fmaf(x, u, (float)(M / 16 * q) * u));
 }
 
-template <int LOGM, int MODE, bool FWD>
+// VIEWS = 2 (fused mode, n <= 16384): the two data views d, d' of one background segment from ONE forward
+// transform.  After pass FC every thread parks its 16 packed spectrum values in the second view's own output row (16 bytes x
+// 16 x T = exactly one row, L2-resident), finishes the first view, reads them back and runs the pointwise stage with the
+// arrival time later by t_shift[b] and the inverse transform into that row.
+template <int LOGM, int MODE, bool FWD, int VIEWS = 1>
 __global__ void __launch_bounds__(Geo<LOGM>::TC, Geo<LOGM>::CTAS) inject_whiten3_kernel(const IwArgs a, int units) {
     using G = Geo<LOGM>;
     constexpr int M = G::M, N = G::N, K = G::K, T = G::T, TC = G::TC, KL = G::KL, RB = G::RB, NB = G::NB, PLANE = G::PLANE;
@@ -111,6 +115,7 @@ __global__ void __launch_bounds__(Geo<LOGM>::TC, Geo<LOGM>::CTAS) inject_whiten3
     __shared__ float2 s_em;           // exp(-2 pi i M dt/T)
     __shared__ float2 sc[32];         // the two self-paired butterflies of thread 0
     __shared__ float4 sx[17][2];      // their operands, prepared by lanes 0..16 of warp 0 long before they are needed
+    __shared__ float4 sraw[17];       // VIEWS = 2: the h0 values those operands are built from, kept for the second view
     // LOGM = 15: blocks 2u and 2u + 1 form the cluster of unit u; t is the thread's index within the segment
     const int rank = LOGM == 15 ? (int)(blockIdx.x & 1) : 0;
     const int unit = LOGM == 15 ? (int)(blockIdx.x >> 1) : (int)blockIdx.x, tid = threadIdx.x;
@@ -133,6 +138,10 @@ __global__ void __launch_bounds__(Geo<LOGM>::TC, Geo<LOGM>::CTAS) inject_whiten3
         if (off < 0 || off + N > a.strip_len) {            // never read out of bounds: poison the row instead
             const float qnan = __int_as_float(0x7fc00000);
             for (int i = t; i < n_out; i += T) out[i] = qnan;
+            if (VIEWS == 2) {
+                float* o2 = a.out2 + (size_t)unit * n_out;
+                for (int i = t; i < n_out; i += T) o2[i] = qnan;
+            }
             return;
         }
         x = a.noise + (size_t)d * a.strip_len + off;
@@ -230,16 +239,19 @@ __global__ void __launch_bounds__(Geo<LOGM>::TC, Geo<LOGM>::CTAS) inject_whiten3
         __sincosf(turns * -6.283185307179586f, &s, &co);
         return make_float2(co, s);
     };
-    if (MODE == MODE_FUSED && tid <= 16) {
-        if (tid < 16) {
-            const float2 e = unit_phase(KL * tid);
-            float* spf = reinterpret_cast<float*>(sp);
-            spf[(tid >> 1) * 4 + (tid & 1)] = e.x;
-            spf[(tid >> 1) * 4 + 2 + (tid & 1)] = e.y;
-        } else {
-            s_em = unit_phase(M);
+    auto view_constants = [&]() {                            // the S table and e(M) of the current arrival time
+        if (MODE == MODE_FUSED && tid <= 16) {
+            if (tid < 16) {
+                const float2 e = unit_phase(KL * tid);
+                float* spf = reinterpret_cast<float*>(sp);
+                spf[(tid >> 1) * 4 + (tid & 1)] = e.x;
+                spf[(tid >> 1) * 4 + 2 + (tid & 1)] = e.y;
+            } else {
+                s_em = unit_phase(M);
+            }
         }
-    }
+    };
+    view_constants();
 
     // Operands of the pointwise stage in the slot layout (spec_layout.cuh): pulled into L1 now, a whole pass ahead of
     // their use, so that the 16-byte requests of the pointwise stage find them there instead of waiting on L2.
@@ -271,6 +283,7 @@ __global__ void __launch_bounds__(Geo<LOGM>::TC, Geo<LOGM>::CTAS) inject_whiten3
     float sfa = 0.f, sfb = 0.f;
     float2 sha = make_float2(0.f, 0.f), shb = make_float2(0.f, 0.f);
     bool sin_a = false, sin_b = false;
+    auto special_loads = [&]() {
     if (sl >= 0 && sl <= 16) {
         const float* filt = a.filt + (size_t)d * a.filt_stride;
         sfa = __ldg(filt + sk);
@@ -285,6 +298,8 @@ __global__ void __launch_bounds__(Geo<LOGM>::TC, Geo<LOGM>::CTAS) inject_whiten3
             if (sin_b) { const float* hp = hsrc + slot::h0_index(KL, M - sk); shb = make_float2(__ldg(hp), __ldg(hp + 2)); }
         }
     }
+    };
+    special_loads();
 
     // the factor conj(w32^n3) of the self-paired column klow = KL/2 (lane B of thread 0 in FC, whose twiddles are those of
     // klow = 0, i.e. 1): one complex product in the 16 threads that produce that column
@@ -406,6 +421,7 @@ __global__ void __launch_bounds__(Geo<LOGM>::TC, Geo<LOGM>::CTAS) inject_whiten3
         }
     }
     }
+    auto special_prepare = [&]() {
     if (sl >= 0 && sl <= 16) {
         float2 ia = make_float2(0.f, 0.f), ib = make_float2(0.f, 0.f);            // what the injection adds to 2 X[k], 2 X[M-k]
         if (MODE == MODE_HDET) {
@@ -419,7 +435,10 @@ __global__ void __launch_bounds__(Geo<LOGM>::TC, Geo<LOGM>::CTAS) inject_whiten3
         const float2 w = twiddle<N>(sk);
         sx[sl][0] = make_float4(sfa, sfb, ia.x, ia.y);
         sx[sl][1] = make_float4(ib.x, ib.y, w.x, w.y);
+        if (VIEWS == 2) sraw[sl] = make_float4(sha.x, sha.y, shb.x, shb.y);
     }
+    };
+    special_prepare();
 
     // ---- FC: radix 16 over n3; lane A klow = t, lane B klow = 512 - t ----
     const int ka = t, kb = (t == 0) ? KL / 2 : KL - t;
@@ -467,6 +486,38 @@ __global__ void __launch_bounds__(Geo<LOGM>::TC, Geo<LOGM>::CTAS) inject_whiten3
         if constexpr (LOGM == 15) cg::this_cluster().sync(); else __syncthreads();
     }
 
+    ulonglong2* park = nullptr;
+    if constexpr (VIEWS == 2) {
+        park = reinterpret_cast<ulonglong2*>(a.out2 + (size_t)unit * N) + t;
+#pragma unroll
+        for (int q = 0; q < 16; ++q) park[q * T] = make_ulonglong2(v[q].r, v[q].i);
+    }
+#pragma unroll 1
+    for (int view = 0; view < VIEWS; ++view) {              // (the body, down to the stores of I3, keeps its indentation)
+    if (VIEWS == 2 && view == 1) {
+        // second view: arrival time later by t_shift[b]; the S table and the operands of the self-paired bins again, then
+        // the spectrum back from the row it was parked in.  (Every thread is past the last barrier of the first view, so
+        // nobody reads the first view's constants any more; the barrier below also fences the planes, which slower threads
+        // may still be reading in I3.)
+        delta += a.t_shift[b] * (double)a.inv_tseg;
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            const ulonglong2 pv = __ldcg(park + q * T);
+            v[q] = C2{pv.x, pv.y};
+        }
+        view_constants();
+        if (sl >= 0 && sl <= 16) {                           // the injected terms with the new phase; filter values and twiddle stay
+            const float4 r4 = sraw[sl];
+            const float2 cc = make_float2(cre, cim);
+            const float2 ia = sl == 0 ? make_float2(0.f, 0.f) : amplfi::cmul(make_float2(r4.x, r4.y), amplfi::cmul(cc, unit_phase(sk)));
+            const float2 ib = sl == 0 ? make_float2(0.f, 0.f) : amplfi::cmul(make_float2(r4.z, r4.w), amplfi::cmul(cc, unit_phase(M - sk)));
+            const float4 s0 = sx[sl][0], s1 = sx[sl][1];
+            sx[sl][0] = make_float4(s0.x, s0.y, ia.x, ia.y);
+            sx[sl][1] = make_float4(ib.x, ib.y, s1.z, s1.w);
+        }
+        __syncthreads();
+        out = a.out2 + (size_t)unit * n_out;
+    }
     // ---- a-7 inject, a-8 whiten + band-limit ----
     // v[k3] = (Z[t + 512 k3] | Z[512 - t + 512 k3]) = (A[k3] | B[k3]).  Unit w < 8 (u = 2w) works on the two bin pairs
     //   lane 0: k0 = t + 512 u <-> M - k0 : (A[u], B[15-u]),      lane 1: k1 = k0 + 512 <-> M - k1 : (A[u+1], B[14-u])
@@ -779,6 +830,7 @@ __global__ void __launch_bounds__(Geo<LOGM>::TC, Geo<LOGM>::CTAS) inject_whiten3
             }
         }
     }
+    }   // views
 }
 
 __global__ void init_tables3_kernel() {
@@ -916,14 +968,14 @@ int init_iw3_tables(cudaStream_t st) {
     return AMPLFI_OK;
 }
 
-template <int LOGM, int MODE, bool FWD>
+template <int LOGM, int MODE, bool FWD, int VIEWS = 1>
 static int launch_iw3_t(const IwArgs& a, int units, cudaStream_t st) {
     using G = v3::Geo<LOGM>;
     static std::atomic<unsigned> attr_done{0};
-    const int rc = ensure_dynamic_smem(v3::inject_whiten3_kernel<LOGM, MODE, FWD>, G::SMEM_BYTES, attr_done);
+    const int rc = ensure_dynamic_smem(v3::inject_whiten3_kernel<LOGM, MODE, FWD, VIEWS>, G::SMEM_BYTES, attr_done);
     if (rc) return rc;
     if constexpr (G::CL == 1) {
-        v3::inject_whiten3_kernel<LOGM, MODE, FWD><<<units, G::TC, G::SMEM_BYTES, st>>>(a, units);
+        v3::inject_whiten3_kernel<LOGM, MODE, FWD, VIEWS><<<units, G::TC, G::SMEM_BYTES, st>>>(a, units);
     } else {                        // one cluster of G::CL CTAs per unit
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3((unsigned)units * G::CL);
@@ -946,6 +998,18 @@ static int launch_iw3_t(const IwArgs& a, int units, cudaStream_t st) {
 
 template <int LOGM>
 static int launch_iw3_l(const IwArgs& a, int mode, int units, cudaStream_t st) {
+    if (a.out2 != nullptr) {        // two data views from one forward transform
+        if constexpr (LOGM <= 13) {
+            if (mode != MODE_FUSED || a.noise == nullptr || a.t_shift == nullptr || a.crop != 0 || (reinterpret_cast<size_t>(a.out2) & 15)) {
+                set_error("inject_whiten3: the two-view launch needs the fused mode and a 16-byte aligned second output");
+                return AMPLFI_ERR_INVALID_ARG;
+            }
+            return launch_iw3_t<LOGM, MODE_FUSED, true, 2>(a, units, st);
+        } else {
+            set_error("inject_whiten3: no two-view launch for this segment length");
+            return AMPLFI_ERR_UNSUPPORTED_SIZE;
+        }
+    }
     if (a.noise == nullptr) {       // inverse-only launches (time-domain waveform, filter design)
         if (mode == MODE_HDET) return launch_iw3_t<LOGM, MODE_HDET, false>(a, units, st);
         if (mode == MODE_FUSED) return launch_iw3_t<LOGM, MODE_FUSED, false>(a, units, st);

@@ -107,7 +107,7 @@ __global__ void __launch_bounds__(256, 4) waveform_kernel(const WfCoef* __restri
     float2* oa = out_a + (size_t)b * n_bins;
     float2* ob = POL ? out_b + (size_t)b * n_bins : nullptr;
     // The plan's h0 workspace (POL == false) is only ever read inside the band, widened to the 32-bin windows of
-    // the consumers' warp-uniform band test (inject_whiten13.cu): bins further than 64 from the band are not written.
+    // the consumers' warp-uniform band test: bins further than 64 from the band are not written.
     int k_first = 0, k_last = n_bins - 1;
     if (!POL) {
         if (k_lo > k_hi) return;

@@ -299,8 +299,10 @@ def test_assemble_batch_equals_two_call_path():
     assert row_err(ref_gpu, oracle_inject_whiten(wl, "fused")).max() <= TOL
 
 
-def test_gather_out_of_range_offset_poisons_row_only():
-    wl = WL.make_c2(batch=4, strip_len=1 << 18)
+@pytest.mark.parametrize("cfg", ["c2", "c4"])
+def test_gather_out_of_range_offset_poisons_row_only(cfg):
+    # c4 (n = 65536): both CTAs of a unit's cluster must leave before any cluster barrier, the other units run on
+    wl = WL.make_c2(batch=4, strip_len=1 << 18) if cfg == "c2" else WL.make_c4(batch=4, strip_len=1 << 22)
     wl.offsets[1, 0] = wl.strip.shape[1] - wl.n + 1
     wl.offsets[2, 2] = -1
     got, _ = run_inject_whiten(wl, "none")
@@ -325,7 +327,7 @@ def test_c3_parity_snr12():
 @pytest.mark.parametrize("mode", ["fused", "hdet", "none"])
 def test_c4_parity(mode):
     # configs[4] shape (fs 4096, 16 s = 65536 samples, Welch 4 s windows from 128 s, PSD grid ratio 4) at reduced
-    # batch and strip; n = 65536 runs the decimated three-kernel path.  One offset is odd (unaligned gather).
+    # batch and strip; n = 65536 runs the two-CTA cluster kernel.  One offset is odd (unaligned gather).
     wl = WL.make_c4(batch=6, strip_len=1 << 22)
     wl.offsets[1, 2] |= 1
     wl.offsets[2, 0] = wl.strip.shape[1] - wl.n
@@ -336,7 +338,7 @@ def test_c4_parity(mode):
 
 
 def test_c4_many_chunks_sampled_rows():
-    # more units than one L2-resident chunk (148 units): every chunk boundary is crossed; sampled rows vs the oracle
+    # more units than one wave of clusters (74 units); sampled rows vs the oracle
     wl = WL.make_c4(batch=120, strip_len=1 << 22)
     got, psd = run_inject_whiten(wl, "fused")
     assert got.shape == (120, 3, 65536) and np.all(np.isfinite(got))
@@ -456,7 +458,7 @@ def test_batch_not_a_multiple_of_the_wave(batch):
 
 
 def test_full_size_c4_sampled_rows():
-    # BASELINE configs[4] at its full size (batch 8192 x 3 x 65536 = 6.4 GB out, 166 chunks of the long-segment path),
+    # BASELINE configs[4] at its full size (batch 8192 x 3 x 65536 = 6.4 GB out, 24576 clusters of the n = 65536 kernel),
     # in the launch configuration bench.py --config c4 times
     wl = WL.make_c4()
     plan = A.Plan(wl.n, wl.fs, wl.det_ids, wl.batch, nperseg=wl.nperseg)
