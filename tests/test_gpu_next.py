@@ -302,7 +302,7 @@ def test_sine_gaussian_parity(n, fs):
 
 # ------------------------------------------------------------------------------------------ plans side by side
 def test_two_plans_side_by_side_and_plan_reuse():
-    """Two plans of different lengths alive at once (they share the packed kernel's twiddle tables), one of them reused for
+    """Two plans of different lengths alive at once (they share the device-wide twiddle tables), one of them reused for
     another batch size, approximant and mode: results equal those of fresh plans bit for bit."""
     par16, noise16, psd16 = _make_inputs(16384, 2048.0, 4, [0, 1], 4242)
     par8, noise8, psd8 = _make_inputs(8192, 2048.0, 3, [0, 1], 4243)

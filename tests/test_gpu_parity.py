@@ -337,7 +337,7 @@ def test_c4_parity(mode):
     assert row_err(got, oracle_inject_whiten(wl, mode, psd=psd)).max() <= TOL
 
 
-def test_c4_many_chunks_sampled_rows():
+def test_c4_many_waves_sampled_rows():
     # more units than one wave of clusters (74 units); sampled rows vs the oracle
     wl = WL.make_c4(batch=120, strip_len=1 << 22)
     got, psd = run_inject_whiten(wl, "fused")
