@@ -152,8 +152,8 @@ int amplfi_psd_welch(const amplfi_plan* plan, const float* bg, long n_bg, long r
  *   psd      [n_det, n_psd] fp32, S * 2^140; n_psd == K, or n_psd == (n/r)/2+1 for an integer r >= 1, in
  *            which case S is linearly interpolated in frequency onto the segment grid.
  *   out      [batch, n_det, n] fp32.
- * batch <= the plan's max_batch.  n = 2^16 runs as a cluster of two thread blocks sharing the transform through
- * distributed shared memory; n >= 2^17 is decimated by n / 2^15 around the 2^15-sample transform, the intermediate
+ * batch <= the plan's max_batch.  n = 2^16 and 2^17 run as a cluster of two / four thread blocks sharing the transform
+ * through distributed shared memory; n >= 2^18 is decimated by n / 2^15 around the 2^15-sample transform, the intermediate
  * spectra of a chunk of segments staying in L2 (three launches per chunk). */
 int amplfi_inject_whiten(const amplfi_plan* plan, int batch, const float* noise, const long* offsets,
                          long strip_len, const float* h_det, int approximant, const double* params,

@@ -38,7 +38,7 @@ struct amplfi_plan {
                            //                  amplfi_waveform_td ((F+, Fx, dt) = (1,0,0), (0,1,0) per sample)
     float2* h0;            // [max_batch * n_bins]   fused path: 2 fs h0
     float* filt;           // [n_det * filt_stride]  whitening filter incl. 1/(2n); rows padded to 16 B
-    float* filt_slots;     // n = 4096 .. 65536: the same filter in the slot layout of the fused kernel [n_det * n/2] (spec_layout.cuh)
+    float* filt_slots;     // n = 4096 .. 131072: the same filter in the slot layout of the fused kernel [n_det * n/2] (spec_layout.cuh)
     int filt_stride;       // n_bins rounded up to a multiple of 4
     float* filt_flat;      // [filt_stride] constant 1/(2n): the "no filter" row of the inverse-only launches
     float2* fir_spec;      // [n_det * n_bins]  truncated-filter construction: spectrum-side workspace
@@ -85,7 +85,7 @@ const double* kerr_qnm_table();
 int launch_prepare(const amplfi_plan* p, int approximant, int batch, const double* params, double gmst,
                    double f_lo, double f_hi, double amp_mul, int* flags, cudaStream_t st);
 int launch_waveform_pol(const amplfi_plan* p, int batch, float* hp, float* hc, cudaStream_t st);
-int launch_waveform_h0(const amplfi_plan* p, int batch, cudaStream_t st, int slots);   // slots: spec_layout.cuh (n = 4096 .. 65536)
+int launch_waveform_h0(const amplfi_plan* p, int batch, cudaStream_t st, int slots);   // slots: spec_layout.cuh (n = 4096 .. 131072)
 int launch_project(const amplfi_plan* p, int batch, const float* hp, const float* hc, float* h_det,
                    double* resp_out, cudaStream_t st);
 int launch_tables(amplfi_plan* p, cudaStream_t st);

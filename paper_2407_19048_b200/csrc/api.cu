@@ -48,7 +48,7 @@ static int dev_alloc(T** ptr, size_t count) {
 }
 
 // segment lengths of the three-pass fused kernel (inject_whiten_v3.cu), whose h0 workspace is in the slot layout
-static bool v3_family(const amplfi_plan* p) { return p->logm >= 11 && p->logm <= 15; }
+static bool v3_family(const amplfi_plan* p) { return p->logm >= 11 && p->logm <= 16; }
 
 static bool known_approximant(int a) { return a == AMPLFI_TAYLORF2 || a == AMPLFI_IMRPHENOMD || a == AMPLFI_SINE_GAUSSIAN; }
 
@@ -193,12 +193,12 @@ int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_
     if (!rc) rc = dev_alloc(&p->h0, (size_t)max_batch * p->n_bins);
     p->filt_stride = (p->n_bins + 3) & ~3;
     if (!rc) rc = dev_alloc(&p->filt, (size_t)n_det * p->filt_stride);
-    if (!rc && p->logm >= 11 && p->logm <= 15) rc = dev_alloc(&p->filt_slots, (size_t)n_det * (n / 2));
+    if (!rc && p->logm >= 11 && p->logm <= 16) rc = dev_alloc(&p->filt_slots, (size_t)n_det * (n / 2));
     if (!rc) rc = dev_alloc(&p->filt_flat, (size_t)p->filt_stride);
     if (!rc) rc = dev_alloc(&p->fir_spec, (size_t)n_det * p->n_bins);
     if (!rc) rc = dev_alloc(&p->fir_time, (size_t)n_det * n);
     if (!rc) rc = dev_alloc(&p->d_det_ids, (size_t)3);
-    if (!rc && p->logm >= 16) {
+    if (!rc && p->logm >= 17) {
         // n/32768 CTAs per unit, one CTA per SM: a chunk is two full waves and its spectra (39 MB) stay in L2
         const int rdec = n / 32768;
         p->long_chunk = (2 * (sms > 0 ? sms : 148)) / rdec;
@@ -221,7 +221,7 @@ int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_
         if (e != cudaSuccess) { set_error("amplfi_plan_create: stream/event: %s", cudaGetErrorString(e)); rc = AMPLFI_ERR_CUDA; }
     }
     if (!rc) rc = launch_tables(p, nullptr);
-    if (!rc && p->logm >= 11 && p->logm <= 15) rc = init_iw3_tables(nullptr);
+    if (!rc && p->logm >= 11 && p->logm <= 16) rc = init_iw3_tables(nullptr);
     if (!rc) {
         fill_kernel<<<(p->filt_stride + 255) / 256, 256>>>(p->filt_flat, p->filt_stride, (float)(1.0 / (2.0 * (double)n)));
         count_launch();

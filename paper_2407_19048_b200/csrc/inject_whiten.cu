@@ -294,7 +294,7 @@ int launch_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
     a.crop = 0; a.phase64 = 0; a.out2 = nullptr; a.t_shift = nullptr;
     a.n_det = p->n_det; a.two_fs = (float)(2.0 * p->fs); a.inv_tseg = (float)(1.0 / p->t_seg);
     a.prefetch_ahead = (p->logm >= 11 && p->logm <= 14 ? 1 : 2) * p->sm_count * (8192 / (p->n / 2 < 8192 ? p->n / 2 : 8192));   // one wave ahead
-    if (p->logm == 15) a.prefetch_ahead = p->sm_count / 2;      // one cluster of two CTAs per unit
+    if (p->logm >= 15) a.prefetch_ahead = p->sm_count >> (p->logm - 14);      // one cluster of 2 / 4 CTAs per unit
     if (opts != nullptr) {
         a.n_det = opts->n_det;
         if (opts->resp != nullptr) a.resp = opts->resp;
@@ -307,8 +307,8 @@ int launch_inject_whiten(const amplfi_plan* p, int batch, const float* noise, co
     switch (p->logm) {
         case 9: return launch_iw_mode<9>(a, mode, units, st);
         case 10: return launch_iw_mode<10>(a, mode, units, st);
-        case 11: case 12: case 13: case 14: case 15: return launch_iw3(a, p->logm, mode, units, st);
-        case 16: case 17: case 18: case 19: return launch_inject_whiten_long(p, a, mode, units, st);
+        case 11: case 12: case 13: case 14: case 15: case 16: return launch_iw3(a, p->logm, mode, units, st);
+        case 17: case 18: case 19: return launch_inject_whiten_long(p, a, mode, units, st);
         default:
             set_error("amplfi_inject_whiten: segment length %d not supported by this build", p->n);
             return AMPLFI_ERR_UNSUPPORTED_SIZE;

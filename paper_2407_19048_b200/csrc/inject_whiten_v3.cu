@@ -1,4 +1,4 @@
-// inject_whiten_v3.cu -- fused gather -> FFT -> inject -> whiten -> iFFT, third generation (n = 4096 ... 65536; all five configs).
+// inject_whiten_v3.cu -- fused gather -> FFT -> inject -> whiten -> iFFT, third generation (n = 4096 ... 131072; all five configs).
 // PAPER.md:103 (background chunks sliced from the GPU-resident strip), PAPER.md:105 (inject, whiten with the estimated PSD).
 //
 // M = 8192 complex points = 32 * 16 * 16: THREE passes per direction (two shared-memory exchanges instead of three),
@@ -45,11 +45,15 @@ using namespace tn;
 // n3 >> 3 at d2 * 272 + (n3 & 7) * 34 + k1.  FA, FB1, FB2 and I2b, I2a, I3 then touch their own CTA only; FC reads half
 // of its operands from the peer through distributed shared memory and I1 writes half of its results there: one remote
 // exchange per direction, bracketed by the two cluster barriers.
+// n = 131072 (LOGM = 16): the same with M = 32 * (8 * 16) * 16 in a cluster of FOUR CTAs, four rows n3 each (element
+// (d2, n3, k1) in CTA n3 >> 2 at d2 * 136 + (n3 & 3) * 34 + k1); three quarters of every FC column are remote.
 template <int LOGM>
 struct Geo {
     static constexpr int M = 1 << LOGM, N = 2 * M, K = M + 1;
     static constexpr int T = M / 32;                  // threads per segment
-    static constexpr int CL = LOGM == 15 ? 2 : 1;     // CTAs per segment (cluster size)
+    static constexpr int CL = LOGM >= 15 ? 1 << (LOGM - 14) : 1;     // CTAs per segment (cluster size: 2, 4)
+    static constexpr int NR = 16 / CL;                // rows n3 of a column held by one CTA
+    static constexpr int RB2 = LOGM == 16 ? 16 : 8;   // LOGM >= 14: radix of the second half of the middle pass
     static constexpr int TC = T / CL;                 // threads per CTA
     static constexpr int KL = M / 16;                 // span of klow = k1 + 32 k2
     static constexpr int RB = LOGM <= 13 ? M / 512 : (LOGM == 14 ? 4 : 8);   // radix of the middle pass (LOGM >= 14: of its first half)
@@ -59,7 +63,6 @@ struct Geo {
     static constexpr int CTAS = TC >= 512 ? 1 : 512 / TC; // per SM (registers: 128 per thread)
 };
 constexpr int ROW = 34, BLK = 16 * ROW;               // 34, 544 floats
-constexpr int BLKH = 8 * ROW;                         // 272: one d2 block of a CTA of the LOGM = 15 cluster (8 rows)
 
 // FB: per-lane twiddles of W = w_(32 RB)^k1, k1 = 2 kap (lane A), 2 kap + 1 (lane B): (cA, cB, tauA, tauB)
 // I2: shared twiddles of W = w_(16 RB)^n3 (used conjugated): (c, tau)
@@ -73,8 +76,9 @@ struct Tables {
     float2 i2b_14[16][4], i2a_14[128][2];
     // LOGM = 15: fb1 W = w_256^k1 [kap], fb2 W = w_2048^(k1 + 32 k2a) [8 kap + k2a], i2b W = w_128^n3 [n3],
     //            i2a W = w_1024^(n3 + 16 n2b) [16 n2b + n3]; radix-8 rows (W^4, W^2, W, W w8)
-    float4 fb1_15[16][4], fb2_15[128][4];
-    float2 i2b_15[16][4], i2a_15[128][4];
+    // (n = 131072, [1]: fb2 and i2b are radix-16 rows, i2a has 256 rows 16 n2b + n3)
+    float4 fb1_c[2][16][4], fb2_c[2][128][8];
+    float2 i2b_c[2][16][8], i2a_c[2][256][4];
 };
 static __device__ Tables g_tab;
 
@@ -117,16 +121,27 @@ __global__ void __launch_bounds__(Geo<LOGM>::TC, Geo<LOGM>::CTAS) inject_whiten3
     __shared__ float4 sx[17][2];      // their operands, prepared by lanes 0..16 of warp 0 long before they are needed
     __shared__ float4 sraw[17];       // VIEWS = 2: the h0 values those operands are built from, kept for the second view
     // LOGM = 15: blocks 2u and 2u + 1 form the cluster of unit u; t is the thread's index within the segment
-    const int rank = LOGM == 15 ? (int)(blockIdx.x & 1) : 0;
-    const int unit = LOGM == 15 ? (int)(blockIdx.x >> 1) : (int)blockIdx.x, tid = threadIdx.x;
+    constexpr int CL = G::CL, NR = G::NR, RB2 = G::RB2, BLKC = NR * ROW;      // cluster geometry (CL = 1: unused)
+    const int rank = CL > 1 ? (int)(blockIdx.x & (CL - 1)) : 0;
+    const int unit = CL > 1 ? (int)(blockIdx.x / CL) : (int)blockIdx.x, tid = threadIdx.x;
     const int t = rank * TC + tid;
     const int b = unit / a.n_det, d = unit - b * a.n_det;
-    float* rre = nullptr;                                    // the peer CTA's planes (LOGM = 15)
-    float* rim = nullptr;
-    if constexpr (LOGM == 15) {
-        rre = cg::this_cluster().map_shared_rank(re, rank ^ 1);
-        rim = cg::this_cluster().map_shared_rank(im, rank ^ 1);
-    }
+    // the planes of CTA c of the cluster (generic addresses; mapped where they are used, so that no pointer stays live)
+    auto peer_re = [&](int c) { return cg::this_cluster().map_shared_rank(re, c); };
+    auto peer_im = [&](int c) { return cg::this_cluster().map_shared_rank(im, c); };
+    // run `body` with the CTA's rank as a compile-time constant (row ownership then selects plain shared-memory accesses)
+    auto with_rank = [&](auto body) {
+        if constexpr (CL == 2) {
+            if (rank == 0) body(std::integral_constant<int, 0>{}); else body(std::integral_constant<int, 1>{});
+        } else if constexpr (CL == 4) {
+            switch (rank) {
+                case 0: body(std::integral_constant<int, 0>{}); break;
+                case 1: body(std::integral_constant<int, 1>{}); break;
+                case 2: body(std::integral_constant<int, 2>{}); break;
+                default: body(std::integral_constant<int, 3>{}); break;
+            }
+        }
+    };
 
     // ---- a-5 gather ----
     const float* x = nullptr;
@@ -166,10 +181,11 @@ __global__ void __launch_bounds__(Geo<LOGM>::TC, Geo<LOGM>::CTAS) inject_whiten3
         }
     }
 
-    // FA / I3: point j = 16 n2 + n3 of the 16 RB.. columns (LOGM <= 14: j = tid; LOGM = 15: the CTA's 8 values of n3)
-    const int n2 = LOGM == 15 ? tid >> 3 : tid >> 4, n3 = LOGM == 15 ? 8 * rank + (tid & 7) : tid & 15;
+    // FA / I3: point j = 16 n2 + n3 (one CTA: j = tid; cluster: the CTA's NR values of n3)
+    const int n3l = CL > 1 ? tid & (NR - 1) : tid & 15;      // row within the CTA
+    const int n2 = CL > 1 ? tid / NR : tid >> 4, n3 = CL > 1 ? NR * rank + n3l : n3l;
     const int j = 16 * n2 + n3;
-    const int oj = LOGM == 15 ? n2 * BLKH + (tid & 7) * ROW : n2 * BLK + n3 * ROW;     // element (n2, n3, k1 = 0)
+    const int oj = CL > 1 ? n2 * BLKC + n3l * ROW : n2 * BLK + n3 * ROW;     // element (n2, n3, k1 = 0)
     // FB / I2: butterfly i of this thread is (kap, n3) = ((tid + T i) >> 4, tid & 15): element (d2 = 0, n3, k1 = 2 kap)
     auto ob_of = [&](int i) { return n3 * ROW + 2 * ((tid + T * i) >> 4); };
 
@@ -334,48 +350,50 @@ __global__ void __launch_bounds__(Geo<LOGM>::TC, Geo<LOGM>::CTAS) inject_whiten3
             for (int k2 = 0; k2 < RB; ++k2) sts2(re, im, ob + k2 * BLK, v[k2]);
         }
     }
-    } else if constexpr (LOGM == 15) {
-    // ---- n = 65536: FB1 radix 8 over n2a, FB2 radix 8 over n2b (2 butterflies per thread each), both inside the CTA ----
-    // element (d2a, d2b, n3l, k1) at (8 d2a + d2b) * BLKH + n3l * ROW + k1; bit 3 of the lane index is given to an index
-    // that moves the address by 16 banks (n2b & 1 in FB1: 272 = 16 mod 32; bit 3 of kap in FB2), so that the 64-bit
-    // accesses of a half-warp (8 values of n3l x 2) stay conflict-free
+    } else if constexpr (CL > 1) {
+    // ---- clusters (n = 65536, 131072): FB1 radix 8 over n2a, FB2 radix RB2 = 8 / 16 over n2b, both inside the CTA ----
+    // element (d2a, d2b, n3l, k1) at (RB2 d2a + d2b) * BLKC + n3l * ROW + k1.  The lane bits above n3l are given to indices that
+    // move the address by 8 / 16 banks (FB1: the low bits of n2b, BLKC = 16 or 8 mod 32; FB2: the high bits of kap), so that
+    // the 64-bit accesses of a half-warp stay conflict-free.
+    constexpr int LB = NR == 8 ? 3 : 2, HB = 4 - LB;         // lane bits of n3l; high bits of kap taken from the lane index
     if (FWD) {
         __syncthreads();
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
-            const int c = tid + TC * i, n2b = (c >> 3) & 7, kap = c >> 6;
+            const int c = tid + TC * i, n2b = (c >> LB) & (RB2 - 1), kap = c >> 6;
             Tw2 tw[8];
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
-                const float4 f = __ldg(&g_tab.fb1_15[kap][e]);
+                const float4 f = __ldg(&g_tab.fb1_c[LOGM - 15][kap][e]);
                 tw[e] = Tw2{pack(f.x, f.y), pack(f.z, f.w)};
             }
-            const int o = n2b * BLKH + (tid & 7) * ROW + 2 * kap;
+            const int o = n2b * BLKC + n3l * ROW + 2 * kap;
             C2 v[8];
 #pragma unroll
-            for (int r = 0; r < 8; ++r) v[brev<8>(r)] = lds2(re, im, o + r * 8 * BLKH);
+            for (int r = 0; r < 8; ++r) v[brev<8>(r)] = lds2(re, im, o + r * RB2 * BLKC);
             dit8<false>(v, tw);
 #pragma unroll
-            for (int q = 0; q < 8; ++q) sts2(re, im, o + q * 8 * BLKH, v[q]);
+            for (int q = 0; q < 8; ++q) sts2(re, im, o + q * RB2 * BLKC, v[q]);
         }
         __syncthreads();
 #pragma unroll
-        for (int i = 0; i < 2; ++i) {
-            const int c = tid + TC * i, k2a = (c >> 4) & 7, kap = 8 * ((c >> 3) & 1) + ((c >> 7) & 7);
+        for (int i = 0; i < 16 / RB2; ++i) {
+            const int c = tid + TC * i, k2a = (c >> 4) & 7;
+            const int kap = (((c >> LB) & ((1 << HB) - 1)) << (4 - HB)) | ((c >> 7) & ((1 << (4 - HB)) - 1));
             Tw2 tw[8];
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                const float4 f = __ldg(&g_tab.fb2_15[8 * kap + k2a][e]);
+            for (int e = 0; e < RB2 / 2; ++e) {
+                const float4 f = __ldg(&g_tab.fb2_c[LOGM - 15][8 * kap + k2a][e]);
                 tw[e] = Tw2{pack(f.x, f.y), pack(f.z, f.w)};
             }
-            const int o = k2a * 8 * BLKH + (tid & 7) * ROW + 2 * kap;
-            C2 v[8];
+            const int o = k2a * RB2 * BLKC + n3l * ROW + 2 * kap;
+            C2 v[RB2];
 #pragma unroll
-            for (int r = 0; r < 8; ++r) v[brev<8>(r)] = lds2(re, im, o + r * BLKH);
-            dit8<false, Tw2, true>(v, tw);                   // k2b >= 4 (klow >= KL/2) stored conjugated
-            if (kap == 0 && k2a == 0) column_factor(v[4]);   // column KL/2 = 1024: k1 = 0, k2a = 0, k2b = 4
+            for (int r = 0; r < RB2; ++r) v[brev<RB2>(r)] = lds2(re, im, o + r * BLKC);
+            dit_r<RB2, false, Tw2, true>(v, tw);             // k2b >= RB2/2 (klow >= KL/2) stored conjugated
+            if (kap == 0 && k2a == 0) column_factor(v[RB2 / 2]);      // column KL/2: k1 = 0, k2a = 0, k2b = RB2/2
 #pragma unroll
-            for (int q = 0; q < 8; ++q) sts2(re, im, o + q * BLKH, v[q]);
+            for (int q = 0; q < RB2; ++q) sts2(re, im, o + q * BLKC, v[q]);
         }
     }
     } else {
@@ -443,9 +461,9 @@ __global__ void __launch_bounds__(Geo<LOGM>::TC, Geo<LOGM>::CTAS) inject_whiten3
     // ---- FC: radix 16 over n3; lane A klow = t, lane B klow = 512 - t ----
     const int ka = t, kb = (t == 0) ? KL / 2 : KL - t;
     // column klow = k1 + 32 k2 lives at d2 = k2 (n = 32768: klow = k1 + 32 k2a + 128 k2b at d2 = 8 k2a + k2b)
-    // (n = 65536: klow = k1 + 32 k2a + 256 k2b at d2 = 8 k2a + k2b, blocks of BLKH in each CTA)
+    // (clusters: klow = k1 + 32 k2a + 256 k2b at d2 = RB2 k2a + k2b, blocks of BLKC in each CTA)
     auto column = [](int klow) {
-        if (LOGM == 15) return (8 * ((klow >> 5) & 7) + (klow >> 8)) * BLKH + (klow & 31);
+        if (CL > 1) return (RB2 * ((klow >> 5) & 7) + (klow >> 8)) * BLKC + (klow & 31);
         return (LOGM <= 13 ? (klow >> 5) : 8 * ((klow >> 5) & 3) + (klow >> 7)) * BLK + (klow & 31);
     };
     const int oa = column(ka), obb = column(kb);
@@ -458,21 +476,22 @@ __global__ void __launch_bounds__(Geo<LOGM>::TC, Geo<LOGM>::CTAS) inject_whiten3
     if (FWD) {
         Tw1 tw[8];
         pass_twiddles<M>((float)ka, tw);
-        if constexpr (LOGM == 15) {
-            cg::this_cluster().sync();                       // both CTAs have stored their columns (and have started)
-            // rows n3 = 8 h + l of a column sit in CTA h: eight from this CTA's planes, eight from the peer's
-            auto load = [&](auto own_first) {
-                constexpr bool OWN_FIRST = decltype(own_first)::value;
+        if constexpr (CL > 1) {
+            cg::this_cluster().sync();                       // every CTA has stored its rows of the columns (and has started)
+            // row n3 = NR c + l of a column sits in CTA c: NR rows from this CTA's planes, the others from the peers'
+            with_rank([&](auto rk) {
+                constexpr int RK = decltype(rk)::value;
 #pragma unroll
-                for (int r = 0; r < 16; ++r) {
-                    const int o = (r & 7) * ROW;
-                    if ((r < 8) == OWN_FIRST)
-                        v[brev<16>(r)] = C2{pack(re[oa + o], re[obb + o]), pack(im[oa + o], im[obb + o])};
-                    else
-                        v[brev<16>(r)] = C2{pack(rre[oa + o], rre[obb + o]), pack(rim[oa + o], rim[obb + o])};
+                for (int c = 0; c < CL; ++c) {
+                    const float* qr = c == RK ? re : peer_re(c);
+                    const float* qi = c == RK ? im : peer_im(c);
+#pragma unroll
+                    for (int l = 0; l < NR; ++l) {
+                        const int r = NR * c + l, o = l * ROW;
+                        v[brev<16>(r)] = C2{pack(qr[oa + o], qr[obb + o]), pack(qi[oa + o], qi[obb + o])};
+                    }
                 }
-            };
-            if (rank == 0) load(std::true_type{}); else load(std::false_type{});
+            });
         } else {
             __syncthreads();
 #pragma unroll
@@ -483,7 +502,7 @@ __global__ void __launch_bounds__(Geo<LOGM>::TC, Geo<LOGM>::CTAS) inject_whiten3
     } else {
 #pragma unroll
         for (int r = 0; r < 16; ++r) v[r] = C2{0ull, 0ull};
-        if constexpr (LOGM == 15) cg::this_cluster().sync(); else __syncthreads();
+        if constexpr (CL > 1) cg::this_cluster().sync(); else __syncthreads();
     }
 
     ulonglong2* park = nullptr;
@@ -666,25 +685,23 @@ __global__ void __launch_bounds__(Geo<LOGM>::TC, Geo<LOGM>::CTAS) inject_whiten3
 #pragma unroll
         for (int r = 0; r < 16; ++r) w[brev<16>(r)] = v[r];
         dit16_const<true>(w);
-        if constexpr (LOGM == 15) {
-            auto store = [&](auto own_first) {
-                constexpr bool OWN_FIRST = decltype(own_first)::value;
+        if constexpr (CL > 1) {
+            with_rank([&](auto rk) {
+                constexpr int RK = decltype(rk)::value;
 #pragma unroll
-                for (int q = 0; q < 16; ++q) {
-                    float ar, br, ai, bi;
-                    unpack(w[q].r, ar, br);
-                    unpack(w[q].i, ai, bi);
-                    const int o = (q & 7) * ROW;
-                    if ((q < 8) == OWN_FIRST) {
-                        re[oa + o] = ar; im[oa + o] = ai;
-                        re[obb + o] = br; im[obb + o] = bi;
-                    } else {
-                        rre[oa + o] = ar; rim[oa + o] = ai;
-                        rre[obb + o] = br; rim[obb + o] = bi;
+                for (int c = 0; c < CL; ++c) {
+                    float* qr = c == RK ? re : peer_re(c);
+                    float* qi = c == RK ? im : peer_im(c);
+#pragma unroll
+                    for (int l = 0; l < NR; ++l) {
+                        float ar, br, ai, bi;
+                        unpack(w[NR * c + l].r, ar, br);
+                        unpack(w[NR * c + l].i, ai, bi);
+                        qr[oa + l * ROW] = ar; qi[oa + l * ROW] = ai;
+                        qr[obb + l * ROW] = br; qi[obb + l * ROW] = bi;
                     }
                 }
-            };
-            if (rank == 0) store(std::true_type{}); else store(std::false_type{});
+            });
         } else {
 #pragma unroll
         for (int q = 0; q < 16; ++q) {
@@ -717,44 +734,46 @@ __global__ void __launch_bounds__(Geo<LOGM>::TC, Geo<LOGM>::CTAS) inject_whiten3
             for (int q = 0; q < RB; ++q) sts2(re, im, ob + q * BLK, w[q]);
         }
     }
-    } else if constexpr (LOGM == 15) {
-    // ---- n = 65536: I2b inverse radix 8 over k2b (twiddles by n3), I2a inverse radix 8 over k2a (twiddles by n3, n2b) ----
+    } else if constexpr (CL > 1) {
+    // ---- clusters: I2b inverse radix RB2 over k2b (twiddles by n3), I2a inverse radix 8 over k2a (twiddles by n3, n2b) ----
     {
+        constexpr int LB = NR == 8 ? 3 : 2, HB = 4 - LB;
         Tw1 tw[8];
 #pragma unroll
-        for (int e = 0; e < 4; ++e) {
-            const float2 f = __ldg(&g_tab.i2b_15[n3][e]);
+        for (int e = 0; e < RB2 / 2; ++e) {
+            const float2 f = __ldg(&g_tab.i2b_c[LOGM - 15][n3][e]);
             tw[e] = Tw1{f.x, f.y};
         }
-        cg::this_cluster().sync();                           // the peer's I1 results have arrived
+        cg::this_cluster().sync();                           // the peers' I1 results have arrived
 #pragma unroll
-        for (int i = 0; i < 2; ++i) {
-            const int c = tid + TC * i, k2a = (c >> 4) & 7, kap = 8 * ((c >> 3) & 1) + ((c >> 7) & 7);
-            const int o = k2a * 8 * BLKH + (tid & 7) * ROW + 2 * kap;
-            C2 w[8];
+        for (int i = 0; i < 16 / RB2; ++i) {
+            const int c = tid + TC * i, k2a = (c >> 4) & 7;
+            const int kap = (((c >> LB) & ((1 << HB) - 1)) << (4 - HB)) | ((c >> 7) & ((1 << (4 - HB)) - 1));
+            const int o = k2a * RB2 * BLKC + n3l * ROW + 2 * kap;
+            C2 w[RB2];
 #pragma unroll
-            for (int r = 0; r < 8; ++r) w[brev<8>(r)] = lds2(re, im, o + r * BLKH);
-            dit8<true>(w, tw);
+            for (int r = 0; r < RB2; ++r) w[brev<RB2>(r)] = lds2(re, im, o + r * BLKC);
+            dit_r<RB2, true>(w, tw);
 #pragma unroll
-            for (int q = 0; q < 8; ++q) sts2(re, im, o + q * BLKH, w[q]);
+            for (int q = 0; q < RB2; ++q) sts2(re, im, o + q * BLKC, w[q]);
         }
         __syncthreads();
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
-            const int c = tid + TC * i, n2b = (c >> 3) & 7, kap = c >> 6;
+            const int c = tid + TC * i, n2b = (c >> LB) & (RB2 - 1), kap = c >> 6;
             Tw1 ta[8];
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
-                const float2 f = __ldg(&g_tab.i2a_15[16 * n2b + n3][e]);
+                const float2 f = __ldg(&g_tab.i2a_c[LOGM - 15][16 * n2b + n3][e]);
                 ta[e] = Tw1{f.x, f.y};
             }
-            const int o = n2b * BLKH + (tid & 7) * ROW + 2 * kap;
+            const int o = n2b * BLKC + n3l * ROW + 2 * kap;
             C2 w[8];
 #pragma unroll
-            for (int r = 0; r < 8; ++r) w[brev<8>(r)] = lds2(re, im, o + r * 8 * BLKH);
+            for (int r = 0; r < 8; ++r) w[brev<8>(r)] = lds2(re, im, o + r * RB2 * BLKC);
             dit8<true>(w, ta);
 #pragma unroll
-            for (int q = 0; q < 8; ++q) sts2(re, im, o + q * 8 * BLKH, w[q]);
+            for (int q = 0; q < 8; ++q) sts2(re, im, o + q * RB2 * BLKC, w[q]);
         }
     }
     } else {
@@ -914,37 +933,54 @@ __global__ void init_tables3_14_kernel() {
     }
 }
 
-// n = 65536 (M = 32768): radix-8 rows (W^4, W^2, W, W w8) of the four middle-pass tables
-__global__ void init_tables3_15_kernel() {
-    constexpr int m = 32768;
-    auto ct = [](int e, float& c, float& tau) {
+// clusters (n = 65536, 131072; lg = 0, 1): the four middle-pass tables; radix-8 rows (W^4, W^2, W, W w8), radix-16 rows as in
+// pass_twiddles (W^8, W^4, W^2, W^2 w8, W w16^q)
+__global__ void init_tables3_cluster_kernel() {
+    const int lg = blockIdx.y;                                 // 0: M = 32768 (RB2 = 8), 1: M = 65536 (RB2 = 16)
+    const int m = 32768 << lg, rb2 = 8 << lg;
+    auto ct = [m](int e, float& c, float& tau) {
         double s, co;
         sincospi(-2.0 * (double)(e & (m - 1)) / (double)m, &s, &co);
         if (fabs(co) < 1e-12) co = 1e-12;
         c = (float)co;
         tau = (float)(s / co);
     };
-    auto e8 = [](int x, int ent) { return ent == 0 ? 4 * x : (ent == 1 ? 2 * x : x + m / 8 * (ent - 2)); };
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;       // 0 .. 511
-    const int row = i >> 2, ent = i & 3;                       // row 0 .. 127
-    if (row < 16) {                                            // fb1: W = w_256^k1 = w_M^(128 k1), lanes k1 = 2 kap, 2 kap + 1
+    auto e8 = [m](int x, int ent) { return ent == 0 ? 4 * x : (ent == 1 ? 2 * x : x + m / 8 * (ent - 2)); };
+    auto e16 = [m](int x, int ent) {
+        switch (ent) {
+            case 0: return 8 * x;
+            case 1: return 4 * x;
+            case 2: return 2 * x;
+            case 3: return 2 * x + m / 8;
+            default: return x + m / 16 * (ent - 4);
+        }
+    };
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;       // 0 .. 2047
+    const int row = i >> 3, ent = i & 7;                       // row 0 .. 255
+    if (row < 16 && ent < 4) {                                 // fb1: W = w_256^k1 = w_M^((M/256) k1), lanes k1 = 2 kap, 2 kap + 1
         float4 f;
-        ct(e8(128 * (2 * row), ent), f.x, f.z);
-        ct(e8(128 * (2 * row + 1), ent), f.y, f.w);
-        g_tab.fb1_15[row][ent] = f;
-        float2 g;                                              // i2b: W = w_128^n3 = w_M^(256 n3)
-        ct(e8(256 * row, ent), g.x, g.y);
-        g_tab.i2b_15[row][ent] = g;
+        ct(e8((m / 256) * (2 * row), ent), f.x, f.z);
+        ct(e8((m / 256) * (2 * row + 1), ent), f.y, f.w);
+        g_tab.fb1_c[lg][row][ent] = f;
     }
-    if (row < 128) {                                           // fb2: W = w_2048^(k1 + 32 k2a) = w_M^(16 (k1 + 32 k2a)), row = 8 kap + k2a
+    if (row < 16 && ent < rb2 / 2) {                           // i2b: W = w_(M/256)^n3 = w_M^(256 n3), radix rb2
+        float2 g;
+        const int x = 256 * row;
+        ct(rb2 == 8 ? e8(x, ent) : e16(x, ent), g.x, g.y);
+        g_tab.i2b_c[lg][row][ent] = g;
+    }
+    if (row < 128 && ent < rb2 / 2) {                          // fb2: W = w_(M/16)^(k1 + 32 k2a), row = 8 kap + k2a, radix rb2
         const int kap = row >> 3, k2a = row & 7;
+        const int xa = 16 * (2 * kap + 32 * k2a), xb = 16 * (2 * kap + 1 + 32 * k2a);
         float4 f;
-        ct(e8(16 * (2 * kap + 32 * k2a), ent), f.x, f.z);
-        ct(e8(16 * (2 * kap + 1 + 32 * k2a), ent), f.y, f.w);
-        g_tab.fb2_15[row][ent] = f;
-        float2 g;                                              // i2a: W = w_1024^(n3 + 16 n2b) = w_M^(32 row), row = 16 n2b + n3
+        ct(rb2 == 8 ? e8(xa, ent) : e16(xa, ent), f.x, f.z);
+        ct(rb2 == 8 ? e8(xb, ent) : e16(xb, ent), f.y, f.w);
+        g_tab.fb2_c[lg][row][ent] = f;
+    }
+    if (row < 16 * rb2 && ent < 4) {                           // i2a: W = w_M^(32 (n3 + 16 n2b)), row = 16 n2b + n3, radix 8
+        float2 g;
         ct(e8(32 * row, ent), g.x, g.y);
-        g_tab.i2a_15[row][ent] = g;
+        g_tab.i2a_c[lg][row][ent] = g;
     }
 }
 
@@ -959,7 +995,7 @@ int init_iw3_tables(cudaStream_t st) {
     if (done.load(std::memory_order_acquire) & bit) return AMPLFI_OK;
     v3::init_tables3_kernel<<<1, 384, 0, st>>>();
     v3::init_tables3_14_kernel<<<1, 256, 0, st>>>();
-    v3::init_tables3_15_kernel<<<1, 512, 0, st>>>();
+    v3::init_tables3_cluster_kernel<<<dim3(8, 2), 256, 0, st>>>();
     count_launch(3);
     const int rc = check_launch("init_tables3_kernel");
     if (rc) return rc;
@@ -1024,6 +1060,7 @@ static int launch_iw3_l(const IwArgs& a, int mode, int units, cudaStream_t st) {
 }
 
 int launch_iw3(const IwArgs& a, int logm, int mode, int units, cudaStream_t st) {
+    if (logm == 16) return launch_iw3_l<16>(a, mode, units, st);
     if (logm == 15) return launch_iw3_l<15>(a, mode, units, st);
     if (logm == 14) return launch_iw3_l<14>(a, mode, units, st);
     if (logm == 13) return launch_iw3_l<13>(a, mode, units, st);

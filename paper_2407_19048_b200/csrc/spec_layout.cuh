@@ -1,5 +1,5 @@
 // spec_layout.cuh -- kernel-native ("slot") layout of the per-bin operands of the three-pass fused kernel
-// (inject_whiten_v3.cu: n = 4096 ... 65536, i.e. M = n/2 = 2048 ... 32768 complex points).
+// (inject_whiten_v3.cu: n = 4096 ... 131072, i.e. M = n/2 = 2048 ... 65536 complex points).
 //
 // With KL = M/16 and T = KL/2 threads, thread t (0 .. T-1) and unit w (0..7) work on the two bin pairs (u = 2w)
 //     lane 0:  k0 = t + KL u      with partner M - k0,        lane 1:  k1 = t + KL (u + 1)   with partner M - k1
@@ -19,7 +19,7 @@
 namespace amplfi {
 namespace slot {
 
-// geometry of a segment length: kl = M / 16 (128 ... 2048), T = kl / 2 threads, M = 16 kl
+// geometry of a segment length: kl = M / 16 (128 ... 4096), T = kl / 2 threads, M = 16 kl
 __host__ __device__ __forceinline__ int h0_row(int kl) { return 32 * kl; }        // floats per sample (2M)
 __host__ __device__ __forceinline__ int filt_row(int kl) { return 16 * kl; }      // floats per detector (M)
 

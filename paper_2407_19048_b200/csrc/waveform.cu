@@ -226,7 +226,7 @@ int launch_waveform_pol(const amplfi_plan* p, int batch, float* hp, float* hc, c
 }
 
 int launch_waveform_h0(const amplfi_plan* p, int batch, cudaStream_t st, int slots) {
-    if (slots) {            // slot layout of the three-pass fused kernel (n = 4096 .. 65536)
+    if (slots) {            // slot layout of the three-pass fused kernel (n = 4096 .. 131072)
         const int kl = p->n / 32;
         const int nthr = kl / 2 > 512 ? 512 : kl / 2;
         dim3 grid(batch >= 1024 ? 2 : (batch >= 64 ? 4 : 8), batch, (kl / 2) / nthr);
