@@ -198,6 +198,9 @@ def run_b200(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the B200 arm has no CPU fallback")
+    if local >= torch.cuda.device_count():
+        raise SystemExit("bench.py: rank %d wants cuda:%d but this node has %d GPU(s); one rank per GPU, ranks are never stacked on a device"
+                         % (rank, local, torch.cuda.device_count()))
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     dist = None
