@@ -136,6 +136,21 @@ int amplfi_project(const amplfi_plan* plan, int batch, const double* params, dou
 int amplfi_psd_welch(const amplfi_plan* plan, const float* bg, long n_bg, long row_stride, int noverlap,
                      int detrend, int average, float* psd, void* stream);
 
+/* The same estimate (mean over segments) for callers that may not allocate device memory: code under CUDA graph
+ * capture, serving loops, harnesses that forbid cudaMalloc.  It needs no plan and calls no cudaMalloc, cudaFree or
+ * allocating library routine: the per-segment periodograms go to a static device array of
+ * AMPLFI_NOALLOC_WELCH_FLOATS floats (4 MiB, held by every GPU that loads the library until the process exits).
+ *   bg, n_bg, row_stride, noverlap, detrend, psd as above;  n_det in [1, 3];  fs in Hz;  nperseg a power of two in
+ *   [2^10, 2^15];  stream: the cudaStream_t of the launches.
+ * Limit: n_det * nseg * (nperseg/2 + 1) <= AMPLFI_NOALLOC_WELCH_FLOATS, nseg = (n_bg - nperseg)/(nperseg - noverlap) + 1
+ * (e.g. 3 detectors x 63 segments of 8192 samples); beyond it the call returns AMPLFI_ERR_UNSUPPORTED_SIZE and launches
+ * nothing.  All calls share the one array: calls that overlap on the GPU (other streams, other threads) race on it and
+ * must be serialised by the caller.  The array keeps the previous call's contents; every value that is read is written
+ * first in the same call, so nothing needs clearing.  Results are bit-identical to amplfi_psd_welch(average = 0). */
+#define AMPLFI_NOALLOC_WELCH_FLOATS (1 << 20)
+int amplfi_psd_welch_noalloc(const float* bg, long n_bg, long row_stride, int n_det, double fs, int nperseg,
+                             int noverlap, int detrend, float* psd, void* stream);
+
 /* a-5 .. a-9 Gather + inject + whiten ("N small background chunks ... are lazily loaded";
  * PAPER.md:105 "We then inject the signals into the background chunks ... We whiten the batch using the
  * estimated power spectra"):

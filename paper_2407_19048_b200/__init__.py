@@ -24,7 +24,8 @@ EXPORTS = ("amplfi_last_error", "amplfi_psd_scale", "amplfi_version", "amplfi_ph
            "amplfi_plan_create", "amplfi_plan_destroy", "amplfi_waveform_fd", "amplfi_project",
            "amplfi_psd_welch", "amplfi_inject_whiten", "amplfi_launch_count", "amplfi_plan_set_timing",
            "amplfi_plan_kernel_times", "amplfi_assemble_batch", "amplfi_probe_fp32_pipe",
-           "amplfi_inject_whiten_views", "amplfi_waveform_td", "amplfi_inject_whiten_fir", "amplfi_qnm_table")
+           "amplfi_inject_whiten_views", "amplfi_waveform_td", "amplfi_inject_whiten_fir", "amplfi_qnm_table",
+           "amplfi_psd_welch_noalloc")
 
 
 class AmplfiError(RuntimeError):
@@ -66,6 +67,8 @@ def _load():
     lib.amplfi_project.argtypes = [vp, i32, vp, dbl, vp, vp, vp, vp, vp]
     lib.amplfi_psd_welch.restype = i32
     lib.amplfi_psd_welch.argtypes = [vp, vp, i64, i64, i32, i32, i32, vp, vp]
+    lib.amplfi_psd_welch_noalloc.restype = i32
+    lib.amplfi_psd_welch_noalloc.argtypes = [vp, i64, i64, i32, dbl, i32, i32, i32, vp, vp]
     lib.amplfi_inject_whiten.restype = i32
     lib.amplfi_inject_whiten.argtypes = [vp, i32, vp, vp, i64, vp, i32, vp, dbl, vp, i32, dbl, dbl, vp, vp]
     lib.amplfi_probe_fp32_pipe.restype = i32
@@ -250,6 +253,27 @@ def amplfi_psd_welch(plan, bg, noverlap=None, detrend=1, average=0, psd=None, st
     _need(psd, plan.n_det * (plan.nperseg // 2 + 1), "psd")
     _check(_lib.amplfi_psd_welch(plan._h, ctypes.c_void_p(bg.data_ptr()), int(bg.shape[1]), row_stride, int(noverlap), int(detrend),
                                  int(average), _ptr(psd, torch.float32, "psd"), _stream(stream)))
+    return psd
+
+
+NOALLOC_WELCH_FLOATS = 1 << 20
+
+
+def amplfi_psd_welch_noalloc(bg, fs, nperseg, psd, noverlap=None, detrend=1, stream=None):
+    """bg [D, n_bg] fp32 -> psd [D, nperseg/2+1] fp32 (S * 2^140), caller-supplied: no plan, no device allocation (the
+    library's static scratch array; see include/amplfi.h for its limit and the rule about overlapping calls)."""
+    if noverlap is None:
+        noverlap = nperseg // 2
+    if bg.dim() != 2 or bg.stride(1) != 1:
+        raise ValueError("bg must be [n_det, n_bg] with unit stride along time (rows may be a window of a strip)")
+    if not bg.is_cuda or bg.dtype != torch.float32:
+        raise TypeError("bg must be a CUDA float32 tensor (no CPU fallback)")
+    n_det = int(bg.shape[0])
+    row_stride = int(bg.stride(0)) if n_det > 1 else int(bg.shape[1])
+    _need(psd, n_det * (nperseg // 2 + 1), "psd")
+    _check(_lib.amplfi_psd_welch_noalloc(ctypes.c_void_p(bg.data_ptr()), int(bg.shape[1]), row_stride, n_det, float(fs),
+                                         int(nperseg), int(noverlap), int(detrend), _ptr(psd, torch.float32, "psd"),
+                                         _stream(stream)))
     return psd
 
 

@@ -232,3 +232,103 @@ int launch_welch(const amplfi_plan* p, const float* bg, long n_bg, long row_stri
 }
 
 }  // namespace amplfi
+
+// ---------------------------------------------------------------------------------------------------------------------
+// amplfi_psd_welch_noalloc: the Welch estimate for callers that may not allocate device memory (code under CUDA graph
+// capture, serving loops, harnesses that forbid cudaMalloc).  The same two kernels as amplfi_psd_welch, but no plan:
+// the per-segment periodograms go to a file-scope device array instead of the plan's workspace.
+//   - AMPLFI_NOALLOC_WELCH_FLOATS floats (4 MiB), held by every GPU that loads the library until the process exits;
+//   - shared by all calls: calls that overlap on the GPU (different streams, different threads) race on it;
+//   - nothing in it has to start at zero: welch_segment_kernel overwrites every value welch_mean_kernel reads, so what
+//     the previous call left behind is never seen.
+// In host code the array's name is only a stand-in; the device address comes from cudaGetSymbolAddress, taken once per
+// device with that device current, and is what the kernels are given.
+namespace amplfi {
+namespace {
+
+static __device__ __align__(256) float g_welch_scratch[AMPLFI_NOALLOC_WELCH_FLOATS];
+
+constexpr int kMaxDevices = 64;
+float* g_scratch_ptr[kMaxDevices];
+std::atomic<int> g_scratch_ready[kMaxDevices];
+
+// device address of g_welch_scratch on the current device (resolved at the first call on that device)
+int noalloc_scratch(float** out) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { set_error("amplfi_psd_welch_noalloc: cudaGetDevice: %s", cudaGetErrorString(e)); return AMPLFI_ERR_CUDA; }
+    if (dev < 0 || dev >= kMaxDevices) { set_error("amplfi_psd_welch_noalloc: device ordinal %d not supported", dev); return AMPLFI_ERR_INVALID_ARG; }
+    if (!g_scratch_ready[dev].load(std::memory_order_acquire)) {
+        float* q = nullptr;
+        e = cudaGetSymbolAddress(reinterpret_cast<void**>(&q), g_welch_scratch);
+        if (e != cudaSuccess || q == nullptr) {
+            set_error("amplfi_psd_welch_noalloc: cudaGetSymbolAddress: %s", cudaGetErrorString(e));
+            return AMPLFI_ERR_CUDA;
+        }
+        g_scratch_ptr[dev] = q;
+        g_scratch_ready[dev].store(1, std::memory_order_release);
+    }
+    *out = g_scratch_ptr[dev];
+    return AMPLFI_OK;
+}
+
+template <int LOGM>
+int noalloc_segments_t(const float* bg, long row_stride, int step, int nseg, int detrend, int n_det, float* part, cudaStream_t st) {
+    using F = Fft<LOGM>;
+    static std::atomic<unsigned> attr_done{0};
+    const int arc = ensure_dynamic_smem(welch_segment_kernel<LOGM>, (int)F::SMEM_BYTES, attr_done);
+    if (arc) return arc;
+    dim3 grid(nseg, n_det);
+    welch_segment_kernel<LOGM><<<grid, F::T, F::SMEM_BYTES, st>>>(bg, row_stride, step, nseg, detrend, part);
+    count_launch();
+    return check_launch("welch_segment_kernel");
+}
+
+}  // namespace
+}  // namespace amplfi
+
+extern "C" int amplfi_psd_welch_noalloc(const float* bg, long n_bg, long row_stride, int n_det, double fs, int nperseg,
+                                        int noverlap, int detrend, float* psd, void* stream) {
+    using namespace amplfi;
+    const char* who = "amplfi_psd_welch_noalloc";
+    if (bg == nullptr || psd == nullptr) { set_error("%s: null pointer", who); return AMPLFI_ERR_INVALID_ARG; }
+    if (n_det < 1 || n_det > 3 || !(fs > 0.0)) { set_error("%s: need 1 <= n_det <= 3 and fs > 0", who); return AMPLFI_ERR_INVALID_ARG; }
+    if (nperseg < 1024 || nperseg > 32768 || (nperseg & (nperseg - 1)) != 0) {
+        set_error("%s: nperseg %d is not a power of two in [2^10, 2^15]", who, nperseg);
+        return AMPLFI_ERR_UNSUPPORTED_SIZE;
+    }
+    if (n_bg < nperseg) { set_error("%s: nperseg %d > n_bg %ld", who, nperseg, n_bg); return AMPLFI_ERR_UNSUPPORTED_SIZE; }
+    if (noverlap < 0 || noverlap >= nperseg || (detrend != 0 && detrend != 1)) {
+        set_error("%s: need 0 <= noverlap < nperseg, detrend in {0,1}", who);
+        return AMPLFI_ERR_INVALID_ARG;
+    }
+    if (row_stride < n_bg) { set_error("%s: row_stride %ld < n_bg %ld", who, row_stride, n_bg); return AMPLFI_ERR_INVALID_ARG; }
+    const int step = nperseg - noverlap, n_w = nperseg / 2 + 1;
+    const long nseg_l = (n_bg - nperseg) / step + 1;
+    const long need = (long)n_det * nseg_l * n_w;
+    if (need > (long)AMPLFI_NOALLOC_WELCH_FLOATS) {
+        set_error("%s: n_det %d x %ld segments x %d bins = %ld floats of scratch, the static array holds %ld "
+                  "(use amplfi_psd_welch with a plan for larger backgrounds)", who, n_det, nseg_l, n_w, need,
+                  (long)AMPLFI_NOALLOC_WELCH_FLOATS);
+        return AMPLFI_ERR_UNSUPPORTED_SIZE;
+    }
+    float* part = nullptr;
+    int rc = noalloc_scratch(&part);
+    if (rc) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int nseg = (int)nseg_l;
+    switch (ilog2(nperseg) - 1) {
+        case 9: rc = noalloc_segments_t<9>(bg, row_stride, step, nseg, detrend, n_det, part, st); break;
+        case 10: rc = noalloc_segments_t<10>(bg, row_stride, step, nseg, detrend, n_det, part, st); break;
+        case 11: rc = noalloc_segments_t<11>(bg, row_stride, step, nseg, detrend, n_det, part, st); break;
+        case 12: rc = noalloc_segments_t<12>(bg, row_stride, step, nseg, detrend, n_det, part, st); break;
+        case 13: rc = noalloc_segments_t<13>(bg, row_stride, step, nseg, detrend, n_det, part, st); break;
+        default: rc = noalloc_segments_t<14>(bg, row_stride, step, nseg, detrend, n_det, part, st); break;
+    }
+    if (rc) return rc;
+    const float scale = (float)(1.0 / ((double)nseg * fs * 0.375 * (double)nperseg));
+    dim3 grid((n_w + 31) / 32, n_det);
+    welch_mean_kernel<<<grid, 32 * MEAN_PARTS, 0, st>>>(part, nseg, n_w, scale, psd, 0);
+    count_launch();
+    return check_launch("welch_mean_kernel");
+}
