@@ -46,10 +46,12 @@ __host__ __device__ __forceinline__ int filt_index(int kl, int k) {
 }
 // bins of slot (second, w, t): lane 0 and lane 1
 __host__ __device__ __forceinline__ void slot_bins(int kl, int second, int w, int t, int& kA, int& kB) {
-    const int m = 16 * kl;
-    if (second == 0) { kA = t + kl * 2 * w; kB = kA + kl; }
-    else if (t != 0) { kA = m - t - kl * 2 * w; kB = kA - kl; }
-    else { kA = kl / 2 + kl * (15 - 2 * w); kB = kA - kl; }           // thread 0: bins KL/2 + KL (15 - u)
+    // first: (t + kl 2w, + kl);  second: (M - t - kl 2w, - kl), thread 0: the self-paired bins kl/2 + kl (15 - 2w), - kl
+    // (branch-free: the producer kernel evaluates this once per slot group)
+    const int base = kl * 2 * w;
+    const int tt = t != 0 ? t : kl / 2;
+    kA = second ? 16 * kl - base - tt : base + t;
+    kB = second ? kA - kl : kA + kl;
 }
 // does warp `wi` (threads 32 wi .. 32 wi + 31) need the slots (second, w) for the band [k_lo, k_hi]?
 // (for wi = 0 the windows are widened by thread 0's self-paired bins, which sit KL/2 away from the warp's other bins)

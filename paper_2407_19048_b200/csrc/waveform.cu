@@ -171,16 +171,21 @@ __global__ void __launch_bounds__(512, 2) waveform_slots_kernel(const WfCoef* __
     {
         const int* src = reinterpret_cast<const int*>(coef + b);
         int* dst = reinterpret_cast<int*>(&c);
-        for (int q = threadIdx.x; q < (int)(sizeof(WfCoef) / sizeof(int)); q += blockDim.x) dst[q] = src[q];      // (64 .. 256 threads)
+        constexpr int NW = (int)(sizeof(WfCoef) / sizeof(int));           // 78 words; CTAs have 64 .. 512 threads
+        static_assert(NW <= 128, "two rounds of a 64-thread CTA must cover WfCoef");
+        const int q = threadIdx.x;
+        if (q < NW) dst[q] = src[q];
+        if (q + 64 < NW && blockDim.x == 64) dst[q + 64] = src[q + 64];
     }
     __syncthreads();
     if (!c.valid || c.k_lo > c.k_hi) return;
     const int k_lo = c.k_lo, k_hi = c.k_hi;
-    float4* row = reinterpret_cast<float4*>(h0 + (size_t)b * slot::h0_row(kl));
+    float4* row = reinterpret_cast<float4*>(h0 + (size_t)b * slot::h0_row(kl)) + t;
     // groups of this warp: bit g = second * 8 + w set iff the consumer reads it (one ballot instead of a test per group);
     // the CTAs of a sample share them round-robin
     const int lane_id = t & 31;
-    unsigned todo = __ballot_sync(0xffffffffu, lane_id < 16 && (lane_id % gridDim.x) == blockIdx.x &&
+    // (gridDim.x is 2, 4 or 8: launch_waveform_h0)
+    unsigned todo = __ballot_sync(0xffffffffu, lane_id < 16 && (lane_id & (gridDim.x - 1)) == blockIdx.x &&
                                                    slot::window_needed(kl, lane_id >> 3, lane_id & 7, wi, k_lo, k_hi));
 #pragma unroll 1
     while (todo) {
@@ -196,7 +201,7 @@ __global__ void __launch_bounds__(512, 2) waveform_slots_kernel(const WfCoef* __
             if (inB) { ciB = tab_ci[kB]; lnB = tab_lnk[kB]; }
         }
         float2 hA = make_float2(0.f, 0.f), hB = make_float2(0.f, 0.f);
-#pragma unroll 1
+#pragma unroll
         for (int lane = 0; lane < 2; ++lane) {
             const int k = lane ? kB : kA;
             float2 h = make_float2(0.f, 0.f);
@@ -206,7 +211,7 @@ __global__ void __launch_bounds__(512, 2) waveform_slots_kernel(const WfCoef* __
             }
             if (lane) hB = h; else hA = h;
         }
-        row[g * nt + t] = make_float4(hA.x, hB.x, hA.y, hB.y);
+        row[g * nt] = make_float4(hA.x, hB.x, hA.y, hB.y);
     }
 }
 
