@@ -48,6 +48,8 @@ struct amplfi_plan {
     int* d_det_ids;        // [3]
     float2* long_spec;     // n >= 65536: sub-spectra of one chunk of units [long_chunk, n/32768, 16392] (L2-resident)
     int long_chunk;        // units per chunk
+    float* long_filt_rows; // n >= 2^18: the filter in the [c][e] row layout of inject_whiten_long.cu [n_det, n/32768 + 1, 16384]
+    float2* long_h0_rows;  // ... and the fused path's h0 [max_batch, n/32768 + 1, 16384]
     // amplfi_assemble_batch: PSD chain runs on `side`, forked from / joined into the caller's stream
     cudaStream_t side;
     cudaEvent_t ev_fork, ev_join;
@@ -148,6 +150,7 @@ int setup_inject_whiten_attrs();
 
 // inject_whiten_long.cu (n = 2^16 .. 2^20: decimation by n/32768 around the 32768-sample transform)
 size_t long_scratch_floats2(int chunk_units, int rdec);
+size_t long_row_elems(int rdec);
 int launch_inject_whiten_long(const amplfi_plan* p, const IwArgs& a, int mode, int units, cudaStream_t st);
 
 }  // namespace amplfi

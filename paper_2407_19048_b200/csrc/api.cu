@@ -199,11 +199,22 @@ int amplfi_plan_create(int n, double fs, int n_det, const int* det_ids, int max_
     if (!rc) rc = dev_alloc(&p->fir_time, (size_t)n_det * n);
     if (!rc) rc = dev_alloc(&p->d_det_ids, (size_t)3);
     if (!rc && p->logm >= 17) {
-        // n/32768 CTAs per unit, one CTA per SM: a chunk is two full waves and its spectra (39 MB) stay in L2
-        const int rdec = n / 32768;
-        p->long_chunk = (2 * (sms > 0 ? sms : 148)) / rdec;
-        if (p->long_chunk < 1) p->long_chunk = 1;
+        // four-step path (inject_whiten_long.cu): n/32768 + 1 rows of 16384 complex points per unit, one CTA per row and SM;
+        // a chunk is two full waves of rows and its scratch (39 MB) stays in L2
+        const int rdec = n / 16384, rows = rdec / 2 + 1;
+        // units per chunk: the count (scratch <= 64 MB) whose rows fill whole waves of SMs best
+        const int nsm = sms > 0 ? sms : 148;
+        const int umax = (int)((64u << 20) / ((size_t)rows * 16384 * 8));
+        double best = 0.0;
+        p->long_chunk = 1;
+        for (int u = 1; u <= (umax < 1 ? 1 : umax); ++u) {
+            const int ctas = u * rows, waves = (ctas + nsm - 1) / nsm;
+            const double util = (double)ctas / ((double)waves * nsm);
+            if (util >= best) { best = util; p->long_chunk = u; }
+        }
         rc = dev_alloc(&p->long_spec, amplfi::long_scratch_floats2(p->long_chunk, rdec));
+        if (!rc) rc = dev_alloc(&p->long_filt_rows, (size_t)3 * amplfi::long_row_elems(rdec));
+        if (!rc) rc = dev_alloc(&p->long_h0_rows, (size_t)max_batch * amplfi::long_row_elems(rdec));
     }
     if (!rc && nperseg) rc = dev_alloc(&p->welch_part, (size_t)n_det * p->welch_max_seg * (nperseg / 2 + 1));
     if (!rc) {
@@ -271,7 +282,7 @@ void amplfi_plan_destroy(amplfi_plan* p) {
     if (p->ev_join) cudaEventDestroy(p->ev_join);
     cudaFree(p->tab_ci); cudaFree(p->tab_lnk); cudaFree(p->pd_table); cudaFree(p->coef); cudaFree(p->resp);
     cudaFree(p->resp2); cudaFree(p->filt_slots); cudaFree(p->filt_flat); cudaFree(p->fir_spec); cudaFree(p->fir_time);
-    cudaFree(p->h0); cudaFree(p->filt); cudaFree(p->welch_part); cudaFree(p->d_det_ids); cudaFree(p->long_spec);
+    cudaFree(p->h0); cudaFree(p->filt); cudaFree(p->welch_part); cudaFree(p->d_det_ids); cudaFree(p->long_spec); cudaFree(p->long_filt_rows); cudaFree(p->long_h0_rows);
     delete p;
 }
 

@@ -247,7 +247,10 @@ int launch_waveform_h0(const amplfi_plan* p, int batch, cudaStream_t st, int slo
         count_launch();
         return check_launch("sine_gaussian_kernel<h0>");
     }
-    dim3 grid(WF_SLICES, batch);
+    // (long segments come in small batches: more CTAs per sample then, up to about eight resident CTAs per SM)
+    int slices = (8 * p->sm_count) / (batch > 0 ? batch : 1);
+    slices = slices < WF_SLICES ? WF_SLICES : (slices > 64 ? 64 : slices);
+    dim3 grid(slices, batch);
     waveform_kernel<false><<<grid, 256, 0, st>>>(p->coef, p->tab_ci, p->tab_lnk, p->n_bins, p->h0, nullptr);
     count_launch();
     return check_launch("waveform_kernel<h0>");

@@ -33,7 +33,7 @@ def _make_inputs(n, fs, batch, dets, seed):
 # ------------------------------------------------------------------------------------------ two views
 @pytest.mark.parametrize("n,fs,approx", [(16384, 2048.0, A.IMRPHENOMD), (8192, 2048.0, A.TAYLORF2), (65536, 4096.0, A.IMRPHENOMD),
                                          (2048, 2048.0, A.IMRPHENOMD), (4096, 2048.0, A.IMRPHENOMD), (8192, 4096.0, A.IMRPHENOMD),
-                                         (131072, 4096.0, A.IMRPHENOMD)])
+                                         (131072, 4096.0, A.IMRPHENOMD), (262144, 4096.0, A.IMRPHENOMD)])
 def test_two_views_parity(n, fs, approx):
     dets = [0, 1, 2]
     batch = 6
@@ -100,7 +100,8 @@ def test_two_views_out_of_range_offset_poisons_both_views(n):
 
 # ------------------------------------------------------------------------------------------ time-domain waveform
 @pytest.mark.parametrize("approx", [A.TAYLORF2, A.IMRPHENOMD])
-@pytest.mark.parametrize("n,fs", [(8192, 2048.0), (16384, 2048.0), (65536, 4096.0), (1024, 2048.0), (4096, 2048.0), (131072, 4096.0)])
+@pytest.mark.parametrize("n,fs", [(8192, 2048.0), (16384, 2048.0), (65536, 4096.0), (1024, 2048.0), (4096, 2048.0), (131072, 4096.0),
+                                   (262144, 4096.0)])
 def test_waveform_td_parity(approx, n, fs):
     par = edge_params(0.6 * n / fs)
     par = np.concatenate([par, par[:1]])
@@ -139,7 +140,8 @@ def test_welch_median_parity(nperseg, n_bg, fs):
 
 # ------------------------------------------------------------------------------------------ truncated whitening filter
 @pytest.mark.parametrize("n,fs,fdur", [(16384, 2048.0, 1.0), (8192, 2048.0, 0.5), (65536, 4096.0, 2.0), (2048, 2048.0, 0.25),
-                                       (16384, 2048.0, 8.0), (4096, 2048.0, 0.5), (131072, 4096.0, 2.0)])
+                                       (16384, 2048.0, 8.0), (4096, 2048.0, 0.5), (131072, 4096.0, 2.0),
+                                       (262144, 4096.0, 2.0)])
 @pytest.mark.parametrize("crop", [True, False])
 def test_inject_whiten_fir_parity(n, fs, fdur, crop):
     if crop and fdur * fs >= n:

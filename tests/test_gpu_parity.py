@@ -299,10 +299,14 @@ def test_assemble_batch_equals_two_call_path():
     assert row_err(ref_gpu, oracle_inject_whiten(wl, "fused")).max() <= TOL
 
 
-@pytest.mark.parametrize("cfg", ["c2", "c4"])
+@pytest.mark.parametrize("cfg", ["c2", "c4", "long"])
 def test_gather_out_of_range_offset_poisons_row_only(cfg):
-    # c4 (n = 65536): both CTAs of a unit's cluster must leave before any cluster barrier, the other units run on
-    wl = WL.make_c2(batch=4, strip_len=1 << 18) if cfg == "c2" else WL.make_c4(batch=4, strip_len=1 << 22)
+    # c4 (n = 65536): both CTAs of a unit's cluster must leave before any cluster barrier, the other units run on;
+    # long (n = 262144): the four-step path, whose first and last kernels both test the offset
+    if cfg == "c2":
+        wl = WL.make_c2(batch=4, strip_len=1 << 18)
+    else:
+        wl = WL.make_c4(batch=4, strip_len=1 << 22, t_seg=16.0 if cfg == "c4" else 64.0)
     wl.offsets[1, 0] = wl.strip.shape[1] - wl.n + 1
     wl.offsets[2, 2] = -1
     got, _ = run_inject_whiten(wl, "none")
