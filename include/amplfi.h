@@ -168,8 +168,8 @@ int amplfi_psd_welch_noalloc(const float* bg, long n_bg, long row_stride, int n_
  *            which case S is linearly interpolated in frequency onto the segment grid.
  *   out      [batch, n_det, n] fp32.
  * batch <= the plan's max_batch.  n = 2^16 and 2^17 run as a cluster of two / four thread blocks sharing the transform
- * through distributed shared memory; n >= 2^18 is decimated by n / 2^15 around the 2^15-sample transform, the intermediate
- * spectra of a chunk of segments staying in L2 (three launches per chunk). */
+ * through distributed shared memory; n >= 2^18 runs as a four-step transform around rows of 16384 complex points, the
+ * rows of a chunk of segments staying in L2 (three launches per chunk). */
 int amplfi_inject_whiten(const amplfi_plan* plan, int batch, const float* noise, const long* offsets,
                          long strip_len, const float* h_det, int approximant, const double* params,
                          double gmst, const float* psd, int n_psd, double f_lo, double f_hi,
