@@ -367,7 +367,7 @@ def test_other_segment_lengths(n, fs):
     assert row_err(got, ref).max() <= TOL
 
 
-@pytest.mark.parametrize("n", [2048, 4096, 8192, 16384, 32768, 65536, 131072])
+@pytest.mark.parametrize("n", [2048, 4096, 8192, 16384, 32768, 65536, 131072, 262144])
 def test_full_band_including_dc_and_nyquist(n):
     # f_lo = 0, f_hi = fs/2: the DC and Nyquist bins take the special path of the packed real FFT (every kernel family)
     fs = 2048.0
