@@ -149,6 +149,10 @@ struct LongEdgeArgs {
     int n_det, unit0, n_full, crop;
 };
 
+// cos / sin of 2 pi i / 64, i < 32 (the one stage of the 64-point register transform that fft_core.cuh does not cover)
+__device__ constexpr float kCos64[32] = {1.000000000e+00f, 9.951847267e-01f, 9.807852804e-01f, 9.569403357e-01f, 9.238795325e-01f, 8.819212643e-01f, 8.314696123e-01f, 7.730104534e-01f, 7.071067812e-01f, 6.343932842e-01f, 5.555702330e-01f, 4.713967368e-01f, 3.826834324e-01f, 2.902846773e-01f, 1.950903220e-01f, 9.801714033e-02f, 0.000000000e+00f, -9.801714033e-02f, -1.950903220e-01f, -2.902846773e-01f, -3.826834324e-01f, -4.713967368e-01f, -5.555702330e-01f, -6.343932842e-01f, -7.071067812e-01f, -7.730104534e-01f, -8.314696123e-01f, -8.819212643e-01f, -9.238795325e-01f, -9.569403357e-01f, -9.807852804e-01f, -9.951847267e-01f};
+__device__ constexpr float kSin64[32] = {0.000000000e+00f, 9.801714033e-02f, 1.950903220e-01f, 2.902846773e-01f, 3.826834324e-01f, 4.713967368e-01f, 5.555702330e-01f, 6.343932842e-01f, 7.071067812e-01f, 7.730104534e-01f, 8.314696123e-01f, 8.819212643e-01f, 9.238795325e-01f, 9.569403357e-01f, 9.807852804e-01f, 9.951847267e-01f, 1.000000000e+00f, 9.951847267e-01f, 9.807852804e-01f, 9.569403357e-01f, 9.238795325e-01f, 8.819212643e-01f, 8.314696123e-01f, 7.730104534e-01f, 7.071067812e-01f, 6.343932842e-01f, 5.555702330e-01f, 4.713967368e-01f, 3.826834324e-01f, 2.902846773e-01f, 1.950903220e-01f, 9.801714033e-02f};
+
 // R-point transforms in registers for R = 16, 32 (fft_core.cuh) and 64 (one radix-2 stage around two 32-point ones):
 // forward: natural-order input, output c left in v[edge_pos<R>(c)];  inverse (unnormalised): input c taken from there,
 // natural-order output
@@ -163,7 +167,7 @@ __device__ __forceinline__ void edge_fft_fwd(float2 (&v)[R]) {
 #pragma unroll
         for (int i = 0; i < 32; ++i) {
             lo[i] = cadd(v[i], v[i + 32]);
-            hi[i] = cmul(csub(v[i], v[i + 32]), twiddle<64>(i));
+            hi[i] = cmul(csub(v[i], v[i + 32]), make_float2(kCos64[i], -kSin64[i]));      // w_64^i
         }
         fft_dif_fwd<32>(lo);                                    // even c
         fft_dif_fwd<32>(hi);                                    // odd c
@@ -183,7 +187,7 @@ __device__ __forceinline__ void edge_fft_inv(float2 (&v)[R]) {
         fft_dit_inv<32>(hi);
 #pragma unroll
         for (int i = 0; i < 32; ++i) {
-            const float2 t = cmul_conj(hi[i], twiddle<64>(i));
+            const float2 t = cmul_conj(hi[i], make_float2(kCos64[i], -kSin64[i]));
             v[i] = cadd(lo[i], t);
             v[i + 32] = csub(lo[i], t);
         }
