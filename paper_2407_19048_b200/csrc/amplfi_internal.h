@@ -46,7 +46,7 @@ struct amplfi_plan {
     float* welch_part;     // [n_det * max_seg * (nperseg/2+1)]
     int welch_max_seg;
     int* d_det_ids;        // [3]
-    float2* long_spec;     // n >= 65536: sub-spectra of one chunk of units [long_chunk, n/32768, 16392] (L2-resident)
+    float2* long_spec;     // n >= 2^18: rows of one chunk of units [long_chunk, n/32768 + 1, 16384] (L2-resident)
     int long_chunk;        // units per chunk
     float* long_filt_rows; // n >= 2^18: the filter in the [c][e] row layout of inject_whiten_long.cu [n_det, n/32768 + 1, 16384]
     float2* long_h0_rows;  // ... and the fused path's h0 [max_batch, n/32768 + 1, 16384]
@@ -148,7 +148,7 @@ int launch_shift_resp(const amplfi_plan* p, int batch, const double* t_shift, cu
 int launch_td_resp(const amplfi_plan* p, int batch, cudaStream_t st);
 int setup_inject_whiten_attrs();
 
-// inject_whiten_long.cu (n = 2^16 .. 2^20: decimation by n/32768 around the 32768-sample transform)
+// inject_whiten_long.cu (n = 2^18 .. 2^20: four-step transform around rows of 16384 complex points)
 size_t long_scratch_floats2(int chunk_units, int rdec);
 size_t long_row_elems(int rdec);
 int launch_inject_whiten_long(const amplfi_plan* p, const IwArgs& a, int mode, int units, cudaStream_t st);
