@@ -488,8 +488,9 @@ def measure_small(A, WL, torch, dev, stream, config, runs):
     return res
 
 
-def measure_throughput(A, torch, dev, stream, wl, steps, warmup):
-    """ms per step, samples/s and launches per step of amplfi_psd_welch + fused amplfi_inject_whiten on a strip workload."""
+def measure_throughput(A, torch, dev, stream, wl, steps, warmup, kernel_time=False):
+    """ms per step, samples/s and launches per step of amplfi_psd_welch + fused amplfi_inject_whiten on a strip workload
+    (kernel_time: also the mean device time of the inject+whiten launches, bracketed by events inside the library)."""
     B, D, N = wl.batch, wl.n_det, wl.n
     plan = A.Plan(N, wl.fs, wl.det_ids, B, nperseg=wl.nperseg)
     strip = torch.from_numpy(wl.strip).to(dev)
@@ -507,6 +508,8 @@ def measure_throughput(A, torch, dev, stream, wl, steps, warmup):
     for _ in range(warmup):
         step()
     torch.cuda.synchronize()
+    if kernel_time:
+        plan.set_timing(True)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     l0 = A.launch_count()
     e0.record(stream)
@@ -515,11 +518,18 @@ def measure_throughput(A, torch, dev, stream, wl, steps, warmup):
     e1.record(stream)
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / steps
+    k_ms = None
+    if kernel_time:
+        kt = plan.kernel_times_ms()
+        plan.set_timing(False)
+        k_ms = sum(kt) / len(kt) if kt else None
     assert bool(torch.isfinite(out[:: max(1, B // 16)]).all())
     sps = B * D * N / (ms * 1e-3)
     n_l = (A.launch_count() - l0) // steps
     del plan, strip, out
     torch.cuda.empty_cache()
+    if kernel_time:
+        return ms, sps, n_l, k_ms
     return ms, sps, n_l
 
 
@@ -530,10 +540,16 @@ C4_WORKLOAD = ("c4 bandwidth stress: batch 8192 x H1+L1+V1, fs 4096 Hz, 16 s seg
 def measure_c4(A, WL, torch, dev, stream, steps, batch=8192):
     peak, peak_src = peaks()
     wl = WL.make_c4(batch=batch)
-    ms, sps, n_l = measure_throughput(A, torch, dev, stream, wl, steps, 3)
+    ms, sps, n_l, k_ms = measure_throughput(A, torch, dev, stream, wl, steps, 3, kernel_time=True)
+    kernel = None
+    if k_ms:
+        gbs = 8.0 * wl.batch * wl.n_det * wl.n / (k_ms * 1e-3) / 1e9
+        kernel = {"kernel": "v3::inject_whiten3_kernel<15, fused> (clusters of two CTAs)", "kernel_ms": k_ms, "achieved": gbs,
+                  "unit": "GB/s", "frac": gbs / peak, "kernel_share_of_step": k_ms / ms}
     return {"metric": METRIC.replace("2048 Hz", "4096 Hz"), "value": sps, "unit": UNIT, "ms_per_step": ms,
             "higher_is_better": True, "dtype": "f32", "data": "synthetic", "gpu_launches_per_step": int(n_l),
             "hbm_gbs_step": 8.0 * sps / 1e9, "frac_of_measured_hbm": 8.0 * sps / 1e9 / peak, "peak_source": peak_src,
+            "roofline_kernel": kernel,
             "config": {"workload": C4_WORKLOAD, "batch": batch}}
 
 # ------------------------------------------------------------------------------------------------
